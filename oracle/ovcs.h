@@ -1,0 +1,91 @@
+/* oracle/ovcs.h — CPU ORACLE for the batched Atari 2600 VCS hot path.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may load it.  It shares no code,
+ * header, table or helper with the CUDA path (paper_2606_22447_b200/csrc) and neither
+ * includes the other.
+ *
+ * What it is: a plain, slow, single-threaded, one-CPU-cycle-at-a-time model of the
+ * machine the paper re-implements (§1, L55 Fig. 1, L61 "Why the Atari VCS
+ * Is Good Ground Truth": 6507 CPU + TIA + RIOT + bank-switched cartridge), in hard mode
+ * (§3: "opcode bytes index an integer dispatch table, the ALU is integer
+ * arithmetic, and flags are bits").  The paper does not define the chips at register
+ * level; the register-level machine model is SURVEY.md §8(c) C.1–C.12 (tags [P] paper,
+ * [D] public 6502/6532/TIA documentation, [R] reading).  Every function in ovcs.c cites
+ * the clause it follows.  All readings are listed in DESIGN.md §3.
+ *
+ * Parity status: pinned by tests/test_oracle_*.py (-m "not gpu") against the opcode
+ * matrix, wide-integer ADC/SBC definitions, base-100 BCD arithmetic, the RIOT closed
+ * form, hand-assembled programs with hand-derived RAM/screens.  PARITY UNPINNED (no
+ * source other than the [R] readings exists in this container): per-register TIA write
+ * latencies, mid-line HMOVE, RSYNC, double/quad-size player 1-clock shift, bus residue
+ * in TIA reads, same-cycle INTIM/underflow, F8 start bank, power-on timer/RAM state, y0,
+ * and decimal-mode results for invalid BCD operands (cited algorithm only).
+ */
+#ifndef OVCS_H
+#define OVCS_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ovcs_s ovcs_t;
+
+typedef struct { const uint8_t *data; uint32_t size; /* 2048 | 4096 | 8192 (F8) */ } ovcs_rom;
+typedef struct { int32_t y0, max_lines, f8_start_bank; uint32_t flags; } ovcs_config;
+
+/* Same 32-byte record as include/vcs.h's vcs_regs; retyped, not shared. */
+typedef struct {
+  uint64_t cycles;
+  uint32_t frame;
+  uint16_t pc; uint8_t a, x, y, sp, p;
+  uint8_t bank;
+  uint16_t line; uint8_t cyc_in_line;
+  uint8_t status;            /* bit0 illegal-opcode halt, bit1 frame cap was hit */
+  uint8_t intim, timint, pad[6];
+} ovcs_regs;
+
+/* Debug view of the TIA/RIOT latches, for the hand-program pins (tests only). */
+typedef struct {
+  uint8_t posP0, posP1, posM0, posM1, posBL;
+  uint8_t fresh, hmove_blank, vsync, vblank, latch_en, wsync;
+  uint8_t inpt4_latch, grp0_new, grp0_old, grp1_new, grp1_old;
+  uint16_t cx;
+  uint8_t timer, tflag, shift; uint16_t sub;
+  uint64_t clocks_rendered;      /* colour clocks rendered since reset: must equal 3*cycles */
+} ovcs_debug;
+
+enum { OVCS_OK = 0, OVCS_EINVAL = -1, OVCS_ENOMEM = -3, OVCS_EROM = -4 };
+
+/* All pointers are HOST pointers.  roms/env_rom/seeds are copied. */
+int  ovcs_create(ovcs_t **out, int32_t batch, const ovcs_rom *roms, int32_t n_roms,
+                 const int32_t *env_rom, const uint64_t *seeds, const ovcs_config *cfg);
+int  ovcs_reset(ovcs_t *h, const uint8_t *mask /* [batch] or NULL = all */);
+int  ovcs_step(ovcs_t *h, const uint8_t *actions /* [batch] */, int32_t frameskip);
+/* Same as ovcs_step restricted to envs [lo,hi): lets a test fan independent envs over
+ * OS threads; the oracle code itself stays single-threaded per env. */
+int  ovcs_step_range(ovcs_t *h, const uint8_t *actions, int32_t frameskip, int32_t lo, int32_t hi);
+int  ovcs_get_ram(ovcs_t *h, uint8_t *out /* [batch][128] */);
+int  ovcs_get_regs(ovcs_t *h, ovcs_regs *out /* [batch] */);
+int  ovcs_get_screen(ovcs_t *h, uint8_t *out /* [batch][210][160] */);
+int  ovcs_destroy(ovcs_t *h);
+
+/* Test hooks: one env at a time. */
+int  ovcs_set_action(ovcs_t *h, int32_t env, int32_t action);  /* latch pins only (C.11)  */
+int  ovcs_step_instruction(ovcs_t *h, int32_t env);             /* returns frame-end events */
+int  ovcs_tick(ovcs_t *h, int32_t env);                         /* one idle CPU cycle       */
+int  ovcs_get_debug(ovcs_t *h, int32_t env, ovcs_debug *out);
+int  ovcs_get_back(ovcs_t *h, int32_t env, uint8_t *out /* [210][160] */);
+int  ovcs_set_cpu(ovcs_t *h, int32_t env, int a, int x, int y, int sp, int p, int pc); /* <0 = keep */
+int  ovcs_poke_ram(ovcs_t *h, int32_t env, int idx, int value);
+
+/* Bare ALU entry points for the brute-force pins (C.6).  flags in/out use the P layout. */
+void ovcs_alu_adc(int a, int m, int p_in, int *a_out, int *p_out);
+void ovcs_alu_sbc(int a, int m, int p_in, int *a_out, int *p_out);
+/* splitmix64: advances *state, returns the draw. */
+uint64_t ovcs_splitmix64(uint64_t *state);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
