@@ -1,0 +1,257 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the vcs_step hot path on BASELINE.json's headline config.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+Workload (N=1): BASELINE.json configs[3] — 65,536 envs over 256 seed-generated ROMs (128 x 4 KB, 128 x 8 KB F8),
+uniform random actions, frameskip 4.  One "step" = one vcs_step(actions, 4) over the whole batch = one launch
+of the persistent interpreter kernel.  `value` = env-steps/s with the action stream resident in HBM;
+`e2e` = the same through the host-pointer C ABI (actions H2D, RAM + regs + screens D2H every step).
+N>1 (torchrun): every rank runs its own 65,536-env shard, no collective on the data path (weak scaling).
+`--impl reference` times the CPU oracle (oracle/) on host cores on a bounded sample of the same workload.
+Prints ONE JSON line on rank 0."""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FRAMESKIP = 4
+METRIC = "env-steps/s (frameskip 4) at batch 65536"
+# SURVEY §8(d) lower-bound work model: thread-instructions per 6502 instruction / TIA segment / scanline
+MODEL_PER_INSTR, MODEL_PER_SEGMENT, MODEL_PER_LINE = 40, 80, 40
+
+
+def oracle_sample(w, n_envs: int, steps: int, threads: int):
+    """Time the oracle, as it stands, on `n_envs` envs (spread over the ROMs) for `steps` env-steps."""
+    from oracle.ovcs_py import OracleVCS
+    idx = (np.arange(n_envs) * (w.batch // n_envs) + (np.arange(n_envs) * 37) % max(1, w.batch // n_envs)).astype(np.int64)
+    o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx])
+    acts = w.actions(0, steps + 1)
+    o.step(acts[0][idx], FRAMESKIP, threads=threads)                    # untimed: first (short) frame, page-in
+    c0 = o.regs()["cycles"].astype(np.int64).sum()
+    d0 = [o.debug(e) for e in range(n_envs)]
+    t0 = time.perf_counter()
+    for t in range(1, steps + 1):
+        o.step(acts[t][idx], FRAMESKIP, threads=threads)
+    dt = time.perf_counter() - t0
+    c1 = o.regs()["cycles"].astype(np.int64).sum()
+    d1 = [o.debug(e) for e in range(n_envs)]
+    per = n_envs * steps
+    work = dict(instr=sum(b.n_instr - a.n_instr for a, b in zip(d0, d1)) / per,
+                tia_writes=sum(b.n_tia_writes - a.n_tia_writes for a, b in zip(d0, d1)) / per,
+                lines=(c1 - c0) / 76.0 / per, cycles=(c1 - c0) / per)
+    return dict(value=per / dt, seconds=dt, cycles_per_s=(c1 - c0) / dt, work=work,
+                sample=f"{n_envs} envs (one per {w.batch // n_envs} of config 4's batch, spread over its ROMs) x {steps} env-steps of frameskip 4")
+
+
+class ClockSampler(threading.Thread):
+    FIELDS = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, gpu_index: int):
+        super().__init__(daemon=True)
+        self.gpu, self.rows, self.stop_flag, self.active = gpu_index, [], False, False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if self.active and out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
+                "power_w_max": max(float(r[2]) for r in self.rows), "samples": len(self.rows)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from vcs_inputs import make_workload
+    import __graft_entry__ as g
+    from oracle import ovcs_py
+    ovcs_py.build()
+    w = make_workload(4)
+    cores = os.cpu_count() or 1
+    n_envs = max(cores, 32)
+    for _ in range(args.warmup):
+        oracle_sample(w, n_envs, 1, cores)
+    t0 = time.perf_counter(); vals = []
+    for _ in range(args.steps):
+        vals.append(oracle_sample(w, n_envs, 1, cores))
+    total = sum(v["seconds"] for v in vals)
+    value = n_envs * len(vals) / total
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "env-steps/s", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / len(vals), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+            "config": {"workload": "config4: 65536 envs, 256 seeded ROMs (128x4K + 128x8K F8), random actions, frameskip 4",
+                       "note": "each step is a bounded sample of the workload (see cpu_baseline.sample)"},
+            "cpu_baseline": {"value": value, "unit": "env-steps/s", "cores": cores, "kind": "oracle", "sample": vals[0]["sample"] + " per step",
+                             "emulated_cycles_per_s": sum(v["cycles_per_s"] * v["seconds"] for v in vals) / total},
+            "e2e": {"value": value, "unit": "env-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--batch", type=int, default=65536, help="envs per GPU (default: BASELINE config 4)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as g
+    g.build()
+    from paper_2606_22447_b200 import VCS
+    from vcs_inputs import make_workload
+
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libvcsb200 has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    K, W = args.steps, max(args.warmup, 3)
+    B = args.batch
+    n_roms = 256 if B % 256 == 0 else 1
+    w = make_workload(4, batch=B, n_roms=n_roms)
+    if world > 1:                                   # every rank its own env seeds / action streams (same ROM set)
+        w.seeds = w.seeds ^ np.uint64(0x1000000 * rank); w._act_seeds = w._act_seeds ^ np.uint64(0x1000000 * rank)
+    env = VCS(w.roms, w.seeds, w.env_rom)
+    acts_host = w.actions(0, W + K)
+    acts = torch.from_numpy(acts_host).cuda()
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local); sampler.start()
+    for t in range(W):
+        env.step(acts[t], FRAMESKIP)
+    barrier()
+    cyc0 = env.regs_host()["cycles"].astype(np.int64).sum()
+    l0 = env.launch_count()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+    sampler.active = True
+    barrier()
+    evs[0].record(stream)
+    for t in range(K):
+        env.step(acts[W + t], FRAMESKIP)
+        evs[t + 1].record(stream)
+    barrier()
+    sampler.active = False
+    launches = env.launch_count() - l0
+    total_ms = evs[0].elapsed_time(evs[K])
+    kern_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(K)]
+    cyc1 = env.regs_host()["cycles"].astype(np.int64).sum()
+    tt = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+    cc = torch.tensor([float(cyc1 - cyc0)], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX); dist.all_reduce(cc, op=dist.ReduceOp.SUM)
+    total_ms = float(tt.item()); cycles = float(cc.item())
+    value = world * B * K / (total_ms * 1e-3)
+
+    # ---- e2e: host-pointer C ABI, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        Ke = max(2, min(K, 5))
+        scr_host = torch.empty((B, 210, 160), dtype=torch.uint8).pin_memory().numpy()
+        env.step_host(acts_host[0], FRAMESKIP); env.screen_host(out=scr_host)            # warm the staging buffers
+        barrier()
+        t0 = time.perf_counter()
+        for t in range(Ke):
+            env.step_host(acts_host[W + t], FRAMESKIP)
+            env.ram_host(); env.regs_host(); env.screen_host(out=scr_host)
+        barrier()
+        dt = torch.tensor([time.perf_counter() - t0], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        t0 = time.perf_counter()
+        for t in range(Ke):
+            env.step_host(acts_host[W + t], FRAMESKIP)
+            env.ram_host(); env.regs_host()
+        barrier()
+        dt2 = torch.tensor([time.perf_counter() - t0], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(dt2, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * B * Ke / float(dt.item()), "unit": "env-steps/s", "h2d_bytes_per_step": B,
+               "d2h_bytes_per_step": B * (128 + 32 + 210 * 160), "steps": Ke,
+               "what": "vcs_step_host + vcs_get_ram_host + vcs_get_regs_host + vcs_get_screen_host (pinned screen buffer)",
+               "ram_regs_only": {"value": world * B * Ke / float(dt2.item()), "d2h_bytes_per_step": B * 160}}
+    sampler.stop_flag = True
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    clocks = sampler.summary()
+    cpu = None
+    work = None
+    if not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        s = oracle_sample(make_workload(4), max(64, cores), 2, cores)
+        work = s["work"]
+        cpu = {"value": s["value"], "unit": "env-steps/s", "cores": cores, "kind": "oracle", "sample": s["sample"],
+               "emulated_cycles_per_s": s["cycles_per_s"], "seconds": s["seconds"]}
+    # ---- roofline: integer-issue bound.  peak = 148 SM x 4 schedulers x 32 lanes x SM clock (1 warp-instruction
+    # per scheduler per clock); achieved = SURVEY §8(d)'s lower-bound work model x envs / kernel time.
+    sm_mhz = clocks.get("sm_mhz") or peaks.get("sm_max_mhz") or 1965.0
+    peak = 148 * 4 * 32 * sm_mhz * 1e6
+    kms = float(np.mean(kern_ms))
+    roof = {"bound": "alu", "unit": "thread-instr/s", "peak": peak, "peak_basis": f"148 SM x 4 x 32 lanes x {sm_mhz:.0f} MHz (median SM clock sampled under load)",
+            "kernel": "vcs_step_kernel", "kernel_ms": kms, "traffic": None}
+    if work:
+        ops = MODEL_PER_INSTR * work["instr"] + MODEL_PER_SEGMENT * work["tia_writes"] + MODEL_PER_LINE * work["lines"]
+        roof.update(achieved=ops * B / (kms * 1e-3), algorithmic_thread_instr_per_env_step=ops, work_per_env_step=work)
+        roof["frac"] = roof["achieved"] / peak
+    hbm_bytes = B * (210 * 160 + 2 * (128 + 4 * 15 + 8) + 1)
+    roof["hbm"] = {"algorithmic_bytes_per_launch": hbm_bytes, "achieved_gbs": hbm_bytes / (kms * 1e-3) / 1e9,
+                   "peak_gbs": peaks.get("hbm_gbs"), "frac": (hbm_bytes / (kms * 1e-3) / 1e9) / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None}
+    line = {"metric": METRIC, "value": value, "unit": "env-steps/s", "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
+            "data": "synthetic", "emulated_cycles_per_s": cycles / (total_ms * 1e-3), "frames_per_s": value * FRAMESKIP,
+            "config": {"workload": "config4: 65536 envs/GPU, 256 seeded ROMs (128x4K + 128x8K F8), uniform random actions, frameskip 4",
+                       "batch_per_gpu": B, "frameskip": FRAMESKIP, "l2": "per-step working set 2.2 GB (screens) > 126 MB L2; no explicit flush",
+                       "target_env_steps_per_s": 1e7},
+            "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, "roofline": roof, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

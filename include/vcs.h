@@ -1,0 +1,102 @@
+/* include/vcs.h — C ABI of libvcsb200: a batched, cycle-exact Atari 2600 VCS (hard mode) on one B200.
+ *
+ * The operation: §1 / L55 Fig. 1 / L61 — a 6507 CPU executing cartridge ROM, a TIA that
+ * turns register writes into pixels cycle by cycle, a RIOT (128 B RAM, interval timer, joystick/switch
+ * I/O), bank-switched cartridges; hard mode per L73 §3 ("opcode bytes index an integer dispatch table,
+ * the ALU is integer arithmetic, and flags are bits"); output frame 210x160 palette indices (L69, L167);
+ * deterministic given ROM, action stream and seed (L63).  The register-level machine model is
+ * SURVEY.md §8(c) C.1–C.12, restated in DESIGN.md §2–3.  Entry points follow SURVEY.md §8(b).
+ *
+ * Conventions
+ *   - Every function returns VCS_OK (0) or a negative error; none throws or aborts.
+ *   - "host" pointers are ordinary CPU memory, "device" pointers are CUDA device memory of the GPU that
+ *     was current when vcs_create ran.  No torch types cross this boundary.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  vcs_reset,
+ *     vcs_step and vcs_get_* only enqueue work on that stream and return; ordering is stream ordering.
+ *     vcs_create / vcs_destroy synchronise the device.
+ *   - The library owns all per-environment state and the front screen buffer.  The caller owns the
+ *     action buffer and every output buffer.  roms / env_rom / seeds are copied by vcs_create.
+ *   - There is no CPU fallback: without a CUDA device vcs_create returns VCS_ECUDA.
+ */
+#ifndef VCS_H
+#define VCS_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vcs_s *vcs_t;
+
+enum { VCS_OK = 0, VCS_EINVAL = -1, VCS_ECUDA = -2, VCS_ENOMEM = -3, VCS_EROM = -4 };
+
+/* One cartridge image (host memory).  size 2048 (2K, mirrored), 4096 (4K) or 8192 (F8: any bus access
+ * to $1FF8/$1FF9 selects bank 0/1 — SURVEY C.9; "writes to special addresses swap which
+ * 4KB ROM page is visible"). */
+typedef struct { const uint8_t *data; uint32_t size; } vcs_rom;
+
+/* y0: scanline shown as screen row 0 (default 34, must be >= 2);  max_lines: frame cap in scanlines
+ * (default 320) — a frame that has not ended by a VSYNC 1->0 write after max_lines*76 CPU cycles is
+ * ended at the next instruction boundary;  f8_start_bank: bank selected at reset for
+ * 8 KB images (default 1);  flags: reserved, must be 0. */
+typedef struct { int32_t y0, max_lines, f8_start_bank; uint32_t flags; } vcs_config;
+
+/* 32 bytes per environment, little-endian. */
+typedef struct {
+  uint64_t cycles;           /* CPU cycles since reset, WSYNC stalls included                     */
+  uint32_t frame;            /* completed frames since reset                                       */
+  uint16_t pc; uint8_t a, x, y, sp, p;   /* p: bit5 always 1, bit4 always 0                        */
+  uint8_t  bank;             /* current cartridge bank                                             */
+  uint16_t line; uint8_t cyc_in_line;    /* beam: scanline in frame, cycles % 76                   */
+  uint8_t  status;           /* bit0 undocumented-opcode halt, bit1 frame cap was hit,
+                                bit2 bus pattern outside the kernel's modelled set */
+  uint8_t  intim, timint, _pad[6];       /* timer value and TIMINT bit 7, read without side effects */
+} vcs_regs;
+
+/* Create `batch` consoles.  roms[n_roms], env_rom[batch] (index into roms; NULL = all 0) and
+ * seeds[batch] are HOST arrays.  seeds[e] seeds env e's power-on RAM: the first 16 draws of
+ * splitmix64(seeds[e]), little-endian.  cfg NULL = defaults.
+ * On return every env is in its reset state (C.2) and the screens are zero.
+ * Errors: VCS_EINVAL (NULL/size/range), VCS_EROM (size not 2048/4096/8192), VCS_ECUDA, VCS_ENOMEM. */
+int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms,
+               const int32_t *env_rom, const uint64_t *seeds, const vcs_config *cfg);
+
+/* Reset the envs with mask_dev[e] != 0 (DEVICE uint8[batch]; NULL = all) to the C.2 state. */
+int vcs_reset(vcs_t h, const uint8_t *mask_dev, void *cuda_stream);
+
+/* One env-step for every env: latch the action (DEVICE uint8[batch]; ALE numbering 0..17, >= 18 is
+ * NOOP — SURVEY C.11) into SWCHA / INPT4, then run whole instructions until `frameskip` frame-end
+ * events have occurred (C.10).  The last completed frame becomes the front screen.
+ * frameskip must satisfy 1 <= frameskip and frameskip*max_lines*76 < 2^31. */
+int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_stream);
+
+/* Copies into caller-owned DEVICE buffers. */
+int vcs_get_ram(vcs_t h, uint8_t *out_dev /* [batch][128] */, void *cuda_stream);
+int vcs_get_regs(vcs_t h, vcs_regs *out_dev /* [batch] */, void *cuda_stream);
+int vcs_get_screen(vcs_t h, uint8_t *out_dev /* [batch][210][160] */, void *cuda_stream);
+
+/* Convenience for hosts without their own device buffers: vcs_step / vcs_get_* with HOST pointers.
+ * The host<->device copies run on `cuda_stream`; the call returns after they complete. */
+int vcs_step_host(vcs_t h, const uint8_t *actions_host, int32_t frameskip, void *cuda_stream);
+int vcs_get_ram_host(vcs_t h, uint8_t *out_host, void *cuda_stream);
+int vcs_get_regs_host(vcs_t h, vcs_regs *out_host, void *cuda_stream);
+int vcs_get_screen_host(vcs_t h, uint8_t *out_host, void *cuda_stream);
+
+/* Device pointer to the library-owned front screen [batch][210][160] (valid until vcs_destroy; contents
+ * change with every vcs_step).  Zero-copy alternative to vcs_get_screen. */
+int vcs_screen_ptr(vcs_t h, const uint8_t **out_dev_ptr);
+
+/* Number of kernel launches this handle has enqueued so far (bench bookkeeping). */
+int64_t vcs_launch_count(vcs_t h);
+
+/* Introspection, no GPU needed: copies the interpreter's 256-entry decode table (HOST uint16[256];
+ * entry = addressing mode | operation<<4 | access kind<<10, operation 0 = undocumented opcode) so that a
+ * CPU-only test can check it against the documented 151-opcode matrix. */
+int vcs_optable(uint16_t *out256_host);
+
+int vcs_destroy(vcs_t h);
+const char *vcs_last_error(vcs_t h);     /* handle-owned string; "" when no error. h may be NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

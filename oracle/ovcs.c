@@ -33,6 +33,7 @@ typedef struct {
   /* cart */
   const uint8_t *rom; uint32_t rom_size; uint8_t bank;
   uint64_t seed;
+  uint64_t n_instr, n_tia_writes;    /* instrumentation only (bench work model); never read by the model */
   uint8_t *back, *front;
 } env_t;
 
@@ -281,7 +282,7 @@ static void bus_write(ctx_t *c, uint16_t addr, uint8_t v) {
   tick(c);
   int n = (int)((e->cyc - 1) % LINE_CYC);
   if (a & 0x1000) { cart_hotspot(e, a); return; }
-  if ((a & 0x0080) == 0) { tia_write(e, a, v, n); return; }
+  if ((a & 0x0080) == 0) { e->n_tia_writes++; tia_write(e, a, v, n); return; }
   if ((a & 0x0200) == 0) { e->ram[a & 0x7F] = v; return; }
   riot_write(e, a, v);
 }

@@ -53,6 +53,7 @@ typedef struct {
   uint16_t cx;
   uint8_t timer, tflag, shift; uint16_t sub;
   uint64_t clocks_rendered;      /* colour clocks rendered since reset: must equal 3*cycles */
+  uint64_t n_instr, n_tia_writes; /* instrumentation: instructions executed / TIA register writes since reset */
 } ovcs_debug;
 
 enum { OVCS_OK = 0, OVCS_EINVAL = -1, OVCS_ENOMEM = -3, OVCS_EROM = -4 };

@@ -45,7 +45,7 @@ class Debug(C.Structure):
                                          "vblank", "latch_en", "wsync", "inpt4_latch", "grp0_new", "grp0_old",
                                          "grp1_new", "grp1_old")] + \
                [("cx", C.c_uint16), ("timer", C.c_uint8), ("tflag", C.c_uint8), ("shift", C.c_uint8),
-                ("sub", C.c_uint16), ("clocks_rendered", C.c_uint64)]
+                ("sub", C.c_uint16), ("clocks_rendered", C.c_uint64), ("n_instr", C.c_uint64), ("n_tia_writes", C.c_uint64)]
 
 
 _lib = None

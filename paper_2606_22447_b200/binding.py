@@ -1,0 +1,169 @@
+"""Thin ctypes binding over libvcsb200.so (include/vcs.h).  Argument marshalling only: every step of the
+emulation runs in the CUDA kernels.  PyTorch supplies device memory and streams, nothing else.
+
+There is no CPU fallback: if the shared library is missing, or no CUDA device is present, construction
+raises.  This module never imports anything from oracle/.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_PKG, "libvcsb200.so")
+
+VCS_OK, VCS_EINVAL, VCS_ECUDA, VCS_ENOMEM, VCS_EROM = 0, -1, -2, -3, -4
+_ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
+
+EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
+           "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_launch_count",
+           "vcs_optable", "vcs_destroy", "vcs_last_error"]
+
+REGS_DTYPE = np.dtype([("cycles", "<u8"), ("frame", "<u4"), ("pc", "<u2"), ("a", "u1"), ("x", "u1"), ("y", "u1"),
+                       ("sp", "u1"), ("p", "u1"), ("bank", "u1"), ("line", "<u2"), ("cyc_in_line", "u1"),
+                       ("status", "u1"), ("intim", "u1"), ("timint", "u1"), ("pad", "u1", (6,))])
+assert REGS_DTYPE.itemsize == 32
+
+
+class VcsRom(C.Structure):
+    _fields_ = [("data", C.POINTER(C.c_uint8)), ("size", C.c_uint32)]
+
+
+class VcsConfig(C.Structure):
+    _fields_ = [("y0", C.c_int32), ("max_lines", C.c_int32), ("f8_start_bank", C.c_int32), ("flags", C.c_uint32)]
+
+
+class VcsError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libvcsb200.so; raises (never falls back) when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_SO):
+        raise VcsError(f"{_SO} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                       "(or paper_2606_22447_b200/build.py).  There is no CPU fallback.")
+    L = C.CDLL(_SO)
+    P = C.c_void_p
+    L.vcs_create.argtypes = [C.POINTER(P), C.c_int32, C.POINTER(VcsRom), C.c_int32, P, P, C.POINTER(VcsConfig)]
+    L.vcs_reset.argtypes = [P, P, P]
+    L.vcs_step.argtypes = [P, P, C.c_int32, P]
+    L.vcs_step_host.argtypes = [P, P, C.c_int32, P]
+    for f in ("vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host"):
+        getattr(L, f).argtypes = [P, P, P]
+    L.vcs_screen_ptr.argtypes = [P, C.POINTER(P)]
+    L.vcs_launch_count.argtypes = [P]; L.vcs_launch_count.restype = C.c_int64
+    L.vcs_optable.argtypes = [P]
+    L.vcs_destroy.argtypes = [P]
+    L.vcs_last_error.argtypes = [P]; L.vcs_last_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def optable() -> np.ndarray:
+    out = np.zeros(256, dtype=np.uint16)
+    assert load_library().vcs_optable(out.ctypes.data) == 0
+    return out
+
+
+def _stream_ptr(stream) -> int | None:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+class VCS:
+    """A batch of consoles on the current CUDA device (vcs_create ... vcs_destroy)."""
+
+    def __init__(self, roms, seeds, env_rom=None, y0=34, max_lines=320, f8_start_bank=1):
+        import torch
+        if not torch.cuda.is_available():
+            raise VcsError("no CUDA device: libvcsb200 has no CPU fallback")
+        self.torch = torch
+        L = self.L = load_library()
+        seeds = np.ascontiguousarray(seeds, dtype=np.uint64)
+        self.batch = int(seeds.shape[0])
+        bufs = [(C.c_uint8 * len(r)).from_buffer_copy(bytes(r)) for r in roms]
+        arr = (VcsRom * len(roms))()
+        for i, b in enumerate(bufs):
+            arr[i].data = C.cast(b, C.POINTER(C.c_uint8)); arr[i].size = len(b)
+        er = None if env_rom is None else np.ascontiguousarray(env_rom, dtype=np.int32)
+        cfg = VcsConfig(y0, max_lines, f8_start_bank, 0)
+        self.h = C.c_void_p()
+        rc = L.vcs_create(C.byref(self.h), self.batch, arr, len(roms), None if er is None else er.ctypes.data,
+                          seeds.ctypes.data, C.byref(cfg))
+        if rc != 0:
+            msg = L.vcs_last_error(self.h).decode() if self.h else ""
+            if self.h:
+                L.vcs_destroy(self.h); self.h = C.c_void_p()
+            raise VcsError(f"vcs_create: {_ERR.get(rc, rc)} {msg}")
+        self.device = torch.device("cuda", torch.cuda.current_device())
+
+    def _chk(self, rc, what):
+        if rc != 0:
+            raise VcsError(f"{what}: {_ERR.get(rc, rc)} {self.L.vcs_last_error(self.h).decode()}")
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.vcs_destroy(self.h); self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- device-pointer API (torch tensors carry the memory)
+    def reset(self, mask=None, stream=None):
+        ptr = None
+        if mask is not None:
+            assert mask.is_cuda and mask.dtype == self.torch.uint8 and mask.numel() == self.batch and mask.is_contiguous()
+            ptr = mask.data_ptr()
+        self._chk(self.L.vcs_reset(self.h, ptr, _stream_ptr(stream)), "vcs_reset")
+
+    def step(self, actions, frameskip=4, stream=None):
+        assert actions.is_cuda and actions.dtype == self.torch.uint8 and actions.numel() == self.batch and actions.is_contiguous()
+        self._chk(self.L.vcs_step(self.h, actions.data_ptr(), int(frameskip), _stream_ptr(stream)), "vcs_step")
+
+    def get_ram(self, out=None, stream=None):
+        t = self.torch
+        out = t.empty((self.batch, 128), dtype=t.uint8, device=self.device) if out is None else out
+        self._chk(self.L.vcs_get_ram(self.h, out.data_ptr(), _stream_ptr(stream)), "vcs_get_ram"); return out
+
+    def get_regs(self, out=None, stream=None):
+        t = self.torch
+        out = t.empty((self.batch, 32), dtype=t.uint8, device=self.device) if out is None else out
+        self._chk(self.L.vcs_get_regs(self.h, out.data_ptr(), _stream_ptr(stream)), "vcs_get_regs"); return out
+
+    def get_screen(self, out=None, stream=None):
+        t = self.torch
+        out = t.empty((self.batch, 210, 160), dtype=t.uint8, device=self.device) if out is None else out
+        self._chk(self.L.vcs_get_screen(self.h, out.data_ptr(), _stream_ptr(stream)), "vcs_get_screen"); return out
+
+    # ---- host-pointer API (numpy in / out; the copies happen inside the C call)
+    def step_host(self, actions: np.ndarray, frameskip=4, stream=None):
+        a = np.ascontiguousarray(actions, dtype=np.uint8); assert a.shape == (self.batch,)
+        self._chk(self.L.vcs_step_host(self.h, a.ctypes.data, int(frameskip), _stream_ptr(stream)), "vcs_step_host")
+
+    def ram_host(self, stream=None) -> np.ndarray:
+        out = np.empty((self.batch, 128), dtype=np.uint8)
+        self._chk(self.L.vcs_get_ram_host(self.h, out.ctypes.data, _stream_ptr(stream)), "vcs_get_ram_host"); return out
+
+    def regs_host(self, stream=None) -> np.ndarray:
+        out = np.empty(self.batch, dtype=REGS_DTYPE)
+        self._chk(self.L.vcs_get_regs_host(self.h, out.ctypes.data, _stream_ptr(stream)), "vcs_get_regs_host"); return out
+
+    def screen_host(self, out=None, stream=None) -> np.ndarray:
+        out = np.empty((self.batch, 210, 160), dtype=np.uint8) if out is None else out
+        self._chk(self.L.vcs_get_screen_host(self.h, out.ctypes.data, _stream_ptr(stream)), "vcs_get_screen_host"); return out
+
+    def launch_count(self) -> int:
+        return int(self.L.vcs_launch_count(self.h))

@@ -1,0 +1,265 @@
+// vcs_api.cu — the extern "C" boundary of libvcsb200 (include/vcs.h), plus the small
+// reset / read-out kernels.  Argument marshalling and launches only: every step of the emulation runs in
+// vcs_step.cu's kernel.  No CPU fallback exists: without a CUDA device vcs_create fails with VCS_ECUDA.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/vcs.h"
+#include "vcs_step.cuh"
+
+using namespace vcs;
+
+struct vcs_s : Handle {};
+
+namespace {
+
+int fail(Handle *h, int code, const char *what, cudaError_t ce = cudaSuccess) {
+  if (h) {
+    if (ce != cudaSuccess) snprintf(h->err, sizeof h->err, "%s: %s", what, cudaGetErrorString(ce));
+    else snprintf(h->err, sizeof h->err, "%s", what);
+  }
+  return code;
+}
+#define CU(h, call) do { cudaError_t ce_ = (call); if (ce_ != cudaSuccess) return fail(h, VCS_ECUDA, #call, ce_); } while (0)
+
+__device__ unsigned long long splitmix64(unsigned long long &s) {
+  s += 0x9E3779B97F4A7C15ull;
+  unsigned long long z = s;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+// C.2 power-on / reset state
+__global__ void reset_kernel(StepParams p, const unsigned long long *seeds, const uint8_t *mask, int f8_start_bank) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= p.batch || (mask && !mask[e])) return;
+  const int B = p.batch;
+  const RomMeta rm = p.rom_meta[p.env_rom[e]];
+  const uint8_t *rom = p.rom_blob + rm.offset;
+  const uint32_t bank = (rm.size == 8192) ? (uint32_t)(f8_start_bank & 1) : 0u;
+  const uint32_t mask_a = (rm.size == 2048) ? 0x7FFu : 0xFFFu;
+  const uint32_t pc = rom[(bank << 12) + (0xFFCu & mask_a)] | ((uint32_t)rom[(bank << 12) + (0xFFDu & mask_a)] << 8);
+  for (int w = 0; w < ST_WORDS; ++w) p.st[w * B + e] = 0;
+  p.st[W_AXYS * B + e] = 0xFDu << 24;
+  p.st[W_PC * B + e] = pc | (0x24u << 16);
+  p.st[W_BEAM * B + e] = bank << 24;
+  p.st[W_TIMER * B + e] = 0xFFu | (10u << 8);
+  p.st[W_FLAGS * B + e] = TF_INPT4_LATCH | TF_INPT5_LATCH;
+  p.cyc[e] = 0;
+  unsigned long long s = seeds[e];
+  for (int k = 0; k < 16; ++k) {
+    unsigned long long z = splitmix64(s);
+    p.ram[(2 * k) * B + e] = (uint32_t)z;
+    p.ram[(2 * k + 1) * B + e] = (uint32_t)(z >> 32);
+  }
+}
+__global__ void clear_screen_kernel(uint8_t *screen, const uint8_t *mask) {
+  const int e = blockIdx.x;
+  if (mask && !mask[e]) return;
+  uint4 *dst = reinterpret_cast<uint4 *>(screen + (size_t)e * (SCR_W * SCR_H));
+  for (int i = threadIdx.x; i < SCR_W * SCR_H / 16; i += blockDim.x) dst[i] = make_uint4(0, 0, 0, 0);
+}
+__global__ void get_ram_kernel(const uint32_t *ram, uint32_t *out, int B) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= 32ll * B) return;
+  const int e = (int)(idx >> 5), i = (int)(idx & 31);
+  out[idx] = ram[(size_t)i * B + e];
+}
+__global__ void get_regs_kernel(const uint32_t *st, const unsigned long long *cyc, uint4 *out, int B) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= B) return;
+  const uint32_t axys = st[W_AXYS * B + e], pcw = st[W_PC * B + e], beam = st[W_BEAM * B + e], tm = st[W_TIMER * B + e];
+  const unsigned long long c = cyc[e];
+  uint4 lo, hi;
+  lo.x = (uint32_t)c; lo.y = (uint32_t)(c >> 32); lo.z = st[W_FRAME * B + e];
+  lo.w = (pcw & 0xFFFFu) | ((axys & 0xFFu) << 16) | (((axys >> 8) & 0xFFu) << 24);                 // pc, a, x
+  hi.x = ((axys >> 16) & 0xFFu) | ((axys >> 24) << 8) | (((pcw >> 16) & 0xFFu) << 16) | ((beam >> 24) << 24);   // y, sp, p, bank
+  hi.y = ((beam >> 8) & 0xFFFFu) | (((beam & 0xFFu) % LINE_CYC) << 16) | ((pcw >> 24) << 24);                    // line, cyc_in_line, status
+  hi.z = (tm & 0xFFu) | ((((tm >> 12) & 1u) << 7) << 8);                                            // intim, timint
+  hi.w = 0;
+  out[2 * e] = lo; out[2 * e + 1] = hi;
+}
+
+StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
+  StepParams p;
+  p.st = h->d_st; p.ram = h->d_ram; p.cyc = h->d_cyc; p.screen = h->d_screen;
+  p.rom_blob = h->d_rom_blob; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
+  p.actions = actions; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
+  return p;
+}
+
+int ensure_stage(Handle *h, size_t bytes) {
+  if (h->h_pinned_bytes >= bytes) return VCS_OK;
+  if (h->h_pinned) cudaFreeHost(h->h_pinned);
+  if (h->d_actions_stage) cudaFree(h->d_actions_stage);
+  h->h_pinned = nullptr; h->d_actions_stage = nullptr; h->h_pinned_bytes = 0;
+  CU(h, cudaMallocHost((void **)&h->h_pinned, bytes));
+  CU(h, cudaMalloc((void **)&h->d_actions_stage, bytes));
+  h->h_pinned_bytes = bytes;
+  return VCS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, const int32_t *env_rom,
+               const uint64_t *seeds, const vcs_config *cfg) {
+  if (!out) return VCS_EINVAL;
+  *out = nullptr;
+  if (batch < 1 || !roms || n_roms < 1 || !seeds) return VCS_EINVAL;
+  for (int r = 0; r < n_roms; ++r) {
+    if (!roms[r].data) return VCS_EINVAL;
+    if (roms[r].size != 2048 && roms[r].size != 4096 && roms[r].size != 8192) return VCS_EROM;
+  }
+  if (env_rom) for (int i = 0; i < batch; ++i) if (env_rom[i] < 0 || env_rom[i] >= n_roms) return VCS_EINVAL;
+  vcs_config c = {34, 320, 1, 0};
+  if (cfg) c = *cfg;
+  if (c.y0 < 2 || c.max_lines < 1 || c.max_lines > 65535 || c.flags != 0) return VCS_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return VCS_ECUDA;     // no CPU fallback
+  vcs_s *h = new (std::nothrow) vcs_s();
+  if (!h) return VCS_ENOMEM;
+  memset(static_cast<Handle *>(h), 0, sizeof(Handle));
+  h->batch = batch; h->n_roms = n_roms; h->y0 = c.y0; h->max_lines = c.max_lines; h->f8_start_bank = c.f8_start_bank;
+  *out = h;                                           // so that the caller can read vcs_last_error and destroy
+
+  std::vector<RomMeta> meta(n_roms);
+  size_t blob = 0;
+  for (int r = 0; r < n_roms; ++r) { meta[r].offset = (uint32_t)blob; meta[r].size = roms[r].size; blob += roms[r].size; }
+  std::vector<uint8_t> hb(blob);
+  for (int r = 0; r < n_roms; ++r) memcpy(hb.data() + meta[r].offset, roms[r].data, roms[r].size);
+  std::vector<int32_t> er(batch, 0);
+  if (env_rom) memcpy(er.data(), env_rom, sizeof(int32_t) * batch);
+
+  const size_t B = (size_t)batch;
+  CU(h, cudaMalloc((void **)&h->d_st, sizeof(uint32_t) * ST_WORDS * B));
+  CU(h, cudaMalloc((void **)&h->d_ram, sizeof(uint32_t) * 32 * B));
+  CU(h, cudaMalloc((void **)&h->d_cyc, sizeof(unsigned long long) * B));
+  CU(h, cudaMalloc((void **)&h->d_screen, (size_t)SCR_W * SCR_H * B));
+  CU(h, cudaMalloc((void **)&h->d_rom_blob, blob));
+  CU(h, cudaMalloc((void **)&h->d_rom_meta, sizeof(RomMeta) * n_roms));
+  CU(h, cudaMalloc((void **)&h->d_env_rom, sizeof(int32_t) * B));
+  CU(h, cudaMalloc((void **)&h->d_seeds, sizeof(unsigned long long) * B));
+  CU(h, cudaMemcpy(h->d_rom_blob, hb.data(), blob, cudaMemcpyHostToDevice));
+  CU(h, cudaMemcpy(h->d_rom_meta, meta.data(), sizeof(RomMeta) * n_roms, cudaMemcpyHostToDevice));
+  CU(h, cudaMemcpy(h->d_env_rom, er.data(), sizeof(int32_t) * B, cudaMemcpyHostToDevice));
+  CU(h, cudaMemcpy(h->d_seeds, seeds, sizeof(unsigned long long) * B, cudaMemcpyHostToDevice));
+  upload_optable();
+  CU(h, cudaGetLastError());
+  int rc = vcs_reset(h, nullptr, nullptr);
+  if (rc != VCS_OK) return rc;
+  CU(h, cudaDeviceSynchronize());
+  return VCS_OK;
+}
+
+int vcs_reset(vcs_t h, const uint8_t *mask_dev, void *cuda_stream) {
+  if (!h) return VCS_EINVAL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  StepParams p = params_of(h, nullptr, 1);
+  reset_kernel<<<(h->batch + 127) / 128, 128, 0, s>>>(p, h->d_seeds, mask_dev, h->f8_start_bank);
+  clear_screen_kernel<<<h->batch, 256, 0, s>>>(h->d_screen, mask_dev);
+  h->launches += 2;
+  CU(h, cudaGetLastError());
+  return VCS_OK;
+}
+
+int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_stream) {
+  if (!h) return VCS_EINVAL;
+  if (!actions_dev) return fail(h, VCS_EINVAL, "vcs_step: actions_dev is NULL");
+  if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31))
+    return fail(h, VCS_EINVAL, "vcs_step: frameskip out of range");
+  StepParams p = params_of(h, actions_dev, frameskip);
+  cudaError_t ce = launch_step(p, (cudaStream_t)cuda_stream);
+  h->launches += 1;
+  if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step launch", ce);
+  return VCS_OK;
+}
+
+int vcs_get_ram(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
+  if (!h || !out_dev) return VCS_EINVAL;
+  const long long n = 32ll * h->batch;
+  get_ram_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(h->d_ram, reinterpret_cast<uint32_t *>(out_dev), h->batch);
+  h->launches += 1;
+  CU(h, cudaGetLastError());
+  return VCS_OK;
+}
+int vcs_get_regs(vcs_t h, vcs_regs *out_dev, void *cuda_stream) {
+  if (!h || !out_dev) return VCS_EINVAL;
+  get_regs_kernel<<<(h->batch + 127) / 128, 128, 0, (cudaStream_t)cuda_stream>>>(h->d_st, h->d_cyc, reinterpret_cast<uint4 *>(out_dev), h->batch);
+  h->launches += 1;
+  CU(h, cudaGetLastError());
+  return VCS_OK;
+}
+int vcs_get_screen(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
+  if (!h || !out_dev) return VCS_EINVAL;
+  CU(h, cudaMemcpyAsync(out_dev, h->d_screen, (size_t)SCR_W * SCR_H * h->batch, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+  return VCS_OK;
+}
+int vcs_screen_ptr(vcs_t h, const uint8_t **out_dev_ptr) {
+  if (!h || !out_dev_ptr) return VCS_EINVAL;
+  *out_dev_ptr = h->d_screen; return VCS_OK;
+}
+
+int vcs_step_host(vcs_t h, const uint8_t *actions_host, int32_t frameskip, void *cuda_stream) {
+  if (!h || !actions_host) return VCS_EINVAL;
+  int rc = ensure_stage(h, (size_t)h->batch * 128); if (rc) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  memcpy(h->h_pinned, actions_host, h->batch);
+  CU(h, cudaMemcpyAsync(h->d_actions_stage, h->h_pinned, h->batch, cudaMemcpyHostToDevice, s));
+  rc = vcs_step(h, h->d_actions_stage, frameskip, cuda_stream); if (rc) return rc;
+  CU(h, cudaStreamSynchronize(s));
+  return VCS_OK;
+}
+int vcs_get_ram_host(vcs_t h, uint8_t *out_host, void *cuda_stream) {
+  if (!h || !out_host) return VCS_EINVAL;
+  int rc = ensure_stage(h, (size_t)h->batch * 128); if (rc) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  rc = vcs_get_ram(h, h->d_actions_stage, cuda_stream); if (rc) return rc;
+  CU(h, cudaMemcpyAsync(h->h_pinned, h->d_actions_stage, (size_t)h->batch * 128, cudaMemcpyDeviceToHost, s));
+  CU(h, cudaStreamSynchronize(s));
+  memcpy(out_host, h->h_pinned, (size_t)h->batch * 128);
+  return VCS_OK;
+}
+int vcs_get_regs_host(vcs_t h, vcs_regs *out_host, void *cuda_stream) {
+  if (!h || !out_host) return VCS_EINVAL;
+  int rc = ensure_stage(h, (size_t)h->batch * 128); if (rc) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  rc = vcs_get_regs(h, reinterpret_cast<vcs_regs *>(h->d_actions_stage), cuda_stream); if (rc) return rc;
+  CU(h, cudaMemcpyAsync(h->h_pinned, h->d_actions_stage, (size_t)h->batch * 32, cudaMemcpyDeviceToHost, s));
+  CU(h, cudaStreamSynchronize(s));
+  memcpy(out_host, h->h_pinned, (size_t)h->batch * 32);
+  return VCS_OK;
+}
+int vcs_get_screen_host(vcs_t h, uint8_t *out_host, void *cuda_stream) {
+  if (!h || !out_host) return VCS_EINVAL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  CU(h, cudaMemcpyAsync(out_host, h->d_screen, (size_t)SCR_W * SCR_H * h->batch, cudaMemcpyDeviceToHost, s));
+  CU(h, cudaStreamSynchronize(s));
+  return VCS_OK;
+}
+
+int64_t vcs_launch_count(vcs_t h) { return h ? h->launches : -1; }
+
+int vcs_optable(uint16_t *out256) {
+  if (!out256) return VCS_EINVAL;
+  memcpy(out256, host_optable(), 512); return VCS_OK;
+}
+
+int vcs_destroy(vcs_t h) {
+  if (!h) return VCS_EINVAL;
+  cudaDeviceSynchronize();
+  cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob);
+  cudaFree(h->d_rom_meta); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage);
+  if (h->h_pinned) cudaFreeHost(h->h_pinned);
+  delete h;
+  return VCS_OK;
+}
+
+const char *vcs_last_error(vcs_t h) { return h ? h->err : ""; }
+
+}  // extern "C"

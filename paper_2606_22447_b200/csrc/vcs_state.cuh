@@ -1,0 +1,66 @@
+// vcs_state.cuh — device-side state layout of libvcsb200 (the CUDA path; shares nothing with oracle/).
+//
+// Per environment, in HBM, structure-of-arrays so that a warp's loads/stores coalesce:
+//   st   [ST_WORDS][batch] u32   packed CPU / beam / RIOT / TIA latches (word index below)
+//   ram  [32][batch]       u32   the 128 RIOT RAM bytes, little-endian words
+//   cyc  [batch]           u64   CPU cycles since reset
+//   screen [batch][210][160] u8  front frame, palette indices
+// Machine model: SURVEY.md §8(c) C.1 (state), restated in DESIGN.md §2.
+#pragma once
+#include <stdint.h>
+
+namespace vcs {
+
+constexpr int SCR_W = 160, SCR_H = 210, LINE_CYC = 76, HBLANK = 68, LINE_CLK = 228;
+
+enum StWord {
+  W_AXYS = 0,   // A | X<<8 | Y<<16 | SP<<24
+  W_PC,         // PC | P<<16 | status<<24
+  W_BEAM,       // n (cycle in line) | line<<8 (16 bit) | bank<<24
+  W_FRAME,      // completed frames since reset
+  W_FCYC,       // cycles since the current frame began
+  W_TIMER,      // timer | shift<<8 | tflag<<12 | sub<<16
+  W_PORTS,      // ora | ddra<<8 | orb<<16 | ddrb<<24
+  W_COLU,       // COLUP0 | COLUP1<<8 | COLUPF<<16 | COLUBK<<24
+  W_PF,         // PF0 | PF1<<8 | PF2<<16 | CTRLPF<<24
+  W_GRP,        // GRP0_new | GRP0_old<<8 | GRP1_new<<16 | GRP1_old<<24
+  W_NUSIZ,      // NUSIZ0 | NUSIZ1<<8 | HMP0<<16 | HMP1<<20 | HMM0<<24 | HMM1<<28
+  W_POS,        // posP0 | posP1<<8 | posM0<<16 | posM1<<24
+  W_POS2,       // posBL | HMBL<<8 | rx<<16 (colour clocks of the current line already rendered, 0..228)
+  W_FLAGS,      // TIA / input flag bits, see TF_*
+  W_CX,         // 15 collision latches
+  ST_WORDS
+};
+
+// W_FLAGS bits
+enum : uint32_t {
+  TF_VSYNC = 1u << 0, TF_VBLANK = 1u << 1, TF_LATCHEN = 1u << 2, TF_WSYNC = 1u << 3,
+  TF_REFP0 = 1u << 4, TF_REFP1 = 1u << 5, TF_ENAM0 = 1u << 6, TF_ENAM1 = 1u << 7,
+  TF_ENABL_NEW = 1u << 8, TF_ENABL_OLD = 1u << 9, TF_VDELP0 = 1u << 10, TF_VDELP1 = 1u << 11,
+  TF_VDELBL = 1u << 12, TF_RESMP0 = 1u << 13, TF_RESMP1 = 1u << 14,
+  TF_FRESH_P0 = 1u << 15, TF_FRESH_P1 = 1u << 16, TF_FRESH_M0 = 1u << 17, TF_FRESH_M1 = 1u << 18,
+  TF_HMBLANK = 1u << 19, TF_INPT4_LATCH = 1u << 20, TF_INPT5_LATCH = 1u << 21,
+  TF_FRESH_ALL = TF_FRESH_P0 | TF_FRESH_P1 | TF_FRESH_M0 | TF_FRESH_M1,
+};
+
+// collision latch bit numbers inside W_CX (read map: SURVEY C.8)
+enum { CX_M0P1 = 0, CX_M0P0, CX_M1P0, CX_M1P1, CX_P0PF, CX_P0BL, CX_P1PF, CX_P1BL,
+       CX_M0PF, CX_M0BL, CX_M1PF, CX_M1BL, CX_BLPF, CX_P0P1, CX_M0M1 };
+
+enum : uint32_t { STATUS_ILLEGAL = 1, STATUS_CAP = 2, STATUS_UNMODELLED = 4 };
+
+struct RomMeta { uint32_t offset; uint32_t size; };   // into the ROM blob
+
+struct Handle {                 // host-side bookkeeping behind vcs_t
+  int32_t batch, n_roms;
+  int32_t y0, max_lines, f8_start_bank;
+  uint32_t *d_st; uint32_t *d_ram; unsigned long long *d_cyc; uint8_t *d_screen;
+  uint8_t *d_rom_blob; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
+  uint8_t *d_actions_stage;     // for vcs_step_host
+  uint8_t *h_pinned; size_t h_pinned_bytes;
+  int block_uniform_rom;        // every 128-env block maps to a single ROM
+  long long launches;
+  char err[256];
+};
+
+}  // namespace vcs

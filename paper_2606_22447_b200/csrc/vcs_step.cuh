@@ -1,0 +1,21 @@
+// vcs_step.cuh — launch interface between the host API (vcs_api.cu) and the kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include "vcs_state.cuh"
+
+namespace vcs {
+
+constexpr int STEP_BLOCK = 128;          // threads (= environments) per block of the interpreter kernel
+
+struct StepParams {
+  uint32_t *st; uint32_t *ram; unsigned long long *cyc; uint8_t *screen;
+  const uint8_t *rom_blob; const RomMeta *rom_meta; const int32_t *env_rom;
+  const uint8_t *actions;
+  int32_t batch, frameskip, y0, max_lines;
+};
+
+void upload_optable();
+const uint16_t *host_optable();
+cudaError_t launch_step(const StepParams &p, cudaStream_t stream);
+
+}  // namespace vcs

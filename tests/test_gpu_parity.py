@@ -1,0 +1,216 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element, bit-exact.
+
+RAM (128 B), every vcs_regs field (registers, cycle counter, beam, bank, status, timer) and the 160x210
+palette-index screen are compared after every step (PAPER.md L167 exactness metrics; L592 batched ==
+unbatched).  Inputs are the seeded synthetic configs of SURVEY §8(d) G.2 at sizes the oracle finishes in
+seconds, plus BASELINE's full batch with a sampled subset of envs."""
+import os
+
+import numpy as np
+import pytest
+
+from vcs_inputs import make_workload, hand_rom, SplitMix64, TIA_W, RIOT, env_seeds
+
+pytestmark = pytest.mark.gpu
+NCPU = os.cpu_count() or 1
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def mk(torch, w, **kw):
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    return VCS(w.roms, w.seeds, w.env_rom, **kw), OracleVCS(w.roms, w.seeds, w.env_rom, **kw)
+
+
+def compare(g, o, tag, envs=None, osel=None):
+    """g: CUDA batch; o: oracle batch.  envs: indices into g to compare against all of o (sampling)."""
+    gram, gregs, gscr = g.ram_host(), g.regs_host(), g.screen_host()
+    if envs is not None:
+        gram, gregs, gscr = gram[envs], gregs[envs], gscr[envs]
+    oram, oregs, oscr = o.ram(), o.regs(), o.screen()
+    for f in gregs.dtype.names:
+        bad = np.nonzero((gregs[f] != oregs[f]).reshape(len(oregs), -1).any(axis=1))[0]
+        assert bad.size == 0, f"{tag}: regs.{f} differs for envs {bad[:8]}: gpu {gregs[f][bad[:4]]} oracle {oregs[f][bad[:4]]}"
+    bad = np.nonzero((gram != oram).any(axis=1))[0]
+    assert bad.size == 0, f"{tag}: RAM differs for envs {bad[:8]}"
+    bad = np.nonzero((gscr != oscr).any(axis=(1, 2)))[0]
+    if bad.size:
+        e = bad[0]; ys, xs = np.nonzero(gscr[e] != oscr[e])
+        raise AssertionError(f"{tag}: screen differs for envs {bad[:8]}; env {e}: {ys.size} px, first (row {ys[0]}, x {xs[0]}) "
+                             f"gpu {gscr[e][ys[0], xs[0]]} oracle {oscr[e][ys[0], xs[0]]}")
+
+
+def run_parity(torch, w, steps, frameskip=None, tag="", **kw):
+    g, o = mk(torch, w, **kw)
+    fs = w.frameskip if frameskip is None else frameskip
+    acts = w.actions(0, steps)
+    compare(g, o, f"{tag} reset")
+    for t in range(steps):
+        g.step(torch.from_numpy(acts[t]).cuda(), fs)
+        o.step(acts[t], fs, threads=NCPU)
+        compare(g, o, f"{tag} step {t}")
+    g.close(); o.close()
+
+
+def test_config1_full(torch):
+    """config 1 exactly as BASELINE.json states it: 1 env, 2 KB ROM, 10 frames, NOOP, compare per frame."""
+    run_parity(torch, make_workload(1), 10, tag="config1")
+
+
+def test_config2_every_env_every_step(torch):
+    run_parity(torch, make_workload(2, batch=160), 12, tag="config2")      # 160 = one full block + a ragged tail
+
+
+def test_config3_features(torch):
+    run_parity(torch, make_workload(3, batch=96), 10, tag="config3")
+
+
+def test_config4_heterogeneous_roms_and_f8(torch):
+    run_parity(torch, make_workload(4, batch=256, n_roms=32), 8, tag="config4")
+
+
+@pytest.mark.parametrize("fs", [1, 2, 3, 5])
+def test_frameskips(torch, fs):
+    run_parity(torch, make_workload(3, batch=40), 6, frameskip=fs, tag=f"frameskip{fs}")
+
+
+def test_other_y0_and_cap(torch):
+    run_parity(torch, make_workload(2, batch=33), 4, tag="y0=2", y0=2)
+    run_parity(torch, make_workload(2, batch=33), 4, tag="y0=60,cap=200", y0=60, max_lines=200)   # cap ends frames mid-picture
+    run_parity(torch, make_workload(4, batch=32, n_roms=4), 4, tag="bank0", f8_start_bank=0)
+
+
+def test_batched_equals_unbatched(torch):
+    """env e inside a batch == env e alone."""
+    from paper_2606_22447_b200 import VCS
+    w = make_workload(3, batch=200)
+    acts = w.actions(0, 5)
+    g = VCS(w.roms, w.seeds, w.env_rom)
+    for t in range(5):
+        g.step(torch.from_numpy(acts[t]).cuda(), 4)
+    ram, regs, scr = g.ram_host(), g.regs_host(), g.screen_host()
+    for e in (0, 77, 199):
+        g1 = VCS(w.roms, w.seeds[e:e + 1], w.env_rom[e:e + 1])
+        for t in range(5):
+            g1.step(torch.from_numpy(acts[t][e:e + 1].copy()).cuda(), 4)
+        assert (g1.ram_host()[0] == ram[e]).all() and g1.regs_host()[0] == regs[e] and (g1.screen_host()[0] == scr[e]).all()
+
+
+def test_reset_mask_and_device_getters(torch):
+    w = make_workload(2, batch=64)
+    g, o = mk(torch, w)
+    acts = w.actions(0, 4)
+    for t in range(2):
+        g.step(torch.from_numpy(acts[t]).cuda(), 4); o.step(acts[t], 4, threads=NCPU)
+    mask = (np.arange(64) % 3 == 0).astype(np.uint8)
+    g.reset(torch.from_numpy(mask).cuda()); o.reset(mask)
+    compare(g, o, "after masked reset")
+    for t in range(2, 4):
+        g.step(torch.from_numpy(acts[t]).cuda(), 4); o.step(acts[t], 4, threads=NCPU)
+        compare(g, o, f"masked reset step {t}")
+    # device-pointer getters agree with the host-pointer ones
+    assert (g.get_ram().cpu().numpy() == g.ram_host()).all()
+    assert (g.get_screen().cpu().numpy() == g.screen_host()).all()
+    assert (g.get_regs().cpu().numpy().view(g.regs_host().dtype).reshape(-1) == g.regs_host()).all()
+    # host-pointer step == device-pointer step
+    g2, _ = mk(torch, w)
+    for t in range(2):
+        g2.step_host(acts[t], 4)
+    g3, _ = mk(torch, w)
+    for t in range(2):
+        g3.step(torch.from_numpy(acts[t]).cuda(), 4)
+    assert (g2.ram_host() == g3.ram_host()).all() and (g2.screen_host() == g3.screen_host()).all()
+
+
+def _chaos_rom(seed: int) -> bytes:
+    """Unstructured TIA/RIOT torture: stores and RMWs to every TIA register at arbitrary beam positions,
+    lines crossed mid-instruction, WSYNC/HMOVE/RESxx/VSYNC/VBLANK at random, collision and timer reads.
+    Frames end by VSYNC toggles or by the cap.  Exercises the lazy TIA against the per-clock oracle."""
+    r = SplitMix64(seed)
+    regs = [n for n in TIA_W if not n.startswith("AUD")]
+
+    def build(a):
+        a.org(0xF000); a.op("LDX", "imm", 0xFF); a.op("TXS")
+        a.label("top")
+        for _ in range(330):
+            k = r.rnd(20)
+            if k < 9:
+                reg = r.choice(regs)
+                if reg in ("VSYNC", "WSYNC") and r.chance(2, 3): reg = r.choice(["GRP0", "GRP1", "PF1", "COLUBK", "ENABL", "ENAM0"])
+                a.op(r.choice(["LDA", "LDX", "LDY"]), "imm", r.rnd(256)) if r.chance(2, 3) else None
+                a.op(r.choice(["STA", "STX", "STY"]), "zp", TIA_W[reg])
+            elif k < 11:
+                a.op(r.choice(["INC", "DEC", "ASL", "LSR", "ROL", "ROR"]), "zp", TIA_W[r.choice(regs)])    # RMW on the TIA: two writes
+            elif k < 13:
+                a.op(r.choice(["LDA", "ADC", "EOR", "ORA"]), "zp", r.rnd(16)); a.op("STA", "zp", 0x80 + r.rnd(64))   # CXxx / INPTx reads
+            elif k < 14:
+                a.op("LDA", "imm", r.rnd(256)); a.op("STA", "abs", RIOT[r.choice(["TIM1T", "TIM8T", "TIM64T", "T1024T"])])
+            elif k < 16:
+                a.op("LDA", "abs", RIOT[r.choice(["INTIM", "TIMINT", "SWCHA", "SWCHB"])]); a.op("STA", "zp", 0x80 + r.rnd(64))
+            elif k < 17:
+                a.op("LDA", "imm", r.rnd(256)); a.op("STA", "abs", RIOT[r.choice(["SWACNT", "SWCHA", "SWBCNT", "SWCHB"])])
+            elif k < 18:
+                a.op("LDA", "abx", RIOT["INTIM"] - 0x20 + r.rnd(0x40)); a.op("INX")       # indexed: dummy/real reads around the RIOT
+            else:
+                if r.chance(1, 3): a.op("PHA"); a.op("PLA")
+                else: a.op(r.choice(["NOP", "INX", "DEY", "CLC", "SEC"]))
+        a.op("JMP", "abs", "top")
+    return hand_rom(build)
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_chaos_tia_riot(torch, seed):
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    rom = _chaos_rom(1000 + seed)
+    seeds = env_seeds(50 + seed, 48)
+    kw = dict(max_lines=120 + 37 * seed, y0=2 + 5 * seed)
+    g, o = VCS([rom], seeds, **kw), OracleVCS([rom], seeds, **kw)
+    rng = SplitMix64(seed)
+    for t in range(10):
+        a = np.array([rng.rnd(20) for _ in range(48)], np.uint8)          # includes out-of-range actions (-> NOOP)
+        fs = 1 + t % 3
+        g.step(torch.from_numpy(a).cuda(), fs); o.step(a, fs, threads=NCPU)
+        compare(g, o, f"chaos{seed} step {t}")
+
+
+def test_illegal_opcode_and_cap(torch):
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+
+    def build(a):
+        a.org(0xF000); a.op("LDA", "imm", 0x4C); a.op("STA", "zp", TIA_W["COLUBK"]); a.op("INC", "zp", 0x80)
+        a.op("LDA", "zp", 0x80); a.op("CMP", "imm", 7); a.op("BNE", "rel", -12); a.byte(0x02)     # KIL after a few loops
+    rom = hand_rom(build)
+    seeds = env_seeds(9, 5)
+    g, o = VCS([rom], seeds, max_lines=64), OracleVCS([rom], seeds, max_lines=64)
+    for t in range(4):
+        a = np.zeros(5, np.uint8)
+        g.step(torch.from_numpy(a).cuda(), 2); o.step(a, 2)
+        compare(g, o, f"illegal step {t}")
+    assert (g.regs_host()["status"] & 1).all()
+
+
+def test_full_batch_sampled(torch):
+    """BASELINE config 4 at its full size and in bench.py's launch configuration (65,536 envs, 256 ROMs,
+    frameskip 4): one env per ROM is checked against the oracle after every step."""
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    w = make_workload(4)
+    g = VCS(w.roms, w.seeds, w.env_rom)
+    idx = np.arange(256) * 256 + (np.arange(256) * 37) % 256           # one env per ROM, varying lane/warp
+    o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx])
+    acts = w.actions(0, 3)
+    for t in range(3):
+        g.step(torch.from_numpy(acts[t]).cuda(), 4)
+        o.step(acts[t][idx], 4, threads=NCPU)
+        compare(g, o, f"config4 full step {t}", envs=idx)
+    r = g.regs_host()
+    assert (r["status"] == 0).all() and (r["frame"] == 12).all()
+    assert (abs(r["cycles"].astype(np.int64) - 11 * 19912) < 19912).all()  # every frame is a 262-line NTSC frame (first one starts at reset)
