@@ -89,6 +89,7 @@ StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   p.st = h->d_st; p.ram = h->d_ram; p.cyc = h->d_cyc; p.screen = h->d_screen;
   p.rom_blob = h->d_rom_blob; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
   p.actions = actions; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
+  p.block = h->block; p.rom_smem = h->rom_smem; p.max_rom = h->max_rom;
   return p;
 }
 
@@ -135,6 +136,16 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   for (int r = 0; r < n_roms; ++r) memcpy(hb.data() + meta[r].offset, roms[r].data, roms[r].size);
   std::vector<int32_t> er(batch, 0);
   if (env_rom) memcpy(er.data(), env_rom, sizeof(int32_t) * batch);
+  // launch shape: envs per block (VCS_BLOCK=64|128|256 overrides), and whether every block maps to one ROM so
+  // that the ROM can be staged in shared memory (otherwise the kernel reads it through the read-only path)
+  int want = 128;
+  if (const char *ev = getenv("VCS_BLOCK")) { const int v = atoi(ev); if (v == 64 || v == 128 || v == 256) want = v; }
+  h->max_rom = 0;
+  for (int r = 0; r < n_roms; ++r) if (roms[r].size > h->max_rom) h->max_rom = roms[r].size;
+  auto uniform = [&](int blk) { for (int i = 0; i < batch; ++i) if (er[i] != er[i - i % blk]) return false; return true; };
+  h->block = want; h->rom_smem = 0;
+  for (int blk = want; blk >= 64; blk >>= 1) if (uniform(blk)) { h->block = blk; h->rom_smem = 1; break; }
+  if (getenv("VCS_ROM_GLOBAL")) h->rom_smem = 0;
 
   const size_t B = (size_t)batch;
   CU(h, cudaMalloc((void **)&h->d_st, sizeof(uint32_t) * ST_WORDS * B));

@@ -1,10 +1,13 @@
-// vcs_state.cuh — device-side state layout of libvcsb200 (the CUDA path; shares nothing with oracle/).
+// vcs_state.cuh — state layout of libvcsb200 (the CUDA path; shares nothing with oracle/).
 //
-// Per environment, in HBM, structure-of-arrays so that a warp's loads/stores coalesce:
+// In HBM, per environment, structure-of-arrays so that a warp's loads/stores coalesce:
 //   st   [ST_WORDS][batch] u32   packed CPU / beam / RIOT / TIA latches (word index below)
 //   ram  [32][batch]       u32   the 128 RIOT RAM bytes, little-endian words
 //   cyc  [batch]           u64   CPU cycles since reset
 //   screen [batch][210][160] u8  front frame, palette indices
+// In shared memory, while vcs_step runs: one "file" of S_WORDS words per thread, word i of thread t at
+// smem[i * BLOCK + t] (word-interleaved, so a warp's accesses never bank-conflict whatever per-lane
+// addresses are used), followed by a per-block context, the 256-entry decode table and the block's ROM.
 // Machine model: SURVEY.md §8(c) C.1 (state), restated in DESIGN.md §2.
 #pragma once
 #include <stdint.h>
@@ -16,7 +19,7 @@ constexpr int SCR_W = 160, SCR_H = 210, LINE_CYC = 76, HBLANK = 68, LINE_CLK = 2
 enum StWord {
   W_AXYS = 0,   // A | X<<8 | Y<<16 | SP<<24
   W_PC,         // PC | P<<16 | status<<24
-  W_BEAM,       // n (cycle in line) | line<<8 (16 bit) | bank<<24
+  W_BEAM,       // n (cycle in line, 0..76) | line<<8 (16 bit) | bank<<24
   W_FRAME,      // completed frames since reset
   W_FCYC,       // cycles since the current frame began
   W_TIMER,      // timer | shift<<8 | tflag<<12 | sub<<16
@@ -27,7 +30,7 @@ enum StWord {
   W_NUSIZ,      // NUSIZ0 | NUSIZ1<<8 | HMP0<<16 | HMP1<<20 | HMM0<<24 | HMM1<<28
   W_POS,        // posP0 | posP1<<8 | posM0<<16 | posM1<<24
   W_POS2,       // posBL | HMBL<<8 | rx<<16 (colour clocks of the current line already rendered, 0..228)
-  W_FLAGS,      // TIA / input flag bits, see TF_*
+  W_FLAGS,      // TIA / input flag bits, see TF_* (only the bits below TF_DIRTY0 are architectural)
   W_CX,         // 15 collision latches
   ST_WORDS
 };
@@ -41,13 +44,35 @@ enum : uint32_t {
   TF_FRESH_P0 = 1u << 15, TF_FRESH_P1 = 1u << 16, TF_FRESH_M0 = 1u << 17, TF_FRESH_M1 = 1u << 18,
   TF_HMBLANK = 1u << 19, TF_INPT4_LATCH = 1u << 20, TF_INPT5_LATCH = 1u << 21,
   TF_FRESH_ALL = TF_FRESH_P0 | TF_FRESH_P1 | TF_FRESH_M0 | TF_FRESH_M1,
+  TF_ARCH_MASK = (1u << 22) - 1u,
+  // kernel-only, derived (never stored to HBM): cached object line masks that must be rebuilt, row visibility
+  TF_DIRTY0 = 1u << 22,            // << object index: PF, BL, P0, P1, M0, M1
+  TF_DIRTY_ALL = 63u << 22,
+  TF_ROWVIS = 1u << 28,            // the scanline in progress is a screen row of a frame whose pixels are kept
+  TF_STORING = 1u << 29,           // the frame in progress is the last one of this vcs_step: its pixels are kept
 };
+enum { OB_PF = 0, OB_BL, OB_P0, OB_P1, OB_M0, OB_M1 };
 
 // collision latch bit numbers inside W_CX (read map: SURVEY C.8)
 enum { CX_M0P1 = 0, CX_M0P0, CX_M1P0, CX_M1P1, CX_P0PF, CX_P0BL, CX_P1PF, CX_P1BL,
        CX_M0PF, CX_M0BL, CX_M1PF, CX_M1BL, CX_BLPF, CX_P0P1, CX_M0M1 };
 
 enum : uint32_t { STATUS_ILLEGAL = 1, STATUS_CAP = 2, STATUS_UNMODELLED = 4 };
+
+// per-thread shared-memory file (word index; word i of thread t lives at smem[i*BLOCK + t])
+enum SmWord {
+  S_RAM = 0,                       // 32 words: the 128 RAM bytes
+  S_OBJ = 32,                      // 30 words: cached 160-bit line masks of PF, BL, P0, P1, M0, M1 (5 words each)
+  S_PLANE = 62,                    // 10 words: colour-index bit planes of the scanline in progress (i0[5], i1[5])
+  S_COLU = 72, S_PF, S_GRP, S_NUSIZ, S_POS, S_POS2,   // TIA registers, packed as the W_* words (S_POS2 without rx)
+  S_CX, S_FL, S_RX, S_PX,          // collision latches, flags, clocks rendered, pixels painted of the current line
+  S_LINE, S_FDONE,                 // scanline in frame, frames completed in this step
+  S_PORTS, S_INP,                  // RIOT port latches; ina | fire0<<8
+  S_TMR, S_TTICKS,                 // timer state packed as W_TIMER, valid after S_TTICKS cycles of this step
+  S_WORDS                          // 88
+};
+// per-block context, in words after the thread files
+enum CtxWord { C_SCREEN_LO = 0, C_SCREEN_HI, C_Y0, C_FRAMESKIP, C_BATCH, C_ENV0, C_WORDS = 8 };
 
 struct RomMeta { uint32_t offset; uint32_t size; };   // into the ROM blob
 
@@ -58,7 +83,9 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   uint8_t *d_rom_blob; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
   uint8_t *d_actions_stage;     // for vcs_step_host
   uint8_t *h_pinned; size_t h_pinned_bytes;
-  int block_uniform_rom;        // every 128-env block maps to a single ROM
+  int block;                    // threads (= envs) per block of the interpreter kernel
+  int rom_smem;                 // every block maps to a single ROM: it is staged in shared memory
+  uint32_t max_rom;             // largest ROM image
   long long launches;
   char err[256];
 };

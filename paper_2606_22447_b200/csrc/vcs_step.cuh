@@ -5,17 +5,18 @@
 
 namespace vcs {
 
-constexpr int STEP_BLOCK = 128;          // threads (= environments) per block of the interpreter kernel
 
 struct StepParams {
   uint32_t *st; uint32_t *ram; unsigned long long *cyc; uint8_t *screen;
   const uint8_t *rom_blob; const RomMeta *rom_meta; const int32_t *env_rom;
   const uint8_t *actions;
   int32_t batch, frameskip, y0, max_lines;
+  int32_t block, rom_smem; uint32_t max_rom;     // launch shape: envs per block (64/128/256), ROM staged in smem, largest image
 };
 
 void upload_optable();
 const uint16_t *host_optable();
 cudaError_t launch_step(const StepParams &p, cudaStream_t stream);
+size_t step_smem_bytes(int block, bool roms, uint32_t max_rom);
 
 }  // namespace vcs
