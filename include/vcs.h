@@ -93,6 +93,15 @@ int64_t vcs_launch_count(vcs_t h);
  * CPU-only test can check it against the documented 151-opcode matrix. */
 int vcs_optable(uint16_t *out256_host);
 
+/* Integer-issue micro-benchmark on the current CUDA device: the denominator of the interpreter's roofline
+ * ("the builder must first run an integer micro-benchmark"; "compute/occupancy-
+ * bound, not memory-bound").  kind 0 = alu pipe only (LOP3 + SHF chains; ptxas moves plain adds to the fma pipe as IMAD.IADD), kind 1 = alu + fma pipes interleaved
+ * (LOP3 + IMAD).  Fills every SM with 2048 threads, each running 8 independent chains for `iters` loop trips of
+ * 256 instructions; writes thread-instructions per second (best of 3 after a warm-up run) to
+ * *thread_instr_per_s (HOST) and the duration of that run to *seconds (HOST, may be NULL).  Synchronous; uses
+ * the legacy default stream.  Errors: VCS_EINVAL, VCS_ECUDA, VCS_ENOMEM. */
+int vcs_issue_peak(int32_t kind, int32_t iters, double *thread_instr_per_s, double *seconds);
+
 int vcs_destroy(vcs_t h);
 const char *vcs_last_error(vcs_t h);     /* handle-owned string; "" when no error. h may be NULL */
 

@@ -19,7 +19,7 @@ _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOME
 
 EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
            "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_launch_count",
-           "vcs_optable", "vcs_destroy", "vcs_last_error"]
+           "vcs_optable", "vcs_issue_peak", "vcs_destroy", "vcs_last_error"]
 
 REGS_DTYPE = np.dtype([("cycles", "<u8"), ("frame", "<u4"), ("pc", "<u2"), ("a", "u1"), ("x", "u1"), ("y", "u1"),
                        ("sp", "u1"), ("p", "u1"), ("bank", "u1"), ("line", "<u2"), ("cyc_in_line", "u1"),
@@ -61,6 +61,7 @@ def load_library() -> C.CDLL:
     L.vcs_screen_ptr.argtypes = [P, C.POINTER(P)]
     L.vcs_launch_count.argtypes = [P]; L.vcs_launch_count.restype = C.c_int64
     L.vcs_optable.argtypes = [P]
+    L.vcs_issue_peak.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.vcs_destroy.argtypes = [P]
     L.vcs_last_error.argtypes = [P]; L.vcs_last_error.restype = C.c_char_p
     _lib = L
@@ -71,6 +72,15 @@ def optable() -> np.ndarray:
     out = np.zeros(256, dtype=np.uint16)
     assert load_library().vcs_optable(out.ctypes.data) == 0
     return out
+
+
+def issue_peak(kind: int, iters: int = 4096) -> tuple[float, float]:
+    """(thread-instructions/s, seconds) of the integer-issue micro-benchmark (vcs_issue_peak)."""
+    v, sec = C.c_double(), C.c_double()
+    rc = load_library().vcs_issue_peak(kind, iters, C.byref(v), C.byref(sec))
+    if rc != 0:
+        raise VcsError(f"vcs_issue_peak: {_ERR.get(rc, rc)}")
+    return v.value, sec.value
 
 
 def _stream_ptr(stream) -> int | None:
