@@ -9,7 +9,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 SO = os.path.join(PKG, "libvcsb200.so")
 SOURCES = ["vcs_api.cu", "vcs_step.cu", "vcs_peak.cu"]
-HEADERS = ["vcs_tia.cuh", "vcs_state.cuh", "vcs_step.cuh", "vcs_optable.cuh", os.path.join("..", "..", "include", "vcs.h")]
+HEADERS = ["vcs_decode.cuh", "vcs_tia.cuh", "vcs_state.cuh", "vcs_step.cuh", "vcs_optable.cuh", os.path.join("..", "..", "include", "vcs.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--use_fast_math"]
 

@@ -9,6 +9,7 @@
 
 #include "../../include/vcs.h"
 #include "vcs_step.cuh"
+#include "vcs_decode.cuh"
 
 using namespace vcs;
 
@@ -87,7 +88,7 @@ __global__ void get_regs_kernel(const uint32_t *st, const unsigned long long *cy
 StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   StepParams p;
   p.st = h->d_st; p.ram = h->d_ram; p.cyc = h->d_cyc; p.screen = h->d_screen;
-  p.rom_blob = h->d_rom_blob; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
+  p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
   p.actions = actions; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
   p.block = h->block; p.rom_smem = h->rom_smem; p.max_rom = h->max_rom;
   return p;
@@ -130,8 +131,11 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   *out = h;                                           // so that the caller can read vcs_last_error and destroy
 
   std::vector<RomMeta> meta(n_roms);
-  size_t blob = 0;
-  for (int r = 0; r < n_roms; ++r) { meta[r].offset = (uint32_t)blob; meta[r].size = roms[r].size; blob += roms[r].size; }
+  size_t blob = 0, dwords = 0;
+  for (int r = 0; r < n_roms; ++r) {
+    meta[r].offset = (uint32_t)blob; meta[r].size = roms[r].size; meta[r].doff = (uint32_t)dwords; meta[r].pad = 0;
+    blob += roms[r].size; dwords += (roms[r].size == 8192) ? 8192 : 4096;
+  }
   std::vector<uint8_t> hb(blob);
   for (int r = 0; r < n_roms; ++r) memcpy(hb.data() + meta[r].offset, roms[r].data, roms[r].size);
   std::vector<int32_t> er(batch, 0);
@@ -146,6 +150,23 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   h->block = want; h->rom_smem = 0;
   for (int blk = want; blk >= 64; blk >>= 1) if (uniform(blk)) { h->block = blk; h->rom_smem = 1; break; }
   if (getenv("VCS_ROM_GLOBAL")) h->rom_smem = 0;
+  // pre-decode every byte offset of every bank once (vcs_decode.cuh); the words depend on the launch shape
+  // (zero-page RAM operands are stored as shared-memory offsets)
+  std::vector<uint32_t> dw(dwords + 8, 0);
+  {
+    std::vector<uint8_t> img(4096 + 4, 0), leader(4096);
+    for (int r = 0; r < n_roms; ++r) {
+      const int nb = (roms[r].size == 8192) ? 2 : 1;
+      std::fill(leader.begin(), leader.end(), 0);
+      for (int pass = 0; pass < 2; ++pass)
+        for (int b = 0; b < nb; ++b) {
+          if (roms[r].size == 2048) { memcpy(img.data(), roms[r].data, 2048); memcpy(img.data() + 2048, roms[r].data, 2048); }
+          else memcpy(img.data(), roms[r].data + 4096 * b, 4096);
+          if (pass == 0) mark_leaders(img.data(), leader.data());
+          else decode_bank(img.data(), leader.data(), h->block, dw.data() + meta[r].doff + 4096 * b);
+        }
+    }
+  }
 
   const size_t B = (size_t)batch;
   CU(h, cudaMalloc((void **)&h->d_st, sizeof(uint32_t) * ST_WORDS * B));
@@ -153,6 +174,8 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   CU(h, cudaMalloc((void **)&h->d_cyc, sizeof(unsigned long long) * B));
   CU(h, cudaMalloc((void **)&h->d_screen, (size_t)SCR_W * SCR_H * B));
   CU(h, cudaMalloc((void **)&h->d_rom_blob, blob));
+  CU(h, cudaMalloc((void **)&h->d_drom, sizeof(uint32_t) * dw.size()));
+  CU(h, cudaMemcpy(h->d_drom, dw.data(), sizeof(uint32_t) * dw.size(), cudaMemcpyHostToDevice));
   CU(h, cudaMalloc((void **)&h->d_rom_meta, sizeof(RomMeta) * n_roms));
   CU(h, cudaMalloc((void **)&h->d_env_rom, sizeof(int32_t) * B));
   CU(h, cudaMalloc((void **)&h->d_seeds, sizeof(unsigned long long) * B));
@@ -264,7 +287,7 @@ int vcs_optable(uint16_t *out256) {
 int vcs_destroy(vcs_t h) {
   if (!h) return VCS_EINVAL;
   cudaDeviceSynchronize();
-  cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob);
+  cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom);
   cudaFree(h->d_rom_meta); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   delete h;

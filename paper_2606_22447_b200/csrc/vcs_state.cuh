@@ -74,13 +74,13 @@ enum SmWord {
 // per-block context, in words after the thread files
 enum CtxWord { C_SCREEN_LO = 0, C_SCREEN_HI, C_Y0, C_FRAMESKIP, C_BATCH, C_ENV0, C_WORDS = 8 };
 
-struct RomMeta { uint32_t offset; uint32_t size; };   // into the ROM blob
+struct RomMeta { uint32_t offset; uint32_t size; uint32_t doff; uint32_t pad; };   // byte offset into the ROM blob, size, word offset into the decode blob
 
 struct Handle {                 // host-side bookkeeping behind vcs_t
   int32_t batch, n_roms;
   int32_t y0, max_lines, f8_start_bank;
   uint32_t *d_st; uint32_t *d_ram; unsigned long long *d_cyc; uint8_t *d_screen;
-  uint8_t *d_rom_blob; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
+  uint8_t *d_rom_blob; uint32_t *d_drom; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
   uint8_t *d_actions_stage;     // for vcs_step_host
   uint8_t *h_pinned; size_t h_pinned_bytes;
   int block;                    // threads (= envs) per block of the interpreter kernel

@@ -5,83 +5,94 @@
 // planes live in the thread's shared-memory file; the block's cartridge ROM is staged in shared memory with
 // one bulk asynchronous copy (TMA 1-D, cp.async.bulk + mbarrier) when all of the block's envs share a ROM.
 //
-// Divergence (the measured choice north_star asks for): lanes of a warp are NOT run in lock-step.  Every
-// iteration each lane forms the key (frames done, SP, bank, PC); a warp-wide REDUX.MIN picks the smallest
-// and only the lanes holding it execute one 6507 instruction — all at the same PC of the same ROM, hence
-// the same opcode, the same addressing mode and (for stores) the same TIA register: the decode switch, the
-// TIA write switch and the lazy-TIA catch-up are warp-uniform.  Lower SP first returns lanes from
-// subroutines, lower PC first re-joins forward branches, the frame count bounds how long a lane can wait.
-// On BASELINE config 4 this keeps ~95 % (4 KB ROMs) of the lanes active per iteration versus 18 % active
-// threads per instruction for the lock-step kernel it replaced (profiles/r01_*).
+// Dispatch.  vcs_create pre-decodes every byte offset of every ROM bank into a 32-bit word (vcs_decode.cuh):
+// a fused handler id, the operand (already turned into a shared-memory offset for zero-page RAM), the
+// instruction length and a "leader" flag.  The hot loop loads that word through the read-only path (L1),
+// prefetches the sequentially next one before it dispatches, and jumps ONCE (one BRX) into a handler that is
+// specialised for opcode x address class; only indexed / indirect / absolute modes take a second-level
+// operation switch.  PCs outside cartridge space and the last 16 bytes of a bank decode at run time (H_SLOW).
 //
-// Each instruction runs in four phases shared by all opcodes — addressing (switch on 13 modes) -> ONE
-// generic operand-read site -> ALU (switch on op) -> ONE generic write site.  Cycle accounting is per bus
-// access (C.4/C.5): an access `k` cycles into the instruction happens in cycle `cyc + k`, scanline slot `n + k`.
+// Divergence (the measured choice north_star asks for): lanes of a warp are NOT run in lock-step.  At every
+// scheduling point each lane forms the key (frames done, SP, bank, PC); a warp-wide REDUX.MIN picks the
+// smallest and only the lanes holding it run — all at the same PC of the same ROM, hence the same handler,
+// the same operand and (for stores) the same TIA register: dispatch, the TIA write switch and the lazy-TIA
+// catch-up are warp-uniform.  Lower SP first returns lanes from subroutines, lower PC first re-joins forward
+// branches, the frame count bounds how long a lane can wait.  A group keeps running straight-line code
+// without re-forming until it executes a control transfer or reaches a leader (a static branch/JMP/JSR target
+// or return point — the only places where another lane can be waiting), so the REDUX is paid per basic
+// block, not per instruction.
+//
+// Cycle accounting is per bus access (C.4/C.5): an access `k` cycles into the instruction happens in cycle
+// `cyc + k`, scanline slot `cyc - lstart + k`.
 #include "vcs_tia.cuh"
-#include "vcs_optable.cuh"
+#include "vcs_decode.cuh"
 #include "vcs_step.cuh"
 
 namespace vcs {
 
-__constant__ uint16_t c_optab[256];
+__constant__ uint16_t c_gen[256];       // generic decode per opcode (vcs_decode.cuh generic_entry) for H_SLOW
 
-void upload_optable() { cudaMemcpyToSymbol(c_optab, kOpTable, sizeof(kOpTable)); }
+void upload_optable() {
+  uint16_t g[256];
+  for (int i = 0; i < 256; ++i) g[i] = generic_entry((uint32_t)i);
+  cudaMemcpyToSymbol(c_gen, g, sizeof(g));
+}
 const uint16_t *host_optable() { return kOpTable; }
 
-constexpr uint32_t IB_SLOW = 0x80000000u;
+constexpr int32_t LIM_NOW = (int32_t)0x80000000;     // `lim` value that forces the slow pre-check
 
 template <int BLOCK, bool ROMS>
 struct Cpu {
   using T = Tia<BLOCK>;
   // ---- CPU
   uint32_t A, X, Y, SP, PC;
-  uint32_t fC, fV, fD, fI, zv, nv;     // Z <=> (zv & 0xFF) == 0 ; N <=> nv & 0x80
+  uint32_t fC, fV, fDI, zv, nv;        // fDI: bit3 D, bit2 I ; Z <=> (zv & 0xFF) == 0 ; N <=> nv & 0x80
   uint32_t status;
   // ---- beam / time (cycle counts are relative to the start of this vcs_step call)
   int32_t cyc;        // CPU cycles executed in this step
-  int32_t n;          // cycle-in-line of `cyc` (0..76)
+  int32_t lstart;     // value of `cyc` at which the current scanline began (cycle-in-line n = cyc - lstart, 0..76+)
   int32_t fstart;     // value of `cyc` at which the current frame began (frame_cyc = cyc - fstart)
+  int32_t lim;        // fast path allowed while cyc < lim: min(line end, frame cap), LIM_NOW when WSYNC/halted
+  int32_t cap;        // frame cap in cycles
   uint32_t fdone;     // frames completed in this step (mirror of S_FDONE)
   bool wsync;         // mirror of TF_WSYNC
   // ---- cart
-  uint32_t bank, rom_mask, is_f8;
+  uint32_t bank, is_f8, rom_mask;
   uint32_t rom_off;   // ROMS: byte offset of the ROM image inside smem
-  const uint8_t *rom_g;   // !ROMS: the image in global memory
-  uint32_t ib;        // prefetched opcode | b1<<8 | b2<<16 at PC (IB_SLOW: fetch byte-wise with side effects)
+  const uint8_t *rom_g;    // !ROMS: the image in global memory
+  const uint32_t *dr;      // decode words of this env's ROM (4096 per bank)
+  uint32_t w;         // decode word at (bank, PC) — valid at every scheduling point
+  uint32_t tid4;      // 4 * threadIdx.x
 
   static DEV uint32_t &S(int i) { return T::S(i); }
 
   // ------------------------------------------------------------------ RAM (smem, conflict-free)
-  DEV uint32_t ram_rd(uint32_t a) const { return reinterpret_cast<const uint8_t *>(smem)[(((a & 0x7Cu) * BLOCK) | (a & 3u)) + 4 * threadIdx.x]; }
-  DEV void ram_wr(uint32_t a, uint32_t v) { reinterpret_cast<uint8_t *>(smem)[(((a & 0x7Cu) * BLOCK) | (a & 3u)) + 4 * threadIdx.x] = (uint8_t)v; }
+  DEV uint32_t ram_rd_off(uint32_t off) const { return reinterpret_cast<const uint8_t *>(smem)[off + tid4]; }
+  DEV void ram_wr_off(uint32_t off, uint32_t v) { reinterpret_cast<uint8_t *>(smem)[off + tid4] = (uint8_t)v; }
+  DEV uint32_t ram_rd(uint32_t a) const { return ram_rd_off(((a & 0x7Cu) * BLOCK) | (a & 3u)); }
+  DEV void ram_wr(uint32_t a, uint32_t v) { ram_wr_off(((a & 0x7Cu) * BLOCK) | (a & 3u), v); }
 
   // ------------------------------------------------------------------ ROM
   DEV uint32_t rom_byte(uint32_t off) const {
     if constexpr (ROMS) return reinterpret_cast<const uint8_t *>(smem)[rom_off + off];
     else return __ldg(rom_g + off);
   }
+  DEV void hotspot(uint32_t a) { if (is_f8 && (a | 1u) == 0x1FF9u) bank = a & 1u; }
   DEV uint32_t rom_rd(uint32_t a) {            // a = addr & 0x1FFF with A12 set
-    if (is_f8 && (a | 1u) == 0x1FF9u) bank = a & 1u;
+    hotspot(a);
     return rom_byte((bank << 12) + (a & rom_mask));
   }
-  DEV void hotspot(uint32_t a) { if (is_f8 && (a | 1u) == 0x1FF9u) bank = a & 1u; }
-  // the three bytes at PC in one go when no fetch can have a side effect (cartridge space, below the hotspots)
-  DEV void prefetch() {
-    const uint32_t a = PC & 0x1FFFu;
-    if ((a & 0x1000u) && (a & rom_mask) < rom_mask - 10u) {
-      const uint32_t off = (bank << 12) + (a & rom_mask);
-      uint32_t w0, w1;
-      if constexpr (ROMS) { const uint32_t *r = reinterpret_cast<const uint32_t *>(reinterpret_cast<const uint8_t *>(smem) + rom_off) + (off >> 2); w0 = r[0]; w1 = r[1]; }
-      else { const uint32_t *r = reinterpret_cast<const uint32_t *>(rom_g) + (off >> 2); w0 = __ldg(r); w1 = __ldg(r + 1); }
-      ib = __funnelshift_r(w0, w1, (off & 3u) * 8u) & 0x00FFFFFFu;
-    } else ib = IB_SLOW;
+  // decode word at (bank, PC); H_SLOW outside cartridge space
+  DEV uint32_t fetch() const {
+    if (!(PC & 0x1000u)) return H_SLOW;
+    return __ldg(dr + ((bank << 12) | (PC & 0xFFFu)));
   }
 
   // ------------------------------------------------------------------ RIOT timer, closed form (C.7)
   // advance the (timer, sub, tflag) state in smem to "after `ticks` cycles of this step" and return it unpacked
   DEV void timer_sync(int32_t ticks, uint32_t &timer, uint32_t &sub, uint32_t &shift, uint32_t &tflag) {
-    const uint32_t w = S(S_TMR);
-    timer = w & 0xFFu; shift = (w >> 8) & 0xFu; tflag = (w >> 12) & 1u; sub = w >> 16;
+    const uint32_t tw = S(S_TMR);
+    timer = tw & 0xFFu; shift = (tw >> 8) & 0xFu; tflag = (tw >> 12) & 1u; sub = tw >> 16;
     const uint32_t d = (uint32_t)(ticks - (int32_t)S(S_TTICKS));
     if ((int32_t)d <= 0) return;
     S(S_TTICKS) = (uint32_t)ticks;
@@ -145,19 +156,25 @@ struct Cpu {
     if (a & 0x1000u) hotspot(a);
     else if ((a & 0x0285u) == 0x0284u) { uint32_t t, s, sh, f; timer_sync(cyc + k + 1, t, s, sh, f); timer_put(t, s, sh, 0); }
   }
-  DEV void tia_events(uint32_t ev, int k) {        // after a TIA access k cycles into the instruction
-    n -= LINE_CYC * (int32_t)(ev >> 4);
+  // lim from (lstart, fstart, wsync, status)
+  DEV void relim() {
+    lim = (wsync || (status & (STATUS_ILLEGAL | STATUS_UNMODELLED))) ? LIM_NOW : min(lstart + LINE_CYC, fstart + cap);
+  }
+  DEV void tia_events(uint32_t ev, int k) {        // after a TIA write k cycles into the instruction
+    lstart += LINE_CYC * (int32_t)(ev >> 4);
     wsync = (ev & EV_WSYNC) != 0;
     if (ev & EV_FRAME) { fdone += 1; fstart = cyc + k + 1; }
+    relim();
   }
+  DEV void tia_write(uint32_t r, uint32_t v, int k) { tia_events(T::write(r, v, cyc - lstart + k), k); }
   // the generic operand read (C.3 decode), k cycles into the instruction
   DEV uint32_t bus_read(uint32_t addr, int k) {
     const uint32_t a = addr & 0x1FFFu;
     if ((a & 0x1280u) == 0x0080u) return ram_rd(a);
     if (a & 0x1000u) return rom_rd(a);
     if (a & 0x0080u) return riot_read(a, cyc + k);
-    const uint32_t r = T::read(a & 0xFu, n + k);
-    if (r >> 12) { n -= LINE_CYC * (int32_t)(r >> 12); wsync = false; }
+    const uint32_t r = T::read(a & 0xFu, cyc - lstart + k);
+    if (r >> 12) { lstart += LINE_CYC * (int32_t)(r >> 12); wsync = false; relim(); }
     return r & 0xFFu;
   }
   DEV void bus_write(uint32_t addr, uint32_t v, int k) {
@@ -167,17 +184,17 @@ struct Cpu {
     if (a & 0x0080u) { riot_write(a, v, cyc + k); return; }
     const uint32_t r = a & 0x3Fu;
     if (r > 0x2Cu || (r >= 0x15u && r <= 0x1Au) || r == 0x03u) return;      // no effect (audio: PAPER.md L205)
-    tia_events(T::write(r, v, n + k), k);
+    tia_write(r, v, k);
   }
   DEV uint32_t pack_p() const {
-    return (nv & 0x80u) | (fV << 6) | 0x20u | (fD << 3) | (fI << 2) | (((zv & 0xFFu) == 0) ? 2u : 0u) | fC;
+    return (nv & 0x80u) | (fV << 6) | 0x20u | fDI | (((zv & 0xFFu) == 0) ? 2u : 0u) | fC;
   }
   DEV void unpack_p(uint32_t p) {
-    fC = p & 1u; zv = (p & 2u) ? 0u : 1u; fI = (p >> 2) & 1u; fD = (p >> 3) & 1u; fV = (p >> 6) & 1u; nv = p & 0x80u;
+    fC = p & 1u; zv = (p & 2u) ? 0u : 1u; fDI = p & 0x0Cu; fV = (p >> 6) & 1u; nv = p & 0x80u;
   }
   DEV void adc(uint32_t v) {                               // C.6, binary and NMOS decimal
     const uint32_t a = A, C = fC;
-    if (!fD) {
+    if (!(fDI & 8u)) {
       const uint32_t s = a + v + C;
       fC = s >> 8; fV = ((a ^ s) & (v ^ s) & 0x80u) >> 7; A = s & 0xFFu; zv = nv = A;
       return;
@@ -198,142 +215,254 @@ struct Cpu {
     const uint32_t nb = v ^ 0xFFu, s = a + nb + C;         // flags exactly as binary
     const uint32_t bin = s & 0xFFu;
     fC = s >> 8; fV = ((a ^ s) & (nb ^ s) & 0x80u) >> 7; zv = nv = bin;
-    if (!fD) { A = bin; return; }
+    if (!(fDI & 8u)) { A = bin; return; }
     int al = (int)(a & 0x0Fu) - (int)(v & 0x0Fu) + (int)C - 1;
     if (al < 0) al = ((al - 6) & 0x0F) - 0x10;
     int d = (int)(a & 0xF0u) - (int)(v & 0xF0u) + al;
     if (d < 0) d -= 0x60;
     A = (uint32_t)d & 0xFFu;
   }
+  DEV void read_op(uint32_t o, uint32_t v) {               // o = op - OP_LDA
+    switch (o) {
+      case 0: A = v; zv = nv = v; break;
+      case 1: X = v; zv = nv = v; break;
+      case 2: Y = v; zv = nv = v; break;
+      case 3: A &= v; zv = nv = A; break;
+      case 4: A |= v; zv = nv = A; break;
+      case 5: A ^= v; zv = nv = A; break;
+      case 6: adc(v); break;
+      case 7: sbc(v); break;
+      case 8: fC = (A >= v) ? 1u : 0u; zv = nv = (A - v) & 0xFFu; break;
+      case 9: fC = (X >= v) ? 1u : 0u; zv = nv = (X - v) & 0xFFu; break;
+      case 10: fC = (Y >= v) ? 1u : 0u; zv = nv = (Y - v) & 0xFFu; break;
+      default: zv = A & v; nv = v; fV = (v >> 6) & 1u; break;
+    }
+  }
+  DEV uint32_t rmw_op(uint32_t o, uint32_t s) {            // o = op - OP_ASL
+    uint32_t r;
+    switch (o) {
+      case 0: r = (s << 1) & 0xFFu; fC = s >> 7; break;
+      case 1: r = s >> 1; fC = s & 1u; break;
+      case 2: r = ((s << 1) | fC) & 0xFFu; fC = s >> 7; break;
+      case 3: r = (s >> 1) | (fC << 7); fC = s & 1u; break;
+      case 4: r = (s + 1u) & 0xFFu; break;
+      default: r = (s - 1u) & 0xFFu; break;
+    }
+    zv = nv = r;
+    return r;
+  }
 
-  // ---------------------------------------------------------------- one instruction (C.5)
-  DEV void instruction(const uint16_t *optab) {
-    const uint32_t pc = PC;
-    const bool slow = (ib & IB_SLOW) != 0;
-    const uint32_t opc = slow ? lite_rd(pc) : (ib & 0xFFu);
-    const uint32_t ent = optab[opc];
-    const uint32_t mode = ent & 15u, op = (ent >> 4) & 63u, kind = ent >> 10;
-    if (op == OP_ILL) {                                    // C.12: halt for good, PC stays
-      if (!(status & STATUS_UNMODELLED)) status |= STATUS_ILLEGAL;
-      cyc += 1; n += 1; return;
+  // ---------------------------------------------------------------- the checks ahead of an instruction (C.4, C.10)
+  // entered when cyc >= lim.  Returns false when no instruction may run now (a frame ended at the cap, or
+  // the CPU is halted and idled): the lane goes back to the scheduling point.
+  DEV bool slow_pre() {
+    if (cyc - lstart > LINE_CYC) { T::line_end(); lstart += LINE_CYC; wsync = false; }     // the previous instruction ran over the line end
+    if (cyc - fstart >= cap) {                             // frame cap at the instruction boundary
+      status |= STATUS_CAP; T::frame_end(3u * (uint32_t)(cyc - lstart)); fdone += 1; fstart = cyc;
+      relim(); return false;
     }
-    const uint32_t b1 = slow ? lite_rd(pc + 1) : ((ib >> 8) & 0xFFu);    // operand byte, or the dummy read @PC+1
-    const uint32_t b2f = (ib >> 16) & 0xFFu;
-#define FETCH2() (slow ? lite_rd(pc + 2) : b2f)
-    uint32_t ea = 0, v = 0, wv = 0;
-    int k = 0;                                             // cycles before the operand access
-    int total = 2;
-    uint32_t npc = pc + 2;
-    switch (mode) {
-      case MD_IMP: case MD_ACC: npc = pc + 1; break;
-      case MD_IMM: v = b1; k = 1; break;
-      case MD_ZP:  ea = b1; k = 2; break;
-      case MD_ZPX: ea = (b1 + X) & 0xFFu; k = 3; break;
-      case MD_ZPY: ea = (b1 + Y) & 0xFFu; k = 3; break;
-      case MD_ABS: ea = b1 | (FETCH2() << 8); k = 3; npc = pc + 3; break;
-      case MD_ABX: case MD_ABY: case MD_IZY: {
-        uint32_t lo, hi;
-        if (mode == MD_IZY) { lo = lite_rd(b1); hi = lite_rd((b1 + 1u) & 0xFFu); k = 4; }
-        else { lo = b1; hi = FETCH2(); k = 3; npc = pc + 3; }
-        const uint32_t t = lo + ((mode == MD_ABX) ? X : Y);
-        const uint32_t unc = (hi << 8) | (t & 0xFFu);
-        ea = (unc + (t & 0x100u)) & 0xFFFFu;
-        if (kind != K_READ || (t & 0x100u)) { dummy_rd(unc, k); k += 1; }
-      } break;
-      case MD_IZX: { const uint32_t z = (b1 + X) & 0xFFu; ea = lite_rd(z) | (lite_rd((z + 1u) & 0xFFu) << 8); k = 5; } break;
-      default: break;                                      // MD_REL, MD_SPC: handled by op
+    if (cyc - lstart >= LINE_CYC) { T::line_end(); lstart += LINE_CYC; wsync = false; }     // n == 76 exactly
+    if (status & (STATUS_ILLEGAL | STATUS_UNMODELLED)) {   // halted: idle cycles to the line end / the cap
+      cyc += min(LINE_CYC - (cyc - lstart), cap - (cyc - fstart));
+      return false;
     }
-    if (kind & K_READ) {                                   // K_READ or K_RMW: the one generic read site
-      if (mode != MD_IMM) v = bus_read(ea, k);
-      total = k + 1;
+    if (wsync) {                                           // a12: RDY holds the CPU until the line ends
+      cyc = lstart + LINE_CYC; T::line_end(); lstart = cyc; wsync = false;
     }
-    switch (op) {
-      case OP_LDA: A = v; zv = nv = v; break;
-      case OP_LDX: X = v; zv = nv = v; break;
-      case OP_LDY: Y = v; zv = nv = v; break;
-      case OP_AND: A &= v; zv = nv = A; break;
-      case OP_ORA: A |= v; zv = nv = A; break;
-      case OP_EOR: A ^= v; zv = nv = A; break;
-      case OP_ADC: adc(v); break;
-      case OP_SBC: sbc(v); break;
-      case OP_CMP: case OP_CPX: case OP_CPY: {
-        const uint32_t r = (op == OP_CMP) ? A : (op == OP_CPX) ? X : Y;
-        fC = (r >= v) ? 1u : 0u; zv = nv = (r - v) & 0xFFu; } break;
-      case OP_BIT: zv = A & v; nv = v; fV = (v >> 6) & 1u; break;
-      case OP_STA: wv = A; break;
-      case OP_STX: wv = X; break;
-      case OP_STY: wv = Y; break;
-      case OP_ASL: case OP_LSR: case OP_ROL: case OP_ROR: case OP_INC: case OP_DEC: {
-        const uint32_t s = (mode == MD_ACC) ? A : v; uint32_t r;
-        if (op == OP_ASL)      { r = (s << 1) & 0xFFu; fC = s >> 7; }
-        else if (op == OP_LSR) { r = s >> 1; fC = s & 1u; }
-        else if (op == OP_ROL) { r = ((s << 1) | fC) & 0xFFu; fC = s >> 7; }
-        else if (op == OP_ROR) { r = (s >> 1) | (fC << 7); fC = s & 1u; }
-        else if (op == OP_INC) { r = (s + 1u) & 0xFFu; }
-        else                   { r = (s - 1u) & 0xFFu; }
-        zv = nv = r;
-        if (mode == MD_ACC) A = r; else wv = r;
-      } break;
-      case OP_CLC: fC = 0; break;
-      case OP_SEC: fC = 1; break;
-      case OP_CLD: fD = 0; break;
-      case OP_SED: fD = 1; break;
-      case OP_CLI: fI = 0; break;
-      case OP_SEI: fI = 1; break;
-      case OP_CLV: fV = 0; break;
-      case OP_NOP: break;
-      case OP_DEX: X = (X - 1u) & 0xFFu; zv = nv = X; break;
-      case OP_DEY: Y = (Y - 1u) & 0xFFu; zv = nv = Y; break;
-      case OP_INX: X = (X + 1u) & 0xFFu; zv = nv = X; break;
-      case OP_INY: Y = (Y + 1u) & 0xFFu; zv = nv = Y; break;
-      case OP_TAX: X = A; zv = nv = X; break;
-      case OP_TAY: Y = A; zv = nv = Y; break;
-      case OP_TSX: X = SP; zv = nv = X; break;
-      case OP_TXA: A = X; zv = nv = A; break;
-      case OP_TYA: A = Y; zv = nv = A; break;
-      case OP_TXS: SP = X; break;
-      case OP_BPL: case OP_BMI: case OP_BVC: case OP_BVS: case OP_BCC: case OP_BCS: case OP_BNE: case OP_BEQ: {
-        const uint32_t idx = op - OP_BPL; uint32_t f;
-        switch (idx >> 1) { case 0: f = (nv >> 7) & 1u; break; case 1: f = fV; break; case 2: f = fC; break;
-                            default: f = ((zv & 0xFFu) == 0) ? 1u : 0u; break; }
-        if (f == (idx & 1u)) {
-          const uint32_t next = (pc + 2u) & 0xFFFFu;
-          const uint32_t target = (next + (uint32_t)(int32_t)(int8_t)b1) & 0xFFFFu;
-          hotspot(next & 0x1FFFu);                         // dummy read @PC
-          total = 3;
-          if ((target ^ next) & 0xFF00u) { hotspot(((next & 0xFF00u) | (target & 0xFFu)) & 0x1FFFu); total = 4; }
-          npc = target;
+    relim();
+    return cyc < lim;                                      // (the cap can fall on the line start reached by WSYNC)
+  }
+
+  // ---------------------------------------------------------------- instructions until the next scheduling point
+  DEV void run_block(uint32_t fskip) {
+    for (;;) {
+      if (cyc >= lim) { if (!slow_pre()) return; }
+      const uint32_t pc = PC;
+      uint32_t cw = w;                                     // the word being executed
+      uint32_t hid = cw & 0xFFu;
+      uint32_t pl = (cw >> 8) & 0xFFFFu;
+      const uint32_t di = (bank << 12) | (pc & 0xFFFu);
+      uint32_t wn = 0;                                     // sequential prefetch (valid when hid != H_SLOW)
+      bool seq = hid != H_SLOW;
+      if (seq) wn = __ldg(dr + di + (cw >> DW_LEN_SHIFT));
+      uint32_t npc = pc + (cw >> DW_LEN_SHIFT);
+      int total = 2;
+      bool brk = false;                                    // control transfer / bank access: refetch and re-schedule
+      uint32_t ea = 0, v = 0, wv = 0;
+      int k = 0, i0 = 0;
+      if (hid == H_SLOW) {                                 // byte-wise fetch with side effects, run-time decode
+        const uint32_t opc = lite_rd(pc);
+        const uint32_t g = c_gen[opc];
+        const uint32_t len = g >> 13;
+        hid = g & 0xFFu;
+        uint32_t b1 = 0, b2 = 0;
+        if (hid != H_ILL) { b1 = lite_rd(pc + 1u); if (len == 3) b2 = lite_rd(pc + 2u); }
+        pl = b1 | (b2 << 8);
+        cw = ((g >> 8) & 31u) << DW_OP2_SHIFT;
+        if (hid >= H_BR0 && hid < H_BR0 + 8) {
+          const uint32_t next = (pc + 2u) & 0xFFFFu, target = (next + (uint32_t)(int32_t)(int8_t)b1) & 0xFFFFu;
+          pl = (2u + (uint32_t)(int32_t)(int8_t)b1) & 0xFFFFu;
+          cw = (((target ^ next) & 0xFF00u) ? 4u : 3u) << DW_OP2_SHIFT;
         }
-      } break;
-      case OP_JMP: npc = b1 | (FETCH2() << 8); total = 3; break;
-      case OP_JMPI: { const uint32_t hi = FETCH2();
-        const uint32_t l2 = lite_rd((hi << 8) | b1), h2 = lite_rd((hi << 8) | ((b1 + 1u) & 0xFFu));   // no carry into the page
-        npc = l2 | (h2 << 8); total = 5; } break;
-      case OP_JSR: { const uint32_t ret = (pc + 2u) & 0xFFFFu;     // address of the 3rd byte
-        push(ret >> 8); push(ret & 0xFFu);
-        npc = b1 | (FETCH2() << 8); total = 6; } break;
-      case OP_RTS: { const uint32_t lo = pull(), hi = pull(); const uint32_t r = lo | (hi << 8);
-        hotspot(r & 0x1FFFu); npc = (r + 1u) & 0xFFFFu; total = 6; } break;
-      case OP_RTI: { unpack_p(pull()); const uint32_t lo = pull(), hi = pull(); npc = lo | (hi << 8); total = 6; } break;
-      case OP_PHA: push(A); npc = pc + 1; total = 3; break;
-      case OP_PHP: push(pack_p() | 0x30u); npc = pc + 1; total = 3; break;
-      case OP_PLA: A = pull(); zv = nv = A; npc = pc + 1; total = 4; break;
-      case OP_PLP: unpack_p(pull()); npc = pc + 1; total = 4; break;
-      case OP_BRK: { const uint32_t ret = (pc + 2u) & 0xFFFFu;
-        push(ret >> 8); push(ret & 0xFFu); push(pack_p() | 0x30u);
-        npc = lite_rd(0xFFFEu) | (lite_rd(0xFFFFu) << 8); fI = 1; total = 7; } break;
-      default: break;
-    }
-#undef FETCH2
-    PC = npc & 0xFFFFu;
-    if (kind & K_WRITE) {                                  // K_WRITE: one write; K_RMW: old value, then new
-      const bool rmw = (kind == K_RMW);
-      total = k + (rmw ? 3 : 1);
+        npc = pc + len;
+        brk = true;
+      }
+      const uint32_t op2 = (cw >> DW_OP2_SHIFT) & 31u;
+      switch (hid) {
+        // ---- immediate
+        case H_IMM0 + 0: A = pl; zv = nv = pl; break;
+        case H_IMM0 + 1: X = pl; zv = nv = pl; break;
+        case H_IMM0 + 2: Y = pl; zv = nv = pl; break;
+        case H_IMM0 + 3: A &= pl; zv = nv = A; break;
+        case H_IMM0 + 4: A |= pl; zv = nv = A; break;
+        case H_IMM0 + 5: A ^= pl; zv = nv = A; break;
+        case H_IMM0 + 6: adc(pl); break;
+        case H_IMM0 + 7: sbc(pl); break;
+        case H_IMM0 + 8: fC = (A >= pl) ? 1u : 0u; zv = nv = (A - pl) & 0xFFu; break;
+        case H_IMM0 + 9: fC = (X >= pl) ? 1u : 0u; zv = nv = (X - pl) & 0xFFu; break;
+        case H_IMM0 + 10: fC = (Y >= pl) ? 1u : 0u; zv = nv = (Y - pl) & 0xFFu; break;
+        // ---- zero-page RAM reads (3 cycles)
+        case H_ZR0 + 0: A = ram_rd_off(pl); zv = nv = A; total = 3; break;
+        case H_ZR0 + 1: X = ram_rd_off(pl); zv = nv = X; total = 3; break;
+        case H_ZR0 + 2: Y = ram_rd_off(pl); zv = nv = Y; total = 3; break;
+        case H_ZR0 + 3: A &= ram_rd_off(pl); zv = nv = A; total = 3; break;
+        case H_ZR0 + 4: A |= ram_rd_off(pl); zv = nv = A; total = 3; break;
+        case H_ZR0 + 5: A ^= ram_rd_off(pl); zv = nv = A; total = 3; break;
+        case H_ZR0 + 6: adc(ram_rd_off(pl)); total = 3; break;
+        case H_ZR0 + 7: sbc(ram_rd_off(pl)); total = 3; break;
+        case H_ZR0 + 8: v = ram_rd_off(pl); fC = (A >= v) ? 1u : 0u; zv = nv = (A - v) & 0xFFu; total = 3; break;
+        case H_ZR0 + 9: v = ram_rd_off(pl); fC = (X >= v) ? 1u : 0u; zv = nv = (X - v) & 0xFFu; total = 3; break;
+        case H_ZR0 + 10: v = ram_rd_off(pl); fC = (Y >= v) ? 1u : 0u; zv = nv = (Y - v) & 0xFFu; total = 3; break;
+        case H_ZR0 + 11: v = ram_rd_off(pl); zv = A & v; nv = v; fV = (v >> 6) & 1u; total = 3; break;
+        // ---- zero-page RAM stores
+        case H_STZR0 + 0: ram_wr_off(pl, A); total = 3; break;
+        case H_STZR0 + 1: ram_wr_off(pl, X); total = 3; break;
+        case H_STZR0 + 2: ram_wr_off(pl, Y); total = 3; break;
+        // ---- zero-page TIA register stores (write in the 3rd cycle)
+        case H_STZT0 + 0: tia_write(pl, A, 2); total = 3; break;
+        case H_STZT0 + 1: tia_write(pl, X, 2); total = 3; break;
+        case H_STZT0 + 2: tia_write(pl, Y, 2); total = 3; break;
+        case H_NOP3: total = 3; break;
+        // ---- zero-page RAM read-modify-write (5 cycles)
+        case H_MZR0 + 0: case H_MZR0 + 1: case H_MZR0 + 2: case H_MZR0 + 3: case H_MZR0 + 4: case H_MZR0 + 5:
+          ram_wr_off(pl, rmw_op(hid - H_MZR0, ram_rd_off(pl))); total = 5; break;
+        case H_ACC0 + 0: case H_ACC0 + 1: case H_ACC0 + 2: case H_ACC0 + 3: A = rmw_op(hid - H_ACC0, A); break;
+        // ---- implied
+        case H_IMP0 + 0: fC = 0; break;
+        case H_IMP0 + 1: fC = 1; break;
+        case H_IMP0 + 2: fDI &= ~8u; break;
+        case H_IMP0 + 3: fDI |= 8u; break;
+        case H_IMP0 + 4: fDI &= ~4u; break;
+        case H_IMP0 + 5: fDI |= 4u; break;
+        case H_IMP0 + 6: fV = 0; break;
+        case H_IMP0 + 7: break;
+        case H_IMP0 + 8: X = (X - 1u) & 0xFFu; zv = nv = X; break;
+        case H_IMP0 + 9: Y = (Y - 1u) & 0xFFu; zv = nv = Y; break;
+        case H_IMP0 + 10: X = (X + 1u) & 0xFFu; zv = nv = X; break;
+        case H_IMP0 + 11: Y = (Y + 1u) & 0xFFu; zv = nv = Y; break;
+        case H_IMP0 + 12: X = A; zv = nv = X; break;
+        case H_IMP0 + 13: Y = A; zv = nv = Y; break;
+        case H_IMP0 + 14: X = SP; zv = nv = X; break;
+        case H_IMP0 + 15: A = X; zv = nv = A; break;
+        case H_IMP0 + 16: A = Y; zv = nv = A; break;
+        case H_IMP0 + 17: SP = X; break;
+        // ---- branches: payload = displacement + 2, op2 = cycles when taken
+        case H_BR0 + 0: case H_BR0 + 1: case H_BR0 + 2: case H_BR0 + 3: case H_BR0 + 4: case H_BR0 + 5: case H_BR0 + 6: case H_BR0 + 7: {
+          const uint32_t idx = hid - H_BR0; uint32_t f;
+          switch (idx >> 1) { case 0: f = (nv >> 7) & 1u; break; case 1: f = fV; break; case 2: f = fC; break;
+                              default: f = ((zv & 0xFFu) == 0) ? 1u : 0u; break; }
+          brk = true;
+          if (f == (idx & 1u)) {
+            const uint32_t target = (pc + pl) & 0xFFFFu;
+            if (is_f8) {                                   // the dummy reads @PC and @(old PCH : new PCL)
+              const uint32_t next = (pc + 2u) & 0xFFFFu;
+              hotspot(next & 0x1FFFu);
+              if (op2 == 4u) hotspot(((next & 0xFF00u) | (target & 0xFFu)) & 0x1FFFu);
+            }
+            total = (int)op2; npc = target;
+          }
+        } break;
+        // ---- control transfers and stack
+        case H_JMP: npc = pl; total = 3; brk = true; break;
+        case H_JSR: { const uint32_t ret = (pc + 2u) & 0xFFFFu;     // address of the 3rd byte
+          push(ret >> 8); push(ret & 0xFFu); npc = pl; total = 6; brk = true; } break;
+        case H_RTS: { const uint32_t lo = pull(), hi = pull(); const uint32_t r = lo | (hi << 8);
+          hotspot(r & 0x1FFFu); npc = r + 1u; total = 6; brk = true; } break;
+        case H_PHA: push(A); total = 3; break;
+        case H_PHP: push(pack_p() | 0x30u); total = 3; break;
+        case H_PLA: A = pull(); zv = nv = A; total = 4; break;
+        case H_PLP: unpack_p(pull()); total = 4; break;
+        // ---- generic addressing: reads
+        case H_R0 + 0: v = pl & 0xFFu; total = 2; goto do_read_op;
+        case H_R0 + 1: ea = pl & 0xFFu; k = 2; goto do_read;
+        case H_R0 + 2: ea = (pl + X) & 0xFFu; k = 3; goto do_read;
+        case H_R0 + 3: ea = (pl + Y) & 0xFFu; k = 3; goto do_read;
+        case H_R0 + 4: ea = pl; k = 3; goto do_read;
+        case H_R0 + 5: case H_R0 + 6: case H_R0 + 8: {
+          uint32_t lo, hi;
+          if (hid == H_R0 + 8) { lo = lite_rd(pl & 0xFFu); hi = lite_rd((pl + 1u) & 0xFFu); k = 4; }
+          else { lo = pl & 0xFFu; hi = pl >> 8; k = 3; }
+          const uint32_t t = lo + ((hid == H_R0 + 5) ? X : Y);
+          const uint32_t unc = (hi << 8) | (t & 0xFFu);
+          ea = (unc + (t & 0x100u)) & 0xFFFFu;
+          if (t & 0x100u) { dummy_rd(unc, k); k += 1; }
+        } goto do_read;
+        case H_R0 + 7: { const uint32_t z = (pl + X) & 0xFFu; ea = lite_rd(z) | (lite_rd((z + 1u) & 0xFFu) << 8); k = 5; } goto do_read;
+        // ---- generic addressing: stores
+        case H_W0 + 0: ea = pl & 0xFFu; k = 2; goto do_write;
+        case H_W0 + 1: ea = (pl + X) & 0xFFu; k = 3; goto do_write;
+        case H_W0 + 2: ea = (pl + Y) & 0xFFu; k = 3; goto do_write;
+        case H_W0 + 3: ea = pl; k = 3; goto do_write;
+        case H_W0 + 4: case H_W0 + 5: case H_W0 + 7: {
+          uint32_t lo, hi;
+          if (hid == H_W0 + 7) { lo = lite_rd(pl & 0xFFu); hi = lite_rd((pl + 1u) & 0xFFu); k = 4; }
+          else { lo = pl & 0xFFu; hi = pl >> 8; k = 3; }
+          const uint32_t t = lo + ((hid == H_W0 + 4) ? X : Y);
+          const uint32_t unc = (hi << 8) | (t & 0xFFu);
+          ea = (unc + (t & 0x100u)) & 0xFFFFu;
+          dummy_rd(unc, k); k += 1;
+        } goto do_write;
+        case H_W0 + 6: { const uint32_t z = (pl + X) & 0xFFu; ea = lite_rd(z) | (lite_rd((z + 1u) & 0xFFu) << 8); k = 5; } goto do_write;
+        // ---- generic addressing: read-modify-write
+        case H_M0 + 0: ea = pl & 0xFFu; k = 2; goto do_rmw;
+        case H_M0 + 1: ea = (pl + X) & 0xFFu; k = 3; goto do_rmw;
+        case H_M0 + 2: ea = pl; k = 3; goto do_rmw;
+        case H_M0 + 3: { const uint32_t t = (pl & 0xFFu) + X; const uint32_t unc = (pl & 0xFF00u) | (t & 0xFFu);
+          ea = (unc + (t & 0x100u)) & 0xFFFFu; dummy_rd(unc, 3); k = 4; } goto do_rmw;
+        // ---- rare
+        case H_JMPI: { const uint32_t l2 = lite_rd(pl), h2 = lite_rd((pl & 0xFF00u) | ((pl + 1u) & 0xFFu));   // no carry into the page
+          npc = l2 | (h2 << 8); total = 5; brk = true; } break;
+        case H_RTI: { unpack_p(pull()); const uint32_t lo = pull(), hi = pull(); npc = lo | (hi << 8); total = 6; brk = true; } break;
+        case H_BRK: { const uint32_t ret = (pc + 2u) & 0xFFFFu;
+          push(ret >> 8); push(ret & 0xFFu); push(pack_p() | 0x30u);
+          npc = lite_rd(0xFFFEu) | (lite_rd(0xFFFFu) << 8); fDI |= 4u; total = 7; brk = true; } break;
+        default:                                           // H_ILL — C.12: halt for good, PC stays
+          if (!(status & STATUS_UNMODELLED)) status |= STATUS_ILLEGAL;
+          npc = pc; total = 1; brk = true; lim = LIM_NOW; break;
+        do_read:
+          v = bus_read(ea, k); total = k + 1;
+        do_read_op:
+          read_op(op2, v); break;
+        do_write:
+          wv = (op2 == 0) ? A : (op2 == 1) ? X : Y;
+          i0 = 1; k -= 1; goto do_store;
+        do_rmw:
+          v = bus_read(ea, k);
+          wv = rmw_op(op2, v);
+          i0 = 0; k += 1;
+        do_store:                                          // the one generic write site: [old value,] new value (C.5)
 #pragma unroll 1
-      for (int i = rmw ? 0 : 1; i < 2; ++i)               // the one generic write site
-        bus_write(ea, i ? wv : v, k + (rmw ? 1 + i : 0));
+          for (int i = i0; i < 2; ++i) bus_write(ea, i ? wv : v, k + i);
+          total = k + 2; break;
+      }
+      brk |= bank != (di >> 12);                           // a hotspot access switched banks: wn is from the old one
+      PC = npc & 0xFFFFu;
+      cyc += total;
+      if (status & STATUS_UNMODELLED) lim = LIM_NOW;
+      if (fdone >= fskip) return;
+      if (seq && !brk) { w = wn; if (w & DW_LEADER) return; }
+      else { w = fetch(); return; }
     }
-    cyc += total; n += total;
   }
 };
 
@@ -353,8 +482,7 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
   using T = Tia<BLOCK>;
   __shared__ __align__(8) unsigned long long s_bar;
   uint32_t *s_ctx = smem + S_WORDS * BLOCK;
-  uint16_t *s_optab = reinterpret_cast<uint16_t *>(s_ctx + C_WORDS);
-  constexpr uint32_t ROM_OFF = (S_WORDS * BLOCK + C_WORDS + 128) * 4;     // byte offset of the ROM image in smem
+  constexpr uint32_t ROM_OFF = (S_WORDS * BLOCK + C_WORDS) * 4;          // byte offset of the ROM image in smem
   const int tid = threadIdx.x;
   const int e0 = blockIdx.x * BLOCK;
   const int e = e0 + tid;
@@ -368,7 +496,6 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
     s_ctx[C_Y0] = (uint32_t)p.y0; s_ctx[C_FRAMESKIP] = (uint32_t)p.frameskip; s_ctx[C_BATCH] = (uint32_t)B; s_ctx[C_ENV0] = (uint32_t)e0;
     if constexpr (ROMS) { mbar_init(smem_u32(&s_bar), 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
   }
-  for (int i = tid; i < 256; i += BLOCK) s_optab[i] = c_optab[i];
   __syncthreads();
   if constexpr (ROMS) {                                    // a3: stage the block's ROM (2 KB images twice: the mirror)
     if (tid == 0) {
@@ -401,9 +528,11 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
   } else {
     s.A = s.X = s.Y = s.SP = s.PC = 0; s.unpack_p(0x24); s.status = 0; s.bank = 0; s.fstart = 0;
   }
-  s.cyc = 0; s.n = (int32_t)n0; s.fdone = live ? 0u : (uint32_t)p.frameskip;
-  s.rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu; s.is_f8 = (rm.size == 8192);
-  s.rom_off = ROM_OFF; s.rom_g = p.rom_blob + rm.offset;
+  s.cyc = 0; s.lstart = -(int32_t)n0; s.fdone = live ? 0u : (uint32_t)p.frameskip;
+  s.cap = p.max_lines * LINE_CYC;
+  s.is_f8 = (rm.size == 8192);
+  s.rom_off = ROM_OFF; s.rom_g = p.rom_blob + rm.offset; s.dr = p.drom + rm.doff; s.tid4 = 4u * (uint32_t)tid;
+  s.rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
   // ---- a2 action latch (C.11)
   if (live) {
     uint32_t act = p.actions[e]; if (act >= 18u) act = 0;
@@ -420,11 +549,10 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
     T::S(S_FL) = fl;
   }
   s.wsync = (fl & TF_WSYNC) != 0;
+  s.relim();
   if constexpr (ROMS) mbar_wait(smem_u32(&s_bar), 0);
-  const int32_t cap = p.max_lines * LINE_CYC;
   const uint32_t fskip = (uint32_t)p.frameskip;
-  s.ib = IB_SLOW;
-  if (live) s.prefetch();
+  s.w = live ? s.fetch() : (uint32_t)H_SLOW;
 
   // ---- the hot loop: whole instructions until `frameskip` frame-end events (C.10), min-key lanes first.
   // Line bookkeeping mirrors C.4: the line counter advances with the FIRST cycle of a new line, so an
@@ -435,33 +563,17 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
                        : (min(s.fdone, 63u) << 25) | (s.SP << 17) | (s.bank << 16) | s.PC;
     const uint32_t mk = __reduce_min_sync(0xFFFFFFFFu, key);
     if (mk == 0xFFFFFFFFu) break;
-    if (key == mk) {
-      if (s.cyc - s.fstart >= cap) {                       // frame cap at the instruction boundary
-        s.status |= STATUS_CAP; T::frame_end(3u * (uint32_t)s.n); s.fdone += 1; s.fstart = s.cyc;
-      } else {
-        if (s.n >= LINE_CYC) { T::line_end(); s.n -= LINE_CYC; s.wsync = false; }     // n == 76 exactly (see above)
-        if (s.status & (STATUS_ILLEGAL | STATUS_UNMODELLED)) {  // halted: idle cycles to the line end / the cap
-          const int d = min(LINE_CYC - s.n, cap - (s.cyc - s.fstart));
-          s.cyc += d; s.n += d;
-        } else {
-          if (s.wsync) {                                   // a12: RDY holds the CPU until the line ends
-            s.cyc += LINE_CYC - s.n; T::line_end(); s.n = 0; s.wsync = false;
-          }
-          s.instruction(s_optab);
-          if (s.n > LINE_CYC) { T::line_end(); s.n -= LINE_CYC; s.wsync = false; }
-          s.prefetch();
-        }
-      }
-    }
+    if (key == mk) s.run_block(fskip);
   }
   if (!live) return;
+  if (s.cyc - s.lstart > LINE_CYC) { T::line_end(); s.lstart += LINE_CYC; }      // the last instruction ran over the line end
   // ---- a16 state store
   {
     uint32_t timer, sub, shift, tflag;
     s.timer_sync(s.cyc, timer, sub, shift, tflag);
     p.st[W_AXYS * B + e] = s.A | (s.X << 8) | (s.Y << 16) | (s.SP << 24);
     p.st[W_PC * B + e] = s.PC | (s.pack_p() << 16) | (s.status << 24);
-    p.st[W_BEAM * B + e] = (uint32_t)s.n | (T::S(S_LINE) << 8) | (s.bank << 24);
+    p.st[W_BEAM * B + e] = (uint32_t)(s.cyc - s.lstart) | (T::S(S_LINE) << 8) | (s.bank << 24);
     p.st[W_FRAME * B + e] += s.fdone;
     p.st[W_FCYC * B + e] = (uint32_t)(s.cyc - s.fstart);
     p.st[W_TIMER * B + e] = timer | (shift << 8) | (tflag << 12) | (sub << 16);
@@ -475,7 +587,7 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
 }
 
 size_t step_smem_bytes(int block, bool roms, uint32_t max_rom) {
-  return (size_t)(S_WORDS * block + C_WORDS + 128) * 4 + (roms ? (max_rom < 4096 ? 4096 : max_rom) + 16 : 0);
+  return (size_t)(S_WORDS * block + C_WORDS) * 4 + (roms ? (max_rom < 4096 ? 4096 : max_rom) + 16 : 0);
 }
 
 template <int BLOCK, bool ROMS>
