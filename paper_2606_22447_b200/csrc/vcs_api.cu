@@ -90,7 +90,7 @@ StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   p.st = h->d_st; p.ram = h->d_ram; p.cyc = h->d_cyc; p.screen = h->d_screen;
   p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
   p.actions = actions; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
-  p.block = h->block; p.rom_smem = h->rom_smem; p.max_rom = h->max_rom;
+  p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom;
   return p;
 }
 
@@ -150,6 +150,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   h->block = want; h->rom_smem = 0;
   for (int blk = want; blk >= 64; blk >>= 1) if (uniform(blk)) { h->block = blk; h->rom_smem = 1; break; }
   if (getenv("VCS_ROM_GLOBAL")) h->rom_smem = 0;
+  h->regroup = getenv("VCS_NO_REGROUP") ? 0 : 1;
   // pre-decode every byte offset of every bank once (vcs_decode.cuh); the words depend on the launch shape
   // (zero-page RAM operands are stored as shared-memory offsets)
   std::vector<uint32_t> dw(dwords + 8, 0);

@@ -62,14 +62,16 @@ enum : uint32_t { STATUS_ILLEGAL = 1, STATUS_CAP = 2, STATUS_UNMODELLED = 4 };
 // per-thread shared-memory file (word index; word i of thread t lives at smem[i*BLOCK + t])
 enum SmWord {
   S_RAM = 0,                       // 32 words: the 128 RAM bytes
-  S_OBJ = 32,                      // 30 words: cached 160-bit line masks of PF, BL, P0, P1, M0, M1 (5 words each)
-  S_PLANE = 62,                    // 10 words: colour-index bit planes of the scanline in progress (i0[5], i1[5])
-  S_COLU = 72, S_PF, S_GRP, S_NUSIZ, S_POS, S_POS2,   // TIA registers, packed as the W_* words (S_POS2 without rx)
+  S_PLANE = 32,                    // 10 words: colour-index bit planes of the scanline in progress (i0[5], i1[5])
+  S_COLU = 42, S_PF, S_GRP, S_NUSIZ, S_POS, S_POS2,   // TIA registers, packed as the W_* words (S_POS2 without rx)
   S_CX, S_FL, S_RX, S_PX,          // collision latches, flags, clocks rendered, pixels painted of the current line
   S_LINE, S_FDONE,                 // scanline in frame, frames completed in this step
-  S_PORTS, S_INP,                  // RIOT port latches; ina | fire0<<8
+  S_PORTS, S_INP,                  // RIOT port latches; ina | fire0<<8 | (env index inside the block)<<16
   S_TMR, S_TTICKS,                 // timer state packed as W_TIMER, valid after S_TTICKS cycles of this step
-  S_WORDS                          // 88
+  S_OBJ = 58,                      // 30 words: cached 160-bit line masks of PF, BL, P0, P1, M0, M1 (5 words each);
+                                   //           a derived cache — also the scratch area of a regroup (vcs_step.cu)
+  S_WORDS = 88,
+  S_MOVED = S_OBJ + 8              // a regroup moves words [0, S_MOVED): the state proper + 8 words of saved CPU registers
 };
 // per-block context, in words after the thread files
 enum CtxWord { C_SCREEN_LO = 0, C_SCREEN_HI, C_Y0, C_FRAMESKIP, C_BATCH, C_ENV0, C_WORDS = 8 };
@@ -84,6 +86,7 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   uint8_t *d_actions_stage;     // for vcs_step_host
   uint8_t *h_pinned; size_t h_pinned_bytes;
   int block;                    // threads (= envs) per block of the interpreter kernel
+  int regroup;                  // F8 blocks re-sort their envs across threads at bank-hotspot accesses
   int rom_smem;                 // every block maps to a single ROM: it is staged in shared memory
   uint32_t max_rom;             // largest ROM image
   long long launches;

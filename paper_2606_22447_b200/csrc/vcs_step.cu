@@ -58,6 +58,7 @@ struct Cpu {
   bool wsync;         // mirror of TF_WSYNC
   // ---- cart
   uint32_t bank, is_f8, rom_mask;
+  uint32_t park;      // bit0: this block regroups its envs at bank-hotspot accesses; bit1: this lane is parked for a regroup
   uint32_t rom_off;   // ROMS: byte offset of the ROM image inside smem
   const uint8_t *rom_g;    // !ROMS: the image in global memory
   const uint32_t *dr;      // decode words of this env's ROM (4096 per bank)
@@ -77,7 +78,8 @@ struct Cpu {
     if constexpr (ROMS) return reinterpret_cast<const uint8_t *>(smem)[rom_off + off];
     else return __ldg(rom_g + off);
   }
-  DEV void hotspot(uint32_t a) { if (is_f8 && (a | 1u) == 0x1FF9u) bank = a & 1u; }
+  // any access to $1FF8/$1FF9 selects the bank; in a block that regroups it also parks the lane (park bit 1)
+  DEV void hotspot(uint32_t a) { if (is_f8 && (a | 1u) == 0x1FF9u) { bank = a & 1u; park |= (park & 1u) << 1; } }
   DEV uint32_t rom_rd(uint32_t a) {            // a = addr & 0x1FFF with A12 set
     hotspot(a);
     return rom_byte((bank << 12) + (a & rom_mask));
@@ -273,6 +275,47 @@ struct Cpu {
     return cyc < lim;                                      // (the cap can fall on the line start reached by WSYNC)
   }
 
+  // ---------------------------------------------------------------- block-wide regroup (F8 divergence)
+  // Called by every thread of the block, converged, when every lane is parked at a bank-hotspot access or has
+  // finished the step.  The block's environments are sorted by (frames done, bank, SP, PC) and MOVED between
+  // threads — shared-memory file words [0, S_MOVED) plus the CPU registers — so that each warp again holds
+  // lanes of one bank at one PC.  Environments are independent, so which thread runs which one is free.
+  DEV void regroup(uint32_t fskip) {
+    const int tid = threadIdx.x;
+    S(S_OBJ + 0) = A | (X << 8) | (Y << 16) | (SP << 24);
+    S(S_OBJ + 1) = PC | (pack_p() << 16) | (status << 24);
+    S(S_OBJ + 2) = (uint32_t)cyc; S(S_OBJ + 3) = (uint32_t)lstart; S(S_OBJ + 4) = (uint32_t)fstart;
+    S(S_OBJ + 5) = fdone | (bank << 8) | ((wsync ? 1u : 0u) << 16);
+    const uint32_t skey = (fdone >= fskip) ? 0xFFFFFFFFu : (min(fdone, 63u) << 25) | (bank << 24) | (SP << 16) | PC;
+    S(S_OBJ + 10) = skey;
+    __syncthreads();
+    uint32_t rank = 0;
+    const uint32_t *keys = smem + (S_OBJ + 10) * BLOCK;
+#pragma unroll 4
+    for (int j = 0; j < BLOCK; ++j) { const uint32_t kj = keys[j]; rank += (kj < skey || (kj == skey && j < tid)) ? 1u : 0u; }
+    constexpr int NB = 11;
+    static_assert(S_MOVED % NB == 0, "batching");
+#pragma unroll 1
+    for (int base = 0; base < S_MOVED; base += NB) {
+      uint32_t t[NB];
+#pragma unroll
+      for (int i = 0; i < NB; ++i) t[i] = smem[(base + i) * BLOCK + tid];
+      __syncthreads();                                     // every file's words [base, base+NB) are in registers
+#pragma unroll
+      for (int i = 0; i < NB; ++i) smem[(base + i) * BLOCK + rank] = t[i];
+    }
+    __syncthreads();
+    uint32_t r;
+    r = S(S_OBJ + 0); A = r & 0xFFu; X = (r >> 8) & 0xFFu; Y = (r >> 16) & 0xFFu; SP = r >> 24;
+    r = S(S_OBJ + 1); PC = r & 0xFFFFu; unpack_p((r >> 16) & 0xFFu); status = r >> 24;
+    cyc = (int32_t)S(S_OBJ + 2); lstart = (int32_t)S(S_OBJ + 3); fstart = (int32_t)S(S_OBJ + 4);
+    r = S(S_OBJ + 5); fdone = r & 0xFFu; bank = (r >> 8) & 1u; wsync = ((r >> 16) & 1u) != 0;
+    S(S_FL) |= TF_DIRTY_ALL;                               // the object-mask cache was the scratch area
+    park &= 1u;
+    relim();
+    w = fetch();
+  }
+
   // ---------------------------------------------------------------- instructions until the next scheduling point
   DEV void run_block(uint32_t fskip) {
     for (;;) {
@@ -455,7 +498,7 @@ struct Cpu {
           for (int i = i0; i < 2; ++i) bus_write(ea, i ? wv : v, k + i);
           total = k + 2; break;
       }
-      brk |= bank != (di >> 12);                           // a hotspot access switched banks: wn is from the old one
+      brk |= (bank != (di >> 12)) | ((park & 2u) != 0);    // a hotspot access: wn may be from the other bank
       PC = npc & 0xFFFFu;
       cyc += total;
       if (status & STATUS_UNMODELLED) lim = LIM_NOW;
@@ -485,10 +528,10 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
   constexpr uint32_t ROM_OFF = (S_WORDS * BLOCK + C_WORDS) * 4;          // byte offset of the ROM image in smem
   const int tid = threadIdx.x;
   const int e0 = blockIdx.x * BLOCK;
-  const int e = e0 + tid;
   const int B = p.batch;
-  const bool live = e < B;
-  const RomMeta rm = p.rom_meta[p.env_rom[live ? e : e0]];
+  const int ei = e0 + tid;                                 // the env this thread starts with
+  const bool live0 = ei < B;
+  const RomMeta rm = p.rom_meta[p.env_rom[live0 ? ei : e0]];
 
   if (tid == 0) {
     const unsigned long long scr = reinterpret_cast<unsigned long long>(p.screen);
@@ -510,32 +553,35 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
   Cpu<BLOCK, ROMS> s;
   // ---- a1 state load (coalesced SoA)
   uint32_t n0 = 0, fl = 0;
-  if (live) {
+  if (live0) {
     uint32_t w;
-    w = p.st[W_AXYS * B + e]; s.A = w & 0xFF; s.X = (w >> 8) & 0xFF; s.Y = (w >> 16) & 0xFF; s.SP = w >> 24;
-    w = p.st[W_PC * B + e]; s.PC = w & 0xFFFF; s.unpack_p((w >> 16) & 0xFF); s.status = w >> 24;
-    w = p.st[W_BEAM * B + e]; n0 = w & 0xFF; T::S(S_LINE) = (w >> 8) & 0xFFFF; s.bank = w >> 24;
-    s.fstart = -(int32_t)p.st[W_FCYC * B + e];
-    T::S(S_TMR) = p.st[W_TIMER * B + e]; T::S(S_TTICKS) = 0;
-    T::S(S_PORTS) = p.st[W_PORTS * B + e];
-    T::S(S_COLU) = p.st[W_COLU * B + e]; T::S(S_PF) = p.st[W_PF * B + e]; T::S(S_GRP) = p.st[W_GRP * B + e]; T::S(S_NUSIZ) = p.st[W_NUSIZ * B + e];
-    T::S(S_POS) = p.st[W_POS * B + e]; w = p.st[W_POS2 * B + e]; T::S(S_POS2) = w & 0xFFFF; T::S(S_RX) = w >> 16;
-    fl = (p.st[W_FLAGS * B + e] & TF_ARCH_MASK) | TF_DIRTY_ALL; T::S(S_CX) = p.st[W_CX * B + e];
+    w = p.st[W_AXYS * B + ei]; s.A = w & 0xFF; s.X = (w >> 8) & 0xFF; s.Y = (w >> 16) & 0xFF; s.SP = w >> 24;
+    w = p.st[W_PC * B + ei]; s.PC = w & 0xFFFF; s.unpack_p((w >> 16) & 0xFF); s.status = w >> 24;
+    w = p.st[W_BEAM * B + ei]; n0 = w & 0xFF; T::S(S_LINE) = (w >> 8) & 0xFFFF; s.bank = w >> 24;
+    s.fstart = -(int32_t)p.st[W_FCYC * B + ei];
+    T::S(S_TMR) = p.st[W_TIMER * B + ei]; T::S(S_TTICKS) = 0;
+    T::S(S_PORTS) = p.st[W_PORTS * B + ei];
+    T::S(S_COLU) = p.st[W_COLU * B + ei]; T::S(S_PF) = p.st[W_PF * B + ei]; T::S(S_GRP) = p.st[W_GRP * B + ei]; T::S(S_NUSIZ) = p.st[W_NUSIZ * B + ei];
+    T::S(S_POS) = p.st[W_POS * B + ei]; w = p.st[W_POS2 * B + ei]; T::S(S_POS2) = w & 0xFFFF; T::S(S_RX) = w >> 16;
+    fl = (p.st[W_FLAGS * B + ei] & TF_ARCH_MASK) | TF_DIRTY_ALL; T::S(S_CX) = p.st[W_CX * B + ei];
     T::S(S_PX) = 0; T::S(S_FDONE) = 0;
-    for (int i = 0; i < 32; ++i) smem[(S_RAM + i) * BLOCK + tid] = p.ram[i * B + e];
+    for (int i = 0; i < 32; ++i) smem[(S_RAM + i) * BLOCK + tid] = p.ram[i * B + ei];
     for (int i = 0; i < 10; ++i) smem[(S_PLANE + i) * BLOCK + tid] = 0;
     if (p.frameskip == 1) { fl |= TF_STORING; if ((T::S(S_LINE) - (uint32_t)p.y0) < (uint32_t)SCR_H) fl |= TF_ROWVIS; }
   } else {
     s.A = s.X = s.Y = s.SP = s.PC = 0; s.unpack_p(0x24); s.status = 0; s.bank = 0; s.fstart = 0;
+    T::S(S_INP) = (uint32_t)tid << 16; T::S(S_FL) = 0; T::S(S_TMR) = 0; T::S(S_TTICKS) = 0;
   }
-  s.cyc = 0; s.lstart = -(int32_t)n0; s.fdone = live ? 0u : (uint32_t)p.frameskip;
+  s.cyc = 0; s.lstart = -(int32_t)n0; s.fdone = live0 ? 0u : (uint32_t)p.frameskip;
   s.cap = p.max_lines * LINE_CYC;
   s.is_f8 = (rm.size == 8192);
+  const bool regroups = ROMS && s.is_f8 && p.regroup;      // block-uniform
+  s.park = regroups ? 1u : 0u;
   s.rom_off = ROM_OFF; s.rom_g = p.rom_blob + rm.offset; s.dr = p.drom + rm.doff; s.tid4 = 4u * (uint32_t)tid;
   s.rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
   // ---- a2 action latch (C.11)
-  if (live) {
-    uint32_t act = p.actions[e]; if (act >= 18u) act = 0;
+  if (live0) {
+    uint32_t act = p.actions[ei]; if (act >= 18u) act = 0;
     //            NOOP FIRE UP RIGHT LEFT DOWN UR UL DR DL UF RF LF DF URF ULF DRF DLF
     const uint32_t up = 0x0C4C4u, down = 0x32320u, left = 0x29290u, right = 0x14948u, fire = 0x3FC02u;
     uint32_t ina = 0xFFu;
@@ -544,7 +590,7 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
     if ((left >> act) & 1u) ina &= ~0x40u;
     if ((right >> act) & 1u) ina &= ~0x80u;
     const uint32_t fire0 = (fire >> act) & 1u;
-    T::S(S_INP) = ina | (fire0 << 8);
+    T::S(S_INP) = ina | (fire0 << 8) | ((uint32_t)tid << 16);
     if ((fl & TF_LATCHEN) && fire0) fl &= ~TF_INPT4_LATCH;
     T::S(S_FL) = fl;
   }
@@ -552,19 +598,26 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
   s.relim();
   if constexpr (ROMS) mbar_wait(smem_u32(&s_bar), 0);
   const uint32_t fskip = (uint32_t)p.frameskip;
-  s.w = live ? s.fetch() : (uint32_t)H_SLOW;
+  s.w = live0 ? s.fetch() : (uint32_t)H_SLOW;
 
   // ---- the hot loop: whole instructions until `frameskip` frame-end events (C.10), min-key lanes first.
   // Line bookkeeping mirrors C.4: the line counter advances with the FIRST cycle of a new line, so an
   // instruction that ends exactly on a line boundary leaves n == 76 pending (a frame end at that point
   // makes the finished line "line 0" and the next one line 1).
   for (;;) {
-    const uint32_t key = (s.fdone >= fskip) ? 0xFFFFFFFFu
-                       : (min(s.fdone, 63u) << 25) | (s.SP << 17) | (s.bank << 16) | s.PC;
-    const uint32_t mk = __reduce_min_sync(0xFFFFFFFFu, key);
-    if (mk == 0xFFFFFFFFu) break;
-    if (key == mk) s.run_block(fskip);
+    for (;;) {
+      const uint32_t key = (s.fdone >= fskip) ? 0xFFFFFFFFu : (s.park & 2u) ? 0xFFFFFFFEu
+                         : (min(s.fdone, 63u) << 25) | (s.SP << 17) | (s.bank << 16) | s.PC;
+      const uint32_t mk = __reduce_min_sync(0xFFFFFFFFu, key);
+      if (mk >= 0xFFFFFFFEu) break;                        // every lane is parked or has finished the step
+      if (key == mk) s.run_block(fskip);
+    }
+    if (!regroups) break;
+    if (!__syncthreads_or((s.park & 2u) && s.fdone < fskip)) break;      // nobody left to run in this block
+    s.regroup(fskip);
   }
+  const int e = e0 + (int)(T::S(S_INP) >> 16);             // the env this thread ends up holding
+  const bool live = e < B;
   if (!live) return;
   if (s.cyc - s.lstart > LINE_CYC) { T::line_end(); s.lstart += LINE_CYC; }      // the last instruction ran over the line end
   // ---- a16 state store

@@ -11,7 +11,7 @@ struct StepParams {
   const uint8_t *rom_blob; const uint32_t *drom; const RomMeta *rom_meta; const int32_t *env_rom;
   const uint8_t *actions;
   int32_t batch, frameskip, y0, max_lines;
-  int32_t block, rom_smem; uint32_t max_rom;     // launch shape: envs per block (64/128/256), ROM staged in smem, largest image
+  int32_t block, rom_smem, regroup; uint32_t max_rom;     // launch shape: envs per block (64/128/256), ROM staged in smem, largest image
 };
 
 void upload_optable();

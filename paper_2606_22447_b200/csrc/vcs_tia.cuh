@@ -61,7 +61,7 @@ struct Tia {
   static DEV uint32_t ctx(int i) { return smem[S_WORDS * BLOCK + i]; }
   static DEV uint8_t *row_ptr(uint32_t r) {
     unsigned long long base = (unsigned long long)ctx(C_SCREEN_LO) | ((unsigned long long)ctx(C_SCREEN_HI) << 32);
-    return reinterpret_cast<uint8_t *>(base) + ((size_t)(ctx(C_ENV0) + threadIdx.x) * SCR_H + r) * SCR_W;
+    return reinterpret_cast<uint8_t *>(base) + ((size_t)(ctx(C_ENV0) + (S(S_INP) >> 16)) * SCR_H + r) * SCR_W;
   }
 
   // ------------------------------------------------------------------ cached object line masks
