@@ -153,7 +153,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   h->regroup = getenv("VCS_NO_REGROUP") ? 0 : 1;
   // pre-decode every byte offset of every bank once (vcs_decode.cuh); the words depend on the launch shape
   // (zero-page RAM operands are stored as shared-memory offsets)
-  std::vector<uint32_t> dw(dwords + 8, 0);
+  std::vector<DWord> dw(dwords + 8, DWord{0, 0});
   {
     std::vector<uint8_t> img(4096 + 4, 0), leader(4096);
     for (int r = 0; r < n_roms; ++r) {
@@ -164,7 +164,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
           if (roms[r].size == 2048) { memcpy(img.data(), roms[r].data, 2048); memcpy(img.data() + 2048, roms[r].data, 2048); }
           else memcpy(img.data(), roms[r].data + 4096 * b, 4096);
           if (pass == 0) mark_leaders(img.data(), leader.data());
-          else decode_bank(img.data(), leader.data(), h->block, dw.data() + meta[r].doff + 4096 * b);
+          else decode_bank(img.data(), leader.data(), h->block, nb == 2, dw.data() + meta[r].doff + 4096 * b);
         }
     }
   }
@@ -175,8 +175,8 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   CU(h, cudaMalloc((void **)&h->d_cyc, sizeof(unsigned long long) * B));
   CU(h, cudaMalloc((void **)&h->d_screen, (size_t)SCR_W * SCR_H * B));
   CU(h, cudaMalloc((void **)&h->d_rom_blob, blob));
-  CU(h, cudaMalloc((void **)&h->d_drom, sizeof(uint32_t) * dw.size()));
-  CU(h, cudaMemcpy(h->d_drom, dw.data(), sizeof(uint32_t) * dw.size(), cudaMemcpyHostToDevice));
+  CU(h, cudaMalloc((void **)&h->d_drom, sizeof(DWord) * dw.size()));
+  CU(h, cudaMemcpy(h->d_drom, dw.data(), sizeof(DWord) * dw.size(), cudaMemcpyHostToDevice));
   CU(h, cudaMalloc((void **)&h->d_rom_meta, sizeof(RomMeta) * n_roms));
   CU(h, cudaMalloc((void **)&h->d_env_rom, sizeof(int32_t) * B));
   CU(h, cudaMalloc((void **)&h->d_seeds, sizeof(unsigned long long) * B));

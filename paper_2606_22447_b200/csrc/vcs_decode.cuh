@@ -1,23 +1,27 @@
 // vcs_decode.cuh — the pre-decoded instruction stream of the CUDA interpreter (shares nothing with oracle/).
 //
-// Cartridge ROM is immutable, so vcs_create decodes every byte offset of every bank ONCE into a 32-bit
-// word; the interpreter kernel then dispatches on a fused handler id instead of walking opcode -> mode ->
+// Cartridge ROM is immutable, so vcs_create decodes every byte offset of every bank ONCE into a 64-bit
+// entry; the interpreter kernel then dispatches on a fused handler id instead of walking opcode -> mode ->
 // operation tables per executed instruction (the paper's cost centre is exactly that dispatch: PAPER.md
 // L584/L592, a 256-way switch per step).  The decode is purely static: it never changes what an instruction
-// does (SURVEY.md C.5 bus sequences), it only picks a specialised handler where the operand address class is
-// known from the instruction bytes alone (immediate, zero-page RAM $80-$FF, zero-page TIA register stores).
+// does (SURVEY.md C.5 bus sequences), it only picks a specialised handler where the operand's address class
+// is known from the instruction bytes alone (immediate, RAM, TIA register stores, RIOT timer reads, fixed
+// ROM bytes), and it carries the instruction's base cycle count and length so that the kernel adds them
+// without looking anything up.
 //
-//   bits  7:0   hid      handler id (enum Hid)
-//   bits 23:8   payload  immediate | smem byte offset of a RAM cell | TIA register | b1|b2<<8 | branch displacement+2
-//   bit  24     leader   a static branch / JMP / JSR target, a JSR return point or the instruction after a static
-//                        bank-hotspot access: the warp re-forms its min-key group before executing it
-//   bits 29:25  op2      second-level operation of a generic handler (read op 0..11, store 0..2, RMW 0..5),
-//                        or the cycles of a taken branch (3 | 4)
-//   bits 31:30  len      instruction length in bytes (1..3; 0 for H_SLOW)
+//   .x  bits  6:0   hid      handler id (enum Hid)
+//       bit   7     leader   a static branch / JMP / JSR target, a JSR return point or the instruction after a
+//                            static bank-hotspot access: the warp re-forms its min-key group before executing it
+//       bits 15:8   cy       base cycles (0 for the generic handlers, which count their own bus accesses)
+//       bits 23:16  len      instruction length in bytes (0 for H_SLOW / H_ILL)
+//       bits 31:24  op2      second-level operation of a generic handler (read op 0..11, store 0..2, RMW 0..5),
+//                            or the extra cycles of a taken branch (1 | 2)
+//   .y  payload     immediate | smem byte offset of a RAM cell | TIA register | b1|b2<<8 | signed branch displacement
 //
-// Offsets >= 0xFF0 of a bank (wrap-around, F8 hotspots inside the instruction bytes) and every PC outside
-// cartridge space decode to H_SLOW: the kernel then fetches byte-wise with side effects and builds the
-// word at run time from c_gen[] (generic handlers only).
+// Offsets >= 0xFF0 of a bank (wrap-around, F8 hotspots inside the instruction bytes), branches that leave
+// the 4 KB window or whose dummy reads can touch a hotspot, and every PC outside cartridge space decode to
+// H_SLOW: the kernel then fetches byte-wise with side effects and builds the entry at run time from c_gen[]
+// (generic handlers only).
 #pragma once
 #include <stdint.h>
 #include "vcs_optable.cuh"
@@ -26,93 +30,115 @@ namespace vcs {
 
 enum Hid : uint32_t {
   H_SLOW = 0,
-  H_IMM0 = 1,        // +0..10: LDA LDX LDY AND ORA EOR ADC SBC CMP CPX CPY #imm
-  H_ZR0 = 12,        // +0..11: LDA .. CPY, BIT  zp ($80-$FF: RAM)
-  H_STZR0 = 24,      // +0..2 : STA STX STY zp RAM
-  H_STZT0 = 27,      // +0..2 : STA STX STY zp TIA register (payload = register, one with an effect)
-  H_NOP3 = 30,       // a zp store to a TIA address without effect (audio, RSYNC, $2D-$3F)
-  H_MZR0 = 31,       // +0..5 : ASL LSR ROL ROR INC DEC zp RAM
+  H_IMM0 = 1,        // +0..10: LDA LDX LDY AND ORA EOR ADC SBC CMP CPX CPY #imm (also: absolute reads of a fixed ROM byte)
+  H_ZR0 = 12,        // +0..11: LDA .. CPY, BIT  RAM cell (zp $80-$FF, or an absolute address that decodes to RAM)
+  H_STZR0 = 24,      // +0..2 : STA STX STY RAM cell
+  H_STZT0 = 27,      // +0..2 : STA STX STY TIA register (payload = register, one with an effect), written in the last cycle
+  H_NOP = 30,        // no effect beyond its cycles (NOP; a store to a TIA address without effect: audio, RSYNC, $2D-$3F)
+  H_MZR0 = 31,       // +0..5 : ASL LSR ROL ROR INC DEC RAM cell
   H_ACC0 = 37,       // +0..3 : ASL LSR ROL ROR A
-  H_IMP0 = 41,       // +0..17: CLC SEC CLD SED CLI SEI CLV NOP DEX DEY INX INY TAX TAY TSX TXA TYA TXS
+  H_IMP0 = 41,       // +0..17: CLC SEC CLD SED CLI SEI CLV (NOP) DEX DEY INX INY TAX TAY TSX TXA TYA TXS
   H_BR0 = 59,        // +0..7 : BPL BMI BVC BVS BCC BCS BNE BEQ
   H_JMP = 67, H_JSR, H_RTS, H_PHA, H_PHP, H_PLA, H_PLP,
   H_R0 = 74,         // generic reads : +0..8  IMM ZP ZPX ZPY ABS ABX ABY IZX IZY   (op2 = read op)
   H_W0 = 83,         // generic stores: +0..7  ZP ZPX ZPY ABS ABX ABY IZX IZY       (op2 = STA STX STY)
   H_M0 = 91,         // generic RMW   : +0..3  ZP ZPX ABS ABX                       (op2 = ASL .. DEC)
   H_JMPI = 95, H_RTI, H_BRK, H_ILL,
+  H_RTIM = 99,       // absolute read of INTIM / TIMINT (payload = address, op2 = read op)
   H_COUNT
 };
+static_assert(H_COUNT <= 128, "hid is 7 bits");
 
-constexpr uint32_t DW_LEADER = 1u << 24;
-constexpr int DW_OP2_SHIFT = 25, DW_LEN_SHIFT = 30;
+constexpr uint32_t DW_LEADER = 1u << 7;
+constexpr int DW_CY_SHIFT = 8, DW_LEN_SHIFT = 16, DW_OP2_SHIFT = 24;
 constexpr uint32_t DW_SLOW_LIMIT = 0xFF0;      // bank offsets >= this decode to H_SLOW
 
-// generic (address-class agnostic) decode of one opcode: hid | op2<<8 | len<<13.  Used on the host as the base
-// of every decode word and on the device (c_gen) by the byte-wise slow fetch.
-inline uint16_t generic_entry(uint32_t opc) {
+struct DWord { uint32_t x, y; };
+
+constexpr uint32_t dw_x(uint32_t hid, uint32_t cy, uint32_t len, uint32_t op2) {
+  return hid | (cy << DW_CY_SHIFT) | (len << DW_LEN_SHIFT) | (op2 << DW_OP2_SHIFT);
+}
+
+// generic (address-class agnostic) decode of one opcode in the .x format.  Used on the host as the base of
+// every decode entry and on the device (c_gen) by the byte-wise slow fetch.
+inline uint32_t generic_entry(uint32_t opc) {
   const uint32_t ent = kOpTable[opc], mode = ent & 15u, op = (ent >> 4) & 63u, kind = ent >> 10;
-  uint32_t hid = H_ILL, op2 = 0, len = 1;
   static const uint8_t mode_len[13] = {1, 1, 2, 2, 2, 2, 3, 3, 3, 2, 2, 2, 1};
-  len = mode_len[mode];
-  if (op == OP_ILL) { hid = H_ILL; len = 1; }
-  else if (mode == MD_SPC) {
+  uint32_t len = mode_len[mode];
+  if (op == OP_ILL) return dw_x(H_ILL, 1, 0, 0);
+  if (mode == MD_SPC) {
     switch (op) {
-      case OP_JMP: hid = H_JMP; len = 3; break;   case OP_JMPI: hid = H_JMPI; len = 3; break;
-      case OP_JSR: hid = H_JSR; len = 3; break;   case OP_RTS: hid = H_RTS; break;
-      case OP_RTI: hid = H_RTI; break;            case OP_PHA: hid = H_PHA; break;
-      case OP_PHP: hid = H_PHP; break;            case OP_PLA: hid = H_PLA; break;
-      case OP_PLP: hid = H_PLP; break;            default: hid = H_BRK; len = 2; break;
+      case OP_JMP: return dw_x(H_JMP, 3, 3, 0);    case OP_JMPI: return dw_x(H_JMPI, 5, 3, 0);
+      case OP_JSR: return dw_x(H_JSR, 6, 3, 0);    case OP_RTS: return dw_x(H_RTS, 6, 1, 0);
+      case OP_RTI: return dw_x(H_RTI, 6, 1, 0);    case OP_PHA: return dw_x(H_PHA, 3, 1, 0);
+      case OP_PHP: return dw_x(H_PHP, 3, 1, 0);    case OP_PLA: return dw_x(H_PLA, 4, 1, 0);
+      case OP_PLP: return dw_x(H_PLP, 4, 1, 0);    default: return dw_x(H_BRK, 7, 2, 0);
     }
   }
-  else if (mode == MD_REL) hid = H_BR0 + (op - OP_BPL);
-  else if (mode == MD_IMP) hid = H_IMP0 + (op - OP_CLC);
-  else if (mode == MD_ACC) hid = H_ACC0 + (op - OP_ASL);
-  else if (kind == K_READ) { hid = H_R0 + (mode - MD_IMM); op2 = op - OP_LDA; }
-  else if (kind == K_WRITE) { hid = H_W0 + (mode - MD_ZP); op2 = op - OP_STA; }
-  else {                                          // K_RMW: zp, zpx, abs, abx
-    const uint32_t mi = (mode == MD_ZP) ? 0u : (mode == MD_ZPX) ? 1u : (mode == MD_ABS) ? 2u : 3u;
-    hid = H_M0 + mi; op2 = op - OP_ASL;
-  }
-  return (uint16_t)(hid | (op2 << 8) | (len << 13));
+  if (mode == MD_REL) return dw_x(H_BR0 + (op - OP_BPL), 2, 2, 1);
+  if (mode == MD_IMP) return (op == OP_NOP) ? dw_x(H_NOP, 2, 1, 0) : dw_x(H_IMP0 + (op - OP_CLC), 2, 1, 0);
+  if (mode == MD_ACC) return dw_x(H_ACC0 + (op - OP_ASL), 2, 1, 0);
+  if (kind == K_READ) return dw_x(H_R0 + (mode - MD_IMM), 0, len, op - OP_LDA);
+  if (kind == K_WRITE) return dw_x(H_W0 + (mode - MD_ZP), 0, len, op - OP_STA);
+  const uint32_t mi = (mode == MD_ZP) ? 0u : (mode == MD_ZPX) ? 1u : (mode == MD_ABS) ? 2u : 3u;   // K_RMW
+  return dw_x(H_M0 + mi, 0, len, op - OP_ASL);
 }
 
 inline bool tia_write_has_effect(uint32_t r) {    // r = address & 0x3F (SURVEY C.8 write map)
   return !(r > 0x2Cu || (r >= 0x15u && r <= 0x1Au) || r == 0x03u);
 }
+inline bool is_hotspot(uint32_t a13) { return (a13 | 1u) == 0x1FF9u; }
 
-// One bank image (4096 bytes; 2 KB carts are passed mirrored) -> 4096 decode words.  `leader` is the bank-
+// One bank image (4096 bytes; 2 KB carts are passed mirrored) -> 4096 decode entries.  `leader` is the bank-
 // independent leader bitmap (4096 flags) filled by mark_leaders() for every bank of the cartridge first.
-inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, uint32_t *out) {
+inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, bool f8, DWord *out) {
   for (uint32_t off = 0; off < 4096; ++off) {
-    if (off >= DW_SLOW_LIMIT) { out[off] = H_SLOW | (leader[off] ? DW_LEADER : 0u); continue; }
+    const uint32_t lead = leader[off] ? DW_LEADER : 0u;
+    if (off >= DW_SLOW_LIMIT) { out[off].x = H_SLOW | lead; out[off].y = 0; continue; }
     const uint32_t opc = img[off], b1 = img[off + 1], b2 = img[off + 2];
     const uint32_t ent = kOpTable[opc], mode = ent & 15u, op = (ent >> 4) & 63u, kind = ent >> 10;
-    const uint16_t g = generic_entry(opc);
-    uint32_t hid = g & 0xFFu, op2 = (g >> 8) & 31u;
-    const uint32_t len = g >> 13;
+    uint32_t x = generic_entry(opc);
+    const uint32_t len = (x >> DW_LEN_SHIFT) & 0xFFu;
     uint32_t payload = (len == 3) ? (b1 | (b2 << 8)) : (len == 2) ? b1 : 0u;
+    const uint32_t abs13 = (b1 | (b2 << 8)) & 0x1FFFu;
+    const bool zp = (mode == MD_ZP), ab = (mode == MD_ABS);
+    const uint32_t cyz = zp ? 0u : 1u;                                     // absolute = zero page + 1 cycle
     if (op != OP_ILL) {
-      if (mode == MD_IMM) { hid = H_IMM0 + (op - OP_LDA); op2 = 0; }
-      else if (mode == MD_ZP && b1 >= 0x80u) {
-        payload = ((b1 & 0x7Cu) * (uint32_t)block) | (b1 & 3u);          // byte offset of the cell in the RAM words
-        if (kind == K_READ) hid = H_ZR0 + (op - OP_LDA);
-        else if (kind == K_WRITE) hid = H_STZR0 + (op - OP_STA);
-        else hid = H_MZR0 + (op - OP_ASL);
-        op2 = 0;
+      const uint32_t a13 = zp ? b1 : abs13;
+      const bool is_ram = zp ? (b1 >= 0x80u) : (ab && (a13 & 0x1280u) == 0x0080u);
+      if (mode == MD_IMM) x = dw_x(H_IMM0 + (op - OP_LDA), 2, 2, 0);
+      else if ((zp || ab) && is_ram) {
+        payload = ((a13 & 0x7Cu) * (uint32_t)block) | (a13 & 3u);          // byte offset of the cell in the RAM words
+        if (kind == K_READ) x = dw_x(H_ZR0 + (op - OP_LDA), 3 + cyz, len, 0);
+        else if (kind == K_WRITE) x = dw_x(H_STZR0 + (op - OP_STA), 3 + cyz, len, 0);
+        else x = dw_x(H_MZR0 + (op - OP_ASL), 5 + cyz, len, 0);
       }
-      else if (mode == MD_ZP && kind == K_WRITE) {                         // b1 < 0x80: a TIA register
-        const uint32_t r = b1 & 0x3Fu;
-        if (tia_write_has_effect(r)) { hid = H_STZT0 + (op - OP_STA); payload = r; }
-        else { hid = H_NOP3; payload = 0; }
-        op2 = 0;
+      else if ((zp || ab) && kind == K_WRITE && (a13 & 0x1080u) == 0) {    // a TIA register
+        const uint32_t r = a13 & 0x3Fu;
+        if (tia_write_has_effect(r)) { x = dw_x(H_STZT0 + (op - OP_STA), 3 + cyz, len, 0); payload = r; }
+        else { x = dw_x(H_NOP, 3 + cyz, len, 0); payload = 0; }
+      }
+      else if (ab && kind == K_READ && (a13 & 0x1284u) == 0x0284u) {       // INTIM / TIMINT
+        x = dw_x(H_RTIM, 4, 3, op - OP_LDA); payload = a13;
+      }
+      else if (ab && kind == K_READ && op != OP_BIT && (a13 & 0x1000u) && !(f8 && is_hotspot(a13))) {   // a fixed ROM byte
+        x = dw_x(H_IMM0 + (op - OP_LDA), 4, 3, 0); payload = img[a13 & 0xFFFu];                        // of this bank
       }
       else if (mode == MD_REL) {
-        const uint32_t next = 0x1000u + off + 2u, target = (next + (uint32_t)(int32_t)(int8_t)b1) & 0xFFFFu;
-        payload = (2u + (uint32_t)(int32_t)(int8_t)b1) & 0xFFFFu;
-        op2 = ((target ^ next) & 0xFF00u) ? 4u : 3u;
+        const int32_t disp = (int32_t)(int8_t)b1;
+        const int32_t toff = (int32_t)off + 2 + disp;                      // target offset inside the 4 KB window
+        const uint32_t next = 0x1000u + off + 2u, target = (uint32_t)((int32_t)next + disp);
+        const uint32_t dummy2 = (next & 0xFF00u) | (target & 0xFFu);
+        if (toff < 0 || toff >= 4096 || (f8 && (is_hotspot(next & 0x1FFFu) || is_hotspot(dummy2 & 0x1FFFu))))
+          x = H_SLOW;                                                      // run-time decode keeps every side effect
+        else {
+          payload = (uint32_t)disp;
+          x = (x & 0x00FFFFFFu) | ((((target ^ next) & 0xFF00u) ? 2u : 1u) << DW_OP2_SHIFT);
+        }
       }
     }
-    out[off] = hid | (payload << 8) | (leader[off] ? DW_LEADER : 0u) | (op2 << DW_OP2_SHIFT) | (len << DW_LEN_SHIFT);
+    if ((x & 0x7Fu) == H_SLOW) { out[off].x = H_SLOW | lead; out[off].y = 0; }
+    else { out[off].x = x | lead; out[off].y = payload; }
   }
 }
 

@@ -11,6 +11,7 @@
 // Machine model: SURVEY.md §8(c) C.1 (state), restated in DESIGN.md §2.
 #pragma once
 #include <stdint.h>
+#include <cuda_runtime.h>
 
 namespace vcs {
 
@@ -82,7 +83,7 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   int32_t batch, n_roms;
   int32_t y0, max_lines, f8_start_bank;
   uint32_t *d_st; uint32_t *d_ram; unsigned long long *d_cyc; uint8_t *d_screen;
-  uint8_t *d_rom_blob; uint32_t *d_drom; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
+  uint8_t *d_rom_blob; uint2 *d_drom; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
   uint8_t *d_actions_stage;     // for vcs_step_host
   uint8_t *h_pinned; size_t h_pinned_bytes;
   int block;                    // threads (= envs) per block of the interpreter kernel

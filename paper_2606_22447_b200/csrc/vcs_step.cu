@@ -5,12 +5,16 @@
 // planes live in the thread's shared-memory file; the block's cartridge ROM is staged in shared memory with
 // one bulk asynchronous copy (TMA 1-D, cp.async.bulk + mbarrier) when all of the block's envs share a ROM.
 //
-// Dispatch.  vcs_create pre-decodes every byte offset of every ROM bank into a 32-bit word (vcs_decode.cuh):
-// a fused handler id, the operand (already turned into a shared-memory offset for zero-page RAM), the
-// instruction length and a "leader" flag.  The hot loop loads that word through the read-only path (L1),
-// prefetches the sequentially next one before it dispatches, and jumps ONCE (one BRX) into a handler that is
-// specialised for opcode x address class; only indexed / indirect / absolute modes take a second-level
-// operation switch.  PCs outside cartridge space and the last 16 bytes of a bank decode at run time (H_SLOW).
+// Dispatch.  vcs_create pre-decodes every byte offset of every ROM bank into a 64-bit entry (vcs_decode.cuh):
+// a fused handler id, the instruction's base cycles and length, a "leader" flag and a 32-bit operand (already
+// turned into a shared-memory offset for RAM cells).  The hot loop loads that entry through the read-only
+// path (L1), prefetches the sequentially next one before it dispatches, adds cycles and length straight from
+// the entry and jumps ONCE (one BRX) into a handler that is specialised for opcode x address class; only
+// indexed / indirect / absolute-I/O modes take a second-level operation switch and count their own bus
+// accesses.  PCs outside cartridge space and the last 16 bytes of a bank decode at run time (H_SLOW).
+//
+// The program counter is kept as (di, pbase): di = bank<<12 | PC & 0xFFF indexes the decode entries and
+// PC = (pbase + di) & 0xFFFF; straight-line code and in-window branches only touch di.
 //
 // Divergence (the measured choice north_star asks for): lanes of a warp are NOT run in lock-step.  At every
 // scheduling point each lane forms the key (frames done, SP, bank, PC); a warp-wide REDUX.MIN picks the
@@ -22,31 +26,36 @@
 // or return point — the only places where another lane can be waiting), so the REDUX is paid per basic
 // block, not per instruction.
 //
-// Cycle accounting is per bus access (C.4/C.5): an access `k` cycles into the instruction happens in cycle
-// `cyc + k`, scanline slot `cyc - lstart + k`.
+// Cycle accounting is per bus access (C.4/C.5).  Specialised handlers add the entry's cycle count before
+// they run (their one side-effecting access is the last cycle: cycle index cyc - 1 afterwards); generic
+// handlers run with `cyc` at the instruction's first cycle, an access `k` cycles into the instruction
+// happens in cycle `cyc + k`, scanline slot `cyc - lstart + k`, and add their total at the end.
 #include "vcs_tia.cuh"
 #include "vcs_decode.cuh"
 #include "vcs_step.cuh"
 
 namespace vcs {
 
-__constant__ uint16_t c_gen[256];       // generic decode per opcode (vcs_decode.cuh generic_entry) for H_SLOW
+__constant__ uint32_t c_gen[256];       // generic decode per opcode (vcs_decode.cuh generic_entry) for H_SLOW
 
 void upload_optable() {
-  uint16_t g[256];
+  uint32_t g[256];
   for (int i = 0; i < 256; ++i) g[i] = generic_entry((uint32_t)i);
   cudaMemcpyToSymbol(c_gen, g, sizeof(g));
 }
 const uint16_t *host_optable() { return kOpTable; }
 
 constexpr int32_t LIM_NOW = (int32_t)0x80000000;     // `lim` value that forces the slow pre-check
+constexpr uint32_t KEY_PARKED = 0xFFFE0000u;         // keys >= this: parked for a regroup / finished the step
+constexpr uint32_t NOSLOT = 0xFFFFFFFFu;             // a thread of the spare warp that holds no environment right now
 
-template <int BLOCK, bool ROMS>
+template <int BLOCK, bool ROMS, int THREADS>
 struct Cpu {
   using T = Tia<BLOCK>;
   // ---- CPU
-  uint32_t A, X, Y, SP, PC;
-  uint32_t fC, fV, fDI, zv, nv;        // fDI: bit3 D, bit2 I ; Z <=> (zv & 0xFF) == 0 ; N <=> nv & 0x80
+  uint32_t A, X, Y, SP;
+  uint32_t di, pbase;                  // PC = (pbase + di) & 0xFFFF ; di = bank<<12 | PC & 0xFFF
+  uint32_t fC, fV, fDI, zn;            // fDI: bit3 D, bit2 I ; Z <=> (zn & 0xFF) == 0 ; N <=> (zn & 0x180) != 0
   uint32_t status;
   // ---- beam / time (cycle counts are relative to the start of this vcs_step call)
   int32_t cyc;        // CPU cycles executed in this step
@@ -55,21 +64,30 @@ struct Cpu {
   int32_t lim;        // fast path allowed while cyc < lim: min(line end, frame cap), LIM_NOW when WSYNC/halted
   int32_t cap;        // frame cap in cycles
   uint32_t fdone;     // frames completed in this step (mirror of S_FDONE)
+  uint32_t fskip;     // frames to run
+  uint32_t keyhi;     // scheduling key without the PC: frames done << 25 | SP << 17 | bank << 16 (or KEY_PARKED / ~0)
   bool wsync;         // mirror of TF_WSYNC
   // ---- cart
-  uint32_t bank, is_f8, rom_mask;
-  uint32_t park;      // bit0: this block regroups its envs at bank-hotspot accesses; bit1: this lane is parked for a regroup
+  uint32_t is_f8, rom_mask;
+  uint32_t park;      // bit0: this block regroups its envs at bank-hotspot accesses; bit1: this lane is parked for a
+                      // regroup; bit2: a bank hotspot was accessed by the instruction in flight
   uint32_t rom_off;   // ROMS: byte offset of the ROM image inside smem
   const uint8_t *rom_g;    // !ROMS: the image in global memory
-  const uint32_t *dr;      // decode words of this env's ROM (4096 per bank)
-  uint32_t w;         // decode word at (bank, PC) — valid at every scheduling point
-  uint32_t tid4;      // 4 * threadIdx.x
+  const uint2 *dr;         // decode entries of this env's ROM (4096 per bank)
+  uint2 w;            // decode entry at (bank, PC) — valid at every scheduling point
+  uint32_t sl, sl4;   // this thread's file slot (word i of the file lives at smem[i*BLOCK + sl]) and 4*sl
 
-  static DEV uint32_t &S(int i) { return T::S(i); }
+  DEV uint32_t &S(int i) const { return T::S(sl, i); }
+
+  DEV uint32_t pc() const { return (pbase + di) & 0xFFFFu; }
+  DEV void set_pc(uint32_t p) { const uint32_t nd = (di & 0x1000u) | (p & 0xFFFu); pbase = p - nd; di = nd; }
+  DEV void rekey() {
+    keyhi = (fdone >= fskip) ? 0xFFFFFFFFu : (park & 2u) ? KEY_PARKED : (min(fdone, 63u) << 25) | (SP << 17) | ((di & 0x1000u) << 4);
+  }
 
   // ------------------------------------------------------------------ RAM (smem, conflict-free)
-  DEV uint32_t ram_rd_off(uint32_t off) const { return reinterpret_cast<const uint8_t *>(smem)[off + tid4]; }
-  DEV void ram_wr_off(uint32_t off, uint32_t v) { reinterpret_cast<uint8_t *>(smem)[off + tid4] = (uint8_t)v; }
+  DEV uint32_t ram_rd_off(uint32_t off) const { return reinterpret_cast<const uint8_t *>(smem)[off + sl4]; }
+  DEV void ram_wr_off(uint32_t off, uint32_t v) { reinterpret_cast<uint8_t *>(smem)[off + sl4] = (uint8_t)v; }
   DEV uint32_t ram_rd(uint32_t a) const { return ram_rd_off(((a & 0x7Cu) * BLOCK) | (a & 3u)); }
   DEV void ram_wr(uint32_t a, uint32_t v) { ram_wr_off(((a & 0x7Cu) * BLOCK) | (a & 3u), v); }
 
@@ -79,15 +97,22 @@ struct Cpu {
     else return __ldg(rom_g + off);
   }
   // any access to $1FF8/$1FF9 selects the bank; in a block that regroups it also parks the lane (park bit 1)
-  DEV void hotspot(uint32_t a) { if (is_f8 && (a | 1u) == 0x1FF9u) { bank = a & 1u; park |= (park & 1u) << 1; } }
+  DEV void hotspot(uint32_t a) {
+    if (is_f8 && (a | 1u) == 0x1FF9u) {
+      const uint32_t nd = (di & 0xFFFu) | ((a & 1u) << 12);
+      pbase += di - nd; di = nd;                     // PC is unchanged
+      park |= 4u | ((park & 1u) << 1);
+      rekey();
+    }
+  }
   DEV uint32_t rom_rd(uint32_t a) {            // a = addr & 0x1FFF with A12 set
     hotspot(a);
-    return rom_byte((bank << 12) + (a & rom_mask));
+    return rom_byte((di & 0x1000u) + (a & rom_mask));
   }
-  // decode word at (bank, PC); H_SLOW outside cartridge space
-  DEV uint32_t fetch() const {
-    if (!(PC & 0x1000u)) return H_SLOW;
-    return __ldg(dr + ((bank << 12) | (PC & 0xFFFu)));
+  // decode entry at (bank, PC); H_SLOW outside cartridge space
+  DEV uint2 fetch() const {
+    if (!((pbase + di) & 0x1000u)) return make_uint2(H_SLOW, 0);
+    return __ldg(dr + di);
   }
 
   // ------------------------------------------------------------------ RIOT timer, closed form (C.7)
@@ -109,7 +134,21 @@ struct Cpu {
     sub = (sub + d) & mask;
   }
   DEV void timer_put(uint32_t timer, uint32_t sub, uint32_t shift, uint32_t tflag) { S(S_TMR) = timer | (shift << 8) | (tflag << 12) | (sub << 16); }
-  DEV uint32_t riot_read(uint32_t a, int32_t c) {     // access in cycle index c (tick c happened first)
+  // INTIM / TIMINT read in cycle index c (tick c happened first)
+  DEV uint32_t timer_read(uint32_t a, int32_t c) {
+    const uint32_t tw = S(S_TMR);
+    const uint32_t d = (uint32_t)(c + 1 - (int32_t)S(S_TTICKS));
+    if (!(tw & 0x1000u) && (int32_t)d > 0) {          // before the underflow nothing has to be written back
+      const uint32_t timer = tw & 0xFFu, k = ((tw >> 16) + d) >> ((tw >> 8) & 0xFu);
+      if (k <= timer) return (a & 1u) ? 0u : timer - k;
+    }
+    uint32_t timer, sub, shift, tflag;
+    timer_sync(c + 1, timer, sub, shift, tflag);
+    if (!(a & 1u)) { timer_put(timer, sub, shift, 0); return timer; }         // INTIM clears the flag
+    timer_put(timer, sub, shift, tflag);
+    return tflag << 7;                                                        // TIMINT
+  }
+  DEV uint32_t riot_read(uint32_t a, int32_t c) {     // access in cycle index c
     if ((a & 4u) == 0) {
       const uint32_t ports = S(S_PORTS);
       const uint32_t ora = byte_of(ports, 0), ddra = byte_of(ports, 1), orb = byte_of(ports, 2), ddrb = byte_of(ports, 3);
@@ -120,11 +159,7 @@ struct Cpu {
         default: return ddrb;
       }
     }
-    uint32_t timer, sub, shift, tflag;
-    timer_sync(c + 1, timer, sub, shift, tflag);
-    if ((a & 5u) == 4u) { timer_put(timer, sub, shift, 0); return timer; }   // INTIM clears the flag
-    timer_put(timer, sub, shift, tflag);
-    return tflag << 7;                                                        // TIMINT
+    return timer_read(a, c);
   }
   DEV void riot_write(uint32_t a, uint32_t v, int32_t c) {
     if ((a & 4u) == 0) { S(S_PORTS) = set_byte(S(S_PORTS), a & 3u, v); return; }
@@ -137,20 +172,21 @@ struct Cpu {
 
   // side-effect-light read used for instruction bytes, zero-page pointers, JMP() vectors and stack
   // pulls: cartridge (incl. F8 hotspots) or RAM.  Anything else is outside the modelled set (status bit 2).
+  DEV void unmodelled() { status |= STATUS_UNMODELLED; lim = LIM_NOW; }
   DEV uint32_t lite_rd(uint32_t addr) {
     const uint32_t a = addr & 0x1FFFu;
     if (a & 0x1000u) return rom_rd(a);
     if ((a & 0x0280u) == 0x0080u) return ram_rd(a);
-    status |= STATUS_UNMODELLED; return 0;
+    unmodelled(); return 0;
   }
   DEV void push(uint32_t v) {
-    if (SP & 0x80u) ram_wr(SP, v); else status |= STATUS_UNMODELLED;
+    if (SP & 0x80u) ram_wr(SP, v); else unmodelled();
     SP = (SP - 1u) & 0xFFu;
   }
   DEV uint32_t pull() {
     SP = (SP + 1u) & 0xFFu;
     if (SP & 0x80u) return ram_rd(SP);
-    status |= STATUS_UNMODELLED; return 0;
+    unmodelled(); return 0;
   }
   // dummy read of an indexed mode's uncorrected address in cycle cyc+k: only INTIM and F8 hotspots react
   DEV void dummy_rd(uint32_t addr, int k) {
@@ -162,20 +198,25 @@ struct Cpu {
   DEV void relim() {
     lim = (wsync || (status & (STATUS_ILLEGAL | STATUS_UNMODELLED))) ? LIM_NOW : min(lstart + LINE_CYC, fstart + cap);
   }
-  DEV void tia_events(uint32_t ev, int k) {        // after a TIA write k cycles into the instruction
+  // after a TIA access that reported events; fc = cycle count at which a frame that just ended did so
+  DEV void tia_events(uint32_t ev, int32_t fc) {
     lstart += LINE_CYC * (int32_t)(ev >> 4);
     wsync = (ev & EV_WSYNC) != 0;
-    if (ev & EV_FRAME) { fdone += 1; fstart = cyc + k + 1; }
+    if (ev & EV_FRAME) { fdone += 1; fstart = fc; rekey(); }
     relim();
   }
-  DEV void tia_write(uint32_t r, uint32_t v, int k) { tia_events(T::write(r, v, cyc - lstart + k), k); }
+  // generic handlers: a TIA write k cycles into the instruction (cyc = its first cycle)
+  DEV void tia_write(uint32_t r, uint32_t v, int k) {
+    const uint32_t ev = T::write(sl, r, v, cyc - lstart + k);
+    if (ev) tia_events(ev, cyc + k + 1);
+  }
   // the generic operand read (C.3 decode), k cycles into the instruction
   DEV uint32_t bus_read(uint32_t addr, int k) {
     const uint32_t a = addr & 0x1FFFu;
     if ((a & 0x1280u) == 0x0080u) return ram_rd(a);
     if (a & 0x1000u) return rom_rd(a);
     if (a & 0x0080u) return riot_read(a, cyc + k);
-    const uint32_t r = T::read(a & 0xFu, cyc - lstart + k);
+    const uint32_t r = T::read(sl, a & 0xFu, cyc - lstart + k);
     if (r >> 12) { lstart += LINE_CYC * (int32_t)(r >> 12); wsync = false; relim(); }
     return r & 0xFFu;
   }
@@ -189,25 +230,24 @@ struct Cpu {
     tia_write(r, v, k);
   }
   DEV uint32_t pack_p() const {
-    return (nv & 0x80u) | (fV << 6) | 0x20u | fDI | (((zv & 0xFFu) == 0) ? 2u : 0u) | fC;
+    return ((zn & 0x180u) ? 0x80u : 0u) | (fV << 6) | 0x20u | fDI | (((zn & 0xFFu) == 0) ? 2u : 0u) | fC;
   }
   DEV void unpack_p(uint32_t p) {
-    fC = p & 1u; zv = (p & 2u) ? 0u : 1u; fDI = p & 0x0Cu; fV = (p >> 6) & 1u; nv = p & 0x80u;
+    fC = p & 1u; zn = ((p & 0x80u) << 1) | ((p & 2u) ? 0u : 1u); fDI = p & 0x0Cu; fV = (p >> 6) & 1u;
   }
   DEV void adc(uint32_t v) {                               // C.6, binary and NMOS decimal
     const uint32_t a = A, C = fC;
     if (!(fDI & 8u)) {
       const uint32_t s = a + v + C;
-      fC = s >> 8; fV = ((a ^ s) & (v ^ s) & 0x80u) >> 7; A = s & 0xFFu; zv = nv = A;
+      fC = s >> 8; fV = ((a ^ s) & (v ^ s) & 0x80u) >> 7; A = s & 0xFFu; zn = A;
       return;
     }
     int al = (int)(a & 0x0Fu) + (int)(v & 0x0Fu) + (int)C;
     if (al >= 0x0A) al = ((al + 6) & 0x0F) + 0x10;
     int s = (int)(a & 0xF0u) + (int)(v & 0xF0u) + al;
     const int sv = (int)(int8_t)(a & 0xF0u) + (int)(int8_t)(v & 0xF0u) + al;
-    nv = (uint32_t)s & 0x80u;
+    zn = (((a + v + C) & 0xFFu) ? 1u : 0u) | (((uint32_t)s & 0x80u) << 1);   // Z from the binary sum, N from the high-nibble sum
     fV = (sv < -128 || sv > 127) ? 1u : 0u;
-    zv = (a + v + C) & 0xFFu;
     if (s >= 0xA0) s += 0x60;
     fC = (s >= 0x100) ? 1u : 0u;
     A = (uint32_t)s & 0xFFu;
@@ -216,7 +256,7 @@ struct Cpu {
     const uint32_t a = A, C = fC;
     const uint32_t nb = v ^ 0xFFu, s = a + nb + C;         // flags exactly as binary
     const uint32_t bin = s & 0xFFu;
-    fC = s >> 8; fV = ((a ^ s) & (nb ^ s) & 0x80u) >> 7; zv = nv = bin;
+    fC = s >> 8; fV = ((a ^ s) & (nb ^ s) & 0x80u) >> 7; zn = bin;
     if (!(fDI & 8u)) { A = bin; return; }
     int al = (int)(a & 0x0Fu) - (int)(v & 0x0Fu) + (int)C - 1;
     if (al < 0) al = ((al - 6) & 0x0F) - 0x10;
@@ -224,20 +264,22 @@ struct Cpu {
     if (d < 0) d -= 0x60;
     A = (uint32_t)d & 0xFFu;
   }
+  DEV void cmp(uint32_t r, uint32_t v) { fC = (r >= v) ? 1u : 0u; zn = (r - v) & 0xFFu; }
+  DEV void bit(uint32_t v) { zn = (A & v) | ((v & 0x80u) << 1); fV = (v >> 6) & 1u; }
   DEV void read_op(uint32_t o, uint32_t v) {               // o = op - OP_LDA
     switch (o) {
-      case 0: A = v; zv = nv = v; break;
-      case 1: X = v; zv = nv = v; break;
-      case 2: Y = v; zv = nv = v; break;
-      case 3: A &= v; zv = nv = A; break;
-      case 4: A |= v; zv = nv = A; break;
-      case 5: A ^= v; zv = nv = A; break;
+      case 0: A = v; zn = v; break;
+      case 1: X = v; zn = v; break;
+      case 2: Y = v; zn = v; break;
+      case 3: A &= v; zn = A; break;
+      case 4: A |= v; zn = A; break;
+      case 5: A ^= v; zn = A; break;
       case 6: adc(v); break;
       case 7: sbc(v); break;
-      case 8: fC = (A >= v) ? 1u : 0u; zv = nv = (A - v) & 0xFFu; break;
-      case 9: fC = (X >= v) ? 1u : 0u; zv = nv = (X - v) & 0xFFu; break;
-      case 10: fC = (Y >= v) ? 1u : 0u; zv = nv = (Y - v) & 0xFFu; break;
-      default: zv = A & v; nv = v; fV = (v >> 6) & 1u; break;
+      case 8: cmp(A, v); break;
+      case 9: cmp(X, v); break;
+      case 10: cmp(Y, v); break;
+      default: bit(v); break;
     }
   }
   DEV uint32_t rmw_op(uint32_t o, uint32_t s) {            // o = op - OP_ASL
@@ -250,7 +292,7 @@ struct Cpu {
       case 4: r = (s + 1u) & 0xFFu; break;
       default: r = (s - 1u) & 0xFFu; break;
     }
-    zv = nv = r;
+    zn = r;
     return r;
   }
 
@@ -258,18 +300,18 @@ struct Cpu {
   // entered when cyc >= lim.  Returns false when no instruction may run now (a frame ended at the cap, or
   // the CPU is halted and idled): the lane goes back to the scheduling point.
   DEV bool slow_pre() {
-    if (cyc - lstart > LINE_CYC) { T::line_end(); lstart += LINE_CYC; wsync = false; }     // the previous instruction ran over the line end
+    if (cyc - lstart > LINE_CYC) { T::line_end(sl); lstart += LINE_CYC; wsync = false; }     // the previous instruction ran over the line end
     if (cyc - fstart >= cap) {                             // frame cap at the instruction boundary
-      status |= STATUS_CAP; T::frame_end(3u * (uint32_t)(cyc - lstart)); fdone += 1; fstart = cyc;
-      relim(); return false;
+      status |= STATUS_CAP; T::frame_end(sl, 3u * (uint32_t)(cyc - lstart)); fdone += 1; fstart = cyc;
+      rekey(); relim(); return false;
     }
-    if (cyc - lstart >= LINE_CYC) { T::line_end(); lstart += LINE_CYC; wsync = false; }     // n == 76 exactly
+    if (cyc - lstart >= LINE_CYC) { T::line_end(sl); lstart += LINE_CYC; wsync = false; }     // n == 76 exactly
     if (status & (STATUS_ILLEGAL | STATUS_UNMODELLED)) {   // halted: idle cycles to the line end / the cap
       cyc += min(LINE_CYC - (cyc - lstart), cap - (cyc - fstart));
       return false;
     }
     if (wsync) {                                           // a12: RDY holds the CPU until the line ends
-      cyc = lstart + LINE_CYC; T::line_end(); lstart = cyc; wsync = false;
+      cyc = lstart + LINE_CYC; T::line_end(sl); lstart = cyc; wsync = false;
     }
     relim();
     return cyc < lim;                                      // (the cap can fall on the line start reached by WSYNC)
@@ -280,115 +322,142 @@ struct Cpu {
   // finished the step.  The block's environments are sorted by (frames done, bank, SP, PC) and MOVED between
   // threads — shared-memory file words [0, S_MOVED) plus the CPU registers — so that each warp again holds
   // lanes of one bank at one PC.  Environments are independent, so which thread runs which one is free.
-  DEV void regroup(uint32_t fskip) {
-    const int tid = threadIdx.x;
-    S(S_OBJ + 0) = A | (X << 8) | (Y << 16) | (SP << 24);
-    S(S_OBJ + 1) = PC | (pack_p() << 16) | (status << 24);
-    S(S_OBJ + 2) = (uint32_t)cyc; S(S_OBJ + 3) = (uint32_t)lstart; S(S_OBJ + 4) = (uint32_t)fstart;
-    S(S_OBJ + 5) = fdone | (bank << 8) | ((wsync ? 1u : 0u) << 16);
-    const uint32_t skey = (fdone >= fskip) ? 0xFFFFFFFFu : (min(fdone, 63u) << 25) | (bank << 24) | (SP << 16) | PC;
-    S(S_OBJ + 10) = skey;
+  DEV void regroup() {
+    const bool has = sl != NOSLOT;
+    uint32_t skey = 0xFFFFFFFFu;
+    if (has) {
+      const uint32_t bank = di >> 12, PC = pc();
+      S(S_OBJ + 0) = A | (X << 8) | (Y << 16) | (SP << 24);
+      S(S_OBJ + 1) = PC | (pack_p() << 16) | (status << 24);
+      S(S_OBJ + 2) = (uint32_t)cyc; S(S_OBJ + 3) = (uint32_t)lstart; S(S_OBJ + 4) = (uint32_t)fstart;
+      S(S_OBJ + 5) = fdone | (bank << 8) | ((wsync ? 1u : 0u) << 16);
+      skey = (fdone >= fskip) ? 0xFFFFFFFFu : (min(fdone, 63u) << 25) | (bank << 24) | (SP << 16) | PC;
+      S(S_OBJ + 6) = skey;
+    }
     __syncthreads();
     uint32_t rank = 0;
-    const uint32_t *keys = smem + (S_OBJ + 10) * BLOCK;
+    const uint32_t *keys = smem + (S_OBJ + 6) * BLOCK;
+    if (has) {
 #pragma unroll 4
-    for (int j = 0; j < BLOCK; ++j) { const uint32_t kj = keys[j]; rank += (kj < skey || (kj == skey && j < tid)) ? 1u : 0u; }
+      for (int j = 0; j < BLOCK; ++j) { const uint32_t kj = keys[j]; rank += (kj < skey || (kj == skey && (uint32_t)j < sl)) ? 1u : 0u; }
+    }
     constexpr int NB = 11;
     static_assert(S_MOVED % NB == 0, "batching");
 #pragma unroll 1
     for (int base = 0; base < S_MOVED; base += NB) {
       uint32_t t[NB];
+      if (has) {
 #pragma unroll
-      for (int i = 0; i < NB; ++i) t[i] = smem[(base + i) * BLOCK + tid];
+        for (int i = 0; i < NB; ++i) t[i] = smem[(base + i) * BLOCK + sl];
+      }
       __syncthreads();                                     // every file's words [base, base+NB) are in registers
+      if (has) {
 #pragma unroll
-      for (int i = 0; i < NB; ++i) smem[(base + i) * BLOCK + rank] = t[i];
+        for (int i = 0; i < NB; ++i) smem[(base + i) * BLOCK + rank] = t[i];
+      }
     }
     __syncthreads();
-    uint32_t r;
-    r = S(S_OBJ + 0); A = r & 0xFFu; X = (r >> 8) & 0xFFu; Y = (r >> 16) & 0xFFu; SP = r >> 24;
-    r = S(S_OBJ + 1); PC = r & 0xFFFFu; unpack_p((r >> 16) & 0xFFu); status = r >> 24;
-    cyc = (int32_t)S(S_OBJ + 2); lstart = (int32_t)S(S_OBJ + 3); fstart = (int32_t)S(S_OBJ + 4);
-    r = S(S_OBJ + 5); fdone = r & 0xFFu; bank = (r >> 8) & 1u; wsync = ((r >> 16) & 1u) != 0;
-    S(S_FL) |= TF_DIRTY_ALL;                               // the object-mask cache was the scratch area
+    // which file this thread runs next.  With a spare warp the lowest (frames done, bank) class gets whole warps of
+    // its own and everything else is packed behind it from the next warp boundary on, so that no warp mixes the two
+    // banks; slots inside a warp stay consecutive, hence bank-conflict free.
+    uint32_t ns = threadIdx.x;
+    if constexpr (THREADS != BLOCK) {
+      const uint32_t c0 = keys[0] >> 24;
+      uint32_t n0 = 0;
+#pragma unroll 4
+      for (int j = 0; j < BLOCK; ++j) n0 += ((keys[j] >> 24) == c0) ? 1u : 0u;
+      const uint32_t t0 = ((n0 + 31u) >> 5) << 5, t = threadIdx.x;
+      if (t < t0) ns = (t < n0) ? t : NOSLOT;
+      else { ns = n0 + (t - t0); if (ns >= (uint32_t)BLOCK) ns = NOSLOT; }
+      __syncthreads();                                     // the keys sit in the object-mask cache: nobody resumes before all have read them
+    }
+    sl = ns; sl4 = 4u * ns;
     park &= 1u;
-    relim();
-    w = fetch();
+    if (sl != NOSLOT) {
+      uint32_t r;
+      r = S(S_OBJ + 0); A = r & 0xFFu; X = (r >> 8) & 0xFFu; Y = (r >> 16) & 0xFFu; SP = r >> 24;
+      r = S(S_OBJ + 1); const uint32_t npc = r & 0xFFFFu; unpack_p((r >> 16) & 0xFFu); status = r >> 24;
+      cyc = (int32_t)S(S_OBJ + 2); lstart = (int32_t)S(S_OBJ + 3); fstart = (int32_t)S(S_OBJ + 4);
+      r = S(S_OBJ + 5); fdone = r & 0xFFu; wsync = ((r >> 16) & 1u) != 0;
+      di = (((r >> 8) & 1u) << 12) | (npc & 0xFFFu); pbase = npc - di;
+      S(S_FL) |= TF_DIRTY_ALL;                             // the object-mask cache was the scratch area
+      rekey(); relim();
+      w = fetch();
+    } else {
+      fdone = fskip; wsync = false; status = 0; di = 0; pbase = 0;
+      rekey();
+    }
   }
 
   // ---------------------------------------------------------------- instructions until the next scheduling point
-  DEV void run_block(uint32_t fskip) {
+  DEV void run_block() {
     for (;;) {
       if (cyc >= lim) { if (!slow_pre()) return; }
-      const uint32_t pc = PC;
-      uint32_t cw = w;                                     // the word being executed
-      uint32_t hid = cw & 0xFFu;
-      uint32_t pl = (cw >> 8) & 0xFFFFu;
-      const uint32_t di = (bank << 12) | (pc & 0xFFFu);
-      uint32_t wn = 0;                                     // sequential prefetch (valid when hid != H_SLOW)
-      bool seq = hid != H_SLOW;
-      if (seq) wn = __ldg(dr + di + (cw >> DW_LEN_SHIFT));
-      uint32_t npc = pc + (cw >> DW_LEN_SHIFT);
-      int total = 2;
-      bool brk = false;                                    // control transfer / bank access: refetch and re-schedule
-      uint32_t ea = 0, v = 0, wv = 0;
-      int k = 0, i0 = 0;
-      if (hid == H_SLOW) {                                 // byte-wise fetch with side effects, run-time decode
-        const uint32_t opc = lite_rd(pc);
-        const uint32_t g = c_gen[opc];
-        const uint32_t len = g >> 13;
-        hid = g & 0xFFu;
-        uint32_t b1 = 0, b2 = 0;
-        if (hid != H_ILL) { b1 = lite_rd(pc + 1u); if (len == 3) b2 = lite_rd(pc + 2u); }
-        pl = b1 | (b2 << 8);
-        cw = ((g >> 8) & 31u) << DW_OP2_SHIFT;
-        if (hid >= H_BR0 && hid < H_BR0 + 8) {
-          const uint32_t next = (pc + 2u) & 0xFFFFu, target = (next + (uint32_t)(int32_t)(int8_t)b1) & 0xFFFFu;
-          pl = (2u + (uint32_t)(int32_t)(int8_t)b1) & 0xFFFFu;
-          cw = (((target ^ next) & 0xFF00u) ? 4u : 3u) << DW_OP2_SHIFT;
-        }
-        npc = pc + len;
-        brk = true;
-      }
-      const uint32_t op2 = (cw >> DW_OP2_SHIFT) & 31u;
+      uint32_t cx = w.x, pl = w.y;                         // the entry being executed
+      di += (cx >> DW_LEN_SHIFT) & 0xFFu;
+      uint2 wn = __ldg(dr + di);                           // sequential prefetch
+      cyc += (int32_t)((cx >> DW_CY_SHIFT) & 0xFFu);
+      bool slow = false;                                   // run-time decoded: always refetch and re-schedule afterwards
+      uint32_t ea = 0, v = 0, wv = 0, op2 = 0, hid;
+      int k = 0, i0 = 0, total = 0;
+    dispatch:
+      hid = cx & 0x7Fu;
       switch (hid) {
-        // ---- immediate
-        case H_IMM0 + 0: A = pl; zv = nv = pl; break;
-        case H_IMM0 + 1: X = pl; zv = nv = pl; break;
-        case H_IMM0 + 2: Y = pl; zv = nv = pl; break;
-        case H_IMM0 + 3: A &= pl; zv = nv = A; break;
-        case H_IMM0 + 4: A |= pl; zv = nv = A; break;
-        case H_IMM0 + 5: A ^= pl; zv = nv = A; break;
+        case H_SLOW: {                                     // byte-wise fetch with side effects, run-time decode
+          const uint32_t pc0 = pc();
+          const uint32_t opc = lite_rd(pc0);
+          uint32_t g = c_gen[opc];
+          const uint32_t ln = (g >> DW_LEN_SHIFT) & 0xFFu;
+          uint32_t b1 = 0, b2 = 0;
+          if ((g & 0x7Fu) != H_ILL) { b1 = lite_rd(pc0 + 1u); if (ln == 3) b2 = lite_rd(pc0 + 2u); }
+          pl = b1 | (b2 << 8);
+          if ((g & 0x7Fu) >= H_BR0 && (g & 0x7Fu) < H_BR0 + 8) {
+            const uint32_t next = (pc0 + 2u) & 0xFFFFu, target = (next + (uint32_t)(int32_t)(int8_t)b1) & 0xFFFFu;
+            pl = (uint32_t)(int32_t)(int8_t)b1;
+            g = (g & 0x00FFFFFFu) | ((((target ^ next) & 0xFF00u) ? 2u : 1u) << DW_OP2_SHIFT);
+          }
+          set_pc((pc0 + ln) & 0xFFFFu);
+          cyc += (int32_t)((g >> DW_CY_SHIFT) & 0xFFu);
+          cx = g; slow = true; wn.x = DW_LEADER;
+          goto dispatch;
+        }
+        // ---- immediate (or a fixed ROM byte)
+        case H_IMM0 + 0: A = pl; zn = pl; break;
+        case H_IMM0 + 1: X = pl; zn = pl; break;
+        case H_IMM0 + 2: Y = pl; zn = pl; break;
+        case H_IMM0 + 3: A &= pl; zn = A; break;
+        case H_IMM0 + 4: A |= pl; zn = A; break;
+        case H_IMM0 + 5: A ^= pl; zn = A; break;
         case H_IMM0 + 6: adc(pl); break;
         case H_IMM0 + 7: sbc(pl); break;
-        case H_IMM0 + 8: fC = (A >= pl) ? 1u : 0u; zv = nv = (A - pl) & 0xFFu; break;
-        case H_IMM0 + 9: fC = (X >= pl) ? 1u : 0u; zv = nv = (X - pl) & 0xFFu; break;
-        case H_IMM0 + 10: fC = (Y >= pl) ? 1u : 0u; zv = nv = (Y - pl) & 0xFFu; break;
-        // ---- zero-page RAM reads (3 cycles)
-        case H_ZR0 + 0: A = ram_rd_off(pl); zv = nv = A; total = 3; break;
-        case H_ZR0 + 1: X = ram_rd_off(pl); zv = nv = X; total = 3; break;
-        case H_ZR0 + 2: Y = ram_rd_off(pl); zv = nv = Y; total = 3; break;
-        case H_ZR0 + 3: A &= ram_rd_off(pl); zv = nv = A; total = 3; break;
-        case H_ZR0 + 4: A |= ram_rd_off(pl); zv = nv = A; total = 3; break;
-        case H_ZR0 + 5: A ^= ram_rd_off(pl); zv = nv = A; total = 3; break;
-        case H_ZR0 + 6: adc(ram_rd_off(pl)); total = 3; break;
-        case H_ZR0 + 7: sbc(ram_rd_off(pl)); total = 3; break;
-        case H_ZR0 + 8: v = ram_rd_off(pl); fC = (A >= v) ? 1u : 0u; zv = nv = (A - v) & 0xFFu; total = 3; break;
-        case H_ZR0 + 9: v = ram_rd_off(pl); fC = (X >= v) ? 1u : 0u; zv = nv = (X - v) & 0xFFu; total = 3; break;
-        case H_ZR0 + 10: v = ram_rd_off(pl); fC = (Y >= v) ? 1u : 0u; zv = nv = (Y - v) & 0xFFu; total = 3; break;
-        case H_ZR0 + 11: v = ram_rd_off(pl); zv = A & v; nv = v; fV = (v >> 6) & 1u; total = 3; break;
-        // ---- zero-page RAM stores
-        case H_STZR0 + 0: ram_wr_off(pl, A); total = 3; break;
-        case H_STZR0 + 1: ram_wr_off(pl, X); total = 3; break;
-        case H_STZR0 + 2: ram_wr_off(pl, Y); total = 3; break;
-        // ---- zero-page TIA register stores (write in the 3rd cycle)
-        case H_STZT0 + 0: tia_write(pl, A, 2); total = 3; break;
-        case H_STZT0 + 1: tia_write(pl, X, 2); total = 3; break;
-        case H_STZT0 + 2: tia_write(pl, Y, 2); total = 3; break;
-        case H_NOP3: total = 3; break;
-        // ---- zero-page RAM read-modify-write (5 cycles)
+        case H_IMM0 + 8: cmp(A, pl); break;
+        case H_IMM0 + 9: cmp(X, pl); break;
+        case H_IMM0 + 10: cmp(Y, pl); break;
+        // ---- RAM cell reads
+        case H_ZR0 + 0: A = ram_rd_off(pl); zn = A; break;
+        case H_ZR0 + 1: X = ram_rd_off(pl); zn = X; break;
+        case H_ZR0 + 2: Y = ram_rd_off(pl); zn = Y; break;
+        case H_ZR0 + 3: A &= ram_rd_off(pl); zn = A; break;
+        case H_ZR0 + 4: A |= ram_rd_off(pl); zn = A; break;
+        case H_ZR0 + 5: A ^= ram_rd_off(pl); zn = A; break;
+        case H_ZR0 + 6: adc(ram_rd_off(pl)); break;
+        case H_ZR0 + 7: sbc(ram_rd_off(pl)); break;
+        case H_ZR0 + 8: cmp(A, ram_rd_off(pl)); break;
+        case H_ZR0 + 9: cmp(X, ram_rd_off(pl)); break;
+        case H_ZR0 + 10: cmp(Y, ram_rd_off(pl)); break;
+        case H_ZR0 + 11: bit(ram_rd_off(pl)); break;
+        // ---- RAM cell stores
+        case H_STZR0 + 0: ram_wr_off(pl, A); break;
+        case H_STZR0 + 1: ram_wr_off(pl, X); break;
+        case H_STZR0 + 2: ram_wr_off(pl, Y); break;
+        // ---- TIA register stores (the write is the instruction's last cycle)
+        case H_STZT0 + 0: v = A; goto tia_store;
+        case H_STZT0 + 1: v = X; goto tia_store;
+        case H_STZT0 + 2: v = Y; goto tia_store;
+        case H_NOP: break;
+        // ---- RAM cell read-modify-write
         case H_MZR0 + 0: case H_MZR0 + 1: case H_MZR0 + 2: case H_MZR0 + 3: case H_MZR0 + 4: case H_MZR0 + 5:
-          ram_wr_off(pl, rmw_op(hid - H_MZR0, ram_rd_off(pl))); total = 5; break;
+          ram_wr_off(pl, rmw_op(hid - H_MZR0, ram_rd_off(pl))); break;
         case H_ACC0 + 0: case H_ACC0 + 1: case H_ACC0 + 2: case H_ACC0 + 3: A = rmw_op(hid - H_ACC0, A); break;
         // ---- implied
         case H_IMP0 + 0: fC = 0; break;
@@ -399,43 +468,38 @@ struct Cpu {
         case H_IMP0 + 5: fDI |= 4u; break;
         case H_IMP0 + 6: fV = 0; break;
         case H_IMP0 + 7: break;
-        case H_IMP0 + 8: X = (X - 1u) & 0xFFu; zv = nv = X; break;
-        case H_IMP0 + 9: Y = (Y - 1u) & 0xFFu; zv = nv = Y; break;
-        case H_IMP0 + 10: X = (X + 1u) & 0xFFu; zv = nv = X; break;
-        case H_IMP0 + 11: Y = (Y + 1u) & 0xFFu; zv = nv = Y; break;
-        case H_IMP0 + 12: X = A; zv = nv = X; break;
-        case H_IMP0 + 13: Y = A; zv = nv = Y; break;
-        case H_IMP0 + 14: X = SP; zv = nv = X; break;
-        case H_IMP0 + 15: A = X; zv = nv = A; break;
-        case H_IMP0 + 16: A = Y; zv = nv = A; break;
-        case H_IMP0 + 17: SP = X; break;
-        // ---- branches: payload = displacement + 2, op2 = cycles when taken
-        case H_BR0 + 0: case H_BR0 + 1: case H_BR0 + 2: case H_BR0 + 3: case H_BR0 + 4: case H_BR0 + 5: case H_BR0 + 6: case H_BR0 + 7: {
-          const uint32_t idx = hid - H_BR0; uint32_t f;
-          switch (idx >> 1) { case 0: f = (nv >> 7) & 1u; break; case 1: f = fV; break; case 2: f = fC; break;
-                              default: f = ((zv & 0xFFu) == 0) ? 1u : 0u; break; }
-          brk = true;
-          if (f == (idx & 1u)) {
-            const uint32_t target = (pc + pl) & 0xFFFFu;
-            if (is_f8) {                                   // the dummy reads @PC and @(old PCH : new PCL)
-              const uint32_t next = (pc + 2u) & 0xFFFFu;
-              hotspot(next & 0x1FFFu);
-              if (op2 == 4u) hotspot(((next & 0xFF00u) | (target & 0xFFu)) & 0x1FFFu);
-            }
-            total = (int)op2; npc = target;
-          }
-        } break;
+        case H_IMP0 + 8: X = (X - 1u) & 0xFFu; zn = X; break;
+        case H_IMP0 + 9: Y = (Y - 1u) & 0xFFu; zn = Y; break;
+        case H_IMP0 + 10: X = (X + 1u) & 0xFFu; zn = X; break;
+        case H_IMP0 + 11: Y = (Y + 1u) & 0xFFu; zn = Y; break;
+        case H_IMP0 + 12: X = A; zn = X; break;
+        case H_IMP0 + 13: Y = A; zn = Y; break;
+        case H_IMP0 + 14: X = SP; zn = X; break;
+        case H_IMP0 + 15: A = X; zn = A; break;
+        case H_IMP0 + 16: A = Y; zn = A; break;
+        case H_IMP0 + 17: SP = X; rekey(); break;
+        // ---- branches: payload = signed displacement, op2 = extra cycles when taken
+        case H_BR0 + 0: if (zn & 0x180u) break; goto br_taken;
+        case H_BR0 + 1: if (!(zn & 0x180u)) break; goto br_taken;
+        case H_BR0 + 2: if (fV) break; goto br_taken;
+        case H_BR0 + 3: if (!fV) break; goto br_taken;
+        case H_BR0 + 4: if (fC) break; goto br_taken;
+        case H_BR0 + 5: if (!fC) break; goto br_taken;
+        case H_BR0 + 6: if (!(zn & 0xFFu)) break; goto br_taken;
+        case H_BR0 + 7: if (zn & 0xFFu) break; goto br_taken;
         // ---- control transfers and stack
-        case H_JMP: npc = pl; total = 3; brk = true; break;
-        case H_JSR: { const uint32_t ret = (pc + 2u) & 0xFFFFu;     // address of the 3rd byte
-          push(ret >> 8); push(ret & 0xFFu); npc = pl; total = 6; brk = true; } break;
+        case H_JMP: set_pc(pl); goto ctl;
+        case H_JSR: { const uint32_t ret = (pc() - 1u) & 0xFFFFu;     // address of the 3rd byte
+          push(ret >> 8); push(ret & 0xFFu); rekey(); set_pc(pl); } goto ctl;
         case H_RTS: { const uint32_t lo = pull(), hi = pull(); const uint32_t r = lo | (hi << 8);
-          hotspot(r & 0x1FFFu); npc = r + 1u; total = 6; brk = true; } break;
-        case H_PHA: push(A); total = 3; break;
-        case H_PHP: push(pack_p() | 0x30u); total = 3; break;
-        case H_PLA: A = pull(); zv = nv = A; total = 4; break;
-        case H_PLP: unpack_p(pull()); total = 4; break;
-        // ---- generic addressing: reads
+          rekey(); hotspot(r & 0x1FFFu); set_pc((r + 1u) & 0xFFFFu); } goto ctl;
+        case H_PHA: push(A); rekey(); break;
+        case H_PHP: push(pack_p() | 0x30u); rekey(); break;
+        case H_PLA: A = pull(); zn = A; rekey(); break;
+        case H_PLP: unpack_p(pull()); rekey(); break;
+        // ---- absolute read of INTIM / TIMINT (4th cycle)
+        case H_RTIM: read_op(cx >> DW_OP2_SHIFT, timer_read(pl, cyc - 1)); break;
+        // ---- generic addressing: reads (cyc = first cycle of the instruction; they add `total` themselves)
         case H_R0 + 0: v = pl & 0xFFu; total = 2; goto do_read_op;
         case H_R0 + 1: ea = pl & 0xFFu; k = 2; goto do_read;
         case H_R0 + 2: ea = (pl + X) & 0xFFu; k = 3; goto do_read;
@@ -474,37 +538,58 @@ struct Cpu {
           ea = (unc + (t & 0x100u)) & 0xFFFFu; dummy_rd(unc, 3); k = 4; } goto do_rmw;
         // ---- rare
         case H_JMPI: { const uint32_t l2 = lite_rd(pl), h2 = lite_rd((pl & 0xFF00u) | ((pl + 1u) & 0xFFu));   // no carry into the page
-          npc = l2 | (h2 << 8); total = 5; brk = true; } break;
-        case H_RTI: { unpack_p(pull()); const uint32_t lo = pull(), hi = pull(); npc = lo | (hi << 8); total = 6; brk = true; } break;
-        case H_BRK: { const uint32_t ret = (pc + 2u) & 0xFFFFu;
-          push(ret >> 8); push(ret & 0xFFu); push(pack_p() | 0x30u);
-          npc = lite_rd(0xFFFEu) | (lite_rd(0xFFFFu) << 8); fDI |= 4u; total = 7; brk = true; } break;
+          set_pc(l2 | (h2 << 8)); } goto ctl;
+        case H_RTI: { unpack_p(pull()); const uint32_t lo = pull(), hi = pull(); rekey(); set_pc(lo | (hi << 8)); } goto ctl;
+        case H_BRK: { const uint32_t ret = pc();             // address of the opcode + 2
+          push(ret >> 8); push(ret & 0xFFu); push(pack_p() | 0x30u); rekey();
+          const uint32_t l2 = lite_rd(0xFFFEu), h2 = lite_rd(0xFFFFu);
+          set_pc(l2 | (h2 << 8)); fDI |= 4u; } goto ctl;
         default:                                           // H_ILL — C.12: halt for good, PC stays
           if (!(status & STATUS_UNMODELLED)) status |= STATUS_ILLEGAL;
-          npc = pc; total = 1; brk = true; lim = LIM_NOW; break;
+          lim = LIM_NOW; goto ctl;
         do_read:
           v = bus_read(ea, k); total = k + 1;
         do_read_op:
-          read_op(op2, v); break;
+          read_op(cx >> DW_OP2_SHIFT, v); goto gen_end;
         do_write:
+          op2 = cx >> DW_OP2_SHIFT;
           wv = (op2 == 0) ? A : (op2 == 1) ? X : Y;
           i0 = 1; k -= 1; goto do_store;
         do_rmw:
           v = bus_read(ea, k);
-          wv = rmw_op(op2, v);
+          wv = rmw_op(cx >> DW_OP2_SHIFT, v);
           i0 = 0; k += 1;
         do_store:                                          // the one generic write site: [old value,] new value (C.5)
 #pragma unroll 1
           for (int i = i0; i < 2; ++i) bus_write(ea, i ? wv : v, k + i);
-          total = k + 2; break;
+          total = k + 2;
+        gen_end:
+          cyc += total;
+          if ((park & 4u) || fdone >= fskip) goto ctl;     // a bank hotspot was touched (the prefetched entry may be the other bank's)
+          break;
+        br_taken:
+          if (slow) {                                      // the dummy reads @PC and @(old PCH : new PCL), any target
+            const uint32_t next = pc(), target = (next + pl) & 0xFFFFu;
+            hotspot(next & 0x1FFFu);
+            if ((cx >> DW_OP2_SHIFT) == 2u) hotspot(((next & 0xFF00u) | (target & 0xFFu)) & 0x1FFFu);
+            set_pc(target);
+          } else di += pl;
+          cyc += (int32_t)(cx >> DW_OP2_SHIFT);
+          goto ctl;
+        tia_store: {
+          const uint32_t ev = T::write(sl, pl, v, cyc - 1 - lstart);
+          if (ev) { tia_events(ev, cyc); if (ev & EV_FRAME) goto ctl; }
+        } break;
       }
-      brk |= (bank != (di >> 12)) | ((park & 2u) != 0);    // a hotspot access: wn may be from the other bank
-      PC = npc & 0xFFFFu;
-      cyc += total;
-      if (status & STATUS_UNMODELLED) lim = LIM_NOW;
-      if (fdone >= fskip) return;
-      if (seq && !brk) { w = wn; if (w & DW_LEADER) return; }
-      else { w = fetch(); return; }
+      // ---- sequential successor
+      w = wn;
+      if (!(w.x & DW_LEADER)) continue;
+      if (slow) w = fetch();
+      return;
+    ctl:                                                   // control transfer, bank access or frame end: refetch, re-schedule
+      park &= ~4u;
+      w = fetch();
+      return;
     }
   }
 };
@@ -520,8 +605,8 @@ DEV void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile("{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @!p bra WAIT_%=;\n}" ::"r"(bar), "r"(parity) : "memory");
 }
 
-template <int BLOCK, bool ROMS>
-__global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams p) {
+template <int BLOCK, bool ROMS, int THREADS>
+__global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepParams p) {
   using T = Tia<BLOCK>;
   __shared__ __align__(8) unsigned long long s_bar;
   uint32_t *s_ctx = smem + S_WORDS * BLOCK;
@@ -530,7 +615,8 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
   const int e0 = blockIdx.x * BLOCK;
   const int B = p.batch;
   const int ei = e0 + tid;                                 // the env this thread starts with
-  const bool live0 = ei < B;
+  const bool filed = tid < BLOCK;                          // threads of the spare warp start without a file
+  const bool live0 = filed && ei < B;
   const RomMeta rm = p.rom_meta[p.env_rom[live0 ? ei : e0]];
 
   if (tid == 0) {
@@ -550,34 +636,38 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
     }
   }
 
-  Cpu<BLOCK, ROMS> s;
+  Cpu<BLOCK, ROMS, THREADS> s;
+  s.sl = filed ? (uint32_t)tid : NOSLOT; s.sl4 = 4u * s.sl;
+  const uint32_t sl = s.sl;
   // ---- a1 state load (coalesced SoA)
-  uint32_t n0 = 0, fl = 0;
+  uint32_t n0 = 0, fl = 0, pc0 = 0, bank0 = 0;
   if (live0) {
     uint32_t w;
     w = p.st[W_AXYS * B + ei]; s.A = w & 0xFF; s.X = (w >> 8) & 0xFF; s.Y = (w >> 16) & 0xFF; s.SP = w >> 24;
-    w = p.st[W_PC * B + ei]; s.PC = w & 0xFFFF; s.unpack_p((w >> 16) & 0xFF); s.status = w >> 24;
-    w = p.st[W_BEAM * B + ei]; n0 = w & 0xFF; T::S(S_LINE) = (w >> 8) & 0xFFFF; s.bank = w >> 24;
+    w = p.st[W_PC * B + ei]; pc0 = w & 0xFFFF; s.unpack_p((w >> 16) & 0xFF); s.status = w >> 24;
+    w = p.st[W_BEAM * B + ei]; n0 = w & 0xFF; T::S(sl, S_LINE) = (w >> 8) & 0xFFFF; bank0 = (w >> 24) & 1u;
     s.fstart = -(int32_t)p.st[W_FCYC * B + ei];
-    T::S(S_TMR) = p.st[W_TIMER * B + ei]; T::S(S_TTICKS) = 0;
-    T::S(S_PORTS) = p.st[W_PORTS * B + ei];
-    T::S(S_COLU) = p.st[W_COLU * B + ei]; T::S(S_PF) = p.st[W_PF * B + ei]; T::S(S_GRP) = p.st[W_GRP * B + ei]; T::S(S_NUSIZ) = p.st[W_NUSIZ * B + ei];
-    T::S(S_POS) = p.st[W_POS * B + ei]; w = p.st[W_POS2 * B + ei]; T::S(S_POS2) = w & 0xFFFF; T::S(S_RX) = w >> 16;
-    fl = (p.st[W_FLAGS * B + ei] & TF_ARCH_MASK) | TF_DIRTY_ALL; T::S(S_CX) = p.st[W_CX * B + ei];
-    T::S(S_PX) = 0; T::S(S_FDONE) = 0;
+    T::S(sl, S_TMR) = p.st[W_TIMER * B + ei]; T::S(sl, S_TTICKS) = 0;
+    T::S(sl, S_PORTS) = p.st[W_PORTS * B + ei];
+    T::S(sl, S_COLU) = p.st[W_COLU * B + ei]; T::S(sl, S_PF) = p.st[W_PF * B + ei]; T::S(sl, S_GRP) = p.st[W_GRP * B + ei]; T::S(sl, S_NUSIZ) = p.st[W_NUSIZ * B + ei];
+    T::S(sl, S_POS) = p.st[W_POS * B + ei]; w = p.st[W_POS2 * B + ei]; T::S(sl, S_POS2) = w & 0xFFFF; T::S(sl, S_RX) = w >> 16;
+    fl = (p.st[W_FLAGS * B + ei] & TF_ARCH_MASK) | TF_DIRTY_ALL; T::S(sl, S_CX) = p.st[W_CX * B + ei];
+    T::S(sl, S_PX) = 0; T::S(sl, S_FDONE) = 0;
     for (int i = 0; i < 32; ++i) smem[(S_RAM + i) * BLOCK + tid] = p.ram[i * B + ei];
     for (int i = 0; i < 10; ++i) smem[(S_PLANE + i) * BLOCK + tid] = 0;
-    if (p.frameskip == 1) { fl |= TF_STORING; if ((T::S(S_LINE) - (uint32_t)p.y0) < (uint32_t)SCR_H) fl |= TF_ROWVIS; }
+    if (p.frameskip == 1) { fl |= TF_STORING; if ((T::S(sl, S_LINE) - (uint32_t)p.y0) < (uint32_t)SCR_H) fl |= TF_ROWVIS; }
   } else {
-    s.A = s.X = s.Y = s.SP = s.PC = 0; s.unpack_p(0x24); s.status = 0; s.bank = 0; s.fstart = 0;
-    T::S(S_INP) = (uint32_t)tid << 16; T::S(S_FL) = 0; T::S(S_TMR) = 0; T::S(S_TTICKS) = 0;
+    s.A = s.X = s.Y = s.SP = 0; s.unpack_p(0x24); s.status = 0; s.fstart = 0;
+    if (filed) { T::S(sl, S_INP) = (uint32_t)tid << 16; T::S(sl, S_FL) = 0; T::S(sl, S_TMR) = 0; T::S(sl, S_TTICKS) = 0; }
   }
-  s.cyc = 0; s.lstart = -(int32_t)n0; s.fdone = live0 ? 0u : (uint32_t)p.frameskip;
+  s.di = (bank0 << 12) | (pc0 & 0xFFFu); s.pbase = pc0 - s.di;
+  s.fskip = (uint32_t)p.frameskip;
+  s.cyc = 0; s.lstart = -(int32_t)n0; s.fdone = live0 ? 0u : s.fskip;
   s.cap = p.max_lines * LINE_CYC;
   s.is_f8 = (rm.size == 8192);
   const bool regroups = ROMS && s.is_f8 && p.regroup;      // block-uniform
   s.park = regroups ? 1u : 0u;
-  s.rom_off = ROM_OFF; s.rom_g = p.rom_blob + rm.offset; s.dr = p.drom + rm.doff; s.tid4 = 4u * (uint32_t)tid;
+  s.rom_off = ROM_OFF; s.rom_g = p.rom_blob + rm.offset; s.dr = p.drom + rm.doff; 
   s.rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
   // ---- a2 action latch (C.11)
   if (live0) {
@@ -590,15 +680,15 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
     if ((left >> act) & 1u) ina &= ~0x40u;
     if ((right >> act) & 1u) ina &= ~0x80u;
     const uint32_t fire0 = (fire >> act) & 1u;
-    T::S(S_INP) = ina | (fire0 << 8) | ((uint32_t)tid << 16);
+    T::S(sl, S_INP) = ina | (fire0 << 8) | ((uint32_t)tid << 16);
     if ((fl & TF_LATCHEN) && fire0) fl &= ~TF_INPT4_LATCH;
-    T::S(S_FL) = fl;
+    T::S(sl, S_FL) = fl;
   }
   s.wsync = (fl & TF_WSYNC) != 0;
-  s.relim();
+  s.relim(); s.rekey();
   if constexpr (ROMS) mbar_wait(smem_u32(&s_bar), 0);
-  const uint32_t fskip = (uint32_t)p.frameskip;
-  s.w = live0 ? s.fetch() : (uint32_t)H_SLOW;
+  const uint32_t fskip = s.fskip;
+  s.w = live0 ? s.fetch() : make_uint2(H_SLOW, 0);
 
   // ---- the hot loop: whole instructions until `frameskip` frame-end events (C.10), min-key lanes first.
   // Line bookkeeping mirrors C.4: the line counter advances with the FIRST cycle of a new line, so an
@@ -606,35 +696,36 @@ __global__ void __launch_bounds__(BLOCK, 512 / BLOCK) vcs_step_kernel(StepParams
   // makes the finished line "line 0" and the next one line 1).
   for (;;) {
     for (;;) {
-      const uint32_t key = (s.fdone >= fskip) ? 0xFFFFFFFFu : (s.park & 2u) ? 0xFFFFFFFEu
-                         : (min(s.fdone, 63u) << 25) | (s.SP << 17) | (s.bank << 16) | s.PC;
+      const uint32_t key = s.keyhi | s.pc();
       const uint32_t mk = __reduce_min_sync(0xFFFFFFFFu, key);
-      if (mk >= 0xFFFFFFFEu) break;                        // every lane is parked or has finished the step
-      if (key == mk) s.run_block(fskip);
+      if (mk >= KEY_PARKED) break;                         // every lane is parked or has finished the step
+      if (key == mk) s.run_block();
     }
     if (!regroups) break;
     if (!__syncthreads_or((s.park & 2u) && s.fdone < fskip)) break;      // nobody left to run in this block
-    s.regroup(fskip);
+    s.regroup();
   }
-  const int e = e0 + (int)(T::S(S_INP) >> 16);             // the env this thread ends up holding
+  if (s.sl == NOSLOT) return;
+  const uint32_t fs = s.sl;                                // the file (and env) this thread ends up holding
+  const int e = e0 + (int)(T::S(fs, S_INP) >> 16);
   const bool live = e < B;
   if (!live) return;
-  if (s.cyc - s.lstart > LINE_CYC) { T::line_end(); s.lstart += LINE_CYC; }      // the last instruction ran over the line end
+  if (s.cyc - s.lstart > LINE_CYC) { T::line_end(fs); s.lstart += LINE_CYC; }      // the last instruction ran over the line end
   // ---- a16 state store
   {
     uint32_t timer, sub, shift, tflag;
     s.timer_sync(s.cyc, timer, sub, shift, tflag);
     p.st[W_AXYS * B + e] = s.A | (s.X << 8) | (s.Y << 16) | (s.SP << 24);
-    p.st[W_PC * B + e] = s.PC | (s.pack_p() << 16) | (s.status << 24);
-    p.st[W_BEAM * B + e] = (uint32_t)(s.cyc - s.lstart) | (T::S(S_LINE) << 8) | (s.bank << 24);
+    p.st[W_PC * B + e] = s.pc() | (s.pack_p() << 16) | (s.status << 24);
+    p.st[W_BEAM * B + e] = (uint32_t)(s.cyc - s.lstart) | (T::S(fs, S_LINE) << 8) | ((s.di >> 12) << 24);
     p.st[W_FRAME * B + e] += s.fdone;
     p.st[W_FCYC * B + e] = (uint32_t)(s.cyc - s.fstart);
     p.st[W_TIMER * B + e] = timer | (shift << 8) | (tflag << 12) | (sub << 16);
-    p.st[W_PORTS * B + e] = T::S(S_PORTS);
-    p.st[W_COLU * B + e] = T::S(S_COLU); p.st[W_PF * B + e] = T::S(S_PF); p.st[W_GRP * B + e] = T::S(S_GRP); p.st[W_NUSIZ * B + e] = T::S(S_NUSIZ);
-    p.st[W_POS * B + e] = T::S(S_POS); p.st[W_POS2 * B + e] = (T::S(S_POS2) & 0xFFFF) | (T::S(S_RX) << 16);
-    p.st[W_FLAGS * B + e] = T::S(S_FL) & TF_ARCH_MASK; p.st[W_CX * B + e] = T::S(S_CX);
-    for (int i = 0; i < 32; ++i) p.ram[i * B + e] = smem[(S_RAM + i) * BLOCK + tid];
+    p.st[W_PORTS * B + e] = T::S(fs, S_PORTS);
+    p.st[W_COLU * B + e] = T::S(fs, S_COLU); p.st[W_PF * B + e] = T::S(fs, S_PF); p.st[W_GRP * B + e] = T::S(fs, S_GRP); p.st[W_NUSIZ * B + e] = T::S(fs, S_NUSIZ);
+    p.st[W_POS * B + e] = T::S(fs, S_POS); p.st[W_POS2 * B + e] = (T::S(fs, S_POS2) & 0xFFFF) | (T::S(fs, S_RX) << 16);
+    p.st[W_FLAGS * B + e] = T::S(fs, S_FL) & TF_ARCH_MASK; p.st[W_CX * B + e] = T::S(fs, S_CX);
+    for (int i = 0; i < 32; ++i) p.ram[i * B + e] = smem[(S_RAM + i) * BLOCK + fs];
     p.cyc[e] += (unsigned long long)s.cyc;
   }
 }
@@ -643,25 +734,28 @@ size_t step_smem_bytes(int block, bool roms, uint32_t max_rom) {
   return (size_t)(S_WORDS * block + C_WORDS) * 4 + (roms ? (max_rom < 4096 ? 4096 : max_rom) + 16 : 0);
 }
 
-template <int BLOCK, bool ROMS>
+template <int BLOCK, bool ROMS, int THREADS>
 static cudaError_t launch_one(const StepParams &p, cudaStream_t stream) {
   const size_t smem_bytes = step_smem_bytes(BLOCK, ROMS, p.max_rom);
   static size_t configured = 0;
   if (configured < smem_bytes) {
-    cudaError_t e = cudaFuncSetAttribute(vcs_step_kernel<BLOCK, ROMS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    cudaError_t e = cudaFuncSetAttribute(vcs_step_kernel<BLOCK, ROMS, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
     configured = smem_bytes;
   }
   const int grid = (p.batch + BLOCK - 1) / BLOCK;
-  vcs_step_kernel<BLOCK, ROMS><<<grid, BLOCK, smem_bytes, stream>>>(p);
+  vcs_step_kernel<BLOCK, ROMS, THREADS><<<grid, THREADS, smem_bytes, stream>>>(p);
   return cudaGetLastError();
 }
 
 cudaError_t launch_step(const StepParams &p, cudaStream_t stream) {
-  if (p.rom_smem) {
-    switch (p.block) { case 64: return launch_one<64, true>(p, stream); case 256: return launch_one<256, true>(p, stream); default: return launch_one<128, true>(p, stream); }
+  if (p.rom_smem && p.regroup && p.max_rom == 8192) {      // F8 carts present: one spare warp per block for the regroup
+    switch (p.block) { case 64: return launch_one<64, true, 96>(p, stream); case 256: return launch_one<256, true, 288>(p, stream); default: return launch_one<128, true, 160>(p, stream); }
   }
-  switch (p.block) { case 64: return launch_one<64, false>(p, stream); case 256: return launch_one<256, false>(p, stream); default: return launch_one<128, false>(p, stream); }
+  if (p.rom_smem) {
+    switch (p.block) { case 64: return launch_one<64, true, 64>(p, stream); case 256: return launch_one<256, true, 256>(p, stream); default: return launch_one<128, true, 128>(p, stream); }
+  }
+  switch (p.block) { case 64: return launch_one<64, false, 64>(p, stream); case 256: return launch_one<256, false, 256>(p, stream); default: return launch_one<128, false, 128>(p, stream); }
 }
 
 }  // namespace vcs

@@ -8,7 +8,7 @@ namespace vcs {
 
 struct StepParams {
   uint32_t *st; uint32_t *ram; unsigned long long *cyc; uint8_t *screen;
-  const uint8_t *rom_blob; const uint32_t *drom; const RomMeta *rom_meta; const int32_t *env_rom;
+  const uint8_t *rom_blob; const uint2 *drom; const RomMeta *rom_meta; const int32_t *env_rom;
   const uint8_t *actions;
   int32_t batch, frameskip, y0, max_lines;
   int32_t block, rom_smem, regroup; uint32_t max_rom;     // launch shape: envs per block (64/128/256), ROM staged in smem, largest image

@@ -57,77 +57,77 @@ enum : uint32_t { EV_FRAME = 1u, EV_WSYNC = 2u, EV_CROSS = 16u };   // EV_CROSS 
 
 template <int BLOCK>
 struct Tia {
-  static DEV uint32_t &S(int i) { return smem[i * BLOCK + threadIdx.x]; }
+  static DEV uint32_t &S(uint32_t sl, int i) { return smem[i * BLOCK + sl]; }
   static DEV uint32_t ctx(int i) { return smem[S_WORDS * BLOCK + i]; }
-  static DEV uint8_t *row_ptr(uint32_t r) {
+  static DEV uint8_t *row_ptr(uint32_t sl, uint32_t r) {
     unsigned long long base = (unsigned long long)ctx(C_SCREEN_LO) | ((unsigned long long)ctx(C_SCREEN_HI) << 32);
-    return reinterpret_cast<uint8_t *>(base) + ((size_t)(ctx(C_ENV0) + (S(S_INP) >> 16)) * SCR_H + r) * SCR_W;
+    return reinterpret_cast<uint8_t *>(base) + ((size_t)(ctx(C_ENV0) + (S(sl, S_INP) >> 16)) * SCR_H + r) * SCR_W;
   }
 
   // ------------------------------------------------------------------ cached object line masks
-  static DEV void obj_clear(int o) {
+  static DEV void obj_clear(uint32_t sl, int o) {
 #pragma unroll
-    for (int w = 0; w < 5; ++w) S(S_OBJ + 5 * o + w) = 0;
+    for (int w = 0; w < 5; ++w) S(sl, S_OBJ + 5 * o + w) = 0;
   }
   // OR a pattern (<= 32 px) whose first pixel is at c (0..159) into object o's line mask, wrapping at 160
-  static DEV void obj_or(int o, uint32_t pat, uint32_t c) {
+  static DEV void obj_or(uint32_t sl, int o, uint32_t pat, uint32_t c) {
     const uint32_t q = c >> 5, s = c & 31u;
     const uint32_t lo = pat << s, hi = __funnelshift_l(pat, 0u, s);
-    uint32_t *p = &smem[(S_OBJ + 5 * o) * BLOCK + threadIdx.x];
+    uint32_t *p = &smem[(S_OBJ + 5 * o) * BLOCK + sl];
     p[q * BLOCK] |= lo;
     if (hi) p[(q == 4 ? 0 : q + 1) * BLOCK] |= hi;
   }
   // copy offsets O(m): {0:[0],1:[0,16],2:[0,32],3:[0,16,32],4:[0,64],5:[0],6:[0,32,64],7:[0]} (C.8)
-  static DEV void obj_copies(int o, uint32_t pat, uint32_t p, uint32_t m, bool fresh) {
+  static DEV void obj_copies(uint32_t sl, int o, uint32_t pat, uint32_t p, uint32_t m, bool fresh) {
     const uint32_t o1 = ((0x02041210u >> (4 * m)) & 0xFu) << 4;        // second copy offset (0 = none)
     const uint32_t o2 = (m == 3) ? 32u : (m == 6) ? 64u : 0u;
-    if (!fresh) obj_or(o, pat, p);
-    if (o1) { uint32_t c = p + o1; if (c >= 160) c -= 160; obj_or(o, pat, c); }
-    if (o2) { uint32_t c = p + o2; if (c >= 160) c -= 160; obj_or(o, pat, c); }
+    if (!fresh) obj_or(sl, o, pat, p);
+    if (o1) { uint32_t c = p + o1; if (c >= 160) c -= 160; obj_or(sl, o, pat, c); }
+    if (o2) { uint32_t c = p + o2; if (c >= 160) c -= 160; obj_or(sl, o, pat, c); }
   }
-  static DEV void rebuild_player(int p, uint32_t fl) {
-    obj_clear(OB_P0 + p);
-    const uint32_t g = byte_of(S(S_GRP), 2 * p + ((fl & (p ? TF_VDELP1 : TF_VDELP0)) ? 1 : 0));
+  static DEV void rebuild_player(uint32_t sl, int p, uint32_t fl) {
+    obj_clear(sl, OB_P0 + p);
+    const uint32_t g = byte_of(S(sl, S_GRP), 2 * p + ((fl & (p ? TF_VDELP1 : TF_VDELP0)) ? 1 : 0));
     if (g == 0) return;
-    const uint32_t m = byte_of(S(S_NUSIZ), p) & 7u;
+    const uint32_t m = byte_of(S(sl, S_NUSIZ), p) & 7u;
     const uint32_t gg = (fl & (p ? TF_REFP1 : TF_REFP0)) ? g : brev8(g);      // bit d = pixel d of the sprite
     const uint32_t pat = (m == 5) ? expand2(gg) : (m == 7) ? expand4(gg) : gg;
-    obj_copies(OB_P0 + p, pat, byte_of(S(S_POS), p), m, fl & (p ? TF_FRESH_P1 : TF_FRESH_P0));
+    obj_copies(sl, OB_P0 + p, pat, byte_of(S(sl, S_POS), p), m, fl & (p ? TF_FRESH_P1 : TF_FRESH_P0));
   }
-  static DEV void rebuild_missile(int p, uint32_t fl) {
-    obj_clear(OB_M0 + p);
+  static DEV void rebuild_missile(uint32_t sl, int p, uint32_t fl) {
+    obj_clear(sl, OB_M0 + p);
     if (!(fl & (p ? TF_ENAM1 : TF_ENAM0)) || (fl & (p ? TF_RESMP1 : TF_RESMP0))) return;
-    const uint32_t ns = byte_of(S(S_NUSIZ), p);
+    const uint32_t ns = byte_of(S(sl, S_NUSIZ), p);
     const uint32_t pat = (1u << (1u << ((ns >> 4) & 3u))) - 1u;
-    obj_copies(OB_M0 + p, pat, byte_of(S(S_POS), 2 + p), ns & 7u, fl & (p ? TF_FRESH_M1 : TF_FRESH_M0));
+    obj_copies(sl, OB_M0 + p, pat, byte_of(S(sl, S_POS), 2 + p), ns & 7u, fl & (p ? TF_FRESH_M1 : TF_FRESH_M0));
   }
-  static DEV void rebuild(uint32_t fl) {
+  static DEV void rebuild(uint32_t sl, uint32_t fl) {
     if (fl & (TF_DIRTY0 << OB_PF)) {
-      const uint32_t pf = S(S_PF);
+      const uint32_t pf = S(sl, S_PF);
       const uint32_t pf20 = (byte_of(pf, 0) >> 4) | (brev8(byte_of(pf, 1)) << 4) | (byte_of(pf, 2) << 12);
       const uint32_t right = (pf & (1u << 24)) ? (__brev(pf20) >> 12) : pf20;      // CTRLPF.REF
       const uint32_t lo = pf20 | (right << 20), hi = right >> 12;                  // 40 playfield bits, 4 px each
-      S(S_OBJ + 0) = expand4(lo); S(S_OBJ + 1) = expand4(lo >> 8); S(S_OBJ + 2) = expand4(lo >> 16);
-      S(S_OBJ + 3) = expand4(lo >> 24); S(S_OBJ + 4) = expand4(hi);
+      S(sl, S_OBJ + 0) = expand4(lo); S(sl, S_OBJ + 1) = expand4(lo >> 8); S(sl, S_OBJ + 2) = expand4(lo >> 16);
+      S(sl, S_OBJ + 3) = expand4(lo >> 24); S(sl, S_OBJ + 4) = expand4(hi);
     }
     if (fl & (TF_DIRTY0 << OB_BL)) {
-      obj_clear(OB_BL);
+      obj_clear(sl, OB_BL);
       if (fl & ((fl & TF_VDELBL) ? TF_ENABL_OLD : TF_ENABL_NEW))
-        obj_or(OB_BL, (1u << (1u << ((S(S_PF) >> 28) & 3u))) - 1u, byte_of(S(S_POS2), 0));
+        obj_or(sl, OB_BL, (1u << (1u << ((S(sl, S_PF) >> 28) & 3u))) - 1u, byte_of(S(sl, S_POS2), 0));
     }
-    if (fl & (TF_DIRTY0 << OB_P0)) rebuild_player(0, fl);
-    if (fl & (TF_DIRTY0 << OB_P1)) rebuild_player(1, fl);
-    if (fl & (TF_DIRTY0 << OB_M0)) rebuild_missile(0, fl);
-    if (fl & (TF_DIRTY0 << OB_M1)) rebuild_missile(1, fl);
+    if (fl & (TF_DIRTY0 << OB_P0)) rebuild_player(sl, 0, fl);
+    if (fl & (TF_DIRTY0 << OB_P1)) rebuild_player(sl, 1, fl);
+    if (fl & (TF_DIRTY0 << OB_M0)) rebuild_missile(sl, 0, fl);
+    if (fl & (TF_DIRTY0 << OB_M1)) rebuild_missile(sl, 1, fl);
   }
 
   // ------------------------------------------------------------------ segment rendering (C.8 pixel function)
   // visible pixels [x0, x1) of the current line with the registers in force; VBLANK is off
-  static DEVNI void render_visible(int x0, int x1) {
-    uint32_t fl = S(S_FL);
-    if (fl & TF_DIRTY_ALL) { rebuild(fl); fl &= ~TF_DIRTY_ALL; S(S_FL) = fl; }
+  static DEVNI void render_visible(uint32_t sl, int x0, int x1) {
+    uint32_t fl = S(sl, S_FL);
+    if (fl & TF_DIRTY_ALL) { rebuild(sl, fl); fl &= ~TF_DIRTY_ALL; S(sl, S_FL) = fl; }
     const bool vis = (fl & TF_ROWVIS) != 0;
-    const uint32_t ctrl = S(S_PF) >> 24;
+    const uint32_t ctrl = S(sl, S_PF) >> 24;
     uint32_t a0 = 0, a1 = 0, a2 = 0, a3 = 0, a4 = 0, a5 = 0, a6 = 0, a7 = 0, a8 = 0, a9 = 0, a10 = 0, a11 = 0, a12 = 0, a13 = 0, a14 = 0;
     const int w1 = (x1 - 1) >> 5;
 #pragma unroll 1
@@ -136,7 +136,7 @@ struct Tia {
       const uint32_t rm = (hi >= 32 ? 0xFFFFFFFFu : ((1u << hi) - 1u)) & ~((1u << lo) - 1u);
       uint32_t act = rm;
       if ((fl & TF_HMBLANK) && w == 0) act &= ~0xFFu;             // HMOVE comb: x 0..7 black, no collisions
-      const uint32_t *o = &smem[(S_OBJ + w) * BLOCK + threadIdx.x];
+      const uint32_t *o = &smem[(S_OBJ + w) * BLOCK + sl];
       const uint32_t PF = o[0] & act, BL = o[5 * BLOCK] & act, P0 = o[10 * BLOCK] & act, P1 = o[15 * BLOCK] & act,
                      M0 = o[20 * BLOCK] & act, M1 = o[25 * BLOCK] & act;
       a0 |= M0 & P1; a1 |= M0 & P0; a2 |= M1 & P0; a3 |= M1 & P1; a4 |= P0 & PF; a5 |= P0 & BL; a6 |= P1 & PF; a7 |= P1 & BL;
@@ -153,7 +153,7 @@ struct Tia {
           e0 = o0; e1 = o1 & ~e0; ef = of & ~(e0 | e1);
         }
         const uint32_t eb = ~(e0 | e1 | ef);
-        uint32_t *pl = &smem[(S_PLANE + w) * BLOCK + threadIdx.x];
+        uint32_t *pl = &smem[(S_PLANE + w) * BLOCK + sl];
         pl[0] = (pl[0] & ~rm) | ((e1 | eb) & rm);
         pl[5 * BLOCK] = (pl[5 * BLOCK] & ~rm) | ((ef | eb) & rm);
       }
@@ -163,31 +163,31 @@ struct Tia {
     c |= a4 ? 1u << CX_P0PF : 0; c |= a5 ? 1u << CX_P0BL : 0; c |= a6 ? 1u << CX_P1PF : 0; c |= a7 ? 1u << CX_P1BL : 0;
     c |= a8 ? 1u << CX_M0PF : 0; c |= a9 ? 1u << CX_M0BL : 0; c |= a10 ? 1u << CX_M1PF : 0; c |= a11 ? 1u << CX_M1BL : 0;
     c |= a12 ? 1u << CX_BLPF : 0; c |= a13 ? 1u << CX_P0P1 : 0; c |= a14 ? 1u << CX_M0M1 : 0;
-    if (c) S(S_CX) |= c;
+    if (c) S(sl, S_CX) |= c;
   }
   // catch the beam up to colour clock `clk` (0..228) of the current line
-  static DEV void render_to(uint32_t clk) {
-    const uint32_t rx = S(S_RX);
+  static DEV void render_to(uint32_t sl, uint32_t clk) {
+    const uint32_t rx = S(sl, S_RX);
     if (clk <= rx) return;
-    S(S_RX) = clk;
+    S(sl, S_RX) = clk;
     const int x0 = (int)max(rx, (uint32_t)HBLANK) - HBLANK, x1 = (int)max(clk, (uint32_t)HBLANK) - HBLANK;
-    if (x1 <= x0 || (S(S_FL) & TF_VBLANK)) return;               // VBLANK: no collisions, painted black
-    render_visible(x0, x1);
+    if (x1 <= x0 || (S(sl, S_FL) & TF_VBLANK)) return;               // VBLANK: no collisions, painted black
+    render_visible(sl, x0, x1);
   }
 
   // ------------------------------------------------------------------ painting: planes + colours -> bytes in HBM
   // the whole row r from pixel 0 (the common case: no colour change inside the visible line)
-  static DEVNI void paint_row_full(uint32_t r, uint32_t fl) {
-    uint4 *dst = reinterpret_cast<uint4 *>(row_ptr(r));
+  static DEVNI void paint_row_full(uint32_t sl, uint32_t r, uint32_t fl) {
+    uint4 *dst = reinterpret_cast<uint4 *>(row_ptr(sl, r));
     if (fl & TF_VBLANK) {
 #pragma unroll
       for (int q = 0; q < 10; ++q) dst[q] = make_uint4(0, 0, 0, 0);
       return;
     }
-    const uint32_t colu = S(S_COLU);
+    const uint32_t colu = S(sl, S_COLU);
 #pragma unroll 1
     for (int w = 0; w < 5; ++w) {
-      const uint32_t i0 = S(S_PLANE + w), i1 = S(S_PLANE + 5 + w);
+      const uint32_t i0 = S(sl, S_PLANE + w), i1 = S(sl, S_PLANE + 5 + w);
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         const uint32_t a = i0 >> (16 * h), b = i1 >> (16 * h);
@@ -199,14 +199,14 @@ struct Tia {
     }
   }
   // pixels [a, b) of row r: from the planes with the colours in force, or zeros
-  static DEVNI void paint_range(uint32_t r, int a, int b, uint32_t fl, bool zero) {
-    uint8_t *row = row_ptr(r);
-    const uint32_t colu = (zero || (fl & TF_VBLANK)) ? 0u : S(S_COLU);
+  static DEVNI void paint_range(uint32_t sl, uint32_t r, int a, int b, uint32_t fl, bool zero) {
+    uint8_t *row = row_ptr(sl, r);
+    const uint32_t colu = (zero || (fl & TF_VBLANK)) ? 0u : S(sl, S_COLU);
     const bool comb = (fl & TF_HMBLANK) != 0;
 #pragma unroll 1
     for (int x = a; x < b;) {
       const int w = x >> 5, s = x & 31;
-      const uint32_t i0 = S(S_PLANE + w) >> s, i1 = S(S_PLANE + 5 + w) >> s;
+      const uint32_t i0 = S(sl, S_PLANE + w) >> s, i1 = S(sl, S_PLANE + 5 + w) >> s;
       if ((x & 3) == 0 && x + 4 <= b) {
         uint32_t n0 = i0 & 0xFu, n1 = i1 & 0xFu;
         n0 = (n0 | (n0 << 6)) & 0x0303u; n0 = (n0 | (n0 << 3)) & 0x1111u;
@@ -222,66 +222,66 @@ struct Tia {
     }
   }
   // before a colour register / VBLANK changes at visible pixel x_now: fix the pixels before it
-  static DEV void paint_upto(int x_now, uint32_t fl) {
-    const int xe = min(max(x_now, 0), SCR_W), px = (int)S(S_PX);
-    if (xe > px) { paint_range(S(S_LINE) - ctx(C_Y0), px, xe, fl, false); S(S_PX) = (uint32_t)xe; }
+  static DEV void paint_upto(uint32_t sl, int x_now, uint32_t fl) {
+    const int xe = min(max(x_now, 0), SCR_W), px = (int)S(sl, S_PX);
+    if (xe > px) { paint_range(sl, S(sl, S_LINE) - ctx(C_Y0), px, xe, fl, false); S(sl, S_PX) = (uint32_t)xe; }
   }
 
   // ------------------------------------------------------------------ line / frame ends
   // the scanline in progress ends: finish it, store its row, start the next one (C.4 new-line bookkeeping)
-  static DEVNI void line_end() {
-    render_to(LINE_CLK);
-    uint32_t fl = S(S_FL);
-    uint32_t line = S(S_LINE);
+  static DEVNI void line_end(uint32_t sl) {
+    render_to(sl, LINE_CLK);
+    uint32_t fl = S(sl, S_FL);
+    uint32_t line = S(sl, S_LINE);
     if (fl & TF_ROWVIS) {
-      const int px = (int)S(S_PX);
-      if (px == 0) paint_row_full(line - ctx(C_Y0), fl);
-      else if (px < SCR_W) paint_range(line - ctx(C_Y0), px, SCR_W, fl, false);
+      const int px = (int)S(sl, S_PX);
+      if (px == 0) paint_row_full(sl, line - ctx(C_Y0), fl);
+      else if (px < SCR_W) paint_range(sl, line - ctx(C_Y0), px, SCR_W, fl, false);
     }
-    line += 1; S(S_LINE) = line; S(S_RX) = 0; S(S_PX) = 0;
+    line += 1; S(sl, S_LINE) = line; S(sl, S_RX) = 0; S(sl, S_PX) = 0;
     const uint32_t fresh = (fl >> 15) & 0xFu;                      // objects whose main copy re-appears
     fl = (fl & ~(TF_WSYNC | TF_HMBLANK | TF_FRESH_ALL | TF_ROWVIS)) | (fresh << (22 + OB_P0));
     if ((fl & TF_STORING) && (line - ctx(C_Y0)) < (uint32_t)SCR_H) fl |= TF_ROWVIS;
-    S(S_FL) = fl;
+    S(sl, S_FL) = fl;
   }
   // C.10 frame end at colour clock `clk` of the current line (which becomes line 0 of the next frame)
-  static DEVNI void frame_end(uint32_t clk) {
-    render_to(clk);
-    uint32_t fl = S(S_FL);
+  static DEVNI void frame_end(uint32_t sl, uint32_t clk) {
+    render_to(sl, clk);
+    uint32_t fl = S(sl, S_FL);
     if (fl & TF_STORING) {
-      const int r = (int)S(S_LINE) - (int)ctx(C_Y0);
+      const int r = (int)S(sl, S_LINE) - (int)ctx(C_Y0);
       if (fl & TF_ROWVIS) {
-        const int x = (int)max(clk, (uint32_t)HBLANK) - HBLANK, px = (int)S(S_PX);
-        if (x > px) paint_range(r, px, x, fl, false);
-        if (max(x, px) < SCR_W) paint_range(r, max(x, px), SCR_W, fl, true);
+        const int x = (int)max(clk, (uint32_t)HBLANK) - HBLANK, px = (int)S(sl, S_PX);
+        if (x > px) paint_range(sl, r, px, x, fl, false);
+        if (max(x, px) < SCR_W) paint_range(sl, r, max(x, px), SCR_W, fl, true);
       }
       const uint4 z = make_uint4(0, 0, 0, 0);                      // rows the beam never reached in this frame
       for (int rr = max(r + 1, 0); rr < SCR_H; ++rr) {
-        uint4 *dst = reinterpret_cast<uint4 *>(row_ptr(rr));
+        uint4 *dst = reinterpret_cast<uint4 *>(row_ptr(sl, rr));
 #pragma unroll
         for (int q = 0; q < 10; ++q) dst[q] = z;
       }
     }
-    const uint32_t fd = S(S_FDONE) + 1;
-    S(S_FDONE) = fd; S(S_LINE) = 0; S(S_PX) = 0;
+    const uint32_t fd = S(sl, S_FDONE) + 1;
+    S(sl, S_FDONE) = fd; S(sl, S_LINE) = 0; S(sl, S_PX) = 0;
     fl &= ~(TF_ROWVIS | TF_STORING);
     if (fd + 1 == ctx(C_FRAMESKIP)) fl |= TF_STORING;
-    S(S_FL) = fl;
+    S(sl, S_FL) = fl;
   }
 
   // ------------------------------------------------------------------ TIA bus accesses (C.8)
   // m = cycle-in-line of the access (>= 76 when the instruction ran over the line end)
-  static DEV uint32_t catch_up(int &m) {
+  static DEV uint32_t catch_up(uint32_t sl, int &m) {
     uint32_t ev = 0;
-    while (m >= LINE_CYC) { line_end(); m -= LINE_CYC; ev += EV_CROSS; }
-    render_to(3u * (uint32_t)(m + 1));
+    while (m >= LINE_CYC) { line_end(sl); m -= LINE_CYC; ev += EV_CROSS; }
+    render_to(sl, 3u * (uint32_t)(m + 1));
     return ev;
   }
   // read of register a&15 -> value | events<<8
-  static DEVNI uint32_t read(uint32_t r, int m) {
+  static DEVNI uint32_t read(uint32_t sl, uint32_t r, int m) {
     if (r < 8) {
-      const uint32_t ev = catch_up(m);
-      const uint32_t cx = S(S_CX);
+      const uint32_t ev = catch_up(sl, m);
+      const uint32_t cx = S(sl, S_CX);
       uint32_t b7, b6;
       switch (r) {
         case 0: b7 = cx >> CX_M0P1; b6 = cx >> CX_M0P0; break;
@@ -295,64 +295,64 @@ struct Tia {
       }
       return ((b7 & 1u) << 7) | ((b6 & 1u) << 6) | (ev << 8);
     }
-    const uint32_t fl = S(S_FL);
-    if (r == 0xC) { const bool lat = (fl & TF_LATCHEN) ? (fl & TF_INPT4_LATCH) != 0 : true; return (!(S(S_INP) & 0x100u) && lat) ? 0x80u : 0u; }
+    const uint32_t fl = S(sl, S_FL);
+    if (r == 0xC) { const bool lat = (fl & TF_LATCHEN) ? (fl & TF_INPT4_LATCH) != 0 : true; return (!(S(sl, S_INP) & 0x100u) && lat) ? 0x80u : 0u; }
     if (r == 0xD) { const bool lat = (fl & TF_LATCHEN) ? (fl & TF_INPT5_LATCH) != 0 : true; return lat ? 0x80u : 0u; }
     return 0;
   }
   static DEV uint32_t flag(uint32_t fl, uint32_t bit, bool on) { return on ? (fl | bit) : (fl & ~bit); }
   static DEV uint32_t dirty(int o) { return TF_DIRTY0 << o; }
   // write of v to register r (= a & 0x3F, one with an effect) in cycle-in-line m -> events
-  static DEVNI uint32_t write(uint32_t r, uint32_t v, int m) {
-    uint32_t ev = catch_up(m);
+  static DEVNI uint32_t write(uint32_t sl, uint32_t r, uint32_t v, int m) {
+    uint32_t ev = catch_up(sl, m);
     const int x_now = 3 * (m + 1) - HBLANK;
-    uint32_t fl = S(S_FL);
+    uint32_t fl = S(sl, S_FL);
     switch (r) {
       case 0x00: { const bool nv = (v >> 1) & 1u;
-                   if ((fl & TF_VSYNC) && !nv) { frame_end(3u * (uint32_t)(m + 1)); ev |= EV_FRAME; fl = S(S_FL); }
+                   if ((fl & TF_VSYNC) && !nv) { frame_end(sl, 3u * (uint32_t)(m + 1)); ev |= EV_FRAME; fl = S(sl, S_FL); }
                    fl = flag(fl, TF_VSYNC, nv); } break;
-      case 0x01: if (fl & TF_ROWVIS) paint_upto(x_now, fl);
+      case 0x01: if (fl & TF_ROWVIS) paint_upto(sl, x_now, fl);
                  fl = flag(fl, TF_VBLANK, (v >> 1) & 1u); fl = flag(fl, TF_LATCHEN, (v >> 6) & 1u);
                  if (!(fl & TF_LATCHEN)) fl |= TF_INPT4_LATCH | TF_INPT5_LATCH;
-                 if ((fl & TF_LATCHEN) && (S(S_INP) & 0x100u)) fl &= ~TF_INPT4_LATCH;
+                 if ((fl & TF_LATCHEN) && (S(sl, S_INP) & 0x100u)) fl &= ~TF_INPT4_LATCH;
                  break;
       case 0x02: fl |= TF_WSYNC; break;
-      case 0x04: S(S_NUSIZ) = set_byte(S(S_NUSIZ), 0, v & 0x37u); fl |= dirty(OB_P0) | dirty(OB_M0); break;
-      case 0x05: S(S_NUSIZ) = set_byte(S(S_NUSIZ), 1, v & 0x37u); fl |= dirty(OB_P1) | dirty(OB_M1); break;
+      case 0x04: S(sl, S_NUSIZ) = set_byte(S(sl, S_NUSIZ), 0, v & 0x37u); fl |= dirty(OB_P0) | dirty(OB_M0); break;
+      case 0x05: S(sl, S_NUSIZ) = set_byte(S(sl, S_NUSIZ), 1, v & 0x37u); fl |= dirty(OB_P1) | dirty(OB_M1); break;
       case 0x06: case 0x07: case 0x08: case 0x09:
-                 if (fl & TF_ROWVIS) paint_upto(x_now, fl);
-                 S(S_COLU) = set_byte(S(S_COLU), r - 6, v & 0xFEu); break;
-      case 0x0A: S(S_PF) = set_byte(S(S_PF), 3, v & 0x37u); fl |= dirty(OB_PF) | dirty(OB_BL); break;
+                 if (fl & TF_ROWVIS) paint_upto(sl, x_now, fl);
+                 S(sl, S_COLU) = set_byte(S(sl, S_COLU), r - 6, v & 0xFEu); break;
+      case 0x0A: S(sl, S_PF) = set_byte(S(sl, S_PF), 3, v & 0x37u); fl |= dirty(OB_PF) | dirty(OB_BL); break;
       case 0x0B: fl = flag(fl, TF_REFP0, (v >> 3) & 1u) | dirty(OB_P0); break;
       case 0x0C: fl = flag(fl, TF_REFP1, (v >> 3) & 1u) | dirty(OB_P1); break;
-      case 0x0D: S(S_PF) = set_byte(S(S_PF), 0, v & 0xF0u); fl |= dirty(OB_PF); break;
-      case 0x0E: S(S_PF) = set_byte(S(S_PF), 1, v); fl |= dirty(OB_PF); break;
-      case 0x0F: S(S_PF) = set_byte(S(S_PF), 2, v); fl |= dirty(OB_PF); break;
-      case 0x10: case 0x11: S(S_POS) = set_byte(S(S_POS), r - 0x10, x_now < 0 ? 3 : (x_now + 5) % 160);
+      case 0x0D: S(sl, S_PF) = set_byte(S(sl, S_PF), 0, v & 0xF0u); fl |= dirty(OB_PF); break;
+      case 0x0E: S(sl, S_PF) = set_byte(S(sl, S_PF), 1, v); fl |= dirty(OB_PF); break;
+      case 0x0F: S(sl, S_PF) = set_byte(S(sl, S_PF), 2, v); fl |= dirty(OB_PF); break;
+      case 0x10: case 0x11: S(sl, S_POS) = set_byte(S(sl, S_POS), r - 0x10, x_now < 0 ? 3 : (x_now + 5) % 160);
                  fl |= (r == 0x10) ? (TF_FRESH_P0 | dirty(OB_P0)) : (TF_FRESH_P1 | dirty(OB_P1)); break;
-      case 0x12: case 0x13: S(S_POS) = set_byte(S(S_POS), r - 0x10, x_now < 0 ? 2 : (x_now + 4) % 160);
+      case 0x12: case 0x13: S(sl, S_POS) = set_byte(S(sl, S_POS), r - 0x10, x_now < 0 ? 2 : (x_now + 4) % 160);
                  fl |= (r == 0x12) ? (TF_FRESH_M0 | dirty(OB_M0)) : (TF_FRESH_M1 | dirty(OB_M1)); break;
-      case 0x14: S(S_POS2) = set_byte(S(S_POS2), 0, x_now < 0 ? 2 : (x_now + 4) % 160); fl |= dirty(OB_BL); break;
-      case 0x1B: { const uint32_t g = S(S_GRP); S(S_GRP) = set_byte(set_byte(g, 0, v), 3, byte_of(g, 2)); }   // GRP0; GRP1_old := GRP1_new
+      case 0x14: S(sl, S_POS2) = set_byte(S(sl, S_POS2), 0, x_now < 0 ? 2 : (x_now + 4) % 160); fl |= dirty(OB_BL); break;
+      case 0x1B: { const uint32_t g = S(sl, S_GRP); S(sl, S_GRP) = set_byte(set_byte(g, 0, v), 3, byte_of(g, 2)); }   // GRP0; GRP1_old := GRP1_new
                  fl |= dirty(OB_P0) | dirty(OB_P1); break;
-      case 0x1C: { const uint32_t g = S(S_GRP); S(S_GRP) = set_byte(set_byte(g, 2, v), 1, byte_of(g, 0)); }   // GRP1; GRP0_old := GRP0_new
+      case 0x1C: { const uint32_t g = S(sl, S_GRP); S(sl, S_GRP) = set_byte(set_byte(g, 2, v), 1, byte_of(g, 0)); }   // GRP1; GRP0_old := GRP0_new
                  fl = flag(fl, TF_ENABL_OLD, fl & TF_ENABL_NEW) | dirty(OB_P0) | dirty(OB_P1) | dirty(OB_BL); break;
       case 0x1D: fl = flag(fl, TF_ENAM0, (v >> 1) & 1u) | dirty(OB_M0); break;
       case 0x1E: fl = flag(fl, TF_ENAM1, (v >> 1) & 1u) | dirty(OB_M1); break;
       case 0x1F: fl = flag(fl, TF_ENABL_NEW, (v >> 1) & 1u) | dirty(OB_BL); break;
-      case 0x20: case 0x21: case 0x22: case 0x23: { const int sh = 16 + 4 * (r - 0x20); S(S_NUSIZ) = (S(S_NUSIZ) & ~(0xFu << sh)) | ((v >> 4) << sh); } break;
-      case 0x24: S(S_POS2) = set_byte(S(S_POS2), 1, v >> 4); break;
+      case 0x20: case 0x21: case 0x22: case 0x23: { const int sh = 16 + 4 * (r - 0x20); S(sl, S_NUSIZ) = (S(sl, S_NUSIZ) & ~(0xFu << sh)) | ((v >> 4) << sh); } break;
+      case 0x24: S(sl, S_POS2) = set_byte(S(sl, S_POS2), 1, v >> 4); break;
       case 0x25: fl = flag(fl, TF_VDELP0, v & 1u) | dirty(OB_P0); break;
       case 0x26: fl = flag(fl, TF_VDELP1, v & 1u) | dirty(OB_P1); break;
       case 0x27: fl = flag(fl, TF_VDELBL, v & 1u) | dirty(OB_BL); break;
       case 0x28: case 0x29: { const int p = r - 0x28; const uint32_t bit = p ? TF_RESMP1 : TF_RESMP0; const bool nv = (v >> 1) & 1u;
                  if ((fl & bit) && !nv) {
-                   const uint32_t mm = byte_of(S(S_NUSIZ), p) & 7u, mid = (mm == 5) ? 8u : (mm == 7) ? 16u : 4u;
-                   S(S_POS) = set_byte(S(S_POS), 2 + p, (byte_of(S(S_POS), p) + mid) % 160u);
+                   const uint32_t mm = byte_of(S(sl, S_NUSIZ), p) & 7u, mid = (mm == 5) ? 8u : (mm == 7) ? 16u : 4u;
+                   S(sl, S_POS) = set_byte(S(sl, S_POS), 2 + p, (byte_of(S(sl, S_POS), p) + mid) % 160u);
                  }
                  fl = flag(fl, bit, nv) | dirty(OB_M0 + p); } break;
       case 0x2A: {                                                                              // HMOVE
-                 uint32_t pos = S(S_POS), pos2 = S(S_POS2); const uint32_t nus = S(S_NUSIZ);
+                 uint32_t pos = S(sl, S_POS), pos2 = S(sl, S_POS2); const uint32_t nus = S(sl, S_NUSIZ);
 #pragma unroll
                  for (int k = 0; k < 5; ++k) {
                    const uint32_t h = (k < 4) ? (nus >> (16 + 4 * k)) & 0xFu : byte_of(pos2, 1) & 0xFu;
@@ -362,14 +362,14 @@ struct Tia {
                    if (p >= 160) p -= 160;
                    if (k < 4) pos = set_byte(pos, k, p); else pos2 = set_byte(pos2, 0, p);
                  }
-                 S(S_POS) = pos; S(S_POS2) = pos2;
+                 S(sl, S_POS) = pos; S(sl, S_POS2) = pos2;
                  fl |= dirty(OB_BL) | dirty(OB_P0) | dirty(OB_P1) | dirty(OB_M0) | dirty(OB_M1);
                  if (x_now < 0) fl |= TF_HMBLANK; } break;
-      case 0x2B: S(S_NUSIZ) &= 0x0000FFFFu; S(S_POS2) = set_byte(S(S_POS2), 1, 0); break;      // HMCLR
-      case 0x2C: S(S_CX) = 0; break;                                                            // CXCLR
+      case 0x2B: S(sl, S_NUSIZ) &= 0x0000FFFFu; S(sl, S_POS2) = set_byte(S(sl, S_POS2), 1, 0); break;      // HMCLR
+      case 0x2C: S(sl, S_CX) = 0; break;                                                            // CXCLR
       default: break;
     }
-    S(S_FL) = fl;
+    S(sl, S_FL) = fl;
     return ev | ((fl & TF_WSYNC) ? EV_WSYNC : 0u);
   }
 };
