@@ -89,6 +89,69 @@ inline bool tia_write_has_effect(uint32_t r) {    // r = address & 0x3F (SURVEY 
 }
 inline bool is_hotspot(uint32_t a13) { return (a13 | 1u) == 0x1FF9u; }
 
+// Second step of the decode: the handler ids above are what the out-of-line ("cold") executor understands.  The
+// instructions that make up almost every executed one are re-coded into a handful of data-driven HOT classes run
+// inline by the interpreter loop: the CPU registers A,X,Y,SP live packed in one 32-bit word, so "which register"
+// is a byte-permute selector carried in the entry instead of a separate handler (LDA/LDX/LDY, STA/STX/STY,
+// INX/INY/DEX/DEY, the transfers), and the eight branches share one flag test described by the entry.
+// Everything else keeps its id, offset by HC_COLD.
+enum HotClass : uint32_t {
+  HC_ST_TIA = 1,     // y = TIA register | extract selector << 16
+  HC_LD_IMM = 2,     // y = immediate | insert selector << 16
+  HC_BR = 3,         // y = signed displacement ; aux = flag bit position in P | wanted value << 3 | extra cycles << 4
+  HC_RTIM = 4,       // y = address ; aux = read op
+  HC_INCDEC = 5,     // y = extract selector | insert selector << 16 ; aux = delta (1 | 0xFF)
+  HC_LD_RAM = 6,     // y = smem byte offset | insert selector << 16
+  HC_ST_RAM = 7,     // y = smem byte offset | extract selector << 16
+  HC_XFER = 8,       // y = extract selector | insert selector << 16 ; aux = 1: sets N,Z  0: TXS
+  HC_ALU_IMM = 9,    // y = immediate ; aux = read op (3..10)
+  HC_ALU_RAM = 10,   // y = smem byte offset ; aux = read op (3..11)
+  HC_RMW_RAM = 11,   // y = smem byte offset ; aux = RMW op
+  HC_ACC = 12,       // aux = RMW op on A
+  HC_FLAG = 13,      // y = P bits to clear | P bits to set << 16
+  HC_NOP = 14,
+  HC_JMP = 15,       // y = target
+  HC_COLD = 16       // + Hid: executed by the out-of-line executor
+};
+static_assert(HC_COLD + H_COUNT <= 128, "hid is 7 bits");
+
+inline void hot_class(uint32_t &x, uint32_t &y) {
+  const uint32_t hid = x & 0x7Fu, rest = x & 0x00FFFF00u;                  // cy and len stay
+  static const uint32_t ins[4] = {0x3214u, 0x3240u, 0x3410u, 0x4210u};     // prmt(axys, v, sel): v -> A, X, Y, SP
+  auto ext = [](uint32_t i) { return 0x4440u | i; };                       // prmt(axys, 0, sel): zero-extended byte i
+  auto mk = [&](uint32_t hc, uint32_t aux) { x = hc | rest | (aux << DW_OP2_SHIFT); };
+  if (hid >= H_STZT0 && hid < H_STZT0 + 3) { y = (y & 0xFFu) | (ext(hid - H_STZT0) << 16); mk(HC_ST_TIA, 0); }
+  else if (hid >= H_IMM0 && hid < H_IMM0 + 3) { y = (y & 0xFFu) | (ins[hid - H_IMM0] << 16); mk(HC_LD_IMM, 0); }
+  else if (hid >= H_IMM0 + 3 && hid < H_IMM0 + 11) { y &= 0xFFu; mk(HC_ALU_IMM, hid - H_IMM0); }
+  else if (hid >= H_ZR0 && hid < H_ZR0 + 3) { y = (y & 0xFFFFu) | (ins[hid - H_ZR0] << 16); mk(HC_LD_RAM, 0); }
+  else if (hid >= H_ZR0 + 3 && hid < H_ZR0 + 12) { y &= 0xFFFFu; mk(HC_ALU_RAM, hid - H_ZR0); }
+  else if (hid >= H_STZR0 && hid < H_STZR0 + 3) { y = (y & 0xFFFFu) | (ext(hid - H_STZR0) << 16); mk(HC_ST_RAM, 0); }
+  else if (hid == H_NOP) { y = 0; mk(HC_NOP, 0); }
+  else if (hid >= H_MZR0 && hid < H_MZR0 + 6) { y &= 0xFFFFu; mk(HC_RMW_RAM, hid - H_MZR0); }
+  else if (hid >= H_ACC0 && hid < H_ACC0 + 4) { y = 0; mk(HC_ACC, hid - H_ACC0); }
+  else if (hid >= H_IMP0 && hid < H_IMP0 + 7) {                            // CLC SEC CLD SED CLI SEI CLV
+    static const uint32_t clr[7] = {1, 1, 8, 8, 4, 4, 0x40}, set[7] = {0, 1, 0, 8, 0, 4, 0};
+    y = clr[hid - H_IMP0] | (set[hid - H_IMP0] << 16); mk(HC_FLAG, 0);
+  }
+  else if (hid >= H_IMP0 + 8 && hid < H_IMP0 + 12) {                       // DEX DEY INX INY
+    const uint32_t k = hid - H_IMP0 - 8, r = 1u + (k & 1u);
+    y = ext(r) | (ins[r] << 16); mk(HC_INCDEC, (k < 2) ? 0xFFu : 1u);
+  }
+  else if (hid >= H_IMP0 + 12 && hid < H_IMP0 + 18) {                      // TAX TAY TSX TXA TYA TXS
+    static const uint32_t src[6] = {0, 0, 3, 1, 2, 1}, dst[6] = {1, 2, 1, 0, 0, 3};
+    const uint32_t k = hid - H_IMP0 - 12;
+    y = ext(src[k]) | (ins[dst[k]] << 16); mk(HC_XFER, (k == 5) ? 0u : 1u);
+  }
+  else if (hid >= H_BR0 && hid < H_BR0 + 8) {                              // BPL BMI BVC BVS BCC BCS BNE BEQ
+    static const uint32_t pos[4] = {7, 6, 0, 1};                           // N V C Z in the P layout
+    const uint32_t k = hid - H_BR0, extra = x >> DW_OP2_SHIFT;
+    mk(HC_BR, pos[k >> 1] | ((k & 1u) << 3) | (extra << 4));
+  }
+  else if (hid == H_JMP) mk(HC_JMP, 0);
+  else if (hid == H_RTIM) mk(HC_RTIM, x >> DW_OP2_SHIFT);
+  else x += HC_COLD;                                                       // (hid + HC_COLD stays below 128)
+}
+
 // One bank image (4096 bytes; 2 KB carts are passed mirrored) -> 4096 decode entries.  `leader` is the bank-
 // independent leader bitmap (4096 flags) filled by mark_leaders() for every bank of the cartridge first.
 inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, bool f8, DWord *out) {
@@ -137,8 +200,8 @@ inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, bo
         }
       }
     }
-    if ((x & 0x7Fu) == H_SLOW) { out[off].x = H_SLOW | lead; out[off].y = 0; }
-    else { out[off].x = x | lead; out[off].y = payload; }
+    if ((x & 0x7Fu) == H_SLOW) { out[off].x = (HC_COLD + H_SLOW) | lead; out[off].y = 0; }
+    else { hot_class(x, payload); out[off].x = x | lead; out[off].y = payload; }
   }
 }
 

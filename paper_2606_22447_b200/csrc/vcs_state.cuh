@@ -69,13 +69,16 @@ enum SmWord {
   S_LINE, S_FDONE,                 // scanline in frame, frames completed in this step
   S_PORTS, S_INP,                  // RIOT port latches; ina | fire0<<8 | (env index inside the block)<<16
   S_TMR, S_TTICKS,                 // timer state packed as W_TIMER, valid after S_TTICKS cycles of this step
-  S_OBJ = 58,                      // 30 words: cached 160-bit line masks of PF, BL, P0, P1, M0, M1 (5 words each);
+  S_STATUS, S_FSTART,              // status bits | ROM index << 8; value of the step's cycle count at which the current frame began
+  S_OBJ = 60,                      // 30 words: cached 160-bit line masks of PF, BL, P0, P1, M0, M1 (5 words each);
                                    //           a derived cache — also the scratch area of a regroup (vcs_step.cu)
-  S_WORDS = 88,
+  S_WORDS = 90,
   S_MOVED = S_OBJ + 8              // a regroup moves words [0, S_MOVED): the state proper + 8 words of saved CPU registers
 };
-// per-block context, in words after the thread files
-enum CtxWord { C_SCREEN_LO = 0, C_SCREEN_HI, C_Y0, C_FRAMESKIP, C_BATCH, C_ENV0, C_WORDS = 8 };
+static_assert(S_STATUS == 58, "file layout");
+// per-block context, in words after the thread files (block-uniform values the out-of-line paths need)
+enum CtxWord { C_SCREEN_LO = 0, C_SCREEN_HI, C_Y0, C_FRAMESKIP, C_BATCH, C_ENV0, C_CAP, C_ROMOFF, C_REGROUP,
+               C_META_LO, C_META_HI, C_BLOB_LO, C_BLOB_HI, C_DROM_LO, C_DROM_HI, C_WORDS = 16 };
 
 struct RomMeta { uint32_t offset; uint32_t size; uint32_t doff; uint32_t pad; };   // byte offset into the ROM blob, size, word offset into the decode blob
 

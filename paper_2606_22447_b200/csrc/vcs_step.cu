@@ -48,6 +48,20 @@ const uint16_t *host_optable() { return kOpTable; }
 constexpr int32_t LIM_NOW = (int32_t)0x80000000;     // `lim` value that forces the slow pre-check
 constexpr uint32_t KEY_PARKED = 0xFFFE0000u;         // keys >= this: parked for a regroup / finished the step
 constexpr uint32_t NOSLOT = 0xFFFFFFFFu;             // a thread of the spare warp that holds no environment right now
+constexpr int32_t LIM_WSYNC = LIM_NOW + 1;            // `lim` while WSYNC holds the CPU (and nothing else is pending)
+
+// What the inline interpreter loop keeps in registers.  A, X, Y, SP are the four bytes of `axys`, so that "which
+// register" is a byte-permute selector from the decode entry; `fl` holds C, I, D, V at their P-register bits.
+// Everything else of an environment (status, frame start, TIA/RIOT latches, RAM) lives in its shared-memory file
+// and block-uniform values live in the block context; the out-of-line paths below rebuild a full Cpu from both.
+struct Hot {
+  uint32_t axys, fl, zn;               // Z <=> (zn & 0xFF) == 0 ; N <=> (zn & 0x180) != 0
+  uint32_t di, pbase;                  // PC = (pbase + di) & 0xFFFF ; di = bank<<12 | PC & 0xFFF
+  int32_t cyc, lstart, lim;
+  uint32_t keyhi;                      // scheduling key without the PC
+  uint32_t wx, wy;                     // decode entry at (bank, PC)
+  uint32_t aux;                        // return flag of the out-of-line calls
+};
 
 template <int BLOCK, bool ROMS, int THREADS>
 struct Cpu {
@@ -56,7 +70,7 @@ struct Cpu {
   uint32_t A, X, Y, SP;
   uint32_t di, pbase;                  // PC = (pbase + di) & 0xFFFF ; di = bank<<12 | PC & 0xFFF
   uint32_t fC, fV, fDI, zn;            // fDI: bit3 D, bit2 I ; Z <=> (zn & 0xFF) == 0 ; N <=> (zn & 0x180) != 0
-  uint32_t status;
+  uint32_t status, romid;
   // ---- beam / time (cycle counts are relative to the start of this vcs_step call)
   int32_t cyc;        // CPU cycles executed in this step
   int32_t lstart;     // value of `cyc` at which the current scanline began (cycle-in-line n = cyc - lstart, 0..76+)
@@ -78,6 +92,30 @@ struct Cpu {
   uint32_t sl, sl4;   // this thread's file slot (word i of the file lives at smem[i*BLOCK + sl]) and 4*sl
 
   DEV uint32_t &S(int i) const { return T::S(sl, i); }
+
+  // ---- Hot <-> Cpu (the out-of-line paths run on a full Cpu; see struct Hot)
+  DEV void load(const Hot &h, uint32_t slot) {
+    sl = slot; sl4 = 4u * slot;
+    A = h.axys & 0xFFu; X = (h.axys >> 8) & 0xFFu; Y = (h.axys >> 16) & 0xFFu; SP = h.axys >> 24;
+    fC = h.fl & 1u; fDI = h.fl & 0x0Cu; fV = (h.fl >> 6) & 1u; zn = h.zn;
+    di = h.di; pbase = h.pbase; cyc = h.cyc; lstart = h.lstart; lim = h.lim; keyhi = h.keyhi; w = make_uint2(h.wx, h.wy);
+    const uint32_t sw = S(S_STATUS);
+    status = sw & 0xFFu; romid = sw >> 8; fstart = (int32_t)S(S_FSTART); fdone = S(S_FDONE); wsync = (S(S_FL) & TF_WSYNC) != 0;
+    cap = (int32_t)T::ctx(C_CAP); fskip = T::ctx(C_FRAMESKIP); rom_off = T::ctx(C_ROMOFF);
+    auto ptr = [](int lo) { return (unsigned long long)T::ctx(lo) | ((unsigned long long)T::ctx(lo + 1) << 32); };
+    const RomMeta rm = reinterpret_cast<const RomMeta *>(ptr(C_META_LO))[romid];
+    is_f8 = (rm.size == 8192) ? 1u : 0u; rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
+    rom_g = reinterpret_cast<const uint8_t *>(ptr(C_BLOB_LO)) + rm.offset;
+    dr = reinterpret_cast<const uint2 *>(ptr(C_DROM_LO)) + rm.doff;
+    park = T::ctx(C_REGROUP) | ((keyhi == KEY_PARKED) ? 2u : 0u);
+  }
+  DEV Hot store() const {
+    Hot h;
+    h.axys = A | (X << 8) | (Y << 16) | (SP << 24); h.fl = fC | fDI | (fV << 6); h.zn = zn;
+    h.di = di; h.pbase = pbase; h.cyc = cyc; h.lstart = lstart; h.lim = lim; h.keyhi = keyhi; h.wx = w.x; h.wy = w.y; h.aux = 0;
+    S(S_STATUS) = status | (romid << 8); S(S_FSTART) = (uint32_t)fstart;
+    return h;
+  }
 
   DEV uint32_t pc() const { return (pbase + di) & 0xFFFFu; }
   DEV void set_pc(uint32_t p) { const uint32_t nd = (di & 0x1000u) | (p & 0xFFFu); pbase = p - nd; di = nd; }
@@ -111,7 +149,7 @@ struct Cpu {
   }
   // decode entry at (bank, PC); H_SLOW outside cartridge space
   DEV uint2 fetch() const {
-    if (!((pbase + di) & 0x1000u)) return make_uint2(H_SLOW, 0);
+    if (!((pbase + di) & 0x1000u)) return make_uint2(HC_COLD + H_SLOW, 0);
     return __ldg(dr + di);
   }
 
@@ -196,7 +234,7 @@ struct Cpu {
   }
   // lim from (lstart, fstart, wsync, status)
   DEV void relim() {
-    lim = (wsync || (status & (STATUS_ILLEGAL | STATUS_UNMODELLED))) ? LIM_NOW : min(lstart + LINE_CYC, fstart + cap);
+    lim = (status & (STATUS_ILLEGAL | STATUS_UNMODELLED)) ? LIM_NOW : wsync ? LIM_WSYNC : min(lstart + LINE_CYC, fstart + cap);
   }
   // after a TIA access that reported events; fc = cycle count at which a frame that just ended did so
   DEV void tia_events(uint32_t ev, int32_t fc) {
@@ -341,7 +379,7 @@ struct Cpu {
 #pragma unroll 4
       for (int j = 0; j < BLOCK; ++j) { const uint32_t kj = keys[j]; rank += (kj < skey || (kj == skey && (uint32_t)j < sl)) ? 1u : 0u; }
     }
-    constexpr int NB = 11;
+    constexpr int NB = 17;
     static_assert(S_MOVED % NB == 0, "batching");
 #pragma unroll 1
     for (int base = 0; base < S_MOVED; base += NB) {
@@ -389,15 +427,12 @@ struct Cpu {
     }
   }
 
-  // ---------------------------------------------------------------- instructions until the next scheduling point
-  DEV void run_block() {
-    for (;;) {
-      if (cyc >= lim) { if (!slow_pre()) return; }
-      uint32_t cx = w.x, pl = w.y;                         // the entry being executed
-      di += (cx >> DW_LEN_SHIFT) & 0xFFu;
-      uint2 wn = __ldg(dr + di);                           // sequential prefetch
-      cyc += (int32_t)((cx >> DW_CY_SHIFT) & 0xFFu);
-      bool slow = false;                                   // run-time decoded: always refetch and re-schedule afterwards
+  // ---------------------------------------------------------------- the out-of-line executor: ONE instruction
+  // Runs the entry (cx, pl) in the vcs_decode.cuh Hid numbering; di and cyc have already been advanced by the
+  // entry's length and base cycles.  Leaves w = the entry at the new (bank, PC): the caller re-schedules.
+  DEV void exec_one(uint32_t cx, uint32_t pl) {
+    {
+      bool slow = false;                                   // run-time decoded
       uint32_t ea = 0, v = 0, wv = 0, op2 = 0, hid;
       int k = 0, i0 = 0, total = 0;
     dispatch:
@@ -418,7 +453,7 @@ struct Cpu {
           }
           set_pc((pc0 + ln) & 0xFFFFu);
           cyc += (int32_t)((g >> DW_CY_SHIFT) & 0xFFu);
-          cx = g; slow = true; wn.x = DW_LEADER;
+          cx = g; slow = true;
           goto dispatch;
         }
         // ---- immediate (or a fixed ROM byte)
@@ -581,18 +616,192 @@ struct Cpu {
           if (ev) { tia_events(ev, cyc); if (ev & EV_FRAME) goto ctl; }
         } break;
       }
-      // ---- sequential successor
-      w = wn;
-      if (!(w.x & DW_LEADER)) continue;
-      if (slow) w = fetch();
-      return;
-    ctl:                                                   // control transfer, bank access or frame end: refetch, re-schedule
+    }
+    ctl:                                                   // every path ends here: refetch at the new (bank, PC)
       park &= ~4u;
       w = fetch();
-      return;
-    }
   }
 };
+
+// ---- ALU on the packed registers (C.6).  op = read op (vcs_optable.cuh: LDA LDX LDY AND ORA EOR ADC SBC CMP CPX CPY BIT)
+DEV void hot_adc(Hot &h, uint32_t v) {
+  const uint32_t a = h.axys & 0xFFu, C = h.fl & 1u;
+  uint32_t r, c, ov;
+  if (!(h.fl & 8u)) {
+    const uint32_t s = a + v + C;
+    c = s >> 8; ov = ((a ^ s) & (v ^ s) & 0x80u) >> 1; r = s & 0xFFu; h.zn = r;
+  } else {                                                  // NMOS decimal mode
+    int al = (int)(a & 0x0Fu) + (int)(v & 0x0Fu) + (int)C;
+    if (al >= 0x0A) al = ((al + 6) & 0x0F) + 0x10;
+    int s = (int)(a & 0xF0u) + (int)(v & 0xF0u) + al;
+    const int sv = (int)(int8_t)(a & 0xF0u) + (int)(int8_t)(v & 0xF0u) + al;
+    h.zn = (((a + v + C) & 0xFFu) ? 1u : 0u) | (((uint32_t)s & 0x80u) << 1);
+    ov = (sv < -128 || sv > 127) ? 0x40u : 0u;
+    if (s >= 0xA0) s += 0x60;
+    c = (s >= 0x100) ? 1u : 0u;
+    r = (uint32_t)s & 0xFFu;
+  }
+  h.fl = (h.fl & ~0x41u) | c | ov;
+  h.axys = __byte_perm(h.axys, r, 0x3214u);
+}
+DEV void hot_sbc(Hot &h, uint32_t v) {
+  const uint32_t a = h.axys & 0xFFu, C = h.fl & 1u;
+  const uint32_t nb = v ^ 0xFFu, s = a + nb + C;            // flags exactly as binary
+  uint32_t r = s & 0xFFu;
+  h.zn = r;
+  const uint32_t fl = (h.fl & ~0x41u) | (s >> 8) | (((a ^ s) & (nb ^ s) & 0x80u) >> 1);
+  if (h.fl & 8u) {
+    int al = (int)(a & 0x0Fu) - (int)(v & 0x0Fu) + (int)C - 1;
+    if (al < 0) al = ((al - 6) & 0x0F) - 0x10;
+    int d = (int)(a & 0xF0u) - (int)(v & 0xF0u) + al;
+    if (d < 0) d -= 0x60;
+    r = (uint32_t)d & 0xFFu;
+  }
+  h.fl = fl;
+  h.axys = __byte_perm(h.axys, r, 0x3214u);
+}
+DEV void hot_cmp(Hot &h, uint32_t r, uint32_t v) { h.fl = (h.fl & ~1u) | ((r >= v) ? 1u : 0u); h.zn = (r - v) & 0xFFu; }
+DEV void alu(Hot &h, uint32_t op, uint32_t v) {
+  if (op == 0) { h.axys = __byte_perm(h.axys, v, 0x3214u); h.zn = v; return; }                 // LDA (INTIM polls)
+  if (op == 11) { h.zn = (((h.axys & v) & 0xFFu) ? 1u : 0u) | ((v & 0x80u) << 1); h.fl = (h.fl & ~0x40u) | (v & 0x40u); return; }   // BIT
+  uint32_t a = h.axys & 0xFFu;
+  switch (op) {
+    case 1: h.axys = __byte_perm(h.axys, v, 0x3240u); h.zn = v; break;
+    case 2: h.axys = __byte_perm(h.axys, v, 0x3410u); h.zn = v; break;
+    case 3: a &= v; h.axys = __byte_perm(h.axys, a, 0x3214u); h.zn = a; break;
+    case 4: a |= v; h.axys = __byte_perm(h.axys, a, 0x3214u); h.zn = a; break;
+    case 5: a ^= v; h.axys = __byte_perm(h.axys, a, 0x3214u); h.zn = a; break;
+    case 6: hot_adc(h, v); break;
+    case 7: hot_sbc(h, v); break;
+    case 8: hot_cmp(h, a, v); break;
+    case 9: hot_cmp(h, (h.axys >> 8) & 0xFFu, v); break;
+    default: hot_cmp(h, (h.axys >> 16) & 0xFFu, v); break;
+  }
+}
+// RMW ops (ASL LSR ROL ROR INC DEC) on the value s
+DEV uint32_t rmw(Hot &h, uint32_t o, uint32_t s) {
+  const uint32_t C = h.fl & 1u;
+  uint32_t r, c = C;
+  switch (o) {
+    case 0: r = (s << 1) & 0xFFu; c = s >> 7; break;
+    case 1: r = s >> 1; c = s & 1u; break;
+    case 2: r = ((s << 1) | C) & 0xFFu; c = s >> 7; break;
+    case 3: r = (s >> 1) | (C << 7); c = s & 1u; break;
+    case 4: r = (s + 1u) & 0xFFu; break;
+    default: r = (s - 1u) & 0xFFu; break;
+  }
+  h.fl = (h.fl & ~1u) | c;
+  h.zn = r;
+  return r;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Out-of-line paths.  Each takes the Hot registers by value, rebuilds a Cpu, does its work and hands the registers
+// back: the struct copy through the stack is only paid on these (rare) calls, and the instruction cache keeps the
+// inline loop below to itself.
+template <int BLOCK, bool ROMS, int THREADS>
+__device__ __noinline__ Hot cold_exec(Hot h, uint32_t sl, uint32_t cx, uint32_t pl) {       // one instruction
+  Cpu<BLOCK, ROMS, THREADS> c; c.load(h, sl);
+  c.exec_one((cx & 0xFFFFFF80u) | ((cx & 0x7Fu) - HC_COLD), pl);
+  return c.store();
+}
+template <int BLOCK, bool ROMS, int THREADS>
+__device__ __noinline__ Hot cold_pre(Hot h, uint32_t sl) {                                   // cyc >= lim: line end, WSYNC, cap, halt
+  Cpu<BLOCK, ROMS, THREADS> c; c.load(h, sl);
+  const bool ok = c.slow_pre();
+  Hot r = c.store(); r.aux = ok ? 1u : 0u;
+  return r;
+}
+template <int BLOCK, bool ROMS, int THREADS>
+__device__ __noinline__ Hot cold_events(Hot h, uint32_t sl, uint32_t ev) {                   // a TIA write crossed a line / ended a frame
+  Cpu<BLOCK, ROMS, THREADS> c; c.load(h, sl);
+  if (ev & EV_FRAME) c.fdone -= 1;                          // (S_FDONE, loaded above, already counts the frame that just ended)
+  c.tia_events(ev, c.cyc);
+  Hot r = c.store(); r.aux = (ev & EV_FRAME) ? 1u : 0u;
+  return r;
+}
+template <int BLOCK, bool ROMS, int THREADS>
+__device__ __noinline__ uint32_t cold_timer_read(uint32_t sl, uint32_t a, int32_t c) {       // INTIM / TIMINT around the underflow
+  Cpu<BLOCK, ROMS, THREADS> cp; cp.sl = sl; cp.sl4 = 4u * sl;
+  uint32_t timer, sub, shift, tflag;
+  cp.timer_sync(c + 1, timer, sub, shift, tflag);
+  if (!(a & 1u)) { cp.timer_put(timer, sub, shift, 0); return timer; }
+  cp.timer_put(timer, sub, shift, tflag);
+  return tflag << 7;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// The inline interpreter loop: instructions of this lane's min-key group until the next scheduling point.
+template <int BLOCK, bool ROMS, int THREADS>
+DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
+  using T = Tia<BLOCK>;
+  uint8_t *const ramb = reinterpret_cast<uint8_t *>(smem) + 4u * sl;
+  for (;;) {
+    if (h.cyc >= h.lim) { h = cold_pre<BLOCK, ROMS, THREADS>(h, sl); if (!h.aux) return; }
+    const uint32_t cx = h.wx, pl = h.wy;                   // the entry being executed
+    h.di += (cx >> DW_LEN_SHIFT) & 0xFFu;
+    const uint2 wn = __ldg(dr + h.di);                     // sequential prefetch
+    h.cyc += (int32_t)((cx >> DW_CY_SHIFT) & 0xFFu);
+    const uint32_t cls = cx & 0x7Fu, aux = cx >> DW_OP2_SHIFT;
+    uint32_t v;
+    if (cls == HC_ST_TIA) {
+      const uint32_t ev = T::write(sl, pl & 0xFFu, __byte_perm(h.axys, 0u, pl >> 16), h.cyc - 1 - h.lstart);
+      if (ev) {
+        if (ev == EV_WSYNC) h.lim = LIM_WSYNC;
+        else { h.wx = wn.x; h.wy = wn.y; h = cold_events<BLOCK, ROMS, THREADS>(h, sl, ev); if (h.aux) return; continue; }
+      }
+    }
+    else if (cls == HC_LD_IMM) { h.axys = __byte_perm(h.axys, pl, pl >> 16); h.zn = pl & 0xFFu; }
+    else if (cls == HC_BR) {
+      const uint32_t t = (h.fl & 0x41u) | ((h.zn & 0x180u) ? 0x80u : 0u) | ((h.zn & 0xFFu) ? 0u : 2u);
+      if (((t >> (aux & 7u)) & 1u) == ((aux >> 3) & 1u)) { h.di += pl; h.cyc += (int32_t)(aux >> 4); goto ctl; }
+    }
+    else if (cls == HC_RTIM) {                             // absolute read of INTIM / TIMINT in the 4th cycle
+      const uint32_t tw = T::S(sl, S_TMR);
+      const uint32_t d = (uint32_t)(h.cyc - (int32_t)T::S(sl, S_TTICKS));
+      const uint32_t timer = tw & 0xFFu, kk = ((tw >> 16) + d) >> ((tw >> 8) & 0xFu);
+      if (!(tw & 0x1000u) && (int32_t)d > 0 && kk <= timer) v = (pl & 1u) ? 0u : timer - kk;      // before the underflow
+      else v = cold_timer_read<BLOCK, ROMS, THREADS>(sl, pl, h.cyc - 1);
+      goto do_alu;
+    }
+    else if (cls == HC_INCDEC) {
+      v = (__byte_perm(h.axys, 0u, pl) + aux) & 0xFFu;
+      h.axys = __byte_perm(h.axys, v, pl >> 16); h.zn = v;
+    }
+    else if (cls == HC_LD_RAM) { v = ramb[pl & 0xFFFFu]; h.axys = __byte_perm(h.axys, v, pl >> 16); h.zn = v; }
+    else {
+      switch (cls) {
+        case HC_ST_RAM: ramb[pl & 0xFFFFu] = (uint8_t)__byte_perm(h.axys, 0u, pl >> 16); break;
+        case HC_XFER:
+          v = __byte_perm(h.axys, 0u, pl); h.axys = __byte_perm(h.axys, v, pl >> 16);
+          if (aux) h.zn = v;
+          else if (h.keyhi < KEY_PARKED) h.keyhi = (h.keyhi & ~(0xFFu << 17)) | (v << 17);      // TXS: SP is part of the key
+          break;
+        case HC_ALU_IMM: v = pl; goto do_alu;
+        case HC_ALU_RAM: v = ramb[pl]; goto do_alu;
+        case HC_RMW_RAM: v = rmw(h, aux, ramb[pl]); ramb[pl] = (uint8_t)v; break;
+        case HC_ACC: v = rmw(h, aux, h.axys & 0xFFu); h.axys = __byte_perm(h.axys, v, 0x3214u); break;
+        case HC_FLAG: h.fl = (h.fl & ~pl) | (pl >> 16); break;
+        case HC_NOP: break;
+        case HC_JMP: { const uint32_t nd = (h.di & 0x1000u) | (pl & 0xFFFu); h.pbase = pl - nd; h.di = nd; } goto ctl;
+        default:                                           // everything else: out of line, then re-schedule
+          h = cold_exec<BLOCK, ROMS, THREADS>(h, sl, cx, pl);
+          return;
+      }
+    }
+    goto seq;
+  do_alu:
+    alu(h, aux, v);
+  seq:                                                     // sequential successor
+    h.wx = wn.x; h.wy = wn.y;
+    if (!(wn.x & DW_LEADER)) continue;
+    return;
+  ctl:                                                     // taken branch / jump: fetch at the new PC, re-schedule
+    if (!((h.pbase + h.di) & 0x1000u)) { h.wx = HC_COLD + H_SLOW; h.wy = 0; }
+    else { const uint2 t = __ldg(dr + h.di); h.wx = t.x; h.wy = t.y; }
+    return;
+  }
+}
 
 // ---- TMA 1-D bulk copy helpers (cp.async.bulk + mbarrier; SASS: UBLKCP / SYNCS)
 DEV uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -617,12 +826,17 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   const int ei = e0 + tid;                                 // the env this thread starts with
   const bool filed = tid < BLOCK;                          // threads of the spare warp start without a file
   const bool live0 = filed && ei < B;
-  const RomMeta rm = p.rom_meta[p.env_rom[live0 ? ei : e0]];
+  const uint32_t romid = (uint32_t)p.env_rom[live0 ? ei : e0];
+  const RomMeta rm = p.rom_meta[romid];
 
   if (tid == 0) {
     const unsigned long long scr = reinterpret_cast<unsigned long long>(p.screen);
     s_ctx[C_SCREEN_LO] = (uint32_t)scr; s_ctx[C_SCREEN_HI] = (uint32_t)(scr >> 32);
     s_ctx[C_Y0] = (uint32_t)p.y0; s_ctx[C_FRAMESKIP] = (uint32_t)p.frameskip; s_ctx[C_BATCH] = (uint32_t)B; s_ctx[C_ENV0] = (uint32_t)e0;
+    s_ctx[C_CAP] = (uint32_t)(p.max_lines * LINE_CYC); s_ctx[C_ROMOFF] = ROM_OFF;
+    s_ctx[C_REGROUP] = (ROMS && rm.size == 8192 && p.regroup) ? 1u : 0u;
+    auto put = [&](int lo, const void *q) { const unsigned long long v = reinterpret_cast<unsigned long long>(q); s_ctx[lo] = (uint32_t)v; s_ctx[lo + 1] = (uint32_t)(v >> 32); };
+    put(C_META_LO, p.rom_meta); put(C_BLOB_LO, p.rom_blob); put(C_DROM_LO, p.drom);
     if constexpr (ROMS) { mbar_init(smem_u32(&s_bar), 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
   }
   __syncthreads();
@@ -662,7 +876,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   }
   s.di = (bank0 << 12) | (pc0 & 0xFFFu); s.pbase = pc0 - s.di;
   s.fskip = (uint32_t)p.frameskip;
-  s.cyc = 0; s.lstart = -(int32_t)n0; s.fdone = live0 ? 0u : s.fskip;
+  s.cyc = 0; s.lstart = -(int32_t)n0; s.fdone = live0 ? 0u : s.fskip; s.romid = romid;
   s.cap = p.max_lines * LINE_CYC;
   s.is_f8 = (rm.size == 8192);
   const bool regroups = ROMS && s.is_f8 && p.regroup;      // block-uniform
@@ -687,8 +901,13 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   s.wsync = (fl & TF_WSYNC) != 0;
   s.relim(); s.rekey();
   if constexpr (ROMS) mbar_wait(smem_u32(&s_bar), 0);
-  const uint32_t fskip = s.fskip;
-  s.w = live0 ? s.fetch() : make_uint2(H_SLOW, 0);
+  s.w = live0 ? s.fetch() : make_uint2(HC_COLD + H_SLOW, 0);
+  Hot h;
+  if (filed) { if (!live0) T::S(sl, S_FDONE) = s.fskip; h = s.store(); }
+  else { h.axys = h.fl = h.zn = h.di = h.pbase = 0; h.cyc = h.lstart = 0; h.lim = LIM_NOW; h.wx = HC_COLD + H_SLOW; h.wy = 0; h.aux = 0; }
+  h.keyhi = s.keyhi;
+  const uint2 *const dr = s.dr;
+  uint32_t cur = sl;                                       // the file this thread runs (changes at a regroup)
 
   // ---- the hot loop: whole instructions until `frameskip` frame-end events (C.10), min-key lanes first.
   // Line bookkeeping mirrors C.4: the line counter advances with the FIRST cycle of a new line, so an
@@ -696,20 +915,24 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   // makes the finished line "line 0" and the next one line 1).
   for (;;) {
     for (;;) {
-      const uint32_t key = s.keyhi | s.pc();
+      const uint32_t key = h.keyhi | ((h.pbase + h.di) & 0xFFFFu);
       const uint32_t mk = __reduce_min_sync(0xFFFFFFFFu, key);
       if (mk >= KEY_PARKED) break;                         // every lane is parked or has finished the step
-      if (key == mk) s.run_block();
+      if (key == mk) run_block<BLOCK, ROMS, THREADS>(h, dr, cur);
     }
     if (!regroups) break;
-    if (!__syncthreads_or((s.park & 2u) && s.fdone < fskip)) break;      // nobody left to run in this block
+    if (!__syncthreads_or(h.keyhi == KEY_PARKED)) break;   // nobody left to run in this block
+    if (cur != NOSLOT) s.load(h, cur); else { s.sl = NOSLOT; s.fskip = (uint32_t)p.frameskip; s.park = 1u; }
     s.regroup();
+    cur = s.sl;
+    if (cur != NOSLOT) h = s.store(); else h.keyhi = 0xFFFFFFFFu;
   }
-  if (s.sl == NOSLOT) return;
-  const uint32_t fs = s.sl;                                // the file (and env) this thread ends up holding
+  if (cur == NOSLOT) return;
+  const uint32_t fs = cur;                                 // the file (and env) this thread ends up holding
   const int e = e0 + (int)(T::S(fs, S_INP) >> 16);
   const bool live = e < B;
   if (!live) return;
+  s.load(h, fs);
   if (s.cyc - s.lstart > LINE_CYC) { T::line_end(fs); s.lstart += LINE_CYC; }      // the last instruction ran over the line end
   // ---- a16 state store
   {
