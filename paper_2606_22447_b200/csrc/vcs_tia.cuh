@@ -304,9 +304,14 @@ struct Tia {
   static DEV uint32_t dirty(int o) { return TF_DIRTY0 << o; }
   // write of v to register r (= a & 0x3F, one with an effect) in cycle-in-line m -> events
   static DEVNI uint32_t write(uint32_t sl, uint32_t r, uint32_t v, int m) {
-    uint32_t ev = catch_up(sl, m);
+    uint32_t ev = 0;
+    while (m >= LINE_CYC) { line_end(sl); m -= LINE_CYC; ev += EV_CROSS; }
     const int x_now = 3 * (m + 1) - HBLANK;
     uint32_t fl = S(sl, S_FL);
+    // WSYNC, the colour registers, HMxx and HMCLR change neither an object's line mask nor a collision: outside
+    // the rows whose pixels are kept the catch-up can wait for the next write that does (same masks, same result)
+    constexpr unsigned long long LAZY = (1ull << 0x02) | (0xFull << 0x06) | (0x1Full << 0x20) | (1ull << 0x2B);
+    if ((fl & TF_ROWVIS) || !((LAZY >> r) & 1ull)) { render_to(sl, 3u * (uint32_t)(m + 1)); fl = S(sl, S_FL); }
     switch (r) {
       case 0x00: { const bool nv = (v >> 1) & 1u;
                    if ((fl & TF_VSYNC) && !nv) { frame_end(sl, 3u * (uint32_t)(m + 1)); ev |= EV_FRAME; fl = S(sl, S_FL); }
