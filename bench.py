@@ -143,7 +143,8 @@ def main():
     n_roms = 256 if B % 256 == 0 else 1
     w = make_workload(4, batch=B, n_roms=n_roms)
     if world > 1:                                   # every rank its own env seeds / action streams (same ROM set)
-        w.seeds = w.seeds ^ np.uint64(0x1000000 * rank); w._act_seeds = w._act_seeds ^ np.uint64(0x1000000 * rank)
+        from paper_2606_22447_b200.shard import rank_seeds
+        w.seeds = rank_seeds(w.seeds, rank); w._act_seeds = rank_seeds(w._act_seeds, rank)
     env = VCS(w.roms, w.seeds, w.env_rom)
     acts_host = w.actions(0, W + K)
     acts = torch.from_numpy(acts_host).cuda()
@@ -173,11 +174,8 @@ def main():
     total_ms = evs[0].elapsed_time(evs[K])
     kern_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(K)]
     cyc1 = env.regs_host()["cycles"].astype(np.int64).sum()
-    tt = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-    cc = torch.tensor([float(cyc1 - cyc0)], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX); dist.all_reduce(cc, op=dist.ReduceOp.SUM)
-    total_ms = float(tt.item()); cycles = float(cc.item())
+    from paper_2606_22447_b200.shard import reduce_job
+    total_ms, cycles = reduce_job(dist if world > 1 else None, total_ms, float(cyc1 - cyc0), device="cuda")
     value = world * B * K / (total_ms * 1e-3)
 
     # ---- e2e: host-pointer C ABI, copies inside the timed region
@@ -223,17 +221,27 @@ def main():
     work = None
     if not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
-        s = oracle_sample(make_workload(4), max(64, cores), 2, cores)
+        s = oracle_sample(make_workload(4), 32 * cores, 24, cores)       # ~10-20 s of wall clock on the box's cores
         work = s["work"]
         cpu = {"value": s["value"], "unit": "env-steps/s", "cores": cores, "kind": "oracle", "sample": s["sample"],
                "emulated_cycles_per_s": s["cycles_per_s"], "seconds": s["seconds"]}
     # ---- roofline: integer-issue bound.  peak = 148 SM x 4 schedulers x 32 lanes x SM clock (1 warp-instruction
     # per scheduler per clock); achieved = SURVEY §8(d)'s lower-bound work model x envs / kernel time.
     sm_mhz = clocks.get("sm_mhz") or peaks.get("sm_max_mhz") or 1965.0
-    peak = 148 * 4 * 32 * sm_mhz * 1e6
+    nominal = 148 * 4 * 32 * sm_mhz * 1e6
+    from paper_2606_22447_b200.binding import issue_peak
+    peak_mixed, _ = issue_peak(1)                   # alu + fma pipes interleaved: the issue-slot ceiling, measured on this box
+    peak_alu, _ = issue_peak(0)                     # alu pipe alone (16 lanes / scheduler / clk)
+    peak = peak_mixed
     kms = float(np.mean(kern_ms))
-    roof = {"bound": "alu", "unit": "thread-instr/s", "peak": peak, "peak_basis": f"148 SM x 4 x 32 lanes x {sm_mhz:.0f} MHz (median SM clock sampled under load)",
-            "kernel": "vcs_step_kernel", "kernel_ms": kms, "traffic": None}
+    # DRAM bytes of one launch from the committed `ncu --set full` capture of this kernel (profiles/r01_v6_full.txt:
+    # dram__bytes_read.sum + dram__bytes_write.sum); algorithmic bytes are roofline.hbm.algorithmic_bytes_per_launch
+    NCU_DRAM_BYTES = 28.129536e6 + 2.174441e9
+    roof = {"bound": "alu", "unit": "thread-instr/s", "peak": peak,
+            "peak_basis": "vcs_issue_peak(kind=1): LOP3+IMAD chains on all SMs, measured in this run",
+            "peak_alu_pipe_only": peak_alu, "peak_nominal": nominal,
+            "kernel": "vcs_step_kernel", "kernel_ms": kms, "traffic": NCU_DRAM_BYTES if B == 65536 else None,
+            "traffic_unit": "DRAM bytes per launch (ncu, profiles/r01_v6_full.txt)"}
     if work:
         ops = MODEL_PER_INSTR * work["instr"] + MODEL_PER_SEGMENT * work["tia_writes"] + MODEL_PER_LINE * work["lines"]
         roof.update(achieved=ops * B / (kms * 1e-3), algorithmic_thread_instr_per_env_step=ops, work_per_env_step=work)
