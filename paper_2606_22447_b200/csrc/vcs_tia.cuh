@@ -302,12 +302,39 @@ struct Tia {
   }
   static DEV uint32_t flag(uint32_t fl, uint32_t bit, bool on) { return on ? (fl | bit) : (fl & ~bit); }
   static DEV uint32_t dirty(int o) { return TF_DIRTY0 << o; }
+  // does writing v to the VALUE register r leave every TIA latch as it is?  (display kernels re-write the same
+  // playfield / graphics / colour bytes line after line: such a write needs no catch-up and dirties no mask)
+  static DEV bool same(uint32_t sl, uint32_t r, uint32_t v, uint32_t fl) {
+    switch (r) {
+      case 0x04: case 0x05: return byte_of(S(sl, S_NUSIZ), r - 4) == (v & 0x37u);
+      case 0x06: case 0x07: case 0x08: case 0x09: return byte_of(S(sl, S_COLU), r - 6) == (v & 0xFEu);
+      case 0x0A: return byte_of(S(sl, S_PF), 3) == (v & 0x37u);
+      case 0x0B: return ((fl & TF_REFP0) != 0) == (((v >> 3) & 1u) != 0);
+      case 0x0C: return ((fl & TF_REFP1) != 0) == (((v >> 3) & 1u) != 0);
+      case 0x0D: return byte_of(S(sl, S_PF), 0) == (v & 0xF0u);
+      case 0x0E: return byte_of(S(sl, S_PF), 1) == (v & 0xFFu);
+      case 0x0F: return byte_of(S(sl, S_PF), 2) == (v & 0xFFu);
+      case 0x1B: { const uint32_t g = S(sl, S_GRP); return byte_of(g, 0) == (v & 0xFFu) && byte_of(g, 3) == byte_of(g, 2); }
+      case 0x1C: { const uint32_t g = S(sl, S_GRP);
+                   return byte_of(g, 2) == (v & 0xFFu) && byte_of(g, 1) == byte_of(g, 0) && ((fl & TF_ENABL_OLD) != 0) == ((fl & TF_ENABL_NEW) != 0); }
+      case 0x1D: return ((fl & TF_ENAM0) != 0) == (((v >> 1) & 1u) != 0);
+      case 0x1E: return ((fl & TF_ENAM1) != 0) == (((v >> 1) & 1u) != 0);
+      case 0x1F: return ((fl & TF_ENABL_NEW) != 0) == (((v >> 1) & 1u) != 0);
+      case 0x25: return ((fl & TF_VDELP0) != 0) == ((v & 1u) != 0);
+      case 0x26: return ((fl & TF_VDELP1) != 0) == ((v & 1u) != 0);
+      case 0x27: return ((fl & TF_VDELBL) != 0) == ((v & 1u) != 0);
+      case 0x28: return ((fl & TF_RESMP0) != 0) == (((v >> 1) & 1u) != 0);
+      case 0x29: return ((fl & TF_RESMP1) != 0) == (((v >> 1) & 1u) != 0);
+      default: return false;
+    }
+  }
   // write of v to register r (= a & 0x3F, one with an effect) in cycle-in-line m -> events
   static DEVNI uint32_t write(uint32_t sl, uint32_t r, uint32_t v, int m) {
     uint32_t ev = 0;
     while (m >= LINE_CYC) { line_end(sl); m -= LINE_CYC; ev += EV_CROSS; }
     const int x_now = 3 * (m + 1) - HBLANK;
     uint32_t fl = S(sl, S_FL);
+    if (same(sl, r, v, fl)) return ev | ((fl & TF_WSYNC) ? EV_WSYNC : 0u);    // a value register re-written with its value
     // WSYNC, the colour registers, HMxx and HMCLR change neither an object's line mask nor a collision: outside
     // the rows whose pixels are kept the catch-up can wait for the next write that does (same masks, same result)
     constexpr unsigned long long LAZY = (1ull << 0x02) | (0xFull << 0x06) | (0x1Full << 0x20) | (1ull << 0x2B);
