@@ -94,6 +94,7 @@ struct Cpu {
   DEV uint32_t &S(int i) const { return T::S(sl, i); }
 
   // ---- Hot <-> Cpu (the out-of-line paths run on a full Cpu; see struct Hot)
+  template <bool CART = true>
   DEV void load(const Hot &h, uint32_t slot) {
     sl = slot; sl4 = 4u * slot;
     A = h.axys & 0xFFu; X = (h.axys >> 8) & 0xFFu; Y = (h.axys >> 16) & 0xFFu; SP = h.axys >> 24;
@@ -102,11 +103,13 @@ struct Cpu {
     const uint32_t sw = S(S_STATUS);
     status = sw & 0xFFu; romid = sw >> 8; fstart = (int32_t)S(S_FSTART); fdone = S(S_FDONE); wsync = (S(S_FL) & TF_WSYNC) != 0;
     cap = (int32_t)T::ctx(C_CAP); fskip = T::ctx(C_FRAMESKIP); rom_off = T::ctx(C_ROMOFF);
-    auto ptr = [](int lo) { return (unsigned long long)T::ctx(lo) | ((unsigned long long)T::ctx(lo + 1) << 32); };
-    const RomMeta rm = reinterpret_cast<const RomMeta *>(ptr(C_META_LO))[romid];
-    is_f8 = (rm.size == 8192) ? 1u : 0u; rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
-    rom_g = reinterpret_cast<const uint8_t *>(ptr(C_BLOB_LO)) + rm.offset;
-    dr = reinterpret_cast<const uint2 *>(ptr(C_DROM_LO)) + rm.doff;
+    if constexpr (CART) {                                  // (the line-end / event paths never touch the cartridge)
+      auto ptr = [](int lo) { return (unsigned long long)T::ctx(lo) | ((unsigned long long)T::ctx(lo + 1) << 32); };
+      const RomMeta rm = reinterpret_cast<const RomMeta *>(ptr(C_META_LO))[romid];
+      is_f8 = (rm.size == 8192) ? 1u : 0u; rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
+      rom_g = reinterpret_cast<const uint8_t *>(ptr(C_BLOB_LO)) + rm.offset;
+      dr = reinterpret_cast<const uint2 *>(ptr(C_DROM_LO)) + rm.doff;
+    } else { is_f8 = 0; rom_mask = 0xFFFu; rom_g = nullptr; dr = nullptr; }
     park = T::ctx(C_REGROUP) | ((keyhi == KEY_PARKED) ? 2u : 0u);
   }
   DEV Hot store() const {
@@ -707,14 +710,14 @@ __device__ __noinline__ Hot cold_exec(Hot h, uint32_t sl, uint32_t cx, uint32_t 
 }
 template <int BLOCK, bool ROMS, int THREADS>
 __device__ __noinline__ Hot cold_pre(Hot h, uint32_t sl) {                                   // cyc >= lim: line end, WSYNC, cap, halt
-  Cpu<BLOCK, ROMS, THREADS> c; c.load(h, sl);
+  Cpu<BLOCK, ROMS, THREADS> c; c.template load<false>(h, sl);
   const bool ok = c.slow_pre();
   Hot r = c.store(); r.aux = ok ? 1u : 0u;
   return r;
 }
 template <int BLOCK, bool ROMS, int THREADS>
 __device__ __noinline__ Hot cold_events(Hot h, uint32_t sl, uint32_t ev) {                   // a TIA write crossed a line / ended a frame
-  Cpu<BLOCK, ROMS, THREADS> c; c.load(h, sl);
+  Cpu<BLOCK, ROMS, THREADS> c; c.template load<false>(h, sl);
   if (ev & EV_FRAME) c.fdone -= 1;                          // (S_FDONE, loaded above, already counts the frame that just ended)
   c.tia_events(ev, c.cyc);
   Hot r = c.store(); r.aux = (ev & EV_FRAME) ? 1u : 0u;
