@@ -254,7 +254,8 @@ static void tia_write(env_t *e, uint16_t a, uint8_t v, int n) {
 }
 
 /* ------------------------------------------------------- C.4 the cycle protocol */
-typedef struct { env_t *e; const ovcs_config *cfg; } ctx_t;
+struct osoft_cfg_s; struct osoft_acc_s;
+typedef struct { env_t *e; const ovcs_config *cfg; const void *soft; void *acc; int dummy; } ctx_t;   /* soft != NULL: SOFT-STE mode (ovcs_soft.inc) */
 
 static void tick(ctx_t *c) {
   env_t *e = c->e;
@@ -267,16 +268,22 @@ static void tick(ctx_t *c) {
   for (int k = 0; k < 3; k++) tia_clock(e, 3 * n + k, c->cfg->y0);   /* state before the access */
 }
 
+#include "ovcs_soft.inc"   /* SOFT-STE mode primitives (config 5) */
+static uint8_t soft_rom(ctx_t *c, uint16_t a, uint8_t v) { return osoft_rom_read((const osoft_cfg *)c->soft, (osoft_acc *)c->acc, c->e, a, v); }
+static uint8_t soft_ram(ctx_t *c, int cell, uint8_t v) { return osoft_ram_read((const osoft_cfg *)c->soft, (osoft_acc *)c->acc, c->e, cell, v); }
+
 /* C.3 address decode + the access itself (post-tick) */
 static uint8_t bus_read(ctx_t *c, uint16_t addr) {
   env_t *e = c->e; uint16_t a = addr & 0x1FFF;
   while (e->wsync && (e->cyc % LINE_CYC) != 0) tick(c);   /* RDY halts read cycles only [D] */
   tick(c);
-  if (a & 0x1000) { cart_hotspot(e, a); return cart_peek(e, a); }
+  const int dummy = c->dummy; c->dummy = 0;                /* set by DUMMY_READ: a cycle whose value is discarded */
+  if (a & 0x1000) { cart_hotspot(e, a); uint8_t v = cart_peek(e, a); return (c->soft && !dummy) ? soft_rom(c, a, v) : v; }
   if ((a & 0x0080) == 0) return tia_read(e, a);
-  if ((a & 0x0200) == 0) return e->ram[a & 0x7F];
+  if ((a & 0x0200) == 0) { uint8_t v = e->ram[a & 0x7F]; return (c->soft && !dummy) ? soft_ram(c, a & 0x7F, v) : v; }
   return riot_read(e, a);
 }
+#define DUMMY_READ(c, addr) ((c)->dummy = 1, (void)bus_read((c), (addr)))
 static void bus_write(ctx_t *c, uint16_t addr, uint8_t v) {
   env_t *e = c->e; uint16_t a = addr & 0x1FFF;
   tick(c);

@@ -71,6 +71,19 @@ int  ovcs_get_regs(ovcs_t *h, ovcs_regs *out /* [batch] */);
 int  ovcs_get_screen(ovcs_t *h, uint8_t *out /* [batch][210][160] */);
 int  ovcs_destroy(ovcs_t *h);
 
+/* SOFT-STE forward mode (BASELINE config 5; reading R14 in DESIGN.md §2):
+ * ovcs_step_range with every value-carrying ROM/RAM read returned as round(STE(relaxed read at temperature T, hard))
+ * and every branch as round(STE(pc_soft(alpha), pc_hard)), float32.  out: HOST [batch][8] doubles per env for this
+ * call: sum of soft ROM reads, of soft RAM reads, of branch gates, the three counts, STE/hard mismatches (Theorem 1:
+ * always 0) and the largest |soft - hard|. */
+int  ovcs_step_soft_range(ovcs_t *h, const uint8_t *actions, int32_t frameskip, double T, double alpha,
+                          double *out, int32_t lo, int32_t hi);
+/* the soft primitives themselves, for the pins: eq. (6), eq. (10) with window K, eq. (8), eq. (9) in float32 */
+double ovcs_soft_peek(const double *r, int M, int a);
+double ovcs_soft_peek_relaxed(const double *r, int M, int a, double T, int K);
+double ovcs_soft_gate(double alpha, int s, double f);
+float  ovcs_soft_ste(float soft, float hard);
+
 /* Test hooks: one env at a time. */
 int  ovcs_set_action(ovcs_t *h, int32_t env, int32_t action);  /* latch pins only (C.11)  */
 int  ovcs_step_instruction(ovcs_t *h, int32_t env);             /* returns frame-end events */

@@ -13,7 +13,7 @@ import numpy as np
 
 _DIR = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_DIR, "libovcs.so")
-_SRC = [os.path.join(_DIR, f) for f in ("ovcs.c", "ovcs.h", "ovcs_cpu.inc", "ovcs_api.inc")]
+_SRC = [os.path.join(_DIR, f) for f in ("ovcs.c", "ovcs.h", "ovcs_cpu.inc", "ovcs_api.inc", "ovcs_soft.inc")]
 
 
 def build(force: bool = False) -> str:
@@ -21,7 +21,7 @@ def build(force: bool = False) -> str:
     stale = force or not os.path.exists(_SO) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in _SRC)
     if stale:
         tmp = _SO + f".tmp{os.getpid()}"
-        subprocess.check_call(["gcc", "-O2", "-std=c11", "-Wall", "-shared", "-fPIC", "-o", tmp, _SRC[0]], cwd=_DIR)
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-Wall", "-shared", "-fPIC", "-o", tmp, _SRC[0], "-lm"], cwd=_DIR)
         os.replace(tmp, _SO)
     return _SO
 
@@ -74,6 +74,11 @@ def lib():
         L.ovcs_alu_sbc.argtypes = [C.c_int] * 3 + [C.POINTER(C.c_int)] * 2
         L.ovcs_splitmix64.argtypes = [C.POINTER(C.c_uint64)]
         L.ovcs_splitmix64.restype = C.c_uint64
+        L.ovcs_step_soft_range.argtypes = [P, P, C.c_int32, C.c_double, C.c_double, P, C.c_int32, C.c_int32]
+        L.ovcs_soft_peek.argtypes = [P, C.c_int, C.c_int]; L.ovcs_soft_peek.restype = C.c_double
+        L.ovcs_soft_peek_relaxed.argtypes = [P, C.c_int, C.c_int, C.c_double, C.c_int]; L.ovcs_soft_peek_relaxed.restype = C.c_double
+        L.ovcs_soft_gate.argtypes = [C.c_double, C.c_int, C.c_double]; L.ovcs_soft_gate.restype = C.c_double
+        L.ovcs_soft_ste.argtypes = [C.c_float, C.c_float]; L.ovcs_soft_ste.restype = C.c_float
         _lib = L
     return _lib
 
@@ -123,6 +128,20 @@ class OracleVCS:
         with ThreadPoolExecutor(n) as ex:
             rcs = list(ex.map(lambda i: lib().ovcs_step_range(self.h, a.ctypes.data, frameskip, cuts[i], cuts[i + 1]), range(n)))
         assert all(rc == 0 for rc in rcs)
+
+    def step_soft(self, actions, frameskip, T, alpha, threads=1):
+        """SOFT-STE forward step (config 5).  Returns [batch][8] float64: sum_rom, sum_ram, sum_gate, n_rom, n_ram,
+        n_branch, mismatch, max_pull of this call."""
+        a = np.ascontiguousarray(actions, dtype=np.uint8)
+        assert a.shape == (self.batch,)
+        out = np.zeros((self.batch, 8), dtype=np.float64)
+        n = max(1, min(threads, self.batch))
+        cuts = [self.batch * i // n for i in range(n + 1)]
+        with ThreadPoolExecutor(n) as ex:
+            rcs = list(ex.map(lambda i: lib().ovcs_step_soft_range(self.h, a.ctypes.data, frameskip, float(T), float(alpha),
+                                                                    out.ctypes.data, cuts[i], cuts[i + 1]), range(n)))
+        assert all(rc == 0 for rc in rcs)
+        return out
 
     def ram(self):
         out = np.empty((self.batch, 128), dtype=np.uint8); assert lib().ovcs_get_ram(self.h, out.ctypes.data) == 0; return out
