@@ -69,6 +69,19 @@ int vcs_reset(vcs_t h, const uint8_t *mask_dev, void *cuda_stream);
  * frameskip must satisfy 1 <= frameskip and frameskip*max_lines*76 < 2^31. */
 int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_stream);
 
+/* SOFT-STE forward step (BASELINE config 5; "Hard and Soft Execution", eq. (1)-(4), appendix
+ * eq. (6)-(10), L316 "Numerical scope"; reading R14 in DESIGN.md §2).  Same as vcs_step, but every value-carrying
+ * read of cartridge ROM (the bank the CPU sees as a 4096 x 8 {0,1} bit tensor) or RIOT RAM (a 128-cell tape) is
+ * computed as round(STE(soft, hard)) with soft = the relaxed read of eq. (10) at temperature T (window
+ * |k| <= ceil(17 T), clipped to the tensor, normalised over the cells kept), in float32, and every conditional
+ * branch sets PC = round(STE(pc_nb + sigma(alpha z) delta, pc_hard)).  Dispatch is the hard switch.  By the paper's
+ * Theorem 1/3 the resulting state equals vcs_step's bit for bit.
+ * soft_out_dev: DEVICE float[batch][8], overwritten with this call's per-env sums: soft ROM reads, soft RAM reads,
+ * branch gates, the three counts, reads/branches whose rounded STE value differed from the hard one (always 0),
+ * max |soft - hard|.  0 < T <= 60, alpha finite.  Errors as vcs_step. */
+int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float T, float alpha,
+                  float *soft_out_dev, void *cuda_stream);
+
 /* Copies into caller-owned DEVICE buffers. */
 int vcs_get_ram(vcs_t h, uint8_t *out_dev /* [batch][128] */, void *cuda_stream);
 int vcs_get_regs(vcs_t h, vcs_regs *out_dev /* [batch] */, void *cuda_stream);

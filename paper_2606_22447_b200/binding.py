@@ -17,7 +17,7 @@ _SO = os.path.join(_PKG, "libvcsb200.so")
 VCS_OK, VCS_EINVAL, VCS_ECUDA, VCS_ENOMEM, VCS_EROM = 0, -1, -2, -3, -4
 _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
 
-EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
+EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
            "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_launch_count",
            "vcs_optable", "vcs_issue_peak", "vcs_destroy", "vcs_last_error"]
 
@@ -56,6 +56,7 @@ def load_library() -> C.CDLL:
     L.vcs_reset.argtypes = [P, P, P]
     L.vcs_step.argtypes = [P, P, C.c_int32, P]
     L.vcs_step_host.argtypes = [P, P, C.c_int32, P]
+    L.vcs_step_soft.argtypes = [P, P, C.c_int32, C.c_float, C.c_float, P, P]
     for f in ("vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host"):
         getattr(L, f).argtypes = [P, P, P]
     L.vcs_screen_ptr.argtypes = [P, C.POINTER(P)]
@@ -142,6 +143,15 @@ class VCS:
     def step(self, actions, frameskip=4, stream=None):
         assert actions.is_cuda and actions.dtype == self.torch.uint8 and actions.numel() == self.batch and actions.is_contiguous()
         self._chk(self.L.vcs_step(self.h, actions.data_ptr(), int(frameskip), _stream_ptr(stream)), "vcs_step")
+
+    def step_soft(self, actions, frameskip, T, alpha, out=None, stream=None):
+        """SOFT-STE forward step (vcs_step_soft); returns the device float[batch][8] of per-env soft sums."""
+        t = self.torch
+        assert actions.is_cuda and actions.dtype == t.uint8 and actions.numel() == self.batch and actions.is_contiguous()
+        out = t.empty((self.batch, 8), dtype=t.float32, device=self.device) if out is None else out
+        self._chk(self.L.vcs_step_soft(self.h, actions.data_ptr(), int(frameskip), float(T), float(alpha), out.data_ptr(),
+                                       _stream_ptr(stream)), "vcs_step_soft")
+        return out
 
     def get_ram(self, out=None, stream=None):
         t = self.torch

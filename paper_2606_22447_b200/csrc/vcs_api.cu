@@ -1,6 +1,7 @@
 // vcs_api.cu — the extern "C" boundary of libvcsb200 (include/vcs.h), plus the small
 // reset / read-out kernels.  Argument marshalling and launches only: every step of the emulation runs in
 // vcs_step.cu's kernel.  No CPU fallback exists: without a CUDA device vcs_create fails with VCS_ECUDA.
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -91,6 +92,7 @@ StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
   p.actions = actions; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
   p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom;
+  p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0;
   return p;
 }
 
@@ -184,6 +186,17 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   CU(h, cudaMemcpy(h->d_rom_meta, meta.data(), sizeof(RomMeta) * n_roms, cudaMemcpyHostToDevice));
   CU(h, cudaMemcpy(h->d_env_rom, er.data(), sizeof(int32_t) * B, cudaMemcpyHostToDevice));
   CU(h, cudaMemcpy(h->d_seeds, seeds, sizeof(unsigned long long) * B, cudaMemcpyHostToDevice));
+  if (!getenv("VCS_NO_SOFT_ALLOC")) {                                                   // soft mode: every entry decodes at run time (vcs_step_soft)
+    std::vector<DWord> sl(8192 + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});
+    std::vector<RomMeta> ms(meta); for (auto &m : ms) { m.pad = m.doff; m.doff = 0; }     // pad: offset into the W(T) x ROM table
+    h->soft_tab_n = dwords; h->soft_tab_T = -1.f;
+    CU(h, cudaMalloc((void **)&h->d_soft_tab, sizeof(float) * (dwords + 8)));
+    CU(h, cudaMalloc((void **)&h->d_drom_soft, sizeof(DWord) * sl.size()));
+    CU(h, cudaMemcpy(h->d_drom_soft, sl.data(), sizeof(DWord) * sl.size(), cudaMemcpyHostToDevice));
+    CU(h, cudaMalloc((void **)&h->d_rom_meta_soft, sizeof(RomMeta) * n_roms));
+    CU(h, cudaMemcpy(h->d_rom_meta_soft, ms.data(), sizeof(RomMeta) * n_roms, cudaMemcpyHostToDevice));
+    CU(h, cudaMalloc((void **)&h->d_soft_w, sizeof(float) * 1024));
+  }
   upload_optable();
   CU(h, cudaGetLastError());
   int rc = vcs_reset(h, nullptr, nullptr);
@@ -212,6 +225,33 @@ int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_
   cudaError_t ce = launch_step(p, (cudaStream_t)cuda_stream);
   h->launches += 1;
   if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step launch", ce);
+  return VCS_OK;
+}
+
+int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float T, float alpha, float *soft_out_dev, void *cuda_stream) {
+  if (!h) return VCS_EINVAL;
+  if (!actions_dev || !soft_out_dev) return fail(h, VCS_EINVAL, "vcs_step_soft: NULL buffer");
+  if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31)) return fail(h, VCS_EINVAL, "vcs_step_soft: frameskip out of range");
+  if (!(T > 0.f) || T > 60.f || !(alpha == alpha) || alpha > 1e30f || alpha < -1e30f) return fail(h, VCS_EINVAL, "vcs_step_soft: T or alpha out of range");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int K = (int)ceil(17.0 * (double)T); if (K < 1) K = 1; if (K > 1023) K = 1023;
+  float w[1024];
+  for (int k = 0; k <= K; ++k) w[k] = (float)exp(-(double)k / (double)T);
+  CU(h, cudaMemcpyAsync(h->d_soft_w, w, sizeof(float) * (K + 1), cudaMemcpyHostToDevice, s));
+  CU(h, cudaStreamSynchronize(s));                     // (w is on this stack frame)
+  if (h->soft_tab_T != T) {                            // W(T) x ROM once per temperature
+    cudaError_t ce0 = launch_soft_table(h->d_rom_blob, h->d_rom_meta_soft, h->n_roms, h->d_soft_w, K, h->d_soft_tab, s);
+    h->launches += 1;
+    if (ce0 != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_soft table launch", ce0);
+    h->soft_tab_T = T;
+  }
+  CU(h, cudaMemsetAsync(soft_out_dev, 0, sizeof(float) * 8 * (size_t)h->batch, s));
+  StepParams p = params_of(h, actions_dev, frameskip);
+  p.drom = h->d_drom_soft; p.rom_meta = h->d_rom_meta_soft;
+  p.soft_w = h->d_soft_w; p.soft_tab = h->d_soft_tab; p.soft_out = soft_out_dev; p.soft_alpha = alpha; p.soft_K = K;
+  cudaError_t ce = launch_step(p, s);
+  h->launches += 1;
+  if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_soft launch", ce);
   return VCS_OK;
 }
 
@@ -289,7 +329,7 @@ int vcs_destroy(vcs_t h) {
   if (!h) return VCS_EINVAL;
   cudaDeviceSynchronize();
   cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom);
-  cudaFree(h->d_rom_meta); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage);
+  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   delete h;
   return VCS_OK;

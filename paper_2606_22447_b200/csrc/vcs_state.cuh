@@ -78,7 +78,8 @@ enum SmWord {
 static_assert(S_STATUS == 58, "file layout");
 // per-block context, in words after the thread files (block-uniform values the out-of-line paths need)
 enum CtxWord { C_SCREEN_LO = 0, C_SCREEN_HI, C_Y0, C_FRAMESKIP, C_BATCH, C_ENV0, C_CAP, C_ROMOFF, C_REGROUP,
-               C_META_LO, C_META_HI, C_BLOB_LO, C_BLOB_HI, C_DROM_LO, C_DROM_HI, C_WORDS = 16 };
+               C_META_LO, C_META_HI, C_BLOB_LO, C_BLOB_HI, C_DROM_LO, C_DROM_HI,
+               C_SOFT_OUT_LO, C_SOFT_OUT_HI, C_SOFT_W_LO, C_SOFT_W_HI, C_SOFT_K, C_SOFT_ALPHA, C_SOFT_TAB_LO, C_SOFT_TAB_HI, C_WORDS = 24 };
 
 struct RomMeta { uint32_t offset; uint32_t size; uint32_t doff; uint32_t pad; };   // byte offset into the ROM blob, size, word offset into the decode blob
 
@@ -87,6 +88,8 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   int32_t y0, max_lines, f8_start_bank;
   uint32_t *d_st; uint32_t *d_ram; unsigned long long *d_cyc; uint8_t *d_screen;
   uint8_t *d_rom_blob; uint2 *d_drom; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
+  float *d_soft_tab; float soft_tab_T; size_t soft_tab_n;          // W(T) x ROM: the relaxed read of every ROM cell at the cached temperature
+  uint2 *d_drom_soft; RomMeta *d_rom_meta_soft; float *d_soft_w;   // soft mode: an all-H_SLOW decode table (every byte fetched at run time), metas with doff 0, e^{-k/T}
   uint8_t *d_actions_stage;     // for vcs_step_host
   uint8_t *h_pinned; size_t h_pinned_bytes;
   int block;                    // threads (= envs) per block of the interpreter kernel

@@ -63,7 +63,7 @@ struct Hot {
   uint32_t aux;                        // return flag of the out-of-line calls
 };
 
-template <int BLOCK, bool ROMS, int THREADS>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 struct Cpu {
   using T = Tia<BLOCK>;
   // ---- CPU
@@ -90,6 +90,8 @@ struct Cpu {
   const uint2 *dr;         // decode entries of this env's ROM (4096 per bank)
   uint2 w;            // decode entry at (bank, PC) — valid at every scheduling point
   uint32_t sl, sl4;   // this thread's file slot (word i of the file lives at smem[i*BLOCK + sl]) and 4*sl
+  float *soft;        // SOFT-STE mode (vcs_step_soft): this env's 8 output sums, else nullptr
+  const float *soft_tab;   // ... and the relaxed read of every cell of this env's ROM (4096 per bank)
 
   DEV uint32_t &S(int i) const { return T::S(sl, i); }
 
@@ -109,7 +111,11 @@ struct Cpu {
       is_f8 = (rm.size == 8192) ? 1u : 0u; rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
       rom_g = reinterpret_cast<const uint8_t *>(ptr(C_BLOB_LO)) + rm.offset;
       dr = reinterpret_cast<const uint2 *>(ptr(C_DROM_LO)) + rm.doff;
-    } else { is_f8 = 0; rom_mask = 0xFFFu; rom_g = nullptr; dr = nullptr; }
+      if constexpr (SOFT) {
+        soft = reinterpret_cast<float *>(ptr(C_SOFT_OUT_LO)) + 8 * (size_t)(T::ctx(C_ENV0) + (S(S_INP) >> 16));
+        soft_tab = reinterpret_cast<const float *>(ptr(C_SOFT_TAB_LO)) + rm.pad;
+      } else { soft = nullptr; soft_tab = nullptr; }
+    } else { is_f8 = 0; rom_mask = 0xFFFu; rom_g = nullptr; dr = nullptr; soft = nullptr; soft_tab = nullptr; }
     park = T::ctx(C_REGROUP) | ((keyhi == KEY_PARKED) ? 2u : 0u);
   }
   DEV Hot store() const {
@@ -129,7 +135,7 @@ struct Cpu {
   // ------------------------------------------------------------------ RAM (smem, conflict-free)
   DEV uint32_t ram_rd_off(uint32_t off) const { return reinterpret_cast<const uint8_t *>(smem)[off + sl4]; }
   DEV void ram_wr_off(uint32_t off, uint32_t v) { reinterpret_cast<uint8_t *>(smem)[off + sl4] = (uint8_t)v; }
-  DEV uint32_t ram_rd(uint32_t a) const { return ram_rd_off(((a & 0x7Cu) * BLOCK) | (a & 3u)); }
+  DEV uint32_t ram_rd(uint32_t a) { const uint32_t v = ram_rd_off(((a & 0x7Cu) * BLOCK) | (a & 3u)); if constexpr (SOFT) return soft_ram(a & 0x7Fu, v); else return v; }
   DEV void ram_wr(uint32_t a, uint32_t v) { ram_wr_off(((a & 0x7Cu) * BLOCK) | (a & 3u), v); }
 
   // ------------------------------------------------------------------ ROM
@@ -146,9 +152,11 @@ struct Cpu {
       rekey();
     }
   }
-  DEV uint32_t rom_rd(uint32_t a) {            // a = addr & 0x1FFF with A12 set
+  DEV uint32_t rom_rd(uint32_t a, bool value = true) {   // a = addr & 0x1FFF with A12 set; value: the byte is used (not a dummy cycle)
     hotspot(a);
-    return rom_byte((di & 0x1000u) + (a & rom_mask));
+    const uint32_t v = rom_byte((di & 0x1000u) + (a & rom_mask));
+    if constexpr (SOFT) { if (value) return soft_rom(a & 0xFFFu, v); }
+    return v;
   }
   // decode entry at (bank, PC); H_SLOW outside cartridge space
   DEV uint2 fetch() const {
@@ -214,9 +222,9 @@ struct Cpu {
   // side-effect-light read used for instruction bytes, zero-page pointers, JMP() vectors and stack
   // pulls: cartridge (incl. F8 hotspots) or RAM.  Anything else is outside the modelled set (status bit 2).
   DEV void unmodelled() { status |= STATUS_UNMODELLED; lim = LIM_NOW; }
-  DEV uint32_t lite_rd(uint32_t addr) {
+  DEV uint32_t lite_rd(uint32_t addr, bool value = true) {
     const uint32_t a = addr & 0x1FFFu;
-    if (a & 0x1000u) return rom_rd(a);
+    if (a & 0x1000u) return rom_rd(a, value);
     if ((a & 0x0280u) == 0x0080u) return ram_rd(a);
     unmodelled(); return 0;
   }
@@ -269,6 +277,40 @@ struct Cpu {
     const uint32_t r = a & 0x3Fu;
     if (r > 0x2Cu || (r >= 0x15u && r <= 0x1Au) || r == 0x03u) return;      // no effect (audio: PAPER.md L205)
     tia_write(r, v, k);
+  }
+  // ---------------------------------------------------------------- SOFT-STE mode (include/vcs.h vcs_step_soft; eq. 8-10)
+  DEV void soft_note(int k, float soft_v, float hard, float ste) {
+    soft[k] += soft_v; soft[3 + k] += 1.f;
+    if (rintf(ste) != hard) soft[6] += 1.f;
+    if (k < 2) soft[7] = fmaxf(soft[7], fabsf(soft_v - hard));
+  }
+  DEV uint32_t soft_rom(uint32_t o, uint32_t hard) {       // eq. (10) on the 4096 x 8 bit tensor of the visible bank, then STE + round
+    // the ROM is constant, so W(T) x ROM is computed once per temperature (soft_table_kernel): a fetch is one lookup
+    const float sv = __ldg(soft_tab + (di & 0x1000u) + o);
+    const float h = (float)hard, ste = sv + (h - sv);      // eq. (9), forward
+    soft_note(0, sv, h, ste);
+    return (uint32_t)(int)rintf(ste) & 0xFFu;
+  }
+  DEV uint32_t soft_ram(uint32_t cell, uint32_t hard) {    // eq. (10) on the 128-cell RAM tape
+    const int K = (int)T::ctx(C_SOFT_K);
+    const float *wt = reinterpret_cast<const float *>((unsigned long long)T::ctx(C_SOFT_W_LO) | ((unsigned long long)T::ctx(C_SOFT_W_HI) << 32));
+    float num = 0, den = 0;
+    const int lo = max(-K, -(int)cell), hi = min(K, 127 - (int)cell);
+#pragma unroll 1
+    for (int k = lo; k <= hi; ++k) {
+      const float w = __ldg(wt + abs(k));
+      const uint32_t c = (uint32_t)((int)cell + k);
+      num += w * (float)ram_rd_off(((c & 0x7Cu) * BLOCK) | (c & 3u)); den += w;
+    }
+    const float sv = num / den, h = (float)hard, ste = sv + (h - sv);
+    soft_note(1, sv, h, ste);
+    return (uint32_t)(int)rintf(ste) & 0xFFu;
+  }
+  DEV void soft_branch(uint32_t f, float sense, float delta, bool taken) {   // eq. (8) + STE; the PC itself is set by the hard path
+    const float z = sense * (2.f * (float)f - 1.f), alpha = __uint_as_float(T::ctx(C_SOFT_ALPHA));
+    const float g = 1.f / (1.f + expf(-alpha * z));
+    const float pc_nb = (float)pc(), pc_soft = pc_nb + g * delta, pc_hard = pc_nb + (taken ? delta : 0.f);
+    soft_note(2, g, pc_hard, pc_soft + (pc_hard - pc_soft));
   }
   DEV uint32_t pack_p() const {
     return ((zn & 0x180u) ? 0x80u : 0u) | (fV << 6) | 0x20u | fDI | (((zn & 0xFFu) == 0) ? 2u : 0u) | fC;
@@ -447,7 +489,7 @@ struct Cpu {
           uint32_t g = c_gen[opc];
           const uint32_t ln = (g >> DW_LEN_SHIFT) & 0xFFu;
           uint32_t b1 = 0, b2 = 0;
-          if ((g & 0x7Fu) != H_ILL) { b1 = lite_rd(pc0 + 1u); if (ln == 3) b2 = lite_rd(pc0 + 2u); }
+          if ((g & 0x7Fu) != H_ILL) { b1 = lite_rd(pc0 + 1u, ln >= 2 && (g & 0x7Fu) != H_BRK); if (ln == 3) b2 = lite_rd(pc0 + 2u); }
           pl = b1 | (b2 << 8);
           if ((g & 0x7Fu) >= H_BR0 && (g & 0x7Fu) < H_BR0 + 8) {
             const uint32_t next = (pc0 + 2u) & 0xFFFFu, target = (next + (uint32_t)(int32_t)(int8_t)b1) & 0xFFFFu;
@@ -517,14 +559,15 @@ struct Cpu {
         case H_IMP0 + 16: A = Y; zn = A; break;
         case H_IMP0 + 17: SP = X; rekey(); break;
         // ---- branches: payload = signed displacement, op2 = extra cycles when taken
-        case H_BR0 + 0: if (zn & 0x180u) break; goto br_taken;
-        case H_BR0 + 1: if (!(zn & 0x180u)) break; goto br_taken;
-        case H_BR0 + 2: if (fV) break; goto br_taken;
-        case H_BR0 + 3: if (!fV) break; goto br_taken;
-        case H_BR0 + 4: if (fC) break; goto br_taken;
-        case H_BR0 + 5: if (!fC) break; goto br_taken;
-        case H_BR0 + 6: if (!(zn & 0xFFu)) break; goto br_taken;
-        case H_BR0 + 7: if (zn & 0xFFu) break; goto br_taken;
+        case H_BR0 + 0: case H_BR0 + 1: case H_BR0 + 2: case H_BR0 + 3: case H_BR0 + 4: case H_BR0 + 5: case H_BR0 + 6: case H_BR0 + 7: {
+          const uint32_t kk = hid - H_BR0;                 // BPL BMI BVC BVS BCC BCS BNE BEQ: flag N V C Z, taken when flag == kk & 1
+          uint32_t f;
+          switch (kk >> 1) { case 0: f = (zn & 0x180u) ? 1u : 0u; break; case 1: f = fV; break; case 2: f = fC; break;
+                             default: f = (zn & 0xFFu) ? 0u : 1u; break; }
+          const bool taken = f == (kk & 1u);
+          if constexpr (SOFT) soft_branch(f, (kk & 1u) ? 1.f : -1.f, (float)(int32_t)pl, taken);
+          if (!taken) break;
+        } goto br_taken;
         // ---- control transfers and stack
         case H_JMP: set_pc(pl); goto ctl;
         case H_JSR: { const uint32_t ret = (pc() - 1u) & 0xFFFFu;     // address of the 3rd byte
@@ -702,30 +745,30 @@ DEV uint32_t rmw(Hot &h, uint32_t o, uint32_t s) {
 // Out-of-line paths.  Each takes the Hot registers by value, rebuilds a Cpu, does its work and hands the registers
 // back: the struct copy through the stack is only paid on these (rare) calls, and the instruction cache keeps the
 // inline loop below to itself.
-template <int BLOCK, bool ROMS, int THREADS>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 __device__ __noinline__ Hot cold_exec(Hot h, uint32_t sl, uint32_t cx, uint32_t pl) {       // one instruction
-  Cpu<BLOCK, ROMS, THREADS> c; c.load(h, sl);
+  Cpu<BLOCK, ROMS, THREADS, SOFT> c; c.load(h, sl);
   c.exec_one((cx & 0xFFFFFF80u) | ((cx & 0x7Fu) - HC_COLD), pl);
   return c.store();
 }
-template <int BLOCK, bool ROMS, int THREADS>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 __device__ __noinline__ Hot cold_pre(Hot h, uint32_t sl) {                                   // cyc >= lim: line end, WSYNC, cap, halt
-  Cpu<BLOCK, ROMS, THREADS> c; c.template load<false>(h, sl);
+  Cpu<BLOCK, ROMS, THREADS, SOFT> c; c.template load<false>(h, sl);
   const bool ok = c.slow_pre();
   Hot r = c.store(); r.aux = ok ? 1u : 0u;
   return r;
 }
-template <int BLOCK, bool ROMS, int THREADS>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 __device__ __noinline__ Hot cold_events(Hot h, uint32_t sl, uint32_t ev) {                   // a TIA write crossed a line / ended a frame
-  Cpu<BLOCK, ROMS, THREADS> c; c.template load<false>(h, sl);
+  Cpu<BLOCK, ROMS, THREADS, SOFT> c; c.template load<false>(h, sl);
   if (ev & EV_FRAME) c.fdone -= 1;                          // (S_FDONE, loaded above, already counts the frame that just ended)
   c.tia_events(ev, c.cyc);
   Hot r = c.store(); r.aux = (ev & EV_FRAME) ? 1u : 0u;
   return r;
 }
-template <int BLOCK, bool ROMS, int THREADS>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 __device__ __noinline__ uint32_t cold_timer_read(uint32_t sl, uint32_t a, int32_t c) {       // INTIM / TIMINT around the underflow
-  Cpu<BLOCK, ROMS, THREADS> cp; cp.sl = sl; cp.sl4 = 4u * sl;
+  Cpu<BLOCK, ROMS, THREADS, SOFT> cp; cp.sl = sl; cp.sl4 = 4u * sl;
   uint32_t timer, sub, shift, tflag;
   cp.timer_sync(c + 1, timer, sub, shift, tflag);
   if (!(a & 1u)) { cp.timer_put(timer, sub, shift, 0); return timer; }
@@ -735,12 +778,12 @@ __device__ __noinline__ uint32_t cold_timer_read(uint32_t sl, uint32_t a, int32_
 
 // ---------------------------------------------------------------------------------------------------------------
 // The inline interpreter loop: instructions of this lane's min-key group until the next scheduling point.
-template <int BLOCK, bool ROMS, int THREADS>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
   using T = Tia<BLOCK>;
   uint8_t *const ramb = reinterpret_cast<uint8_t *>(smem) + 4u * sl;
   for (;;) {
-    if (h.cyc >= h.lim) { h = cold_pre<BLOCK, ROMS, THREADS>(h, sl); if (!h.aux) return; }
+    if (h.cyc >= h.lim) { h = cold_pre<BLOCK, ROMS, THREADS, SOFT>(h, sl); if (!h.aux) return; }
     const uint32_t cx = h.wx, pl = h.wy;                   // the entry being executed
     h.di += (cx >> DW_LEN_SHIFT) & 0xFFu;
     const uint2 wn = __ldg(dr + h.di);                     // sequential prefetch
@@ -751,7 +794,7 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
       const uint32_t ev = T::write(sl, pl & 0xFFu, __byte_perm(h.axys, 0u, pl >> 16), h.cyc - 1 - h.lstart);
       if (ev) {
         if (ev == EV_WSYNC) h.lim = LIM_WSYNC;
-        else { h.wx = wn.x; h.wy = wn.y; h = cold_events<BLOCK, ROMS, THREADS>(h, sl, ev); if (h.aux) return; continue; }
+        else { h.wx = wn.x; h.wy = wn.y; h = cold_events<BLOCK, ROMS, THREADS, SOFT>(h, sl, ev); if (h.aux) return; continue; }
       }
     }
     else if (cls == HC_LD_IMM) { h.axys = __byte_perm(h.axys, pl, pl >> 16); h.zn = pl & 0xFFu; }
@@ -764,7 +807,7 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
       const uint32_t d = (uint32_t)(h.cyc - (int32_t)T::S(sl, S_TTICKS));
       const uint32_t timer = tw & 0xFFu, kk = ((tw >> 16) + d) >> ((tw >> 8) & 0xFu);
       if (!(tw & 0x1000u) && (int32_t)d > 0 && kk <= timer) v = (pl & 1u) ? 0u : timer - kk;      // before the underflow
-      else v = cold_timer_read<BLOCK, ROMS, THREADS>(sl, pl, h.cyc - 1);
+      else v = cold_timer_read<BLOCK, ROMS, THREADS, SOFT>(sl, pl, h.cyc - 1);
       goto do_alu;
     }
     else if (cls == HC_INCDEC) {
@@ -788,7 +831,7 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
         case HC_NOP: break;
         case HC_JMP: { const uint32_t nd = (h.di & 0x1000u) | (pl & 0xFFFu); h.pbase = pl - nd; h.di = nd; } goto ctl;
         default:                                           // everything else: out of line, then re-schedule
-          h = cold_exec<BLOCK, ROMS, THREADS>(h, sl, cx, pl);
+          h = cold_exec<BLOCK, ROMS, THREADS, SOFT>(h, sl, cx, pl);
           return;
       }
     }
@@ -817,7 +860,7 @@ DEV void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile("{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @!p bra WAIT_%=;\n}" ::"r"(bar), "r"(parity) : "memory");
 }
 
-template <int BLOCK, bool ROMS, int THREADS>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepParams p) {
   using T = Tia<BLOCK>;
   __shared__ __align__(8) unsigned long long s_bar;
@@ -840,6 +883,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     s_ctx[C_REGROUP] = (ROMS && rm.size == 8192 && p.regroup) ? 1u : 0u;
     auto put = [&](int lo, const void *q) { const unsigned long long v = reinterpret_cast<unsigned long long>(q); s_ctx[lo] = (uint32_t)v; s_ctx[lo + 1] = (uint32_t)(v >> 32); };
     put(C_META_LO, p.rom_meta); put(C_BLOB_LO, p.rom_blob); put(C_DROM_LO, p.drom);
+    put(C_SOFT_OUT_LO, p.soft_out); put(C_SOFT_W_LO, p.soft_w); put(C_SOFT_TAB_LO, p.soft_tab); s_ctx[C_SOFT_K] = (uint32_t)p.soft_K; s_ctx[C_SOFT_ALPHA] = __float_as_uint(p.soft_alpha);
     if constexpr (ROMS) { mbar_init(smem_u32(&s_bar), 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
   }
   __syncthreads();
@@ -853,7 +897,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     }
   }
 
-  Cpu<BLOCK, ROMS, THREADS> s;
+  Cpu<BLOCK, ROMS, THREADS, SOFT> s;
   s.sl = filed ? (uint32_t)tid : NOSLOT; s.sl4 = 4u * s.sl;
   const uint32_t sl = s.sl;
   // ---- a1 state load (coalesced SoA)
@@ -921,7 +965,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
       const uint32_t key = h.keyhi | ((h.pbase + h.di) & 0xFFFFu);
       const uint32_t mk = __reduce_min_sync(0xFFFFFFFFu, key);
       if (mk >= KEY_PARKED) break;                         // every lane is parked or has finished the step
-      if (key == mk) run_block<BLOCK, ROMS, THREADS>(h, dr, cur);
+      if (key == mk) run_block<BLOCK, ROMS, THREADS, SOFT>(h, dr, cur);
     }
     if (!regroups) break;
     if (!__syncthreads_or(h.keyhi == KEY_PARKED)) break;   // nobody left to run in this block
@@ -956,32 +1000,62 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   }
 }
 
+// W(T) x ROM: for every cell o of every bank of every cartridge the relaxed read of eq. (10) on the 4096 x 8 bit
+// tensor (byte = sum_j 2^j * bit plane j), window |k| <= K clipped to the bank, normalised over the cells kept.
+// A banded [4096 x 4096] x [4096 x 8] contraction per bank, done once per temperature instead of once per fetch.
+__global__ void soft_table_kernel(const uint8_t *rom_blob, const RomMeta *meta, const float *wt, int K, float *tab) {
+  const RomMeta rm = meta[blockIdx.y];
+  const int nb = (rm.size == 8192) ? 2 : 1;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;            // bank * 4096 + o
+  if (idx >= nb * 4096) return;
+  const int bank = idx >> 12, o = idx & 0xFFF;
+  const uint32_t mask = (rm.size == 2048) ? 0x7FFu : 0xFFFu;
+  const uint8_t *img = rom_blob + rm.offset + bank * 4096;
+  float pl0 = 0, pl1 = 0, pl2 = 0, pl3 = 0, pl4 = 0, pl5 = 0, pl6 = 0, pl7 = 0, den = 0;
+  const int lo = max(-K, -o), hi = min(K, 4095 - o);
+  for (int k = lo; k <= hi; ++k) {
+    const float w = __ldg(wt + abs(k));
+    const uint32_t b = img[(uint32_t)(o + k) & mask];
+    pl0 += w * (float)(b & 1u); pl1 += w * (float)((b >> 1) & 1u); pl2 += w * (float)((b >> 2) & 1u); pl3 += w * (float)((b >> 3) & 1u);
+    pl4 += w * (float)((b >> 4) & 1u); pl5 += w * (float)((b >> 5) & 1u); pl6 += w * (float)((b >> 6) & 1u); pl7 += w * (float)((b >> 7) & 1u);
+    den += w;
+  }
+  const float inv = 1.f / den;
+  tab[rm.pad + idx] = pl0 * inv + 2.f * (pl1 * inv) + 4.f * (pl2 * inv) + 8.f * (pl3 * inv) + 16.f * (pl4 * inv) + 32.f * (pl5 * inv) + 64.f * (pl6 * inv) + 128.f * (pl7 * inv);
+}
+cudaError_t launch_soft_table(const uint8_t *rom_blob, const RomMeta *meta, int n_roms, const float *w, int K, float *tab, cudaStream_t stream) {
+  soft_table_kernel<<<dim3(8192 / 256, n_roms), 256, 0, stream>>>(rom_blob, meta, w, K, tab);
+  return cudaGetLastError();
+}
+
 size_t step_smem_bytes(int block, bool roms, uint32_t max_rom) {
   return (size_t)(S_WORDS * block + C_WORDS) * 4 + (roms ? (max_rom < 4096 ? 4096 : max_rom) + 16 : 0);
 }
 
-template <int BLOCK, bool ROMS, int THREADS>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 static cudaError_t launch_one(const StepParams &p, cudaStream_t stream) {
   const size_t smem_bytes = step_smem_bytes(BLOCK, ROMS, p.max_rom);
   static size_t configured = 0;
   if (configured < smem_bytes) {
-    cudaError_t e = cudaFuncSetAttribute(vcs_step_kernel<BLOCK, ROMS, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    cudaError_t e = cudaFuncSetAttribute(vcs_step_kernel<BLOCK, ROMS, THREADS, SOFT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
     configured = smem_bytes;
   }
   const int grid = (p.batch + BLOCK - 1) / BLOCK;
-  vcs_step_kernel<BLOCK, ROMS, THREADS><<<grid, THREADS, smem_bytes, stream>>>(p);
+  vcs_step_kernel<BLOCK, ROMS, THREADS, SOFT><<<grid, THREADS, smem_bytes, stream>>>(p);
   return cudaGetLastError();
 }
 
 cudaError_t launch_step(const StepParams &p, cudaStream_t stream) {
+  if (p.soft_out)                                          // SOFT-STE mode: one variant (ROM through the read-only path, no regroup)
+    return launch_one<128, false, 128, true>(p, stream);
   if (p.rom_smem && p.regroup && p.max_rom == 8192) {      // F8 carts present: one spare warp per block for the regroup
-    switch (p.block) { case 64: return launch_one<64, true, 96>(p, stream); case 256: return launch_one<256, true, 288>(p, stream); default: return launch_one<128, true, 160>(p, stream); }
+    switch (p.block) { case 64: return launch_one<64, true, 96, false>(p, stream); case 256: return launch_one<256, true, 288, false>(p, stream); default: return launch_one<128, true, 160, false>(p, stream); }
   }
   if (p.rom_smem) {
-    switch (p.block) { case 64: return launch_one<64, true, 64>(p, stream); case 256: return launch_one<256, true, 256>(p, stream); default: return launch_one<128, true, 128>(p, stream); }
+    switch (p.block) { case 64: return launch_one<64, true, 64, false>(p, stream); case 256: return launch_one<256, true, 256, false>(p, stream); default: return launch_one<128, true, 128, false>(p, stream); }
   }
-  switch (p.block) { case 64: return launch_one<64, false, 64>(p, stream); case 256: return launch_one<256, false, 256>(p, stream); default: return launch_one<128, false, 128>(p, stream); }
+  switch (p.block) { case 64: return launch_one<64, false, 64, false>(p, stream); case 256: return launch_one<256, false, 256, false>(p, stream); default: return launch_one<128, false, 128, false>(p, stream); }
 }
 
 }  // namespace vcs

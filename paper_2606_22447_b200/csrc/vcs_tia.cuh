@@ -85,7 +85,7 @@ struct Tia {
     if (o1) { uint32_t c = p + o1; if (c >= 160) c -= 160; obj_or(sl, o, pat, c); }
     if (o2) { uint32_t c = p + o2; if (c >= 160) c -= 160; obj_or(sl, o, pat, c); }
   }
-  static DEV void rebuild_player(uint32_t sl, int p, uint32_t fl) {
+  static DEVNI void rebuild_player(uint32_t sl, int p, uint32_t fl) {      // out of line, one copy: the hot code must stay small (icache)
     obj_clear(sl, OB_P0 + p);
     const uint32_t g = byte_of(S(sl, S_GRP), 2 * p + ((fl & (p ? TF_VDELP1 : TF_VDELP0)) ? 1 : 0));
     if (g == 0) return;
@@ -94,14 +94,14 @@ struct Tia {
     const uint32_t pat = (m == 5) ? expand2(gg) : (m == 7) ? expand4(gg) : gg;
     obj_copies(sl, OB_P0 + p, pat, byte_of(S(sl, S_POS), p), m, fl & (p ? TF_FRESH_P1 : TF_FRESH_P0));
   }
-  static DEV void rebuild_missile(uint32_t sl, int p, uint32_t fl) {
+  static DEVNI void rebuild_missile(uint32_t sl, int p, uint32_t fl) {
     obj_clear(sl, OB_M0 + p);
     if (!(fl & (p ? TF_ENAM1 : TF_ENAM0)) || (fl & (p ? TF_RESMP1 : TF_RESMP0))) return;
     const uint32_t ns = byte_of(S(sl, S_NUSIZ), p);
     const uint32_t pat = (1u << (1u << ((ns >> 4) & 3u))) - 1u;
     obj_copies(sl, OB_M0 + p, pat, byte_of(S(sl, S_POS), 2 + p), ns & 7u, fl & (p ? TF_FRESH_M1 : TF_FRESH_M0));
   }
-  static DEV void rebuild(uint32_t sl, uint32_t fl) {
+  static DEVNI void rebuild(uint32_t sl, uint32_t fl) {
     if (fl & (TF_DIRTY0 << OB_PF)) {
       const uint32_t pf = S(sl, S_PF);
       const uint32_t pf20 = (byte_of(pf, 0) >> 4) | (brev8(byte_of(pf, 1)) << 4) | (byte_of(pf, 2) << 12);
@@ -385,7 +385,7 @@ struct Tia {
                  fl = flag(fl, bit, nv) | dirty(OB_M0 + p); } break;
       case 0x2A: {                                                                              // HMOVE
                  uint32_t pos = S(sl, S_POS), pos2 = S(sl, S_POS2); const uint32_t nus = S(sl, S_NUSIZ);
-#pragma unroll
+#pragma unroll 1
                  for (int k = 0; k < 5; ++k) {
                    const uint32_t h = (k < 4) ? (nus >> (16 + 4 * k)) & 0xFu : byte_of(pos2, 1) & 0xFu;
                    const int s = (h < 8) ? (int)h : (int)h - 16;
