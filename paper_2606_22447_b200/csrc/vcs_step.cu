@@ -42,6 +42,8 @@ void upload_optable() {
   uint32_t g[256];
   for (int i = 0; i < 256; ++i) g[i] = generic_entry((uint32_t)i);
   cudaMemcpyToSymbol(c_gen, g, sizeof(g));
+  uint32_t td[64]; tia_desc_table(td);
+  cudaMemcpyToSymbol(c_tia_desc, td, sizeof(td));
 }
 const uint16_t *host_optable() { return kOpTable; }
 

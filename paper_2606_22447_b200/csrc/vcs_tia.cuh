@@ -55,6 +55,37 @@ DEV uint32_t spread8(uint32_t b) {
 
 enum : uint32_t { EV_FRAME = 1u, EV_WSYNC = 2u, EV_CROSS = 16u };   // EV_CROSS * (line ends performed)
 
+// ---- descriptors of the plain VALUE registers (SURVEY C.8 write effects that are "store a masked field"): the write
+// path handles them with one piece of code instead of one switch case each (the hot code must stay small: icache).
+//   bits 2:0 kind (0 special, 1 field store into a packed word, 2 flag) ; 5:3 word - S_COLU ; 10:6 bit shift of the
+//   field (kind 2: flag bit number) ; 18:11 value mask ; 21:19 right shift applied to the written value first ;
+//   27:22 objects whose line mask the register feeds ; 28 lazy (no catch-up outside kept rows) ; 29 colour (the
+//   pixels before the write are painted with the old value in a kept row) ; 30 the field is a nibble
+constexpr uint32_t tia_field(int word, int shift, uint32_t mask, int pre, uint32_t dirty, bool lazy, bool paint, bool nib) {
+  return 1u | ((uint32_t)(word - S_COLU) << 3) | ((uint32_t)shift << 6) | (mask << 11) | ((uint32_t)pre << 19) | (dirty << 22) |
+         (lazy ? 1u << 28 : 0u) | (paint ? 1u << 29 : 0u) | (nib ? 1u << 30 : 0u);
+}
+constexpr uint32_t tia_flagd(int bit, int pre, uint32_t dirty) { return 2u | ((uint32_t)bit << 6) | ((uint32_t)pre << 19) | (dirty << 22); }
+constexpr int ctz32(uint32_t v) { int n = 0; while (!(v & 1u)) { v >>= 1; ++n; } return n; }
+inline void tia_desc_table(uint32_t *t) {
+  for (int i = 0; i < 64; ++i) t[i] = 0;
+  const uint32_t PF = 1u << OB_PF, BL = 1u << OB_BL, P0 = 1u << OB_P0, P1 = 1u << OB_P1, M0 = 1u << OB_M0, M1 = 1u << OB_M1;
+  t[0x04] = tia_field(S_NUSIZ, 0, 0x37, 0, P0 | M0, false, false, false);
+  t[0x05] = tia_field(S_NUSIZ, 8, 0x37, 0, P1 | M1, false, false, false);
+  for (int k = 0; k < 4; ++k) t[0x06 + k] = tia_field(S_COLU, 8 * k, 0xFE, 0, 0, true, true, false);
+  t[0x0A] = tia_field(S_PF, 24, 0x37, 0, PF | BL, false, false, false);
+  t[0x0D] = tia_field(S_PF, 0, 0xF0, 0, PF, false, false, false);
+  t[0x0E] = tia_field(S_PF, 8, 0xFF, 0, PF, false, false, false);
+  t[0x0F] = tia_field(S_PF, 16, 0xFF, 0, PF, false, false, false);
+  for (int k = 0; k < 4; ++k) t[0x20 + k] = tia_field(S_NUSIZ, 16 + 4 * k, 0x0F, 4, 0, true, false, true);    // HMP0 HMP1 HMM0 HMM1
+  t[0x24] = tia_field(S_POS2, 8, 0x0F, 4, 0, true, false, false);                                            // HMBL
+  t[0x0B] = tia_flagd(ctz32(TF_REFP0), 3, P0); t[0x0C] = tia_flagd(ctz32(TF_REFP1), 3, P1);
+  t[0x1D] = tia_flagd(ctz32(TF_ENAM0), 1, M0); t[0x1E] = tia_flagd(ctz32(TF_ENAM1), 1, M1);
+  t[0x1F] = tia_flagd(ctz32(TF_ENABL_NEW), 1, BL);
+  t[0x25] = tia_flagd(ctz32(TF_VDELP0), 0, P0); t[0x26] = tia_flagd(ctz32(TF_VDELP1), 0, P1); t[0x27] = tia_flagd(ctz32(TF_VDELBL), 0, BL);
+}
+__constant__ uint32_t c_tia_desc[64];
+
 template <int BLOCK>
 struct Tia {
   static DEV uint32_t &S(uint32_t sl, int i) { return smem[i * BLOCK + sl]; }
@@ -306,23 +337,9 @@ struct Tia {
   // playfield / graphics / colour bytes line after line: such a write needs no catch-up and dirties no mask)
   static DEV bool same(uint32_t sl, uint32_t r, uint32_t v, uint32_t fl) {
     switch (r) {
-      case 0x04: case 0x05: return byte_of(S(sl, S_NUSIZ), r - 4) == (v & 0x37u);
-      case 0x06: case 0x07: case 0x08: case 0x09: return byte_of(S(sl, S_COLU), r - 6) == (v & 0xFEu);
-      case 0x0A: return byte_of(S(sl, S_PF), 3) == (v & 0x37u);
-      case 0x0B: return ((fl & TF_REFP0) != 0) == (((v >> 3) & 1u) != 0);
-      case 0x0C: return ((fl & TF_REFP1) != 0) == (((v >> 3) & 1u) != 0);
-      case 0x0D: return byte_of(S(sl, S_PF), 0) == (v & 0xF0u);
-      case 0x0E: return byte_of(S(sl, S_PF), 1) == (v & 0xFFu);
-      case 0x0F: return byte_of(S(sl, S_PF), 2) == (v & 0xFFu);
       case 0x1B: { const uint32_t g = S(sl, S_GRP); return byte_of(g, 0) == (v & 0xFFu) && byte_of(g, 3) == byte_of(g, 2); }
       case 0x1C: { const uint32_t g = S(sl, S_GRP);
                    return byte_of(g, 2) == (v & 0xFFu) && byte_of(g, 1) == byte_of(g, 0) && ((fl & TF_ENABL_OLD) != 0) == ((fl & TF_ENABL_NEW) != 0); }
-      case 0x1D: return ((fl & TF_ENAM0) != 0) == (((v >> 1) & 1u) != 0);
-      case 0x1E: return ((fl & TF_ENAM1) != 0) == (((v >> 1) & 1u) != 0);
-      case 0x1F: return ((fl & TF_ENABL_NEW) != 0) == (((v >> 1) & 1u) != 0);
-      case 0x25: return ((fl & TF_VDELP0) != 0) == ((v & 1u) != 0);
-      case 0x26: return ((fl & TF_VDELP1) != 0) == ((v & 1u) != 0);
-      case 0x27: return ((fl & TF_VDELBL) != 0) == ((v & 1u) != 0);
       case 0x28: return ((fl & TF_RESMP0) != 0) == (((v >> 1) & 1u) != 0);
       case 0x29: return ((fl & TF_RESMP1) != 0) == (((v >> 1) & 1u) != 0);
       default: return false;
@@ -334,11 +351,35 @@ struct Tia {
     while (m >= LINE_CYC) { line_end(sl); m -= LINE_CYC; ev += EV_CROSS; }
     const int x_now = 3 * (m + 1) - HBLANK;
     uint32_t fl = S(sl, S_FL);
-    if (same(sl, r, v, fl)) return ev | ((fl & TF_WSYNC) ? EV_WSYNC : 0u);    // a value register re-written with its value
-    // WSYNC, the colour registers, HMxx and HMCLR change neither an object's line mask nor a collision: outside
-    // the rows whose pixels are kept the catch-up can wait for the next write that does (same masks, same result)
-    constexpr unsigned long long LAZY = (1ull << 0x02) | (0xFull << 0x06) | (0x1Full << 0x20) | (1ull << 0x2B);
-    if ((fl & TF_ROWVIS) || !((LAZY >> r) & 1ull)) { render_to(sl, 3u * (uint32_t)(m + 1)); fl = S(sl, S_FL); }
+    const uint32_t d = c_tia_desc[r];
+    if (d & 3u) {                                          // a plain value register: field store or flag
+      const uint32_t pv = v >> ((d >> 19) & 7u);
+      uint32_t nfl = fl;
+      uint32_t old = 0, neu = 0; int wi = 0;
+      if (d & 1u) {
+        wi = S_COLU + (int)((d >> 3) & 7u);
+        const uint32_t sh = (d >> 6) & 31u, fm = ((d >> 30) & 1u) ? 0xFu : 0xFFu;
+        old = S(sl, wi); neu = (old & ~(fm << sh)) | ((pv & ((d >> 11) & 0xFFu)) << sh);
+        if (neu == old) return ev | ((fl & TF_WSYNC) ? EV_WSYNC : 0u);        // re-written with the value it holds: nothing changes
+      } else {
+        const uint32_t bit = 1u << ((d >> 6) & 31u);
+        nfl = (pv & 1u) ? (fl | bit) : (fl & ~bit);
+        if (nfl == fl) return ev | ((fl & TF_WSYNC) ? EV_WSYNC : 0u);
+      }
+      // colour, HMxx: neither an object mask nor a collision changes, so outside the kept rows the catch-up can wait
+      if ((fl & TF_ROWVIS) || !((d >> 28) & 1u)) {
+        render_to(sl, 3u * (uint32_t)(m + 1));
+        const uint32_t fl2 = S(sl, S_FL); nfl = (nfl & ~(TF_DIRTY_ALL | 0u)) | (fl2 & (TF_DIRTY_ALL | 0u)); fl = fl2;
+        if (((d >> 29) & 1u) && (fl & TF_ROWVIS)) paint_upto(sl, x_now, fl);
+      }
+      if (d & 1u) S(sl, wi) = neu;
+      nfl |= ((d >> 22) & 63u) << 22;
+      S(sl, S_FL) = nfl;
+      return ev | ((nfl & TF_WSYNC) ? EV_WSYNC : 0u);
+    }
+    if (same(sl, r, v, fl)) return ev | ((fl & TF_WSYNC) ? EV_WSYNC : 0u);    // GRPx / RESMPx re-written with what they hold
+    // WSYNC and HMCLR change neither an object's line mask nor a collision: lazy as above
+    if ((fl & TF_ROWVIS) || !(r == 0x02u || r == 0x2Bu)) { render_to(sl, 3u * (uint32_t)(m + 1)); fl = S(sl, S_FL); }
     switch (r) {
       case 0x00: { const bool nv = (v >> 1) & 1u;
                    if ((fl & TF_VSYNC) && !nv) { frame_end(sl, 3u * (uint32_t)(m + 1)); ev |= EV_FRAME; fl = S(sl, S_FL); }
@@ -349,17 +390,6 @@ struct Tia {
                  if ((fl & TF_LATCHEN) && (S(sl, S_INP) & 0x100u)) fl &= ~TF_INPT4_LATCH;
                  break;
       case 0x02: fl |= TF_WSYNC; break;
-      case 0x04: S(sl, S_NUSIZ) = set_byte(S(sl, S_NUSIZ), 0, v & 0x37u); fl |= dirty(OB_P0) | dirty(OB_M0); break;
-      case 0x05: S(sl, S_NUSIZ) = set_byte(S(sl, S_NUSIZ), 1, v & 0x37u); fl |= dirty(OB_P1) | dirty(OB_M1); break;
-      case 0x06: case 0x07: case 0x08: case 0x09:
-                 if (fl & TF_ROWVIS) paint_upto(sl, x_now, fl);
-                 S(sl, S_COLU) = set_byte(S(sl, S_COLU), r - 6, v & 0xFEu); break;
-      case 0x0A: S(sl, S_PF) = set_byte(S(sl, S_PF), 3, v & 0x37u); fl |= dirty(OB_PF) | dirty(OB_BL); break;
-      case 0x0B: fl = flag(fl, TF_REFP0, (v >> 3) & 1u) | dirty(OB_P0); break;
-      case 0x0C: fl = flag(fl, TF_REFP1, (v >> 3) & 1u) | dirty(OB_P1); break;
-      case 0x0D: S(sl, S_PF) = set_byte(S(sl, S_PF), 0, v & 0xF0u); fl |= dirty(OB_PF); break;
-      case 0x0E: S(sl, S_PF) = set_byte(S(sl, S_PF), 1, v); fl |= dirty(OB_PF); break;
-      case 0x0F: S(sl, S_PF) = set_byte(S(sl, S_PF), 2, v); fl |= dirty(OB_PF); break;
       case 0x10: case 0x11: S(sl, S_POS) = set_byte(S(sl, S_POS), r - 0x10, x_now < 0 ? 3 : (x_now + 5) % 160);
                  fl |= (r == 0x10) ? (TF_FRESH_P0 | dirty(OB_P0)) : (TF_FRESH_P1 | dirty(OB_P1)); break;
       case 0x12: case 0x13: S(sl, S_POS) = set_byte(S(sl, S_POS), r - 0x10, x_now < 0 ? 2 : (x_now + 4) % 160);
@@ -369,14 +399,6 @@ struct Tia {
                  fl |= dirty(OB_P0) | dirty(OB_P1); break;
       case 0x1C: { const uint32_t g = S(sl, S_GRP); S(sl, S_GRP) = set_byte(set_byte(g, 2, v), 1, byte_of(g, 0)); }   // GRP1; GRP0_old := GRP0_new
                  fl = flag(fl, TF_ENABL_OLD, fl & TF_ENABL_NEW) | dirty(OB_P0) | dirty(OB_P1) | dirty(OB_BL); break;
-      case 0x1D: fl = flag(fl, TF_ENAM0, (v >> 1) & 1u) | dirty(OB_M0); break;
-      case 0x1E: fl = flag(fl, TF_ENAM1, (v >> 1) & 1u) | dirty(OB_M1); break;
-      case 0x1F: fl = flag(fl, TF_ENABL_NEW, (v >> 1) & 1u) | dirty(OB_BL); break;
-      case 0x20: case 0x21: case 0x22: case 0x23: { const int sh = 16 + 4 * (r - 0x20); S(sl, S_NUSIZ) = (S(sl, S_NUSIZ) & ~(0xFu << sh)) | ((v >> 4) << sh); } break;
-      case 0x24: S(sl, S_POS2) = set_byte(S(sl, S_POS2), 1, v >> 4); break;
-      case 0x25: fl = flag(fl, TF_VDELP0, v & 1u) | dirty(OB_P0); break;
-      case 0x26: fl = flag(fl, TF_VDELP1, v & 1u) | dirty(OB_P1); break;
-      case 0x27: fl = flag(fl, TF_VDELBL, v & 1u) | dirty(OB_BL); break;
       case 0x28: case 0x29: { const int p = r - 0x28; const uint32_t bit = p ? TF_RESMP1 : TF_RESMP0; const bool nv = (v >> 1) & 1u;
                  if ((fl & bit) && !nv) {
                    const uint32_t mm = byte_of(S(sl, S_NUSIZ), p) & 7u, mid = (mm == 5) ? 8u : (mm == 7) ? 16u : 4u;
@@ -399,6 +421,7 @@ struct Tia {
                  if (x_now < 0) fl |= TF_HMBLANK; } break;
       case 0x2B: S(sl, S_NUSIZ) &= 0x0000FFFFu; S(sl, S_POS2) = set_byte(S(sl, S_POS2), 1, 0); break;      // HMCLR
       case 0x2C: S(sl, S_CX) = 0; break;                                                            // CXCLR
+
       default: break;
     }
     S(sl, S_FL) = fl;
