@@ -144,7 +144,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   if (env_rom) memcpy(er.data(), env_rom, sizeof(int32_t) * batch);
   // launch shape: envs per block (VCS_BLOCK=64|128|256 overrides), and whether every block maps to one ROM so
   // that the ROM can be staged in shared memory (otherwise the kernel reads it through the read-only path)
-  int want = 128;
+  int want = (batch >= 32768) ? 256 : 128;           // big batches: 256 envs per block (measured 8 % faster on config 4: fewer, larger regroup domains)
   if (const char *ev = getenv("VCS_BLOCK")) { const int v = atoi(ev); if (v == 64 || v == 128 || v == 256) want = v; }
   h->max_rom = 0;
   for (int r = 0; r < n_roms; ++r) if (roms[r].size > h->max_rom) h->max_rom = roms[r].size;
