@@ -111,7 +111,8 @@ enum HotClass : uint32_t {
   HC_FLAG = 13,      // y = P bits to clear | P bits to set << 16
   HC_NOP = 14,
   HC_JMP = 15,       // y = target
-  HC_COLD = 16       // + Hid: executed by the out-of-line executor
+  HC_SPIN = 16,      // LDA INTIM ; BNE *-3  /  BIT TIMINT ; BPL *-3 : the timer wait loop, fast-forwarded (aux = 0 / 1 ; y = the poll's own entry .x)
+  HC_COLD = 17       // + Hid: executed by the out-of-line executor
 };
 static_assert(HC_COLD + H_COUNT <= 128, "hid is 7 bits");
 
@@ -202,6 +203,23 @@ inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, bo
     }
     if ((x & 0x7Fu) == H_SLOW) { out[off].x = (HC_COLD + H_SLOW) | lead; out[off].y = 0; }
     else { hot_class(x, payload); out[off].x = x | lead; out[off].y = payload; }
+  }
+}
+
+// Timer wait loops — "LDA INTIM ; BNE back" and "BIT TIMINT ; BPL back", the way every kernel waits for the end of
+// VBLANK / overscan — are marked so that the interpreter can jump to the loop's exit in closed form (same registers,
+// cycles and line ends as running it; see HC_SPIN in vcs_step.cu).  The poll's own entry is kept in .y for the cases
+// the closed form does not cover.
+inline void mark_spins(const uint8_t *img, DWord *out) {
+  for (uint32_t off = 0; off + 5 < DW_SLOW_LIMIT; ++off) {
+    const uint32_t a13 = (img[off + 1] | (img[off + 2] << 8)) & 0x1FFFu;
+    const bool intim = img[off] == 0xAD && (a13 & 0x1285u) == 0x0284u && img[off + 3] == 0xD0;
+    const bool timint = img[off] == 0x2C && (a13 & 0x1285u) == 0x0285u && img[off + 3] == 0x10;
+    if (!(intim || timint) || img[off + 4] != 0xFB) continue;                  // branch back to the poll
+    if (((0x1000u + off + 5u) ^ (0x1000u + off)) & 0xFF00u) continue;          // taken branch must not cross a page (3 cycles)
+    if ((out[off].x & 0x7Fu) != HC_RTIM || (out[off + 3].x & 0x7Fu) != HC_BR) continue;
+    out[off].y = out[off].x & ~DW_LEADER;
+    out[off].x = HC_SPIN | (out[off].x & DW_LEADER) | ((timint ? 1u : 0u) << DW_OP2_SHIFT);
   }
 }
 
