@@ -214,3 +214,47 @@ def test_full_batch_sampled(torch):
     r = g.regs_host()
     assert (r["status"] == 0).all() and (r["frame"] == 12).all()
     assert (abs(r["cycles"].astype(np.int64) - 11 * 19912) < 19912).all()  # every frame is a 262-line NTSC frame (first one starts at reset)
+
+
+def _spin_rom(seed: int) -> bytes:
+    """Timer wait loops in every regime the closed-form fast-forward (HC_SPIN) must get right or hand back to the
+    plain interpreter: all four divisors, INTIM polls that can step over the single cycle TIM1T shows 0, polls started
+    after the underflow, waits with the picture on (line ends render), waits that run into the frame cap."""
+    r = SplitMix64(seed)
+
+    def build(a):
+        a.org(0xF000); a.op("LDX", "imm", 0xFF); a.op("TXS")
+        a.label("top")
+        for i in range(40):
+            div = r.choice(["TIM1T", "TIM8T", "TIM64T", "T1024T"])
+            val = r.rnd(256) if div != "T1024T" else r.rnd(6)
+            if r.chance(1, 2):                                    # picture on or off during the wait
+                a.op("LDA", "imm", r.choice([0, 2])); a.op("STA", "zp", TIA_W["VBLANK"])
+                a.op("LDA", "imm", r.rnd(256)); a.op("STA", "zp", TIA_W[r.choice(["PF1", "GRP0", "COLUBK", "ENABL"])])
+            for _ in range(r.rnd(4)): a.op("NOP")
+            a.op("LDA", "imm", val); a.op("STA", "abs", RIOT[div])
+            if r.chance(1, 4):                                    # let it underflow first: the flag is already set when the poll starts
+                a.op("LDY", "imm", 40 + r.rnd(200)); d = a.newlabel("D"); a.label(d); a.op("DEY"); a.op("BNE", "rel", d)
+            for _ in range(r.rnd(5)): a.op("NOP")
+            w = a.newlabel("W"); a.label(w)
+            if r.chance(1, 2): a.op("LDA", "abs", RIOT["INTIM"]); a.op("BNE", "rel", w)
+            else: a.op("BIT", "abs", RIOT["TIMINT"]); a.op("BPL", "rel", w)
+            a.op("STA", "zp", 0x80 + i); a.op("PHP"); a.op("PLA"); a.op("STA", "zp", 0xC0 + (i & 31))
+            if r.chance(1, 5): a.op("LDA", "imm", 2); a.op("STA", "zp", TIA_W["VSYNC"]); a.op("LDA", "imm", 0); a.op("STA", "zp", TIA_W["VSYNC"])
+        a.op("JMP", "abs", "top")
+    return hand_rom(build)
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_timer_wait_loops(torch, seed):
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    rom = _spin_rom(2000 + seed)
+    seeds = env_seeds(70 + seed, 40)
+    kw = dict(max_lines=90 + 60 * seed)                          # small caps: waits run into the frame cap
+    g, o = VCS([rom], seeds, **kw), OracleVCS([rom], seeds, **kw)
+    for t in range(8):
+        a = np.zeros(40, np.uint8)
+        fs = 1 + t % 4
+        g.step(torch.from_numpy(a).cuda(), fs); o.step(a, fs, threads=NCPU)
+        compare(g, o, f"spin{seed} step {t}")
