@@ -791,32 +791,6 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
     uint2 wn = __ldg(dr + h.di);                           // sequential prefetch
     h.cyc += (int32_t)((cx >> DW_CY_SHIFT) & 0xFFu);
     uint32_t cls = cx & 0x7Fu, aux = cx >> DW_OP2_SHIFT;
-    if (cls == HC_SPIN) {
-      // The timer wait loop in closed form.  Poll i reads the timer in tick cyc + 7 i + 4 (4th cycle of LDA / BIT abs;
-      // a taken branch back is 3 cycles); the loop leaves with the first poll that reads INTIM == 0 (aux 0) or TIMINT
-      // bit 7 set (aux 1), 2 cycles later.  Covered: no underflow flag set yet, the deciding poll lands while the
-      // value is 0 / right after the underflow, no frame cap on the way.  Nothing in the loop touches the TIA, so
-      // the line ends on the way are all it owes the beam.
-      const uint32_t tw = T::S(sl, S_TMR);
-      const uint32_t shift = (tw >> 8) & 0xFu, sub0 = tw >> 16, tv = tw & 0xFFu;
-      const int32_t dfirst = h.cyc + 4 - (int32_t)T::S(sl, S_TTICKS);
-      const int32_t dz = (int32_t)((tv << shift) - sub0), du = (int32_t)(((tv + 1u) << shift) - sub0);   // ticks until the value is 0 / underflows
-      const int32_t need = aux ? du : dz;
-      const int32_t k = (need > dfirst) ? (need - dfirst + 6) / 7 : 0;
-      const int32_t cend = h.cyc + 7 * k + 6;
-      const int32_t fcap = (int32_t)T::S(sl, S_FSTART) + (int32_t)T::ctx(C_CAP);
-      if (!(tw & 0x1000u) && dfirst > 0 && (aux || dfirst + 7 * k < du) && cend - 2 < fcap) {
-        if (aux) { h.zn = ((h.axys & 0x80u) ? 1u : 0u) | 0x100u; h.fl &= ~0x40u; }      // BIT with v = $80
-        else { h.axys &= ~0xFFu; h.zn = 0; }                                             // LDA with v = 0
-        h.cyc = cend; h.di += 5u;
-        while (h.lstart + LINE_CYC <= cend - 2) { T::line_end(sl); h.lstart += LINE_CYC; }
-        h.lim = min(h.lstart + LINE_CYC, fcap);
-        goto ctl;
-      }
-      cx = pl; pl = 0x0284u | aux;                         // not covered: run the poll itself
-      h.di += 3u; h.cyc += 4; wn = __ldg(dr + h.di);
-      cls = HC_RTIM; aux = cx >> DW_OP2_SHIFT;
-    }
     uint32_t v;
     if (cls == HC_ST_TIA) {
       const uint32_t ev = T::write(sl, pl & 0xFFu, __byte_perm(h.axys, 0u, pl >> 16), h.cyc - 1 - h.lstart);
@@ -831,6 +805,7 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
       if (((t >> (aux & 7u)) & 1u) == ((aux >> 3) & 1u)) { h.di += pl; h.cyc += (int32_t)(aux >> 4); goto ctl; }
     }
     else if (cls == HC_RTIM) {                             // absolute read of INTIM / TIMINT in the 4th cycle
+    do_rtim:
       const uint32_t tw = T::S(sl, S_TMR);
       const uint32_t d = (uint32_t)(h.cyc - (int32_t)T::S(sl, S_TTICKS));
       const uint32_t timer = tw & 0xFFu, kk = ((tw >> 16) + d) >> ((tw >> 8) & 0xFu);
@@ -857,6 +832,32 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
         case HC_ACC: v = rmw(h, aux, h.axys & 0xFFu); h.axys = __byte_perm(h.axys, v, 0x3214u); break;
         case HC_FLAG: h.fl = (h.fl & ~pl) | (pl >> 16); break;
         case HC_NOP: break;
+        case HC_SPIN: {
+      // The timer wait loop in closed form.  Poll i reads the timer in tick cyc + 7 i + 4 (4th cycle of LDA / BIT abs;
+      // a taken branch back is 3 cycles); the loop leaves with the first poll that reads INTIM == 0 (aux 0) or TIMINT
+      // bit 7 set (aux 1), 2 cycles later.  Covered: no underflow flag set yet, the deciding poll lands while the
+      // value is 0 / right after the underflow, no frame cap on the way.  Nothing in the loop touches the TIA, so
+      // the line ends on the way are all it owes the beam.
+      const uint32_t tw = T::S(sl, S_TMR);
+      const uint32_t shift = (tw >> 8) & 0xFu, sub0 = tw >> 16, tv = tw & 0xFFu;
+      const int32_t dfirst = h.cyc + 4 - (int32_t)T::S(sl, S_TTICKS);
+      const int32_t dz = (int32_t)((tv << shift) - sub0), du = (int32_t)(((tv + 1u) << shift) - sub0);   // ticks until the value is 0 / underflows
+      const int32_t need = aux ? du : dz;
+      const int32_t k = (need > dfirst) ? (need - dfirst + 6) / 7 : 0;
+      const int32_t cend = h.cyc + 7 * k + 6;
+      const int32_t fcap = (int32_t)T::S(sl, S_FSTART) + (int32_t)T::ctx(C_CAP);
+      if (!(tw & 0x1000u) && dfirst > 0 && (aux || dfirst + 7 * k < du) && cend - 2 < fcap) {
+        if (aux) { h.zn = ((h.axys & 0x80u) ? 1u : 0u) | 0x100u; h.fl &= ~0x40u; }      // BIT with v = $80
+        else { h.axys &= ~0xFFu; h.zn = 0; }                                             // LDA with v = 0
+        h.cyc = cend; h.di += 5u;
+        while (h.lstart + LINE_CYC <= cend - 2) { T::line_end(sl); h.lstart += LINE_CYC; }
+        h.lim = min(h.lstart + LINE_CYC, fcap);
+        goto ctl;
+      }
+      cx = pl; pl = 0x0284u | aux;                         // not covered: run the poll itself
+      h.di += 3u; h.cyc += 4; wn = __ldg(dr + h.di);
+      aux = cx >> DW_OP2_SHIFT;
+        } goto do_rtim;
         case HC_JMP: { const uint32_t nd = (h.di & 0x1000u) | (pl & 0xFFFu); h.pbase = pl - nd; h.di = nd; } goto ctl;
         default:                                           // everything else: out of line, then re-schedule
           h = cold_exec<BLOCK, ROMS, THREADS, SOFT>(h, sl, cx, pl);
