@@ -778,6 +778,17 @@ __device__ __noinline__ uint32_t cold_timer_read(uint32_t sl, uint32_t a, int32_
   return tflag << 7;
 }
 
+// WSYNC released at the end of the line (a12), the common way a line ends: returns the new `lim`, or LIM_NOW when
+// the case is not the plain one (instruction ran over the line end, frame cap in reach) and cold_pre must decide.
+template <int BLOCK>
+__device__ __noinline__ int32_t wsync_line(uint32_t sl, int32_t cyc, int32_t lstart) {
+  using T = Tia<BLOCK>;
+  const int32_t fcap = (int32_t)T::S(sl, S_FSTART) + (int32_t)T::ctx(C_CAP);
+  if (cyc - lstart > LINE_CYC || lstart + 2 * LINE_CYC >= fcap) return LIM_NOW;
+  T::line_end(sl);
+  return lstart + 2 * LINE_CYC;
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // The inline interpreter loop: instructions of this lane's min-key group until the next scheduling point.
 template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
@@ -785,7 +796,12 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
   using T = Tia<BLOCK>;
   uint8_t *const ramb = reinterpret_cast<uint8_t *>(smem) + 4u * sl;
   for (;;) {
-    if (h.cyc >= h.lim) { h = cold_pre<BLOCK, ROMS, THREADS, SOFT>(h, sl); if (!h.aux) return; }
+    if (h.cyc >= h.lim) {
+      int32_t nl = LIM_NOW;
+      if (h.lim == LIM_WSYNC) nl = wsync_line<BLOCK>(sl, h.cyc, h.lstart);
+      if (nl != LIM_NOW) { h.lstart += LINE_CYC; h.cyc = h.lstart; h.lim = nl; }
+      else { h = cold_pre<BLOCK, ROMS, THREADS, SOFT>(h, sl); if (!h.aux) return; }
+    }
     uint32_t cx = h.wx, pl = h.wy;                         // the entry being executed
     h.di += (cx >> DW_LEN_SHIFT) & 0xFFu;
     uint2 wn = __ldg(dr + h.di);                           // sequential prefetch
