@@ -809,6 +809,10 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
     uint32_t cls = cx & 0x7Fu, aux = cx >> DW_OP2_SHIFT;
     uint32_t v;
     if (cls == HC_ST_TIA) {
+      if ((pl & 0xFFu) == 0x02u && h.cyc - 1 - h.lstart < LINE_CYC) {        // STx WSYNC inside the line: only the latch changes
+        T::S(sl, S_FL) |= TF_WSYNC; h.lim = LIM_WSYNC;
+        goto seq;
+      }
       const uint32_t ev = T::write(sl, pl & 0xFFu, __byte_perm(h.axys, 0u, pl >> 16), h.cyc - 1 - h.lstart);
       if (ev) {
         if (ev == EV_WSYNC) h.lim = LIM_WSYNC;
