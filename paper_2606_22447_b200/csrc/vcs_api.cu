@@ -167,7 +167,8 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
           else memcpy(img.data(), roms[r].data + 4096 * b, 4096);
           if (pass == 0) mark_leaders(img.data(), leader.data());
           else { decode_bank(img.data(), leader.data(), h->block, nb == 2, dw.data() + meta[r].doff + 4096 * b);
-                 if (!getenv("VCS_NO_SPIN")) mark_spins(img.data(), dw.data() + meta[r].doff + 4096 * b); }
+                 if (!getenv("VCS_NO_SPIN")) mark_spins(img.data(), dw.data() + meta[r].doff + 4096 * b);
+                 if (!getenv("VCS_NO_FUSE")) fuse_ld_st(dw.data() + meta[r].doff + 4096 * b); }
         }
     }
   }

@@ -112,7 +112,9 @@ enum HotClass : uint32_t {
   HC_NOP = 14,
   HC_JMP = 15,       // y = target
   HC_SPIN = 16,      // LDA INTIM ; BNE *-3  /  BIT TIMINT ; BPL *-3 : the timer wait loop, fast-forwarded (aux = 0 / 1 ; y = the poll's own entry .x)
-  HC_COLD = 17       // + Hid: executed by the out-of-line executor
+  HC_LDST = 17,      // LDx #imm ; STx <TIA register> as one entry: y = imm | (register | source index << 6) << 8 | insert selector << 16 ;
+                     // aux = 1 when the store is absolute ; cy / len cover both instructions
+  HC_COLD = 18       // + Hid: executed by the out-of-line executor
 };
 static_assert(HC_COLD + H_COUNT <= 128, "hid is 7 bits");
 
@@ -220,6 +222,22 @@ inline void mark_spins(const uint8_t *img, DWord *out) {
     if ((out[off].x & 0x7Fu) != HC_RTIM || (out[off + 3].x & 0x7Fu) != HC_BR) continue;
     out[off].y = out[off].x & ~DW_LEADER;
     out[off].x = HC_SPIN | (out[off].x & DW_LEADER) | ((timint ? 1u : 0u) << DW_OP2_SHIFT);
+  }
+}
+
+// "LDx #imm ; STx reg" pairs — the body of every display kernel — become ONE entry at the load's offset (the store's
+// own entry stays for anyone who jumps to it).  The interpreter still honours the instruction boundary between the
+// two: with a line end / cap / WSYNC release pending there, it runs the load alone and the store as its own entry.
+inline void fuse_ld_st(DWord *out) {
+  for (uint32_t off = 0; off + 5 < DW_SLOW_LIMIT; ++off) {
+    const DWord ld = out[off], st = out[off + 2];
+    if ((ld.x & 0x7Fu) != HC_LD_IMM || ((ld.x >> DW_LEN_SHIFT) & 0xFFu) != 2u) continue;    // (a fixed-ROM-byte load is 3 bytes: not fused)
+    if ((st.x & 0x7Fu) != HC_ST_TIA || (st.x & DW_LEADER)) continue;
+    const uint32_t cy2 = (st.x >> DW_CY_SHIFT) & 0xFFu, len2 = (st.x >> DW_LEN_SHIFT) & 0xFFu;
+    if (off + 2 + len2 >= DW_SLOW_LIMIT) continue;
+    const uint32_t reg = st.y & 0x3Fu, src = (st.y >> 16) & 3u;                             // extract selector 0x4440 | src
+    out[off].x = HC_LDST | (ld.x & DW_LEADER) | ((2u + cy2) << DW_CY_SHIFT) | ((2u + len2) << DW_LEN_SHIFT) | ((len2 - 2u) << DW_OP2_SHIFT);
+    out[off].y = (ld.y & 0xFFu) | ((reg | (src << 6)) << 8) | (ld.y & 0xFFFF0000u);
   }
 }
 

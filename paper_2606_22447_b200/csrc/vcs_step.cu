@@ -808,12 +808,22 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
     h.cyc += (int32_t)((cx >> DW_CY_SHIFT) & 0xFFu);
     uint32_t cls = cx & 0x7Fu, aux = cx >> DW_OP2_SHIFT;
     uint32_t v;
-    if (cls == HC_ST_TIA) {
-      if ((pl & 0xFFu) == 0x02u && h.cyc - 1 - h.lstart < LINE_CYC) {        // STx WSYNC inside the line: only the latch changes
+    if (cls == HC_ST_TIA || cls == HC_LDST) {
+      uint32_t reg = pl & 0xFFu;
+      if (cls == HC_LDST) {                                // LDx #imm ; STx reg in one entry
+        h.axys = __byte_perm(h.axys, pl, pl >> 16); h.zn = pl & 0xFFu;
+        if (h.cyc - 3 - (int32_t)aux >= h.lim) {           // boundary work pending between the two: the store runs as its own entry
+          h.di -= 2u + aux; h.cyc -= 3 + (int32_t)aux;
+          goto ctl;
+        }
+        reg = (pl >> 8) & 0x3Fu;
+        v = __byte_perm(h.axys, 0u, 0x4440u | ((pl >> 14) & 3u));
+      } else v = __byte_perm(h.axys, 0u, pl >> 16);
+      if (reg == 0x02u && h.cyc - 1 - h.lstart < LINE_CYC) {                 // STx WSYNC inside the line: only the latch changes
         T::S(sl, S_FL) |= TF_WSYNC; h.lim = LIM_WSYNC;
         goto seq;
       }
-      const uint32_t ev = T::write(sl, pl & 0xFFu, __byte_perm(h.axys, 0u, pl >> 16), h.cyc - 1 - h.lstart);
+      const uint32_t ev = T::write(sl, reg, v, h.cyc - 1 - h.lstart);
       if (ev) {
         if (ev == EV_WSYNC) h.lim = LIM_WSYNC;
         else { h.wx = wn.x; h.wy = wn.y; h = cold_events<BLOCK, ROMS, THREADS, SOFT>(h, sl, ev); if (h.aux) return; continue; }
