@@ -256,6 +256,8 @@ def main():
                        "batch_per_gpu": B, "frameskip": FRAMESKIP, "l2": "per-step working set 2.2 GB (screens) > 126 MB L2; no explicit flush",
                        "target_env_steps_per_s": 1e7},
             "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, "roofline": roof, "cpu_baseline": cpu}
+    if work:      # the paper's own unit (one step = one CPU instruction), from the oracle's instruction count per env-step
+        line["emulated_instructions_per_s"] = value * work["instr"]
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
