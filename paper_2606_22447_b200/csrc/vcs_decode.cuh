@@ -50,6 +50,9 @@ enum Hid : uint32_t {
 static_assert(H_COUNT <= 128, "hid is 7 bits");
 
 constexpr uint32_t DW_LEADER = 1u << 7;
+// one-bit class flags of the four classes that make up most executed entries (bits 12..15; cy itself is < 16): the
+// interpreter tests them before it looks at the class number at all
+constexpr uint32_t DW_F_LDST = 1u << 12, DW_F_STTIA = 1u << 13, DW_F_LDIMM = 1u << 14, DW_F_BR = 1u << 15;
 constexpr int DW_CY_SHIFT = 8, DW_LEN_SHIFT = 16, DW_OP2_SHIFT = 24;
 constexpr uint32_t DW_SLOW_LIMIT = 0xFF0;      // bank offsets >= this decode to H_SLOW
 
@@ -153,6 +156,8 @@ inline void hot_class(uint32_t &x, uint32_t &y) {
   else if (hid == H_JMP) mk(HC_JMP, 0);
   else if (hid == H_RTIM) mk(HC_RTIM, x >> DW_OP2_SHIFT);
   else x += HC_COLD;                                                       // (hid + HC_COLD stays below 128)
+  const uint32_t hc = x & 0x7Fu;
+  x |= (hc == HC_ST_TIA) ? DW_F_STTIA : (hc == HC_LD_IMM) ? DW_F_LDIMM : (hc == HC_BR) ? DW_F_BR : 0u;
 }
 
 // One bank image (4096 bytes; 2 KB carts are passed mirrored) -> 4096 decode entries.  `leader` is the bank-
@@ -233,10 +238,10 @@ inline void fuse_ld_st(DWord *out) {
     const DWord ld = out[off], st = out[off + 2];
     if ((ld.x & 0x7Fu) != HC_LD_IMM || ((ld.x >> DW_LEN_SHIFT) & 0xFFu) != 2u) continue;    // (a fixed-ROM-byte load is 3 bytes: not fused)
     if ((st.x & 0x7Fu) != HC_ST_TIA || (st.x & DW_LEADER)) continue;
-    const uint32_t cy2 = (st.x >> DW_CY_SHIFT) & 0xFFu, len2 = (st.x >> DW_LEN_SHIFT) & 0xFFu;
+    const uint32_t cy2 = (st.x >> DW_CY_SHIFT) & 0xFu, len2 = (st.x >> DW_LEN_SHIFT) & 0xFFu;
     if (off + 2 + len2 >= DW_SLOW_LIMIT) continue;
     const uint32_t reg = st.y & 0x3Fu, src = (st.y >> 16) & 3u;                             // extract selector 0x4440 | src
-    out[off].x = HC_LDST | (ld.x & DW_LEADER) | ((2u + cy2) << DW_CY_SHIFT) | ((2u + len2) << DW_LEN_SHIFT) | ((len2 - 2u) << DW_OP2_SHIFT);
+    out[off].x = HC_LDST | DW_F_LDST | (ld.x & DW_LEADER) | ((2u + cy2) << DW_CY_SHIFT) | ((2u + len2) << DW_LEN_SHIFT) | ((len2 - 2u) << DW_OP2_SHIFT);
     out[off].y = (ld.y & 0xFFu) | ((reg | (src << 6)) << 8) | (ld.y & 0xFFFF0000u);
   }
 }

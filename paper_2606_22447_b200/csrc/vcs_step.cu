@@ -805,12 +805,12 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
     uint32_t cx = h.wx, pl = h.wy;                         // the entry being executed
     h.di += (cx >> DW_LEN_SHIFT) & 0xFFu;
     uint2 wn = __ldg(dr + h.di);                           // sequential prefetch
-    h.cyc += (int32_t)((cx >> DW_CY_SHIFT) & 0xFFu);
+    h.cyc += (int32_t)((cx >> DW_CY_SHIFT) & 0xFu);
     uint32_t cls = cx & 0x7Fu, aux = cx >> DW_OP2_SHIFT;
     uint32_t v;
-    if (cls == HC_ST_TIA || cls == HC_LDST) {
+    if (cx & (DW_F_LDST | DW_F_STTIA)) {
       uint32_t reg = pl & 0xFFu;
-      if (cls == HC_LDST) {                                // LDx #imm ; STx reg in one entry
+      if (cx & DW_F_LDST) {                                // LDx #imm ; STx reg in one entry
         h.axys = __byte_perm(h.axys, pl, pl >> 16); h.zn = pl & 0xFFu;
         if (h.cyc - 3 - (int32_t)aux >= h.lim) {           // boundary work pending between the two: the store runs as its own entry
           h.di -= 2u + aux; h.cyc -= 3 + (int32_t)aux;
@@ -829,8 +829,8 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
         else { h.wx = wn.x; h.wy = wn.y; h = cold_events<BLOCK, ROMS, THREADS, SOFT>(h, sl, ev); if (h.aux) return; continue; }
       }
     }
-    else if (cls == HC_LD_IMM) { h.axys = __byte_perm(h.axys, pl, pl >> 16); h.zn = pl & 0xFFu; }
-    else if (cls == HC_BR) {
+    else if (cx & DW_F_LDIMM) { h.axys = __byte_perm(h.axys, pl, pl >> 16); h.zn = pl & 0xFFu; }
+    else if (cx & DW_F_BR) {
       const uint32_t t = (h.fl & 0x41u) | ((h.zn & 0x180u) ? 0x80u : 0u) | ((h.zn & 0xFFu) ? 0u : 2u);
       if (((t >> (aux & 7u)) & 1u) == ((aux >> 3) & 1u)) { h.di += pl; h.cyc += (int32_t)(aux >> 4); goto ctl; }
     }
