@@ -451,9 +451,16 @@ struct Cpu {
       uint32_t n0 = 0;
 #pragma unroll 4
       for (int j = 0; j < BLOCK; ++j) n0 += ((keys[j] >> 24) == c0) ? 1u : 0u;
-      const uint32_t t0 = ((n0 + 31u) >> 5) << 5, t = threadIdx.x;
-      if (t < t0) ns = (t < n0) ? t : NOSLOT;
-      else { ns = n0 + (t - t0); if (ns >= (uint32_t)BLOCK) ns = NOSLOT; }
+      // both groups spread evenly over the warps they get (in proportion to their sizes): no nearly empty warp
+      // beside full ones, and fewer lanes per warp means fewer divergent groups to run one after the other
+      constexpr uint32_t NW = THREADS / 32;
+      const uint32_t n1 = (uint32_t)BLOCK - n0;
+      uint32_t w0 = (n0 * NW + (uint32_t)BLOCK / 2u) / (uint32_t)BLOCK;
+      w0 = max(w0, (n0 + 31u) >> 5); w0 = min(w0, NW - ((n1 + 31u) >> 5));          // each group fits its warps
+      const uint32_t w1 = NW - w0, wid = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+      if (wid < w0) { const uint32_t per = (n0 + w0 - 1u) / w0, sidx = wid * per + lane; ns = (lane < per && sidx < n0) ? sidx : NOSLOT; }
+      else if (n1) { const uint32_t per = (n1 + w1 - 1u) / w1, sidx = (wid - w0) * per + lane; ns = (lane < per && sidx < n1) ? n0 + sidx : NOSLOT; }
+      else ns = NOSLOT;
       __syncthreads();                                     // the keys sit in the object-mask cache: nobody resumes before all have read them
     }
     sl = ns; sl4 = 4u * ns;
