@@ -48,7 +48,7 @@ typedef struct {
   uint8_t  bank;             /* current cartridge bank                                             */
   uint16_t line; uint8_t cyc_in_line;    /* beam: scanline in frame, cycles % 76                   */
   uint8_t  status;           /* bit0 undocumented-opcode halt, bit1 frame cap was hit,
-                                bit2 bus pattern outside the kernel's modelled set (see DESIGN.md §7) */
+                                bit2 bus pattern outside the kernel's modelled set (see DESIGN.md §2) */
   uint8_t  intim, timint, _pad[6];       /* timer value and TIMINT bit 7, read without side effects */
 } vcs_regs;
 
@@ -56,6 +56,10 @@ typedef struct {
  * seeds[batch] are HOST arrays.  seeds[e] seeds env e's power-on RAM: the first 16 draws of
  * splitmix64(seeds[e]), little-endian.  cfg NULL = defaults.
  * On return every env is in its reset state (C.2) and the screens are zero.
+ * Layout hint (performance only, never results): when every aligned group of 256 (batches >= 32768), 128 or 64
+ * consecutive envs shares one ROM, the ROM is staged in shared memory per block and F8 carts regroup their envs by
+ * bank inside the block; otherwise ROM bytes come through the read-only cache.  Tuning overrides read here from
+ * the environment: VCS_BLOCK=64|128|256, VCS_ROM_GLOBAL, VCS_NO_REGROUP, VCS_NO_SPIN, VCS_NO_FUSE.
  * Errors: VCS_EINVAL (NULL/size/range), VCS_EROM (size not 2048/4096/8192), VCS_ECUDA, VCS_ENOMEM. */
 int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms,
                const int32_t *env_rom, const uint64_t *seeds, const vcs_config *cfg);
