@@ -258,3 +258,44 @@ def test_timer_wait_loops(torch, seed):
         fs = 1 + t % 4
         g.step(torch.from_numpy(a).cuda(), fs); o.step(a, fs, threads=NCPU)
         compare(g, o, f"spin{seed} step {t}")
+
+
+def test_config2_full_batch_every_env(torch):
+    """BASELINE config 2 at its full batch (1024 envs, one 4 KB ROM, uniform random actions, frameskip 4): every env,
+    RAM + regs + screen, every step (40 of the 500 steps: the oracle pays ~80k cycles per env-step)."""
+    g, o = mk(torch, make_workload(2))
+    w = make_workload(2)
+    acts = w.actions(0, 40)
+    for t in range(40):
+        g.step(torch.from_numpy(acts[t]).cuda(), 4); o.step(acts[t], 4, threads=NCPU)
+        compare(g, o, f"config2 full step {t}")
+
+
+def test_config3_full_batch_sampled(torch):
+    """BASELINE config 3 at its full batch (16,384 envs, sticky actions): the stratified subset e % 128 == 0 is checked
+    against the oracle after every step, 60 steps."""
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    w = make_workload(3)
+    idx = np.arange(0, w.batch, 128)
+    g = VCS(w.roms, w.seeds, w.env_rom)
+    o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx])
+    acts = w.actions(0, 60)
+    for t in range(60):
+        g.step(torch.from_numpy(acts[t]).cuda(), 4); o.step(acts[t][idx], 4, threads=NCPU)
+        compare(g, o, f"config3 full step {t}", envs=idx)
+
+
+def test_config4_full_batch_longer(torch):
+    """Config 4 in bench.py's launch configuration for 12 steps (F8 regroups, spare warp, 256-env blocks), one env per
+    ROM against the oracle at every step, plus batched == same envs run as a small batch on the GPU."""
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    w = make_workload(4)
+    idx = np.arange(256) * 256 + (np.arange(256) * 91) % 256
+    g = VCS(w.roms, w.seeds, w.env_rom)
+    o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx])
+    acts = w.actions(0, 12)
+    for t in range(12):
+        g.step(torch.from_numpy(acts[t]).cuda(), 4); o.step(acts[t][idx], 4, threads=NCPU)
+        compare(g, o, f"config4 long step {t}", envs=idx)
