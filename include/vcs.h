@@ -47,7 +47,7 @@ typedef struct {
   uint16_t pc; uint8_t a, x, y, sp, p;   /* p: bit5 always 1, bit4 always 0                        */
   uint8_t  bank;             /* current cartridge bank                                             */
   uint16_t line; uint8_t cyc_in_line;    /* beam: scanline in frame, cycles % 76                   */
-  uint8_t  status;           /* bit0 undocumented-opcode halt, bit1 frame cap was hit,
+  uint8_t  status;           /* bit0 halt on an unimplemented (undocumented) opcode, bit1 frame cap was hit,
                                 bit2 bus pattern outside the kernel's modelled set */
   uint8_t  intim, timint, _pad[6];       /* timer value and TIMINT bit 7, read without side effects */
 } vcs_regs;
@@ -106,8 +106,9 @@ int vcs_screen_ptr(vcs_t h, const uint8_t **out_dev_ptr);
 int64_t vcs_launch_count(vcs_t h);
 
 /* Introspection, no GPU needed: copies the interpreter's 256-entry decode table (HOST uint16[256];
- * entry = addressing mode | operation<<4 | access kind<<10, operation 0 = undocumented opcode) so that a
- * CPU-only test can check it against the documented 151-opcode matrix. */
+ * entry = addressing mode | operation<<4 | access kind<<10, operation 0 = a byte that halts the CPU) so that a
+ * CPU-only test can check it against the documented 151-opcode matrix plus the paper's 38 undocumented bytes
+ * (USBC, the NOP / LAX / SAX family) that also execute (R12). */
 int vcs_optable(uint16_t *out256_host);
 
 /* Integer-issue micro-benchmark on the current CUDA device: the denominator of the interpreter's roofline

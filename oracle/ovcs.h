@@ -15,7 +15,7 @@
  * the clause it follows.  All readings are listed in DESIGN.md §3.
  *
  * Parity status: pinned by tests/test_oracle_*.py (-m "not gpu") against the opcode
- * matrix, wide-integer ADC/SBC definitions, base-100 BCD arithmetic, the RIOT closed
+ * matrices (151 documented + the paper's 38 undocumented bytes, tests/golden/), wide-integer ADC/SBC definitions, base-100 BCD arithmetic, the RIOT closed
  * form, hand-assembled programs with hand-derived RAM/screens.  PARITY UNPINNED (no
  * source other than the [R] readings exists in this container): per-register TIA write
  * latencies, mid-line HMOVE, RSYNC, double/quad-size player 1-clock shift, bus residue

@@ -177,22 +177,24 @@ inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, bo
     if (op != OP_ILL) {
       const uint32_t a13 = zp ? b1 : abs13;
       const bool is_ram = zp ? (b1 >= 0x80u) : (ab && (a13 & 0x1280u) == 0x0080u);
-      if (mode == MD_IMM) x = dw_x(H_IMM0 + (op - OP_LDA), 2, 2, 0);
-      else if ((zp || ab) && is_ram) {
+      const bool rd_std = kind == K_READ && op <= OP_BIT, wr_std = kind == K_WRITE && op <= OP_STY;   // (LAX / NOPR / SAX stay generic)
+      if (mode == MD_IMM && op <= OP_CPY) x = dw_x(H_IMM0 + (op - OP_LDA), 2, 2, 0);
+      else if (mode == MD_IMM) { /* NOP #imm: generic read */ }
+      else if ((zp || ab) && is_ram && (rd_std || wr_std || kind == K_RMW)) {
         payload = ((a13 & 0x7Cu) * (uint32_t)block) | (a13 & 3u);          // byte offset of the cell in the RAM words
         if (kind == K_READ) x = dw_x(H_ZR0 + (op - OP_LDA), 3 + cyz, len, 0);
         else if (kind == K_WRITE) x = dw_x(H_STZR0 + (op - OP_STA), 3 + cyz, len, 0);
         else x = dw_x(H_MZR0 + (op - OP_ASL), 5 + cyz, len, 0);
       }
-      else if ((zp || ab) && kind == K_WRITE && (a13 & 0x1080u) == 0) {    // a TIA register
+      else if ((zp || ab) && wr_std && (a13 & 0x1080u) == 0) {    // a TIA register
         const uint32_t r = a13 & 0x3Fu;
         if (tia_write_has_effect(r)) { x = dw_x(H_STZT0 + (op - OP_STA), 3 + cyz, len, 0); payload = r; }
         else { x = dw_x(H_NOP, 3 + cyz, len, 0); payload = 0; }
       }
-      else if (ab && kind == K_READ && (a13 & 0x1284u) == 0x0284u) {       // INTIM / TIMINT
+      else if (ab && rd_std && (a13 & 0x1284u) == 0x0284u) {       // INTIM / TIMINT
         x = dw_x(H_RTIM, 4, 3, op - OP_LDA); payload = a13;
       }
-      else if (ab && kind == K_READ && op != OP_BIT && (a13 & 0x1000u) && !(f8 && is_hotspot(a13))) {   // a fixed ROM byte
+      else if (ab && rd_std && op != OP_BIT && (a13 & 0x1000u) && !(f8 && is_hotspot(a13))) {   // a fixed ROM byte
         x = dw_x(H_IMM0 + (op - OP_LDA), 4, 3, 0); payload = img[a13 & 0xFFFu];                        // of this bank
       }
       else if (mode == MD_REL) {

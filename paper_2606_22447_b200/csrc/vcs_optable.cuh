@@ -1,5 +1,6 @@
 // vcs_optable.cuh — 6507 decode table for the CUDA interpreter, in opcode order.
-// The 151 documented NMOS 6502 opcodes (SURVEY.md §8(c) C.5 matrix [D]); every other byte
+// The 151 documented NMOS 6502 opcodes (SURVEY.md §8(c) C.5 matrix [D]) plus the 38 undocumented bytes
+// of the paper's ports (USBC + the NOP / LAX / SAX family: tests/golden/undocumented_opcodes.txt); every other byte
 // decodes to OP_ILL (C.12).  Entry = mode | op<<4 | kind<<10.
 #pragma once
 #include <stdint.h>
@@ -13,8 +14,9 @@ enum Op : uint32_t {
   OP_ILL = 0,
   // K_READ (operand value v)
   OP_LDA, OP_LDX, OP_LDY, OP_AND, OP_ORA, OP_EOR, OP_ADC, OP_SBC, OP_CMP, OP_CPX, OP_CPY, OP_BIT,
+  OP_LAX, OP_NOPR,          // undocumented: A = X = v ; read and discard (NOP with an operand)
   // K_WRITE
-  OP_STA, OP_STX, OP_STY,
+  OP_STA, OP_STX, OP_STY, OP_SAX,     // SAX (undocumented): stores A & X
   // K_RMW (or accumulator)
   OP_ASL, OP_LSR, OP_ROL, OP_ROR, OP_INC, OP_DEC,
   // implied
@@ -39,22 +41,22 @@ static_assert(OP_COUNT <= 64, "op field is 6 bits");
 #define SPC(op) E(OP_##op, MD_SPC, K_NONE)
 
 static const uint16_t kOpTable[256] = {
-  /*00*/ SPC(BRK), RD(ORA, IZX), ILL, ILL, ILL, RD(ORA, ZP), RMW(ASL, ZP), ILL, SPC(PHP), RD(ORA, IMM), ACC(ASL), ILL, ILL, RD(ORA, ABS), RMW(ASL, ABS), ILL,
-  /*10*/ BR(BPL), RD(ORA, IZY), ILL, ILL, ILL, RD(ORA, ZPX), RMW(ASL, ZPX), ILL, IMP(CLC), RD(ORA, ABY), ILL, ILL, ILL, RD(ORA, ABX), RMW(ASL, ABX), ILL,
+  /*00*/ SPC(BRK), RD(ORA, IZX), ILL, ILL, RD(NOPR, ZP), RD(ORA, ZP), RMW(ASL, ZP), ILL, SPC(PHP), RD(ORA, IMM), ACC(ASL), ILL, RD(NOPR, ABS), RD(ORA, ABS), RMW(ASL, ABS), ILL,
+  /*10*/ BR(BPL), RD(ORA, IZY), ILL, ILL, RD(NOPR, ZPX), RD(ORA, ZPX), RMW(ASL, ZPX), ILL, IMP(CLC), RD(ORA, ABY), IMP(NOP), ILL, RD(NOPR, ABX), RD(ORA, ABX), RMW(ASL, ABX), ILL,
   /*20*/ SPC(JSR), RD(AND, IZX), ILL, ILL, RD(BIT, ZP), RD(AND, ZP), RMW(ROL, ZP), ILL, SPC(PLP), RD(AND, IMM), ACC(ROL), ILL, RD(BIT, ABS), RD(AND, ABS), RMW(ROL, ABS), ILL,
-  /*30*/ BR(BMI), RD(AND, IZY), ILL, ILL, ILL, RD(AND, ZPX), RMW(ROL, ZPX), ILL, IMP(SEC), RD(AND, ABY), ILL, ILL, ILL, RD(AND, ABX), RMW(ROL, ABX), ILL,
-  /*40*/ SPC(RTI), RD(EOR, IZX), ILL, ILL, ILL, RD(EOR, ZP), RMW(LSR, ZP), ILL, SPC(PHA), RD(EOR, IMM), ACC(LSR), ILL, SPC(JMP), RD(EOR, ABS), RMW(LSR, ABS), ILL,
-  /*50*/ BR(BVC), RD(EOR, IZY), ILL, ILL, ILL, RD(EOR, ZPX), RMW(LSR, ZPX), ILL, IMP(CLI), RD(EOR, ABY), ILL, ILL, ILL, RD(EOR, ABX), RMW(LSR, ABX), ILL,
-  /*60*/ SPC(RTS), RD(ADC, IZX), ILL, ILL, ILL, RD(ADC, ZP), RMW(ROR, ZP), ILL, SPC(PLA), RD(ADC, IMM), ACC(ROR), ILL, SPC(JMPI), RD(ADC, ABS), RMW(ROR, ABS), ILL,
-  /*70*/ BR(BVS), RD(ADC, IZY), ILL, ILL, ILL, RD(ADC, ZPX), RMW(ROR, ZPX), ILL, IMP(SEI), RD(ADC, ABY), ILL, ILL, ILL, RD(ADC, ABX), RMW(ROR, ABX), ILL,
-  /*80*/ ILL, WRT(STA, IZX), ILL, ILL, WRT(STY, ZP), WRT(STA, ZP), WRT(STX, ZP), ILL, IMP(DEY), ILL, IMP(TXA), ILL, WRT(STY, ABS), WRT(STA, ABS), WRT(STX, ABS), ILL,
-  /*90*/ BR(BCC), WRT(STA, IZY), ILL, ILL, WRT(STY, ZPX), WRT(STA, ZPX), WRT(STX, ZPY), ILL, IMP(TYA), WRT(STA, ABY), IMP(TXS), ILL, ILL, WRT(STA, ABX), ILL, ILL,
-  /*A0*/ RD(LDY, IMM), RD(LDA, IZX), RD(LDX, IMM), ILL, RD(LDY, ZP), RD(LDA, ZP), RD(LDX, ZP), ILL, IMP(TAY), RD(LDA, IMM), IMP(TAX), ILL, RD(LDY, ABS), RD(LDA, ABS), RD(LDX, ABS), ILL,
-  /*B0*/ BR(BCS), RD(LDA, IZY), ILL, ILL, RD(LDY, ZPX), RD(LDA, ZPX), RD(LDX, ZPY), ILL, IMP(CLV), RD(LDA, ABY), IMP(TSX), ILL, RD(LDY, ABX), RD(LDA, ABX), RD(LDX, ABY), ILL,
-  /*C0*/ RD(CPY, IMM), RD(CMP, IZX), ILL, ILL, RD(CPY, ZP), RD(CMP, ZP), RMW(DEC, ZP), ILL, IMP(INY), RD(CMP, IMM), IMP(DEX), ILL, RD(CPY, ABS), RD(CMP, ABS), RMW(DEC, ABS), ILL,
-  /*D0*/ BR(BNE), RD(CMP, IZY), ILL, ILL, ILL, RD(CMP, ZPX), RMW(DEC, ZPX), ILL, IMP(CLD), RD(CMP, ABY), ILL, ILL, ILL, RD(CMP, ABX), RMW(DEC, ABX), ILL,
-  /*E0*/ RD(CPX, IMM), RD(SBC, IZX), ILL, ILL, RD(CPX, ZP), RD(SBC, ZP), RMW(INC, ZP), ILL, IMP(INX), RD(SBC, IMM), IMP(NOP), ILL, RD(CPX, ABS), RD(SBC, ABS), RMW(INC, ABS), ILL,
-  /*F0*/ BR(BEQ), RD(SBC, IZY), ILL, ILL, ILL, RD(SBC, ZPX), RMW(INC, ZPX), ILL, IMP(SED), RD(SBC, ABY), ILL, ILL, ILL, RD(SBC, ABX), RMW(INC, ABX), ILL,
+  /*30*/ BR(BMI), RD(AND, IZY), ILL, ILL, RD(NOPR, ZPX), RD(AND, ZPX), RMW(ROL, ZPX), ILL, IMP(SEC), RD(AND, ABY), IMP(NOP), ILL, RD(NOPR, ABX), RD(AND, ABX), RMW(ROL, ABX), ILL,
+  /*40*/ SPC(RTI), RD(EOR, IZX), ILL, ILL, RD(NOPR, ZP), RD(EOR, ZP), RMW(LSR, ZP), ILL, SPC(PHA), RD(EOR, IMM), ACC(LSR), ILL, SPC(JMP), RD(EOR, ABS), RMW(LSR, ABS), ILL,
+  /*50*/ BR(BVC), RD(EOR, IZY), ILL, ILL, RD(NOPR, ZPX), RD(EOR, ZPX), RMW(LSR, ZPX), ILL, IMP(CLI), RD(EOR, ABY), IMP(NOP), ILL, RD(NOPR, ABX), RD(EOR, ABX), RMW(LSR, ABX), ILL,
+  /*60*/ SPC(RTS), RD(ADC, IZX), ILL, ILL, RD(NOPR, ZP), RD(ADC, ZP), RMW(ROR, ZP), ILL, SPC(PLA), RD(ADC, IMM), ACC(ROR), ILL, SPC(JMPI), RD(ADC, ABS), RMW(ROR, ABS), ILL,
+  /*70*/ BR(BVS), RD(ADC, IZY), ILL, ILL, RD(NOPR, ZPX), RD(ADC, ZPX), RMW(ROR, ZPX), ILL, IMP(SEI), RD(ADC, ABY), IMP(NOP), ILL, RD(NOPR, ABX), RD(ADC, ABX), RMW(ROR, ABX), ILL,
+  /*80*/ RD(NOPR, IMM), WRT(STA, IZX), RD(NOPR, IMM), WRT(SAX, IZX), WRT(STY, ZP), WRT(STA, ZP), WRT(STX, ZP), WRT(SAX, ZP), IMP(DEY), RD(NOPR, IMM), IMP(TXA), ILL, WRT(STY, ABS), WRT(STA, ABS), WRT(STX, ABS), WRT(SAX, ABS),
+  /*90*/ BR(BCC), WRT(STA, IZY), ILL, ILL, WRT(STY, ZPX), WRT(STA, ZPX), WRT(STX, ZPY), WRT(SAX, ZPY), IMP(TYA), WRT(STA, ABY), IMP(TXS), ILL, ILL, WRT(STA, ABX), ILL, ILL,
+  /*A0*/ RD(LDY, IMM), RD(LDA, IZX), RD(LDX, IMM), RD(LAX, IZX), RD(LDY, ZP), RD(LDA, ZP), RD(LDX, ZP), RD(LAX, ZP), IMP(TAY), RD(LDA, IMM), IMP(TAX), ILL, RD(LDY, ABS), RD(LDA, ABS), RD(LDX, ABS), RD(LAX, ABS),
+  /*B0*/ BR(BCS), RD(LDA, IZY), ILL, RD(LAX, IZY), RD(LDY, ZPX), RD(LDA, ZPX), RD(LDX, ZPY), RD(LAX, ZPY), IMP(CLV), RD(LDA, ABY), IMP(TSX), ILL, RD(LDY, ABX), RD(LDA, ABX), RD(LDX, ABY), RD(LAX, ABY),
+  /*C0*/ RD(CPY, IMM), RD(CMP, IZX), RD(NOPR, IMM), ILL, RD(CPY, ZP), RD(CMP, ZP), RMW(DEC, ZP), ILL, IMP(INY), RD(CMP, IMM), IMP(DEX), ILL, RD(CPY, ABS), RD(CMP, ABS), RMW(DEC, ABS), ILL,
+  /*D0*/ BR(BNE), RD(CMP, IZY), ILL, ILL, RD(NOPR, ZPX), RD(CMP, ZPX), RMW(DEC, ZPX), ILL, IMP(CLD), RD(CMP, ABY), IMP(NOP), ILL, RD(NOPR, ABX), RD(CMP, ABX), RMW(DEC, ABX), ILL,
+  /*E0*/ RD(CPX, IMM), RD(SBC, IZX), RD(NOPR, IMM), ILL, RD(CPX, ZP), RD(SBC, ZP), RMW(INC, ZP), ILL, IMP(INX), RD(SBC, IMM), IMP(NOP), RD(SBC, IMM), RD(CPX, ABS), RD(SBC, ABS), RMW(INC, ABS), ILL,
+  /*F0*/ BR(BEQ), RD(SBC, IZY), ILL, ILL, RD(NOPR, ZPX), RD(SBC, ZPX), RMW(INC, ZPX), ILL, IMP(SED), RD(SBC, ABY), IMP(NOP), ILL, RD(NOPR, ABX), RD(SBC, ABX), RMW(INC, ABX), ILL,
 };
 #undef E
 #undef ILL

@@ -364,7 +364,9 @@ struct Cpu {
       case 8: cmp(A, v); break;
       case 9: cmp(X, v); break;
       case 10: cmp(Y, v); break;
-      default: bit(v); break;
+      case 11: bit(v); break;
+      case 12: A = v; X = v; zn = v; break;                // LAX
+      default: break;                                      // NOP with an operand: the read happened, nothing is kept
     }
   }
   DEV uint32_t rmw_op(uint32_t o, uint32_t s) {            // o = op - OP_ASL
@@ -643,7 +645,7 @@ struct Cpu {
           read_op(cx >> DW_OP2_SHIFT, v); goto gen_end;
         do_write:
           op2 = cx >> DW_OP2_SHIFT;
-          wv = (op2 == 0) ? A : (op2 == 1) ? X : Y;
+          wv = (op2 == 0) ? A : (op2 == 1) ? X : (op2 == 2) ? Y : (A & X);      // STA STX STY SAX
           i0 = 1; k -= 1; goto do_store;
         do_rmw:
           v = bus_read(ea, k);

@@ -57,3 +57,14 @@ def load_opcode_matrix():
                        "abs" if mn == "JSR" else "imp"
             out[hi * 16 + lo] = (mn, mode, cyc, px)
     return out
+
+
+def load_undocumented():
+    """-> {opcode: (mnemonic, mode, cycles, pagecross)} from tests/golden/undocumented_opcodes.txt"""
+    out = {}
+    for line in open(os.path.join(GOLDEN, "undocumented_opcodes.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        code, mn, mode, cyc = line.split()
+        out[int(code, 16)] = (mn, mode, int(cyc.rstrip("+")), cyc.endswith("+"))
+    return out

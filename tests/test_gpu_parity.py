@@ -299,3 +299,62 @@ def test_config4_full_batch_longer(torch):
     for t in range(12):
         g.step(torch.from_numpy(acts[t]).cuda(), 4); o.step(acts[t][idx], 4, threads=NCPU)
         compare(g, o, f"config4 long step {t}", envs=idx)
+
+
+def _undoc_rom(seed: int) -> bytes:
+    """The paper's 38 undocumented opcode bytes (tests/golden/undocumented_opcodes.txt) mixed into ordinary code:
+    NOPs of every addressing mode (their reads are real bus reads: RIOT timer, TIA collision latches, page crossings),
+    LAX from RAM / ROM / through pointers, SAX into RAM and into TIA registers, USBC in binary and decimal mode."""
+    r = SplitMix64(seed)
+
+    def build(a):
+        a.org(0xF000); a.op("LDX", "imm", 0xFF); a.op("TXS")
+        for zp, target in ((0x90, 0xFAF0), (0x92, 0x00C0), (0x94, 0xF900)):            # pointers for (zp),Y and (zp,X)
+            a.op("LDA", "imm", target & 0xFF); a.op("STA", "zp", zp); a.op("LDA", "imm", target >> 8); a.op("STA", "zp", zp + 1)
+        a.label("top")
+        for i in range(260):
+            k = r.rnd(16)
+            if k < 3: a.byte(r.choice([0x1A, 0x3A, 0x5A, 0x7A, 0xDA, 0xFA]))
+            elif k < 4: a.byte(r.choice([0x80, 0x82, 0x89, 0xC2, 0xE2]), r.rnd(256))
+            elif k < 5: a.byte(r.choice([0x04, 0x44, 0x64]), r.choice([r.rnd(16), 0x80 + r.rnd(128)]))          # zp: TIA read or RAM
+            elif k < 6: a.byte(r.choice([0x14, 0x34, 0x54, 0x74, 0xD4, 0xF4]), r.rnd(256))
+            elif k < 7:
+                lo = RIOT["INTIM"] - 0x10 + r.rnd(0x20) if r.chance(1, 2) else 0xF900 + r.rnd(0x100)
+                a.byte(r.choice([0x0C, 0x1C, 0x3C, 0x5C, 0x7C, 0xDC, 0xFC]), lo & 0xFF, lo >> 8)                # abs / abs,X incl. the RIOT
+            elif k < 9:
+                opc = r.choice([0xA7, 0xB7, 0xAF, 0xBF, 0xA3, 0xB3])
+                if opc in (0xA7, 0xB7): a.byte(opc, 0x80 + r.rnd(0x60))
+                elif opc in (0xAF, 0xBF): t = r.choice([0xF900 + r.rnd(0x1F0), 0x0080 + r.rnd(0x60)]); a.byte(opc, t & 0xFF, t >> 8)
+                else:
+                    if opc == 0xA3: a.op("LDX", "imm", r.rnd(3) * 2)      # (zp,X): keep the pointer cells in RAM (DESIGN.md §2, status bit 2)
+                    a.byte(opc, r.choice([0x90, 0x92, 0x94]) if opc == 0xB3 else 0x90)
+            elif k < 11:
+                opc = r.choice([0x87, 0x97, 0x8F, 0x83])
+                if opc in (0x87, 0x97): a.byte(opc, r.choice([0x80 + r.rnd(0x60), TIA_W[r.choice(["COLUBK", "PF1", "GRP0", "COLUPF", "ENAM0"])]]))
+                elif opc == 0x8F: a.byte(opc, 0x80 + r.rnd(0x60), 0x00)
+                else: a.op("LDX", "imm", r.rnd(3) * 2); a.byte(opc, 0x90)                                        # (zp,X) -> pointer at $90/$92/$94
+            elif k < 12:
+                if r.chance(1, 2): a.op("SED")
+                a.byte(0xEB, r.rnd(256)); a.op("CLD")
+            elif k < 13: a.op(r.choice(["LDX", "LDY", "LDA"]), "imm", r.rnd(4) * 2)
+            elif k < 14: a.op("STA", "zp", TIA_W[r.choice(["WSYNC", "GRP1", "PF2", "HMOVE", "RESP0"])])
+            elif k < 15: a.op("LDA", "imm", r.rnd(256)); a.op("STA", "abs", RIOT[r.choice(["TIM8T", "TIM64T"])])
+            else: a.op(r.choice(["INX", "DEY", "CLC", "SEC", "TXA", "TAY"]))
+        a.op("LDA", "imm", 2); a.op("STA", "zp", TIA_W["VSYNC"]); a.op("LDA", "imm", 0); a.op("STA", "zp", TIA_W["VSYNC"])
+        a.op("JMP", "abs", "top")
+    return hand_rom(build)
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_undocumented_opcodes(torch, seed):
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    rom = _undoc_rom(3000 + seed)
+    seeds = env_seeds(90 + seed, 36)
+    kw = dict(max_lines=200 + 40 * seed)
+    g, o = VCS([rom], seeds, **kw), OracleVCS([rom], seeds, **kw)
+    for t in range(8):
+        a = np.array([(t + e) % 18 for e in range(36)], np.uint8)
+        g.step(torch.from_numpy(a).cuda(), 1 + t % 3); o.step(a, 1 + t % 3, threads=NCPU)
+        compare(g, o, f"undoc{seed} step {t}")
+    assert not (g.regs_host()["status"] & 1).any()                # none of them halts the CPU any more

@@ -5,11 +5,12 @@ import ctypes as C
 import numpy as np
 import pytest
 
-from helpers import oracle_for, run_instr, regs, load_opcode_matrix
+from helpers import oracle_for, run_instr, regs, load_opcode_matrix, load_undocumented
 from vcs_inputs import OPCODES
 
 fC, fZ, fI, fD, fV, fN = 1, 2, 4, 8, 0x40, 0x80
 MATRIX = load_opcode_matrix()
+UNDOC = load_undocumented()          # the paper's 38 undocumented bytes: executed, not halted
 BR_FLAG = {"BPL": (fN, 0), "BMI": (fN, 1), "BVC": (fV, 0), "BVS": (fV, 1), "BCC": (fC, 0), "BCS": (fC, 1), "BNE": (fZ, 0), "BEQ": (fZ, 1)}
 
 
@@ -46,6 +47,14 @@ def _one(opcode, mode, cross, p=0x24):
 
 @pytest.mark.parametrize("opcode", range(256))
 def test_cycles_from_bus_sequences_match_matrix(opcode):
+    if opcode in UNDOC:
+        mn, mode, cyc, px = UNDOC[opcode]
+        n, r, _ = _one(opcode, mode, False)
+        assert n == cyc and not (r["status"] & 1), (hex(opcode), mn, mode)
+        n2, _, _ = _one(opcode, mode, True)
+        assert n2 == cyc + (1 if px else 0), (hex(opcode), "page cross")
+        assert r["pc"] == 0xF000 + {"imp": 1, "abs": 3, "abx": 3, "aby": 3}.get(mode, 2)
+        return
     if opcode not in MATRIX:                                    # C.12: halt, PC stays, status bit 0
         n, r, o = _one(opcode, "imp", False)
         assert n == 1 and r["status"] & 1 and r["pc"] == 0xF000
@@ -237,3 +246,42 @@ def test_izy_izx_pointer_wrap_in_zero_page():
     o = oracle_for(build); o.poke_ram(0, 0x7F, 0x80); o.poke_ram(0, 0, 0x77)  # -> $0080 = ram[0]
     run_instr(o, 2); assert regs(o)["a"] == 0x77
     o.set_cpu(0, a=0); run_instr(o, 2); assert regs(o)["a"] == 0x77
+
+
+def test_undocumented_family_is_38_and_disjoint():
+    assert len(UNDOC) == 38 and not (set(UNDOC) & set(MATRIX))             # 151 + USBC + 37 = 189
+    assert sum(1 for v in UNDOC.values() if v[0] == "NOP") == 27 and sum(1 for v in UNDOC.values() if v[0] == "LAX") == 6
+    assert sum(1 for v in UNDOC.values() if v[0] == "SAX") == 4 and UNDOC[0xEB][0] == "SBC"
+
+
+def test_undocumented_behaviour():
+    """NOPs change nothing but PC and time; LAX loads A and X with N,Z; SAX stores A & X without flags; USBC == SBC."""
+    for code, (mn, mode, _, _) in UNDOC.items():
+        n, r, o = _one(code, mode, False, p=0x24 | fC)
+        ram = o.ram()[0]
+        # operand value seen by the instruction in _one(): imm $12; zp/zpx/zpy -> RAM cell; abs $0080 -> RAM[0]; abx/aby $FA00+1 -> ROM $10/$F0; (zp,X)/(zp),Y -> $FA00(+1)
+        if mn == "NOP":
+            assert (r["a"], r["x"], r["y"], r["sp"], r["p"]) == (0x55, 0 if mode == "izx" else 1, 1, 0xFD, 0x24 | fC), hex(code)
+        elif mn == "LAX":
+            assert r["a"] == r["x"], hex(code)
+            assert bool(r["p"] & fZ) == (r["a"] == 0) and bool(r["p"] & fN) == bool(r["a"] & 0x80)
+        elif mn == "SAX":
+            assert r["p"] == 0x24 | fC and r["a"] == 0x55                    # no flags, registers kept
+    # LAX zp with a known byte; SAX zp stores A & X
+    def build(a):
+        a.org(0xF000); a.byte(0xA7, 0x90); a.byte(0x87, 0x91); a.byte(0xA7, 0x92)
+    o = oracle_for(build)
+    o.set_cpu(0, a=0, x=0, y=0, sp=0xFD, p=0x24, pc=0xF000); o.poke_ram(0, 0x10, 0xC3); o.poke_ram(0, 0x12, 0x00)
+    run_instr(o); r = regs(o); assert r["a"] == 0xC3 and r["x"] == 0xC3 and r["p"] & fN and not r["p"] & fZ
+    o.set_cpu(0, a=0xF0, x=0x3C); run_instr(o); assert o.ram()[0][0x11] == 0x30 and regs(o)["p"] & fN     # flags untouched by SAX
+    run_instr(o); r = regs(o); assert r["a"] == 0 and r["x"] == 0 and r["p"] & fZ
+    # USBC ($EB) == SBC #imm ($E9) on a sample of operands, binary and decimal
+    rng = np.random.default_rng(7)
+    for _ in range(200):
+        a_, m_, p_ = int(rng.integers(256)), int(rng.integers(256)), 0x24 | int(rng.integers(2)) | (8 if rng.integers(2) else 0)
+        res = []
+        for opc in (0xE9, 0xEB):
+            def build(a, opc=opc): a.org(0xF000); a.byte(opc, m_)
+            o = oracle_for(build); o.set_cpu(0, a=a_, x=0, y=0, sp=0xFD, p=p_, pc=0xF000); run_instr(o)
+            r = regs(o); res.append((int(r["a"]), int(r["p"]), int(r["cycles"])))
+        assert res[0] == res[1]
