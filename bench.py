@@ -51,7 +51,7 @@ def oracle_sample(w, n_envs: int, steps: int, threads: int):
                 tia_writes=sum(b.n_tia_writes - a.n_tia_writes for a, b in zip(d0, d1)) / per,
                 lines=(c1 - c0) / 76.0 / per, cycles=(c1 - c0) / per)
     return dict(value=per / dt, seconds=dt, cycles_per_s=(c1 - c0) / dt, work=work,
-                sample=f"{n_envs} envs (one per {w.batch // n_envs} of config 4's batch, spread over its ROMs) x {steps} env-steps of frameskip 4")
+                sample=f"{n_envs} envs (one per {w.batch // n_envs} of {w.name}'s batch, spread over its ROMs) x {steps} env-steps of frameskip 4")
 
 
 class ClockSampler(threading.Thread):
@@ -119,6 +119,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--batch", type=int, default=65536, help="envs per GPU (default: BASELINE config 4)")
+    ap.add_argument("--workload", type=int, default=4, choices=[2, 3, 4],
+                    help="BASELINE config the envs run (default 4, the headline; 2/3 = one shared 4K ROM: the single-game "
+                         "axis of the paper's Table 7, SURVEY §8(f) NEXT-2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -140,8 +143,11 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     K, W = args.steps, max(args.warmup, 3)
     B = args.batch
-    n_roms = 256 if B % 256 == 0 else 1
-    w = make_workload(4, batch=B, n_roms=n_roms)
+    n_roms = (256 if B % 16384 == 0 else 2 if B % 2 == 0 else 1) if args.workload == 4 else 1
+    w = make_workload(args.workload, batch=B, n_roms=n_roms if args.workload == 4 else None)
+    label = {4: f"config4: {B} envs/GPU, {n_roms} seeded ROMs (half 4K, half 8K F8), uniform random actions, frameskip 4",
+             2: f"config2: {B} envs/GPU sharing one seeded 4K ROM, uniform random actions, frameskip 4",
+             3: f"config3: {B} envs/GPU sharing one seeded 4K ROM (indexed/indirect, stack, BCD, timers), sticky actions, frameskip 4"}[args.workload]
     if world > 1:                                   # every rank its own env seeds / action streams (same ROM set)
         from paper_2606_22447_b200.shard import rank_seeds
         w.seeds = rank_seeds(w.seeds, rank); w._act_seeds = rank_seeds(w._act_seeds, rank)
@@ -221,7 +227,7 @@ def main():
     work = None
     if not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
-        s = oracle_sample(make_workload(4), 32 * cores, 24, cores)       # ~10-20 s of wall clock on the box's cores
+        s = oracle_sample(make_workload(args.workload), 32 * cores, 24, cores)       # ~10-20 s of wall clock on the box's cores
         work = s["work"]
         cpu = {"value": s["value"], "unit": "env-steps/s", "cores": cores, "kind": "oracle", "sample": s["sample"],
                "emulated_cycles_per_s": s["cycles_per_s"], "seconds": s["seconds"]}
@@ -252,7 +258,7 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": "env-steps/s", "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
             "data": "synthetic", "emulated_cycles_per_s": cycles / (total_ms * 1e-3), "frames_per_s": value * FRAMESKIP,
-            "config": {"workload": "config4: 65536 envs/GPU, 256 seeded ROMs (128x4K + 128x8K F8), uniform random actions, frameskip 4",
+            "config": {"workload": label,
                        "batch_per_gpu": B, "frameskip": FRAMESKIP, "l2": "per-step working set 2.2 GB (screens) > 126 MB L2; no explicit flush",
                        "target_env_steps_per_s": 1e7},
             "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, "roofline": roof, "cpu_baseline": cpu}
