@@ -73,6 +73,30 @@ int vcs_reset(vcs_t h, const uint8_t *mask_dev, void *cuda_stream);
  * frameskip must satisfy 1 <= frameskip and frameskip*max_lines*76 < 2^31. */
 int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_stream);
 
+/* vcs_step for a subset: envs with mask_dev[e] == 0 (DEVICE uint8[batch]; NULL = every env steps) stay frozen —
+ * no state, cycle counter, frame counter or screen byte of theirs changes.  Environments are independent
+ * (PAPER.md L63), so the others end exactly where vcs_step would have put them.  Used by vcs_boot for per-env
+ * episode starts; errors as vcs_step. */
+int vcs_step_masked(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, const uint8_t *mask_dev, void *cuda_stream);
+
+/* Console switches (SURVEY.md §8(f) NEXT-4 "console switches as inputs"; C.7 port B): switches_dev[e] (DEVICE
+ * uint8[batch], copied) is the level of the SWCHB input pins of env e — bit 0 RESET and bit 1 SELECT (0 = pressed),
+ * bit 3 colour (1) / b&w (0), bits 6 / 7 difficulty P0 / P1; pins 2, 4 and 5 are not connected and always read 1.
+ * NULL restores the default 0x3F (nothing pressed, colour, both difficulties B).  The value stays until the next
+ * call; vcs_reset does not touch it.  A read of SWCHB returns (ORB & DDRB) | (pins & ~DDRB). */
+int vcs_set_switches(vcs_t h, const uint8_t *switches_dev, void *cuda_stream);
+
+/* ALE-style episode start for the envs with mask_dev[e] != 0 (NULL = all) — PAPER.md L167 "the standard ALE boot
+ * (60 no-op frames plus four resets)", Table 8 "Boot sequence: 60 NOOP + 4 RESET frames; episode-start
+ * randomization: 0-30 random NOOPs (Mnih-style)"; SURVEY.md §8(f) NEXT-4.  In order: vcs_reset(mask); noop_frames
+ * single-frame steps with action NOOP; reset_frames single-frame steps with NOOP and the RESET switch held (bit 0
+ * of the env's switch byte forced low, released afterwards); then, if noop_starts_dev != NULL (DEVICE
+ * uint8[batch], drawn by the caller), min(noop_starts_dev[e], max_noop_starts) env-steps of `frameskip` frames with
+ * NOOP for env e.  All other envs stay frozen.  Enqueues noop_frames + reset_frames + max_noop_starts step kernels.
+ * 0 <= noop_frames, reset_frames; 0 <= max_noop_starts <= 255; frameskip as vcs_step.  Errors as vcs_step. */
+int vcs_boot(vcs_t h, const uint8_t *mask_dev, int32_t noop_frames, int32_t reset_frames,
+             const uint8_t *noop_starts_dev, int32_t max_noop_starts, int32_t frameskip, void *cuda_stream);
+
 /* SOFT-STE forward step (BASELINE config 5; "Hard and Soft Execution", eq. (1)-(4), appendix
  * eq. (6)-(10), L316 "Numerical scope"; reading R14 in DESIGN.md §2).  Same as vcs_step, but every value-carrying
  * read of cartridge ROM (the bank the CPU sees as a 4096 x 8 {0,1} bit tensor) or RIOT RAM (a 128-cell tape) is

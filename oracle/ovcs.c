@@ -19,7 +19,7 @@ typedef struct {
   uint32_t line, frame, frame_cyc; uint64_t events; uint64_t clocks;
   /* RIOT */
   uint8_t ram[128]; uint8_t timer; uint16_t sub; uint8_t shift, tflag;
-  uint8_t ora, ddra, orb, ddrb, ina, inb;
+  uint8_t ora, ddra, orb, ddrb, ina, inb, switches_set;
   /* TIA */
   uint8_t vsync, vblank, latch_en, wsync;
   uint8_t nusiz[2], colup[2], colupf, colubk, ctrlpf, refp[2], pf0, pf1, pf2;

@@ -59,6 +59,9 @@ def lib():
         L.ovcs_create.argtypes = [C.POINTER(P), C.c_int32, C.POINTER(Rom), C.c_int32, P, P, C.POINTER(Config)]
         L.ovcs_reset.argtypes = [P, P]
         L.ovcs_step.argtypes = [P, P, C.c_int32]
+        L.ovcs_step_masked.argtypes = [P, P, C.c_int32, P]
+        L.ovcs_set_switches.argtypes = [P, P]
+        L.ovcs_boot.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, C.c_int32]
         L.ovcs_step_range.argtypes = [P, P, C.c_int32, C.c_int32, C.c_int32]
         for f in ("ovcs_get_ram", "ovcs_get_regs", "ovcs_get_screen"):
             getattr(L, f).argtypes = [P, P]
@@ -128,6 +131,23 @@ class OracleVCS:
         with ThreadPoolExecutor(n) as ex:
             rcs = list(ex.map(lambda i: lib().ovcs_step_range(self.h, a.ctypes.data, frameskip, cuts[i], cuts[i + 1]), range(n)))
         assert all(rc == 0 for rc in rcs)
+
+    @staticmethod
+    def _u8(x):
+        return None if x is None else np.ascontiguousarray(x, dtype=np.uint8)
+
+    def step_masked(self, actions, frameskip, mask):
+        a, m = self._u8(actions), self._u8(mask)
+        assert lib().ovcs_step_masked(self.h, a.ctypes.data, frameskip, None if m is None else m.ctypes.data) == 0
+
+    def set_switches(self, switches=None):
+        s = self._u8(switches)
+        assert lib().ovcs_set_switches(self.h, None if s is None else s.ctypes.data) == 0
+
+    def boot(self, mask=None, noop_frames=60, reset_frames=4, noop_starts=None, max_noop_starts=30, frameskip=4):
+        m, k = self._u8(mask), self._u8(noop_starts)
+        assert lib().ovcs_boot(self.h, None if m is None else m.ctypes.data, noop_frames, reset_frames,
+                               None if k is None else k.ctypes.data, max_noop_starts, frameskip) == 0
 
     def step_soft(self, actions, frameskip, T, alpha, threads=1):
         """SOFT-STE forward step (config 5).  Returns [batch][8] float64: sum_rom, sum_ram, sum_gate, n_rom, n_ram,

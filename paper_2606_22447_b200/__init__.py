@@ -2,3 +2,4 @@
 
 The product is libvcsb200.so (CUDA, sm_100a) behind include/vcs.h; this package is its thin binding."""
 from .binding import VCS, VcsError, REGS_DTYPE, EXPORTS, load_library, optable, issue_peak  # noqa: F401
+from .ale import AleVecEnv  # noqa: F401,E402

@@ -17,7 +17,7 @@ _SO = os.path.join(_PKG, "libvcsb200.so")
 VCS_OK, VCS_EINVAL, VCS_ECUDA, VCS_ENOMEM, VCS_EROM = 0, -1, -2, -3, -4
 _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
 
-EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
+EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
            "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_launch_count",
            "vcs_optable", "vcs_issue_peak", "vcs_destroy", "vcs_last_error"]
 
@@ -56,6 +56,9 @@ def load_library() -> C.CDLL:
     L.vcs_reset.argtypes = [P, P, P]
     L.vcs_step.argtypes = [P, P, C.c_int32, P]
     L.vcs_step_host.argtypes = [P, P, C.c_int32, P]
+    L.vcs_step_masked.argtypes = [P, P, C.c_int32, P, P]
+    L.vcs_set_switches.argtypes = [P, P, P]
+    L.vcs_boot.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, C.c_int32, P]
     L.vcs_step_soft.argtypes = [P, P, C.c_int32, C.c_float, C.c_float, P, P]
     for f in ("vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host"):
         getattr(L, f).argtypes = [P, P, P]
@@ -143,6 +146,27 @@ class VCS:
     def step(self, actions, frameskip=4, stream=None):
         assert actions.is_cuda and actions.dtype == self.torch.uint8 and actions.numel() == self.batch and actions.is_contiguous()
         self._chk(self.L.vcs_step(self.h, actions.data_ptr(), int(frameskip), _stream_ptr(stream)), "vcs_step")
+
+    def _u8(self, x, what):
+        if x is None:
+            return None
+        assert x.is_cuda and x.dtype == self.torch.uint8 and x.numel() == self.batch and x.is_contiguous(), what
+        return x.data_ptr()
+
+    def step_masked(self, actions, frameskip, mask, stream=None):
+        """vcs_step_masked: envs with mask == 0 stay frozen."""
+        self._chk(self.L.vcs_step_masked(self.h, self._u8(actions, "actions"), int(frameskip), self._u8(mask, "mask"),
+                                         _stream_ptr(stream)), "vcs_step_masked")
+
+    def set_switches(self, switches=None, stream=None):
+        """vcs_set_switches: SWCHB input pins per env (None = the default 0x3F)."""
+        self._chk(self.L.vcs_set_switches(self.h, self._u8(switches, "switches"), _stream_ptr(stream)), "vcs_set_switches")
+
+    def boot(self, mask=None, noop_frames=60, reset_frames=4, noop_starts=None, max_noop_starts=30, frameskip=4, stream=None):
+        """vcs_boot: ALE-style episode start (reset, NOOP frames, RESET-switch frames, per-env NOOP steps)."""
+        self._chk(self.L.vcs_boot(self.h, self._u8(mask, "mask"), int(noop_frames), int(reset_frames),
+                                  self._u8(noop_starts, "noop_starts"), int(max_noop_starts), int(frameskip),
+                                  _stream_ptr(stream)), "vcs_boot")
 
     def step_soft(self, actions, frameskip, T, alpha, out=None, stream=None):
         """SOFT-STE forward step (vcs_step_soft); returns the device float[batch][8] of per-env soft sums."""

@@ -65,6 +65,19 @@ __global__ void clear_screen_kernel(uint8_t *screen, const uint8_t *mask) {
   uint4 *dst = reinterpret_cast<uint4 *>(screen + (size_t)e * (SCR_W * SCR_H));
   for (int i = threadIdx.x; i < SCR_W * SCR_H / 16; i += blockDim.x) dst[i] = make_uint4(0, 0, 0, 0);
 }
+// vcs_boot helpers: NOOP actions + the switch bytes with RESET held (bit 0 low); the mask of one random-NOOP-start round
+__global__ void boot_prep_kernel(const uint8_t *sw, uint8_t *zero, uint8_t *sw_reset, int B) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e < B) { zero[e] = 0; sw_reset[e] = sw[e] & 0xFEu; }
+}
+__global__ void boot_mask_kernel(const uint8_t *mask, const uint8_t *starts, int k, uint8_t *out, int B) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e < B) out[e] = ((!mask || mask[e]) && (int)starts[e] > k) ? 1 : 0;
+}
+__global__ void fill_kernel(uint8_t *dst, uint8_t v, int B) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e < B) dst[e] = v;
+}
 __global__ void get_ram_kernel(const uint32_t *ram, uint32_t *out, int B) {
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= 32ll * B) return;
@@ -90,7 +103,7 @@ StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   StepParams p;
   p.st = h->d_st; p.ram = h->d_ram; p.cyc = h->d_cyc; p.screen = h->d_screen;
   p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
-  p.actions = actions; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
+  p.actions = actions; p.switches = h->d_switches; p.mask = nullptr; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
   p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom;
   p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0;
   return p;
@@ -188,6 +201,9 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   CU(h, cudaMemcpy(h->d_rom_meta, meta.data(), sizeof(RomMeta) * n_roms, cudaMemcpyHostToDevice));
   CU(h, cudaMemcpy(h->d_env_rom, er.data(), sizeof(int32_t) * B, cudaMemcpyHostToDevice));
   CU(h, cudaMemcpy(h->d_seeds, seeds, sizeof(unsigned long long) * B, cudaMemcpyHostToDevice));
+  CU(h, cudaMalloc((void **)&h->d_switches, (size_t)B));
+  CU(h, cudaMemset(h->d_switches, 0x3F, (size_t)B));
+  CU(h, cudaMalloc((void **)&h->d_boot, 3 * (size_t)B));
   if (!getenv("VCS_NO_SOFT_ALLOC")) {                                                   // soft mode: every entry decodes at run time (vcs_step_soft)
     std::vector<DWord> sl(8192 + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});
     std::vector<RomMeta> ms(meta); for (auto &m : ms) { m.pad = m.doff; m.doff = 0; }     // pad: offset into the W(T) x ROM table
@@ -227,6 +243,57 @@ int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_
   cudaError_t ce = launch_step(p, (cudaStream_t)cuda_stream);
   h->launches += 1;
   if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step launch", ce);
+  return VCS_OK;
+}
+
+int vcs_step_masked(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, const uint8_t *mask_dev, void *cuda_stream) {
+  if (!h) return VCS_EINVAL;
+  if (!actions_dev) return fail(h, VCS_EINVAL, "vcs_step_masked: actions_dev is NULL");
+  if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31))
+    return fail(h, VCS_EINVAL, "vcs_step_masked: frameskip out of range");
+  StepParams p = params_of(h, actions_dev, frameskip);
+  p.mask = mask_dev;
+  cudaError_t ce = launch_step(p, (cudaStream_t)cuda_stream);
+  h->launches += 1;
+  if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_masked launch", ce);
+  return VCS_OK;
+}
+
+int vcs_set_switches(vcs_t h, const uint8_t *switches_dev, void *cuda_stream) {
+  if (!h) return VCS_EINVAL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (switches_dev) CU(h, cudaMemcpyAsync(h->d_switches, switches_dev, (size_t)h->batch, cudaMemcpyDeviceToDevice, s));
+  else { fill_kernel<<<(h->batch + 255) / 256, 256, 0, s>>>(h->d_switches, 0x3F, h->batch); h->launches += 1; CU(h, cudaGetLastError()); }
+  return VCS_OK;
+}
+
+int vcs_boot(vcs_t h, const uint8_t *mask_dev, int32_t noop_frames, int32_t reset_frames, const uint8_t *noop_starts_dev,
+             int32_t max_noop_starts, int32_t frameskip, void *cuda_stream) {
+  if (!h) return VCS_EINVAL;
+  if (noop_frames < 0 || reset_frames < 0 || max_noop_starts < 0 || max_noop_starts > 255 || noop_frames > 100000 || reset_frames > 100000)
+    return fail(h, VCS_EINVAL, "vcs_boot: frame counts out of range");
+  if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31)) return fail(h, VCS_EINVAL, "vcs_boot: frameskip out of range");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const int B = h->batch, nb = (B + 255) / 256;
+  uint8_t *zero = h->d_boot, *itmask = h->d_boot + B, *swr = h->d_boot + 2 * (size_t)B;
+  int rc = vcs_reset(h, mask_dev, cuda_stream); if (rc) return rc;
+  boot_prep_kernel<<<nb, 256, 0, s>>>(h->d_switches, zero, swr, B); h->launches += 1;
+  CU(h, cudaGetLastError());
+  StepParams p = params_of(h, zero, 1);
+  p.mask = mask_dev;
+  for (int f = 0; f < noop_frames + reset_frames; ++f) {
+    p.switches = (f < noop_frames) ? h->d_switches : swr;
+    cudaError_t ce = launch_step(p, s); h->launches += 1;
+    if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_boot launch", ce);
+  }
+  if (noop_starts_dev) {
+    p = params_of(h, zero, frameskip); p.mask = itmask;
+    for (int k = 0; k < max_noop_starts; ++k) {
+      boot_mask_kernel<<<nb, 256, 0, s>>>(mask_dev, noop_starts_dev, k, itmask, B);
+      cudaError_t ce = launch_step(p, s); h->launches += 2;
+      if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_boot launch", ce);
+    }
+  }
   return VCS_OK;
 }
 
@@ -331,7 +398,7 @@ int vcs_destroy(vcs_t h) {
   if (!h) return VCS_EINVAL;
   cudaDeviceSynchronize();
   cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom);
-  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage);
+  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   delete h;
   return VCS_OK;

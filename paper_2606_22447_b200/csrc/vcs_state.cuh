@@ -67,7 +67,7 @@ enum SmWord {
   S_COLU = 42, S_PF, S_GRP, S_NUSIZ, S_POS, S_POS2,   // TIA registers, packed as the W_* words (S_POS2 without rx)
   S_CX, S_FL, S_RX, S_PX,          // collision latches, flags, clocks rendered, pixels painted of the current line
   S_LINE, S_FDONE,                 // scanline in frame, frames completed in this step
-  S_PORTS, S_INP,                  // RIOT port latches; ina | fire0<<8 | (env index inside the block)<<16
+  S_PORTS, S_INP,                  // RIOT port latches; ina | fire0<<8 | switches (5 pins)<<9 | (env index inside the block)<<16
   S_TMR, S_TTICKS,                 // timer state packed as W_TIMER, valid after S_TTICKS cycles of this step
   S_STATUS, S_FSTART,              // status bits | ROM index << 8; value of the step's cycle count at which the current frame began
   S_OBJ = 60,                      // 30 words: cached 160-bit line masks of PF, BL, P0, P1, M0, M1 (5 words each);
@@ -91,6 +91,8 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   float *d_soft_tab; float soft_tab_T; size_t soft_tab_n;          // W(T) x ROM: the relaxed read of every ROM cell at the cached temperature
   uint2 *d_drom_soft; RomMeta *d_rom_meta_soft; float *d_soft_w;   // soft mode: an all-H_SLOW decode table (every byte fetched at run time), metas with doff 0, e^{-k/T}
   uint8_t *d_actions_stage;     // for vcs_step_host
+  uint8_t *d_switches;          // SWCHB input pins per env (vcs_set_switches; 0x3F after vcs_create)
+  uint8_t *d_boot;              // vcs_boot scratch: [batch] NOOP actions, [batch] per-iteration mask, [batch] switches with RESET held
   uint8_t *h_pinned; size_t h_pinned_bytes;
   int block;                    // threads (= envs) per block of the interpreter kernel
   int regroup;                  // F8 blocks re-sort their envs across threads at bank-hotspot accesses

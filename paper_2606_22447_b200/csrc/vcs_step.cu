@@ -206,7 +206,9 @@ struct Cpu {
       switch (a & 3u) {
         case 0: return (ora & ddra) | (S(S_INP) & ~ddra & 0xFFu);
         case 1: return ddra;
-        case 2: return (orb & ddrb) | (0x3Fu & ~ddrb);
+        case 2: { const uint32_t k = S(S_INP) >> 9;        // console switches (vcs_set_switches), pins 2, 4, 5 not connected
+                  const uint32_t inb = 0x34u | (k & 3u) | ((k & 4u) << 1) | ((k & 0x18u) << 3);
+                  return (orb & ddrb) | (inb & ~ddrb); }
         default: return ddrb;
       }
     }
@@ -939,7 +941,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   const int B = p.batch;
   const int ei = e0 + tid;                                 // the env this thread starts with
   const bool filed = tid < BLOCK;                          // threads of the spare warp start without a file
-  const bool live0 = filed && ei < B;
+  const bool live0 = filed && ei < B && (!p.mask || p.mask[ei]);   // vcs_step_masked: envs with mask 0 stay frozen
   const uint32_t romid = (uint32_t)p.env_rom[live0 ? ei : e0];
   const RomMeta rm = p.rom_meta[romid];
 
@@ -1009,7 +1011,8 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     if ((left >> act) & 1u) ina &= ~0x40u;
     if ((right >> act) & 1u) ina &= ~0x80u;
     const uint32_t fire0 = (fire >> act) & 1u;
-    T::S(sl, S_INP) = ina | (fire0 << 8) | ((uint32_t)tid << 16);
+    const uint32_t inb = p.switches[ei];                   // SWCHB input pins: bits 0, 1, 3, 6, 7 packed into S_INP bits 9..13
+    T::S(sl, S_INP) = ina | (fire0 << 8) | (((inb & 3u) | ((inb >> 1) & 4u) | ((inb >> 3) & 0x18u)) << 9) | ((uint32_t)tid << 16);
     if ((fl & TF_LATCHEN) && fire0) fl &= ~TF_INPT4_LATCH;
     T::S(sl, S_FL) = fl;
   }
@@ -1045,7 +1048,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   if (cur == NOSLOT) return;
   const uint32_t fs = cur;                                 // the file (and env) this thread ends up holding
   const int e = e0 + (int)(T::S(fs, S_INP) >> 16);
-  const bool live = e < B;
+  const bool live = e < B && (!p.mask || p.mask[e]);
   if (!live) return;
   s.load(h, fs);
   if (s.cyc - s.lstart > LINE_CYC) { T::line_end(fs); s.lstart += LINE_CYC; }      // the last instruction ran over the line end

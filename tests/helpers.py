@@ -68,3 +68,27 @@ def load_undocumented():
         code, mn, mode, cyc = line.split()
         out[int(code, 16)] = (mn, mode, int(cyc.rstrip("+")), cyc.endswith("+"))
     return out
+
+
+def switch_rom() -> bytes:
+    """A frame loop that samples the console switches once per frame (NEXT-4 tests).  After the VSYNC that ends frame
+    n (n >= 1) it runs: $80 += 1 (frames seen), $82 = SWCHB, $81 += 1 if RESET (bit 0) reads low, COLUBK = $4A when the
+    colour switch (bit 3) reads high else $0E, $85 = SWCHA, $86 = P after BIT SWCHB (N = bit 7, V = bit 6), then 200
+    WSYNC lines.  $80 / $81 are cleared at power-on, so after f frames $80 == f - 1."""
+    def build(a):
+        a.org(0xF000); a.op("LDX", "imm", 0xFF); a.op("TXS"); a.op("LDA", "imm", 0); a.op("STA", "zp", 0x80); a.op("STA", "zp", 0x81)
+        a.label("frame")
+        a.op("LDA", "imm", 2); a.op("STA", "zp", TIA_W["VSYNC"])
+        for _ in range(3): a.op("STA", "zp", TIA_W["WSYNC"])
+        a.op("LDA", "imm", 0); a.op("STA", "zp", TIA_W["VSYNC"])
+        a.op("INC", "zp", 0x80)
+        a.op("LDA", "abs", RIOT["SWCHB"]); a.op("STA", "zp", 0x82)
+        a.op("LSR", "acc"); a.op("BCS", "rel", "held_not"); a.op("INC", "zp", 0x81); a.label("held_not")
+        a.op("LDA", "zp", 0x82); a.op("AND", "imm", 0x08); a.op("BEQ", "rel", "bw")
+        a.op("LDA", "imm", 0x4A); a.op("JMP", "abs", "setc"); a.label("bw"); a.op("LDA", "imm", 0x0E)
+        a.label("setc"); a.op("STA", "zp", TIA_W["COLUBK"])
+        a.op("LDA", "abs", RIOT["SWCHA"]); a.op("STA", "zp", 0x85)
+        a.op("BIT", "abs", RIOT["SWCHB"]); a.op("PHP"); a.op("PLA"); a.op("STA", "zp", 0x86)
+        a.op("LDY", "imm", 200); a.label("line"); a.op("STA", "zp", TIA_W["WSYNC"]); a.op("DEY"); a.op("BNE", "rel", "line")
+        a.op("JMP", "abs", "frame")
+    return hand_rom(build)

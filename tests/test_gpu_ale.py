@@ -1,0 +1,120 @@
+"""CUDA path vs oracle for the ALE-style wrapper pieces (Table 8):
+vcs_set_switches, vcs_step_masked, vcs_boot — bit-exact RAM, regs and screens through the C ABI."""
+import os
+
+import numpy as np
+import pytest
+
+from helpers import switch_rom
+from test_gpu_parity import compare, mk, torch  # noqa: F401
+from vcs_inputs import make_workload, SplitMix64
+
+pytestmark = pytest.mark.gpu
+NCPU = os.cpu_count() or 1
+
+
+def pair(roms, seeds, env_rom=None, **kw):
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    return VCS(roms, seeds, env_rom, **kw), OracleVCS(roms, seeds, env_rom, **kw)
+
+
+def dev(torch, x):
+    return torch.from_numpy(np.ascontiguousarray(x, dtype=np.uint8)).cuda()
+
+
+def test_switches(torch):
+    n = 70                                                       # one block and a ragged tail
+    g, o = pair([switch_rom()], np.arange(1, n + 1, dtype=np.uint64))
+    r = SplitMix64(5)
+    for t in range(6):
+        sw = np.array([r.rnd(256) for _ in range(n)], np.uint8)
+        if t == 3:
+            g.set_switches(None); o.set_switches(None)
+        else:
+            g.set_switches(dev(torch, sw)); o.set_switches(sw)
+        if t == 4:
+            g.reset(); o.reset()                                 # switches are physical: a reset leaves them
+        a = np.array([r.rnd(18) for _ in range(n)], np.uint8)
+        g.step(dev(torch, a), 1 + t % 3); o.step(a, 1 + t % 3)
+        compare(g, o, f"switches step {t}")
+    assert (g.ram_host()[:, 2] == (sw | 0x34)).all()
+
+
+@pytest.mark.parametrize("cfg,batch,n_roms", [(2, 200, None), (4, 256, 32), (4, 96, 6)])
+def test_masked_step(torch, cfg, batch, n_roms):
+    w = make_workload(cfg, batch=batch, n_roms=n_roms)           # config 4: F8 blocks regroup with frozen envs among them
+    g, o = mk(torch, w)
+    acts = w.actions(0, 8)
+    r = SplitMix64(11 + batch)
+    for t in range(8):
+        mask = np.array([r.rnd(3) > 0 for _ in range(batch)], np.uint8)
+        if t == 5: mask[:] = 0
+        if t == 6: mask[: batch // 2] = 0
+        g.step_masked(dev(torch, acts[t]), w.frameskip, dev(torch, mask))
+        o.step_masked(acts[t], w.frameskip, mask)
+        compare(g, o, f"masked cfg{cfg} step {t}")
+    g.step_masked(dev(torch, acts[0]), 2, None); o.step_masked(acts[0], 2, None)
+    compare(g, o, "masked NULL mask")
+
+
+def test_boot_switch_rom(torch):
+    n = 130
+    g, o = pair([switch_rom()], np.arange(100, 100 + n, dtype=np.uint64))
+    starts = (np.arange(n) * 7 % 34).astype(np.uint8)            # 0..33: some above the cap of 30
+    g.boot(None, 60, 4, dev(torch, starts), 30, 4); o.boot(None, 60, 4, starts, 30, 4)
+    compare(g, o, "boot")
+    k = np.minimum(starts, 30).astype(np.int64)
+    assert (g.regs_host()["frame"] == 64 + 4 * k).all() and (g.ram_host()[:, 1] == 4).all()
+
+
+def test_boot_subset_mid_episode(torch):
+    w = make_workload(4, batch=128, n_roms=4)
+    g, o = mk(torch, w)
+    acts = w.actions(0, 6)
+    r = SplitMix64(77)
+    for t in range(6):
+        g.step(dev(torch, acts[t]), 4); o.step(acts[t], 4, threads=NCPU)
+        if t in (1, 4):                                          # "auto-reset" of a few envs: boot them, the rest stay put
+            mask = np.array([r.rnd(5) == 0 for _ in range(128)], np.uint8)
+            starts = np.array([r.rnd(5) for _ in range(128)], np.uint8)
+            g.boot(dev(torch, mask), 5, 2, dev(torch, starts), 4, 4); o.boot(mask, 5, 2, starts, 4, 4)
+        compare(g, o, f"boot subset step {t}")
+    g.boot(None, 3, 1, None, 30, 4); o.boot(None, 3, 1, None, 30, 4)      # no NOOP starts
+    compare(g, o, "boot all")
+
+
+def test_boot_argument_errors(torch):
+    g, _ = pair([switch_rom()], np.arange(4, dtype=np.uint64))
+    for kw in (dict(noop_frames=-1), dict(reset_frames=-1), dict(max_noop_starts=256), dict(frameskip=0)):
+        with pytest.raises(RuntimeError):
+            g.boot(**kw)
+
+
+def test_ale_vec_env_auto_reset(torch):
+    from paper_2606_22447_b200 import AleVecEnv
+    from oracle.ovcs_py import OracleVCS
+    n = 96
+    w = make_workload(4, batch=n, n_roms=6)
+    env = AleVecEnv(w.roms, w.seeds, w.env_rom, frameskip=4, noop_max=5, boot_noop_frames=6, boot_reset_frames=2,
+                    max_episode_steps=4, start_seed=3)
+    o = OracleVCS(w.roms, w.seeds, w.env_rom)
+    starts = env.reset().cpu().numpy()
+    assert starts.max() <= 5 and len(set(starts.tolist())) > 1
+    o.boot(None, 6, 2, starts, 5, 4)
+    compare(env.vcs, o, "ale reset")
+    acts = w.actions(0, 10)
+    r = SplitMix64(9)
+    n_boot = np.ones(n, np.int64)
+    for t in range(10):
+        done = np.array([r.rnd(7) == 0 for _ in range(n)], np.uint8)
+        steps_before = env.episode_steps.cpu().numpy()
+        mask = env.step(dev(torch, acts[t]), dev(torch, done)).cpu().numpy()
+        assert (mask.astype(bool) == (done.astype(bool) | (steps_before + 1 >= 4))).all()
+        o.step(acts[t], 4, threads=NCPU)
+        if mask.any():
+            o.boot(mask, 6, 2, env.last_starts.cpu().numpy(), 5, 4)
+        n_boot += mask
+        compare(env.vcs, o, f"ale step {t}")
+    assert (env.episodes.cpu().numpy() == n_boot).all()
+    env.close()
