@@ -29,9 +29,11 @@ typedef struct vcs_s *vcs_t;
 
 enum { VCS_OK = 0, VCS_EINVAL = -1, VCS_ECUDA = -2, VCS_ENOMEM = -3, VCS_EROM = -4 };
 
-/* One cartridge image (host memory).  size 2048 (2K, mirrored), 4096 (4K) or 8192 (F8: any bus access
- * to $1FF8/$1FF9 selects bank 0/1 — SURVEY C.9; "writes to special addresses swap which
- * 4KB ROM page is visible"). */
+/* One cartridge image (host memory).  size 2048 (2K, mirrored), 4096 (4K), 8192 (F8: any bus access to
+ * $1FF8/$1FF9 selects bank 0/1 — SURVEY C.9; "writes to special addresses swap which 4KB ROM page
+ * is visible"), 16384 (F6: $1FF6..$1FF9 select banks 0..3) or 32768 (F4: $1FF4..$1FFB select banks 0..7) — PAPER.md
+ * L69 / L469, SURVEY §8(f) NEXT-3.  F6 / F4 images power up in bank 0 and are read from global memory (a handle
+ * that holds one does not stage ROMs in shared memory and does not regroup F8 blocks: slower, same results). */
 typedef struct { const uint8_t *data; uint32_t size; } vcs_rom;
 
 /* y0: scanline shown as screen row 0 (default 34, must be >= 2);  max_lines: frame cap in scanlines
@@ -60,7 +62,7 @@ typedef struct {
  * consecutive envs shares one ROM, the ROM is staged in shared memory per block and F8 carts regroup their envs by
  * bank inside the block; otherwise ROM bytes come through the read-only cache.  Tuning overrides read here from
  * the environment: VCS_BLOCK=64|128|256, VCS_ROM_GLOBAL, VCS_NO_REGROUP, VCS_NO_SPIN, VCS_NO_FUSE.
- * Errors: VCS_EINVAL (NULL/size/range), VCS_EROM (size not 2048/4096/8192), VCS_ECUDA, VCS_ENOMEM. */
+ * Errors: VCS_EINVAL (NULL/size/range), VCS_EROM (size not 2048/4096/8192/16384/32768), VCS_ECUDA, VCS_ENOMEM. */
 int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms,
                const int32_t *env_rom, const uint64_t *seeds, const vcs_config *cfg);
 

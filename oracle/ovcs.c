@@ -54,6 +54,10 @@ uint64_t ovcs_splitmix64(uint64_t *s) {
 /* ------------------------------------------------------------- C.9 cartridge */
 static void cart_hotspot(env_t *e, uint16_t a) {          /* any bus access, a = addr&0x1FFF */
   if (e->rom_size == 8192) { if (a == 0x1FF8) e->bank = 0; else if (a == 0x1FF9) e->bank = 1; }
+  /* SURVEY §8(f) NEXT-3, PAPER.md L69 / L469 (F6, F4 among the implemented formats) [D]: the same scheme with more
+   * banks — F6 (16 KB): $1FF6..$1FF9 select banks 0..3;  F4 (32 KB): $1FF4..$1FFB select banks 0..7. */
+  if (e->rom_size == 16384 && a >= 0x1FF6 && a <= 0x1FF9) e->bank = (uint8_t)(a - 0x1FF6);
+  if (e->rom_size == 32768 && a >= 0x1FF4 && a <= 0x1FFB) e->bank = (uint8_t)(a - 0x1FF4);
 }
 static uint8_t cart_peek(const env_t *e, uint16_t a) {
   uint32_t o = a & 0x0FFF;

@@ -31,7 +31,7 @@ extern "C" {
 
 typedef struct ovcs_s ovcs_t;
 
-typedef struct { const uint8_t *data; uint32_t size; /* 2048 | 4096 | 8192 (F8) */ } ovcs_rom;
+typedef struct { const uint8_t *data; uint32_t size; /* 2048 | 4096 | 8192 (F8) | 16384 (F6) | 32768 (F4) */ } ovcs_rom;
 typedef struct { int32_t y0, max_lines, f8_start_bank; uint32_t flags; } ovcs_config;
 
 /* Same 32-byte record as include/vcs.h's vcs_regs; retyped, not shared. */

@@ -42,7 +42,7 @@ __global__ void reset_kernel(StepParams p, const unsigned long long *seeds, cons
   const int B = p.batch;
   const RomMeta rm = p.rom_meta[p.env_rom[e]];
   const uint8_t *rom = p.rom_blob + rm.offset;
-  const uint32_t bank = (rm.size == 8192) ? (uint32_t)(f8_start_bank & 1) : 0u;
+  const uint32_t bank = (rm.size == 8192) ? (uint32_t)(f8_start_bank & 1) : 0u;      // F6 / F4 power up in bank 0 (reading R15)
   const uint32_t mask_a = (rm.size == 2048) ? 0x7FFu : 0xFFFu;
   const uint32_t pc = rom[(bank << 12) + (0xFFCu & mask_a)] | ((uint32_t)rom[(bank << 12) + (0xFFDu & mask_a)] << 8);
   for (int w = 0; w < ST_WORDS; ++w) p.st[w * B + e] = 0;
@@ -131,7 +131,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   if (batch < 1 || !roms || n_roms < 1 || !seeds) return VCS_EINVAL;
   for (int r = 0; r < n_roms; ++r) {
     if (!roms[r].data) return VCS_EINVAL;
-    if (roms[r].size != 2048 && roms[r].size != 4096 && roms[r].size != 8192) return VCS_EROM;
+    if (roms[r].size != 2048 && roms[r].size != 4096 && roms[r].size != 8192 && roms[r].size != 16384 && roms[r].size != 32768) return VCS_EROM;
   }
   if (env_rom) for (int i = 0; i < batch; ++i) if (env_rom[i] < 0 || env_rom[i] >= n_roms) return VCS_EINVAL;
   vcs_config c = {34, 320, 1, 0};
@@ -149,7 +149,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   size_t blob = 0, dwords = 0;
   for (int r = 0; r < n_roms; ++r) {
     meta[r].offset = (uint32_t)blob; meta[r].size = roms[r].size; meta[r].doff = (uint32_t)dwords; meta[r].pad = 0;
-    blob += roms[r].size; dwords += (roms[r].size == 8192) ? 8192 : 4096;
+    blob += roms[r].size; dwords += (roms[r].size < 4096) ? 4096 : roms[r].size;
   }
   std::vector<uint8_t> hb(blob);
   for (int r = 0; r < n_roms; ++r) memcpy(hb.data() + meta[r].offset, roms[r].data, roms[r].size);
@@ -164,7 +164,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   auto uniform = [&](int blk) { for (int i = 0; i < batch; ++i) if (er[i] != er[i - i % blk]) return false; return true; };
   h->block = want; h->rom_smem = 0;
   for (int blk = want; blk >= 64; blk >>= 1) if (uniform(blk)) { h->block = blk; h->rom_smem = 1; break; }
-  if (getenv("VCS_ROM_GLOBAL")) h->rom_smem = 0;
+  if (getenv("VCS_ROM_GLOBAL") || h->max_rom > 8192) h->rom_smem = 0;     // F6 / F4 images stay in global memory (read-only path)
   h->regroup = getenv("VCS_NO_REGROUP") ? 0 : 1;
   // pre-decode every byte offset of every bank once (vcs_decode.cuh); the words depend on the launch shape
   // (zero-page RAM operands are stored as shared-memory offsets)
@@ -172,14 +172,14 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   {
     std::vector<uint8_t> img(4096 + 4, 0), leader(4096);
     for (int r = 0; r < n_roms; ++r) {
-      const int nb = (roms[r].size == 8192) ? 2 : 1;
+      const int nb = (roms[r].size < 4096) ? 1 : (int)(roms[r].size / 4096);
       std::fill(leader.begin(), leader.end(), 0);
       for (int pass = 0; pass < 2; ++pass)
         for (int b = 0; b < nb; ++b) {
           if (roms[r].size == 2048) { memcpy(img.data(), roms[r].data, 2048); memcpy(img.data() + 2048, roms[r].data, 2048); }
           else memcpy(img.data(), roms[r].data + 4096 * b, 4096);
           if (pass == 0) mark_leaders(img.data(), leader.data());
-          else { decode_bank(img.data(), leader.data(), h->block, nb == 2, dw.data() + meta[r].doff + 4096 * b);
+          else { decode_bank(img.data(), leader.data(), h->block, nb, dw.data() + meta[r].doff + 4096 * b);
                  if (!getenv("VCS_NO_SPIN")) mark_spins(img.data(), dw.data() + meta[r].doff + 4096 * b);
                  if (!getenv("VCS_NO_FUSE")) fuse_ld_st(dw.data() + meta[r].doff + 4096 * b); }
         }
@@ -205,7 +205,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   CU(h, cudaMemset(h->d_switches, 0x3F, (size_t)B));
   CU(h, cudaMalloc((void **)&h->d_boot, 3 * (size_t)B));
   if (!getenv("VCS_NO_SOFT_ALLOC")) {                                                   // soft mode: every entry decodes at run time (vcs_step_soft)
-    std::vector<DWord> sl(8192 + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});
+    std::vector<DWord> sl((h->max_rom < 8192 ? 8192 : h->max_rom) + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});
     std::vector<RomMeta> ms(meta); for (auto &m : ms) { m.pad = m.doff; m.doff = 0; }     // pad: offset into the W(T) x ROM table
     h->soft_tab_n = dwords; h->soft_tab_T = -1.f;
     CU(h, cudaMalloc((void **)&h->d_soft_tab, sizeof(float) * (dwords + 8)));

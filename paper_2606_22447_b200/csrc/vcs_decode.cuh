@@ -90,7 +90,8 @@ inline uint32_t generic_entry(uint32_t opc) {
 inline bool tia_write_has_effect(uint32_t r) {    // r = address & 0x3F (SURVEY C.8 write map)
   return !(r > 0x2Cu || (r >= 0x15u && r <= 0x1Au) || r == 0x03u);
 }
-inline bool is_hotspot(uint32_t a13) { return (a13 | 1u) == 0x1FF9u; }
+// bank hotspots of an image with nb banks: F8 $1FF8-9, F6 $1FF6-9, F4 $1FF4-B
+inline bool is_hotspot(uint32_t a13, int nb) { const uint32_t lo = (nb == 8) ? 0x1FF4u : 0x1FFAu - (uint32_t)nb; return nb >= 2 && a13 - lo < (uint32_t)nb; }
 
 // Second step of the decode: the handler ids above are what the out-of-line ("cold") executor understands.  The
 // instructions that make up almost every executed one are re-coded into a handful of data-driven HOT classes run
@@ -162,7 +163,7 @@ inline void hot_class(uint32_t &x, uint32_t &y) {
 
 // One bank image (4096 bytes; 2 KB carts are passed mirrored) -> 4096 decode entries.  `leader` is the bank-
 // independent leader bitmap (4096 flags) filled by mark_leaders() for every bank of the cartridge first.
-inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, bool f8, DWord *out) {
+inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, int nb, DWord *out) {
   for (uint32_t off = 0; off < 4096; ++off) {
     const uint32_t lead = leader[off] ? DW_LEADER : 0u;
     if (off >= DW_SLOW_LIMIT) { out[off].x = H_SLOW | lead; out[off].y = 0; continue; }
@@ -194,7 +195,7 @@ inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, bo
       else if (ab && rd_std && (a13 & 0x1284u) == 0x0284u) {       // INTIM / TIMINT
         x = dw_x(H_RTIM, 4, 3, op - OP_LDA); payload = a13;
       }
-      else if (ab && rd_std && op != OP_BIT && (a13 & 0x1000u) && !(f8 && is_hotspot(a13))) {   // a fixed ROM byte
+      else if (ab && rd_std && op != OP_BIT && (a13 & 0x1000u) && !is_hotspot(a13, nb)) {   // a fixed ROM byte
         x = dw_x(H_IMM0 + (op - OP_LDA), 4, 3, 0); payload = img[a13 & 0xFFFu];                        // of this bank
       }
       else if (mode == MD_REL) {
@@ -202,7 +203,7 @@ inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, bo
         const int32_t toff = (int32_t)off + 2 + disp;                      // target offset inside the 4 KB window
         const uint32_t next = 0x1000u + off + 2u, target = (uint32_t)((int32_t)next + disp);
         const uint32_t dummy2 = (next & 0xFF00u) | (target & 0xFFu);
-        if (toff < 0 || toff >= 4096 || (f8 && (is_hotspot(next & 0x1FFFu) || is_hotspot(dummy2 & 0x1FFFu))))
+        if (toff < 0 || toff >= 4096 || (is_hotspot(next & 0x1FFFu, nb) || is_hotspot(dummy2 & 0x1FFFu, nb)))
           x = H_SLOW;                                                      // run-time decode keeps every side effect
         else {
           payload = (uint32_t)disp;

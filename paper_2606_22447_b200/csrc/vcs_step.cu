@@ -81,10 +81,10 @@ struct Cpu {
   int32_t cap;        // frame cap in cycles
   uint32_t fdone;     // frames completed in this step (mirror of S_FDONE)
   uint32_t fskip;     // frames to run
-  uint32_t keyhi;     // scheduling key without the PC: frames done << 25 | SP << 17 | bank << 16 (or KEY_PARKED / ~0)
+  uint32_t keyhi;     // scheduling key without the PC: frames done << 27 | SP << 19 | bank << 16 (or KEY_PARKED / ~0)
   bool wsync;         // mirror of TF_WSYNC
   // ---- cart
-  uint32_t is_f8, rom_mask;
+  uint32_t hs_lo, hs_n, rom_mask;      // bank hotspots: hs_n addresses from hs_lo (F8 $1FF8 x2, F6 $1FF6 x4, F4 $1FF4 x8); hs_n 0 = none
   uint32_t park;      // bit0: this block regroups its envs at bank-hotspot accesses; bit1: this lane is parked for a
                       // regroup; bit2: a bank hotspot was accessed by the instruction in flight
   uint32_t rom_off;   // ROMS: byte offset of the ROM image inside smem
@@ -110,14 +110,14 @@ struct Cpu {
     if constexpr (CART) {                                  // (the line-end / event paths never touch the cartridge)
       auto ptr = [](int lo) { return (unsigned long long)T::ctx(lo) | ((unsigned long long)T::ctx(lo + 1) << 32); };
       const RomMeta rm = reinterpret_cast<const RomMeta *>(ptr(C_META_LO))[romid];
-      is_f8 = (rm.size == 8192) ? 1u : 0u; rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
+      hs_n = rm.size >> 12; if (hs_n < 2u) hs_n = 0; hs_lo = (hs_n == 8u) ? 0x1FF4u : 0x1FFAu - hs_n; rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
       rom_g = reinterpret_cast<const uint8_t *>(ptr(C_BLOB_LO)) + rm.offset;
       dr = reinterpret_cast<const uint2 *>(ptr(C_DROM_LO)) + rm.doff;
       if constexpr (SOFT) {
         soft = reinterpret_cast<float *>(ptr(C_SOFT_OUT_LO)) + 8 * (size_t)(T::ctx(C_ENV0) + (S(S_INP) >> 16));
         soft_tab = reinterpret_cast<const float *>(ptr(C_SOFT_TAB_LO)) + rm.pad;
       } else { soft = nullptr; soft_tab = nullptr; }
-    } else { is_f8 = 0; rom_mask = 0xFFFu; rom_g = nullptr; dr = nullptr; soft = nullptr; soft_tab = nullptr; }
+    } else { hs_n = 0; hs_lo = 0; rom_mask = 0xFFFu; rom_g = nullptr; dr = nullptr; soft = nullptr; soft_tab = nullptr; }
     park = T::ctx(C_REGROUP) | ((keyhi == KEY_PARKED) ? 2u : 0u);
   }
   DEV Hot store() const {
@@ -129,9 +129,9 @@ struct Cpu {
   }
 
   DEV uint32_t pc() const { return (pbase + di) & 0xFFFFu; }
-  DEV void set_pc(uint32_t p) { const uint32_t nd = (di & 0x1000u) | (p & 0xFFFu); pbase = p - nd; di = nd; }
+  DEV void set_pc(uint32_t p) { const uint32_t nd = (di & 0x7000u) | (p & 0xFFFu); pbase = p - nd; di = nd; }
   DEV void rekey() {
-    keyhi = (fdone >= fskip) ? 0xFFFFFFFFu : (park & 2u) ? KEY_PARKED : (min(fdone, 63u) << 25) | (SP << 17) | ((di & 0x1000u) << 4);
+    keyhi = (fdone >= fskip) ? 0xFFFFFFFFu : (park & 2u) ? KEY_PARKED : (min(fdone, 30u) << 27) | (SP << 19) | ((di & 0x7000u) << 4);
   }
 
   // ------------------------------------------------------------------ RAM (smem, conflict-free)
@@ -145,10 +145,10 @@ struct Cpu {
     if constexpr (ROMS) return reinterpret_cast<const uint8_t *>(smem)[rom_off + off];
     else return __ldg(rom_g + off);
   }
-  // any access to $1FF8/$1FF9 selects the bank; in a block that regroups it also parks the lane (park bit 1)
+  // any access to a hotspot ($1FF8/$1FF9 on F8 carts) selects the bank; in a block that regroups it also parks the lane (park bit 1)
   DEV void hotspot(uint32_t a) {
-    if (is_f8 && (a | 1u) == 0x1FF9u) {
-      const uint32_t nd = (di & 0xFFFu) | ((a & 1u) << 12);
+    if (a - hs_lo < hs_n) {
+      const uint32_t nd = (di & 0xFFFu) | ((a - hs_lo) << 12);
       pbase += di - nd; di = nd;                     // PC is unchanged
       park |= 4u | ((park & 1u) << 1);
       rekey();
@@ -156,7 +156,7 @@ struct Cpu {
   }
   DEV uint32_t rom_rd(uint32_t a, bool value = true) {   // a = addr & 0x1FFF with A12 set; value: the byte is used (not a dummy cycle)
     hotspot(a);
-    const uint32_t v = rom_byte((di & 0x1000u) + (a & rom_mask));
+    const uint32_t v = rom_byte((di & 0x7000u) + (a & rom_mask));
     if constexpr (SOFT) { if (value) return soft_rom(a & 0xFFFu, v); }
     return v;
   }
@@ -290,7 +290,7 @@ struct Cpu {
   }
   DEV uint32_t soft_rom(uint32_t o, uint32_t hard) {       // eq. (10) on the 4096 x 8 bit tensor of the visible bank, then STE + round
     // the ROM is constant, so W(T) x ROM is computed once per temperature (soft_table_kernel): a fetch is one lookup
-    const float sv = __ldg(soft_tab + (di & 0x1000u) + o);
+    const float sv = __ldg(soft_tab + (di & 0x7000u) + o);
     const float h = (float)hard, ste = sv + (h - sv);      // eq. (9), forward
     soft_note(0, sv, h, ste);
     return (uint32_t)(int)rintf(ste) & 0xFFu;
@@ -865,7 +865,7 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
         case HC_XFER:
           v = __byte_perm(h.axys, 0u, pl); h.axys = __byte_perm(h.axys, v, pl >> 16);
           if (aux) h.zn = v;
-          else if (h.keyhi < KEY_PARKED) h.keyhi = (h.keyhi & ~(0xFFu << 17)) | (v << 17);      // TXS: SP is part of the key
+          else if (h.keyhi < KEY_PARKED) h.keyhi = (h.keyhi & ~(0xFFu << 19)) | (v << 19);      // TXS: SP is part of the key
           break;
         case HC_ALU_IMM: v = pl; goto do_alu;
         case HC_ALU_RAM: v = ramb[pl]; goto do_alu;
@@ -899,7 +899,7 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
       h.di += 3u; h.cyc += 4; wn = __ldg(dr + h.di);
       aux = cx >> DW_OP2_SHIFT;
         } goto do_rtim;
-        case HC_JMP: { const uint32_t nd = (h.di & 0x1000u) | (pl & 0xFFFu); h.pbase = pl - nd; h.di = nd; } goto ctl;
+        case HC_JMP: { const uint32_t nd = (h.di & 0x7000u) | (pl & 0xFFFu); h.pbase = pl - nd; h.di = nd; } goto ctl;
         default:                                           // everything else: out of line, then re-schedule
           h = cold_exec<BLOCK, ROMS, THREADS, SOFT>(h, sl, cx, pl);
           return;
@@ -976,7 +976,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     uint32_t w;
     w = p.st[W_AXYS * B + ei]; s.A = w & 0xFF; s.X = (w >> 8) & 0xFF; s.Y = (w >> 16) & 0xFF; s.SP = w >> 24;
     w = p.st[W_PC * B + ei]; pc0 = w & 0xFFFF; s.unpack_p((w >> 16) & 0xFF); s.status = w >> 24;
-    w = p.st[W_BEAM * B + ei]; n0 = w & 0xFF; T::S(sl, S_LINE) = (w >> 8) & 0xFFFF; bank0 = (w >> 24) & 1u;
+    w = p.st[W_BEAM * B + ei]; n0 = w & 0xFF; T::S(sl, S_LINE) = (w >> 8) & 0xFFFF; bank0 = (w >> 24) & 7u;
     s.fstart = -(int32_t)p.st[W_FCYC * B + ei];
     T::S(sl, S_TMR) = p.st[W_TIMER * B + ei]; T::S(sl, S_TTICKS) = 0;
     T::S(sl, S_PORTS) = p.st[W_PORTS * B + ei];
@@ -995,8 +995,8 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   s.fskip = (uint32_t)p.frameskip;
   s.cyc = 0; s.lstart = -(int32_t)n0; s.fdone = live0 ? 0u : s.fskip; s.romid = romid;
   s.cap = p.max_lines * LINE_CYC;
-  s.is_f8 = (rm.size == 8192);
-  const bool regroups = ROMS && s.is_f8 && p.regroup;      // block-uniform
+  s.hs_n = rm.size >> 12; if (s.hs_n < 2u) s.hs_n = 0; s.hs_lo = (s.hs_n == 8u) ? 0x1FF4u : 0x1FFAu - s.hs_n;
+  const bool regroups = ROMS && rm.size == 8192 && p.regroup;      // block-uniform
   s.park = regroups ? 1u : 0u;
   s.rom_off = ROM_OFF; s.rom_g = p.rom_blob + rm.offset; s.dr = p.drom + rm.doff; 
   s.rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
@@ -1076,7 +1076,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
 // A banded [4096 x 4096] x [4096 x 8] contraction per bank, done once per temperature instead of once per fetch.
 __global__ void soft_table_kernel(const uint8_t *rom_blob, const RomMeta *meta, const float *wt, int K, float *tab) {
   const RomMeta rm = meta[blockIdx.y];
-  const int nb = (rm.size == 8192) ? 2 : 1;
+  const int nb = max(1, (int)(rm.size >> 12));
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;            // bank * 4096 + o
   if (idx >= nb * 4096) return;
   const int bank = idx >> 12, o = idx & 0xFFF;
@@ -1095,7 +1095,7 @@ __global__ void soft_table_kernel(const uint8_t *rom_blob, const RomMeta *meta, 
   tab[rm.pad + idx] = pl0 * inv + 2.f * (pl1 * inv) + 4.f * (pl2 * inv) + 8.f * (pl3 * inv) + 16.f * (pl4 * inv) + 32.f * (pl5 * inv) + 64.f * (pl6 * inv) + 128.f * (pl7 * inv);
 }
 cudaError_t launch_soft_table(const uint8_t *rom_blob, const RomMeta *meta, int n_roms, const float *w, int K, float *tab, cudaStream_t stream) {
-  soft_table_kernel<<<dim3(8192 / 256, n_roms), 256, 0, stream>>>(rom_blob, meta, w, K, tab);
+  soft_table_kernel<<<dim3(32768 / 256, n_roms), 256, 0, stream>>>(rom_blob, meta, w, K, tab);
   return cudaGetLastError();
 }
 

@@ -19,7 +19,7 @@ SUBS_ORG, TABLES_ORG, TABLES_END, TRAMP2_ORG = 0xF800, 0xFA00, 0xFE00, 0xFE00
 
 @dataclass(frozen=True)
 class Features:
-    size: int = 2048          # 2048 | 4096 | 8192 (F8)
+    size: int = 2048          # 2048 | 4096 | 8192 (F8) | 16384 (F6) | 32768 (F4)
     joystick: bool = False    # config 2+: SWCHA / INPT4 reads, object update, RESP0 timing, CX reads
     extended: bool = False    # config 3+: indexed/indirect, JSR/RTS, stack, BCD, all timer divisors
 
@@ -30,7 +30,17 @@ FEATURES = {
     3: Features(4096, True, True),
     "4a": Features(4096, True, True),
     "4b": Features(8192, True, True),
+    "f6": Features(16384, True, True),      # F6: four 4 KB banks, hotspots $1FF6-$1FF9
+    "f4": Features(32768, True, True),      # F4: eight 4 KB banks, hotspots $1FF4-$1FFB
 }
+
+
+def _banks(size: int) -> int:
+    return max(1, size // 4096)
+
+
+def _hotspot_lo(size: int) -> int:
+    return {8192: 0x1FF8, 16384: 0x1FF6, 32768: 0x1FF4}[size]
 
 BAND_REGS_1 = ["COLUBK", "COLUPF", "PF0", "PF1", "PF2", "GRP0", "GRP1", "COLUP0", "RESP0", "HMP0", "HMOVE"]
 BAND_REGS_2 = BAND_REGS_1 + ["COLUP1", "NUSIZ0", "NUSIZ1", "CTRLPF", "REFP0", "REFP1", "RESP1", "RESM0",
@@ -196,6 +206,9 @@ def _prologue(a: Asm, feat: Features):
         a.op("BCS", "rel", "t1_b1"); a.op("BIT", "abs", 0x1FF8); a.op("BCC", "rel", "t1_c")
         a.label("t1_b1"); a.op("BIT", "abs", 0x1FF9)
         a.label("t1_c")
+    elif feat.size > 8192:                                             # F6 / F4: bank = RAM bits, selected by an indexed read
+        a.op("LDA", "zp", 0xA7); a.op("EOR", "zp", 0x80); a.op("AND", "imm", _banks(feat.size) - 1); a.op("TAX")
+        a.op("LDA", "abx", _hotspot_lo(feat.size))
 
 
 def _input_block(a: Asm, g: _Gen):
@@ -309,7 +322,7 @@ def _gen_bank(seed: int, feat: Features, bank: int) -> bytes:
     a.label("wait"); a.op("LDA", "abs", RIOT["INTIM"]); a.op("BNE", "rel", "wait")
     a.op("STA", "zp", TIA_W["WSYNC"]); a.op("STA", "zp", TIA_W["VBLANK"])          # A = 0
     _bands(a, g)
-    if feat.size == 8192:                      # trampoline 2 at a fixed address, landing differs per bank
+    if feat.size >= 8192:                      # trampoline 2 at a fixed address, landing differs per bank
         a.op("JMP", "abs", TRAMP2_ORG)
         a.label("after_t2")
     _overscan(a, g)
@@ -321,6 +334,11 @@ def _gen_bank(seed: int, feat: Features, bank: int) -> bytes:
         a.op("BCS", "rel", "t2_b1"); a.op("BIT", "abs", 0x1FF8); a.op("BCC", "rel", "t2_c")
         a.label("t2_b1"); a.op("BIT", "abs", 0x1FF9)
         a.label("t2_c"); a.op("JMP", "abs", "after_t2")
+    elif feat.size > 8192:
+        a.org(TRAMP2_ORG)
+        a.op("LDA", "zp", 0xB3); a.op("EOR", "zp", 0x83); a.op("LSR", "acc"); a.op("AND", "imm", _banks(feat.size) - 1); a.op("TAY")
+        a.op("STA", "aby", _hotspot_lo(feat.size))                     # a write selects the bank as well (any bus access does)
+        a.op("JMP", "abs", "after_t2")
     img = bytearray(a.finish())
     entry = a.labels["entry"]
     for off in (size - 4, size - 2):
@@ -330,6 +348,4 @@ def _gen_bank(seed: int, feat: Features, bank: int) -> bytes:
 
 def make_rom(seed: int, feat: Features) -> bytes:
     """One cartridge image of feat.size bytes from `seed`."""
-    if feat.size == 8192:
-        return _gen_bank(seed, feat, 0) + _gen_bank(seed, feat, 1)
-    return _gen_bank(seed, feat, 0)
+    return b"".join(_gen_bank(seed, feat, b) for b in range(_banks(feat.size)))
