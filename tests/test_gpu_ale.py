@@ -118,3 +118,25 @@ def test_ale_vec_env_auto_reset(torch):
         compare(env.vcs, o, f"ale step {t}")
     assert (env.episodes.cpu().numpy() == n_boot).all()
     env.close()
+
+
+def test_masked_and_boot_full_batch_launch_shape(torch):
+    """Config 4 at its full batch (bench.py's launch configuration: 256-env blocks, spare warp, F8 regroup with frozen
+    envs among the files): masked steps and a mid-episode boot of a subset, one env per ROM against the oracle."""
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    w = make_workload(4)
+    idx = np.arange(256) * 256 + (np.arange(256) * 91) % 256
+    g = VCS(w.roms, w.seeds, w.env_rom)
+    o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx])
+    acts = w.actions(0, 6)
+    rng = np.random.default_rng(5)
+    for t in range(6):
+        mask = (rng.integers(0, 4, w.batch) > 0).astype(np.uint8)
+        g.step_masked(dev(torch, acts[t]), 4, dev(torch, mask)); o.step_masked(acts[t][idx], 4, mask[idx])
+        compare(g, o, f"full masked step {t}", envs=idx)
+        if t == 2:
+            bm = (rng.integers(0, 3, w.batch) == 0).astype(np.uint8)
+            st = rng.integers(0, 4, w.batch).astype(np.uint8)
+            g.boot(dev(torch, bm), 4, 2, dev(torch, st), 3, 4); o.boot(bm[idx], 4, 2, st[idx], 3, 4)
+            compare(g, o, "full boot", envs=idx)
