@@ -122,9 +122,13 @@ def main():
     ap.add_argument("--workload", type=int, default=4, choices=[2, 3, 4],
                     help="BASELINE config the envs run (default 4, the headline; 2/3 = one shared 4K ROM: the single-game "
                          "axis of the paper's Table 7, SURVEY §8(f) NEXT-2)")
+    ap.add_argument("--soft-T", type=float, default=None,
+                    help="run vcs_step_soft (SOFT-STE forward, BASELINE config 5: --workload 2 --batch 4096) at this temperature")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
+    if args.soft_T is not None:
+        args.no_e2e = True
     if args.impl == "reference":
         return run_reference(args)
 
@@ -155,6 +159,12 @@ def main():
     acts_host = w.actions(0, W + K)
     acts = torch.from_numpy(acts_host).cuda()
     stream = torch.cuda.current_stream()
+    if args.soft_T is not None:                     # SOFT-STE forward (alpha 4): same step, soft reads / branches on top
+        label = f"config5 (soft mode, T={args.soft_T}, alpha=4) on " + label
+        soft_out = torch.empty((B, 8), dtype=torch.float32, device="cuda")
+        do_step = lambda a: env.step_soft(a, FRAMESKIP, args.soft_T, 4.0, out=soft_out)
+    else:
+        do_step = lambda a: env.step(a, FRAMESKIP)
 
     def barrier():
         if world > 1:
@@ -163,7 +173,7 @@ def main():
 
     sampler = ClockSampler(local); sampler.start()
     for t in range(W):
-        env.step(acts[t], FRAMESKIP)
+        do_step(acts[t])
     barrier()
     cyc0 = env.regs_host()["cycles"].astype(np.int64).sum()
     l0 = env.launch_count()
@@ -172,7 +182,7 @@ def main():
     barrier()
     evs[0].record(stream)
     for t in range(K):
-        env.step(acts[W + t], FRAMESKIP)
+        do_step(acts[W + t])
         evs[t + 1].record(stream)
     barrier()
     sampler.active = False
@@ -256,8 +266,8 @@ def main():
     roof["hbm"] = {"algorithmic_bytes_per_launch": hbm_bytes, "achieved_gbs": hbm_bytes / (kms * 1e-3) / 1e9,
                    "peak_gbs": peaks.get("hbm_gbs"), "frac": (hbm_bytes / (kms * 1e-3) / 1e9) / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None}
     line = {"metric": METRIC, "value": value, "unit": "env-steps/s", "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
-            "data": "synthetic", "emulated_cycles_per_s": cycles / (total_ms * 1e-3), "frames_per_s": value * FRAMESKIP,
+            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u8" if args.soft_T is None else "u8 + f32 soft reads", "data": "synthetic", "emulated_cycles_per_s": cycles / (total_ms * 1e-3), "frames_per_s": value * FRAMESKIP,
             "config": {"workload": label,
                        "batch_per_gpu": B, "frameskip": FRAMESKIP, "l2": "per-step working set 2.2 GB (screens) > 126 MB L2; no explicit flush",
                        "target_env_steps_per_s": 1e7},

@@ -358,3 +358,26 @@ def test_undocumented_opcodes(torch, seed):
         g.step(torch.from_numpy(a).cuda(), 1 + t % 3); o.step(a, 1 + t % 3, threads=NCPU)
         compare(g, o, f"undoc{seed} step {t}")
     assert not (g.regs_host()["status"] & 1).any()                # none of them halts the CPU any more
+
+
+@pytest.mark.parametrize("cfg,steps,stride", [(2, 500, 8), (3, 2000, 128), (4, 1000, 256)])
+def test_full_length_runs(torch, cfg, steps, stride):
+    """BASELINE configs 2-4 at their full batch AND their full length (500 / 2000 / 1000 env-steps of frameskip 4, the
+    launch configuration bench.py times): a stratified subset of the envs (every `stride`-th, offset varying, so one env
+    per ROM for config 4) runs on the oracle beside the GPU; RAM, regs and screens compared every 250 steps and at the
+    final step (BASELINE.json: "bit-exact RAM/screen at the final step")."""
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    w = make_workload(cfg)
+    n = w.batch // stride
+    idx = np.arange(n) * stride + (np.arange(n) * 91) % stride
+    g = VCS(w.roms, w.seeds, w.env_rom)
+    o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx])
+    chunk = 250
+    for t0 in range(0, steps, chunk):
+        acts = w.actions(t0, t0 + chunk)
+        dacts = torch.from_numpy(acts).cuda()
+        for t in range(chunk):
+            g.step(dacts[t], w.frameskip); o.step(acts[t][idx], w.frameskip, threads=NCPU)
+        compare(g, o, f"config{cfg} full length, step {t0 + chunk}", envs=idx)
+    assert int(g.regs_host()["frame"].min()) >= steps * w.frameskip
