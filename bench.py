@@ -265,7 +265,7 @@ def main():
     hbm_bytes = B * (210 * 160 + 2 * (128 + 4 * 15 + 8) + 1)
     roof["hbm"] = {"algorithmic_bytes_per_launch": hbm_bytes, "achieved_gbs": hbm_bytes / (kms * 1e-3) / 1e9,
                    "peak_gbs": peaks.get("hbm_gbs"), "frac": (hbm_bytes / (kms * 1e-3) / 1e9) / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None}
-    line = {"metric": METRIC, "value": value, "unit": "env-steps/s", "n_gpus": world, "steps": K, "warmup": W,
+    line = {"metric": METRIC if B == 65536 else METRIC.replace("65536", str(B)), "value": value, "unit": "env-steps/s", "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "u8" if args.soft_T is None else "u8 + f32 soft reads", "data": "synthetic", "emulated_cycles_per_s": cycles / (total_ms * 1e-3), "frames_per_s": value * FRAMESKIP,
             "config": {"workload": label,
