@@ -99,6 +99,21 @@ int vcs_set_switches(vcs_t h, const uint8_t *switches_dev, void *cuda_stream);
 int vcs_boot(vcs_t h, const uint8_t *mask_dev, int32_t noop_frames, int32_t reset_frames,
              const uint8_t *noop_starts_dev, int32_t max_noop_starts, int32_t frameskip, void *cuda_stream);
 
+/* The same episode start, amortised: instead of stepping the booting envs on their own (vcs_boot: dozens of launches
+ * that run a handful of envs each), the envs with mask_dev[e] != 0 (NULL = all) are reset and ARMED, and the boot
+ * runs inside the following vcs_step / vcs_step_masked / vcs_step_soft calls of the whole batch: for its first
+ * noop_steps steps an armed env ignores the caller's action (NOOP), for the next reset_steps steps it also has the
+ * RESET switch held, then it takes min(noop_starts_dev[e], max_noop_starts) more NOOP steps, and from the next step
+ * on it follows the caller's actions.  One "step" here is one env-step of whatever frameskip the caller passes: with
+ * frameskip 4, noop_steps 15 and reset_steps 1 are the paper's 60 NOOP + 4 RESET frames (inputs are latched once
+ * per vcs_step, and the protocol's inputs only change at those frame counts, so the frames are the same ones
+ * vcs_boot runs — tests/test_gpu_ale.py).  No extra step launches; frozen envs (vcs_step_masked) do not count down.
+ * noop_steps + reset_steps + max_noop_starts <= 255.  vcs_reset / vcs_boot disarm the envs they touch. */
+int vcs_auto_reset(vcs_t h, const uint8_t *mask_dev, int32_t noop_steps, int32_t reset_steps,
+                   const uint8_t *noop_starts_dev, int32_t max_noop_starts, void *cuda_stream);
+/* out_dev[e] (DEVICE uint8[batch]) = boot steps env e still has to run (0 = it follows the caller's actions). */
+int vcs_get_booting(vcs_t h, uint8_t *out_dev, void *cuda_stream);
+
 /* SOFT-STE forward step (BASELINE config 5; "Hard and Soft Execution", eq. (1)-(4), appendix
  * eq. (6)-(10), L316 "Numerical scope"; reading R14 in DESIGN.md §2).  Same as vcs_step, but every value-carrying
  * read of cartridge ROM (the bank the CPU sees as a 4096 x 8 {0,1} bit tensor) or RIOT RAM (a 128-cell tape) is

@@ -6,7 +6,9 @@ Table 8: "Boot sequence: 60 NOOP + 4 RESET frames; episode-start random
 vcs_set_switches); this class only sequences those calls, draws the NOOP-start counts (seeded, on the device) and
 keeps the episode step counters.  Per-game reward / terminal logic needs the games and is out of scope: the caller
 passes its own `done` mask (e.g. computed from `ram()`), and the envs it names are re-booted in place while the
-others carry on — per-env auto-reset."""
+others carry on — per-env auto-reset.  With `amortised=True` (default when the boot frame counts are multiples of
+`frameskip`) the re-boot is vcs_auto_reset: the env is reset and armed, its boot runs inside the batch's following
+vcs_step calls (no extra launches), and `booting()` says which envs do not yet follow the agent."""
 from __future__ import annotations
 
 from .binding import VCS
@@ -14,7 +16,7 @@ from .binding import VCS
 
 class AleVecEnv:
     def __init__(self, roms, seeds, env_rom=None, frameskip=4, noop_max=30, boot_noop_frames=60, boot_reset_frames=4,
-                 max_episode_steps=None, start_seed=0, **config):
+                 max_episode_steps=None, start_seed=0, amortised=None, **config):
         self.vcs = VCS(roms, seeds, env_rom, **config)
         t = self.torch = self.vcs.torch
         self.batch, self.device = self.vcs.batch, self.vcs.device
@@ -22,6 +24,9 @@ class AleVecEnv:
         self.boot_noop_frames, self.boot_reset_frames = int(boot_noop_frames), int(boot_reset_frames)
         self.max_episode_steps = max_episode_steps
         assert 0 <= self.noop_max <= 255
+        divisible = self.boot_noop_frames % self.frameskip == 0 and self.boot_reset_frames % self.frameskip == 0
+        self.amortised = divisible if amortised is None else bool(amortised)
+        assert divisible or not self.amortised, "amortised boot needs boot frame counts that are multiples of frameskip"
         self._gen = t.Generator(device=self.device); self._gen.manual_seed(int(start_seed))
         self.episode_steps = t.zeros(self.batch, dtype=t.int32, device=self.device)
         self.episodes = t.zeros(self.batch, dtype=t.int32, device=self.device)
@@ -63,8 +68,18 @@ class AleVecEnv:
             return t.zeros(self.batch, dtype=t.uint8, device=self.device)
         mask = over.to(t.uint8).contiguous()
         if bool(mask.any()):
-            self.reset(mask)
+            if self.amortised:
+                self.last_starts = self._draw_starts()
+                self.vcs.auto_reset(mask, self.boot_noop_frames // self.frameskip, self.boot_reset_frames // self.frameskip,
+                                    self.last_starts if self.noop_max > 0 else None, self.noop_max)
+                self.episode_steps.masked_fill_(over, 0); self.episodes += over.to(self.episodes.dtype)
+            else:
+                self.reset(mask)
         return mask
+
+    def booting(self, out=None):
+        """uint8[batch]: boot steps each env still has to run before it follows the agent (0 = playing)."""
+        return self.vcs.get_booting(out)
 
     # ---- observations (device tensors)
     def screen(self, out=None):

@@ -17,7 +17,7 @@ _SO = os.path.join(_PKG, "libvcsb200.so")
 VCS_OK, VCS_EINVAL, VCS_ECUDA, VCS_ENOMEM, VCS_EROM = 0, -1, -2, -3, -4
 _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
 
-EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
+EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
            "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_launch_count",
            "vcs_optable", "vcs_issue_peak", "vcs_destroy", "vcs_last_error"]
 
@@ -59,6 +59,8 @@ def load_library() -> C.CDLL:
     L.vcs_step_masked.argtypes = [P, P, C.c_int32, P, P]
     L.vcs_set_switches.argtypes = [P, P, P]
     L.vcs_boot.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, C.c_int32, P]
+    L.vcs_auto_reset.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, P]
+    L.vcs_get_booting.argtypes = [P, P, P]
     L.vcs_step_soft.argtypes = [P, P, C.c_int32, C.c_float, C.c_float, P, P]
     for f in ("vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host"):
         getattr(L, f).argtypes = [P, P, P]
@@ -167,6 +169,17 @@ class VCS:
         self._chk(self.L.vcs_boot(self.h, self._u8(mask, "mask"), int(noop_frames), int(reset_frames),
                                   self._u8(noop_starts, "noop_starts"), int(max_noop_starts), int(frameskip),
                                   _stream_ptr(stream)), "vcs_boot")
+
+    def auto_reset(self, mask=None, noop_steps=15, reset_steps=1, noop_starts=None, max_noop_starts=30, stream=None):
+        """vcs_auto_reset: reset + arm the masked envs; their boot runs inside the following step calls."""
+        self._chk(self.L.vcs_auto_reset(self.h, self._u8(mask, "mask"), int(noop_steps), int(reset_steps),
+                                        self._u8(noop_starts, "noop_starts"), int(max_noop_starts), _stream_ptr(stream)),
+                  "vcs_auto_reset")
+
+    def get_booting(self, out=None, stream=None):
+        t = self.torch
+        out = t.empty(self.batch, dtype=t.uint8, device=self.device) if out is None else out
+        self._chk(self.L.vcs_get_booting(self.h, out.data_ptr(), _stream_ptr(stream)), "vcs_get_booting"); return out
 
     def step_soft(self, actions, frameskip, T, alpha, out=None, stream=None):
         """SOFT-STE forward step (vcs_step_soft); returns the device float[batch][8] of per-env soft sums."""

@@ -52,6 +52,7 @@ __global__ void reset_kernel(StepParams p, const unsigned long long *seeds, cons
   p.st[W_TIMER * B + e] = 0xFFu | (10u << 8);
   p.st[W_FLAGS * B + e] = TF_INPT4_LATCH | TF_INPT5_LATCH;
   p.cyc[e] = 0;
+  p.boot[e] = 0;
   unsigned long long s = seeds[e];
   for (int k = 0; k < 16; ++k) {
     unsigned long long z = splitmix64(s);
@@ -73,6 +74,17 @@ __global__ void boot_prep_kernel(const uint8_t *sw, uint8_t *zero, uint8_t *sw_r
 __global__ void boot_mask_kernel(const uint8_t *mask, const uint8_t *starts, int k, uint8_t *out, int B) {
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e < B) out[e] = ((!mask || mask[e]) && (int)starts[e] > k) ? 1 : 0;
+}
+// vcs_auto_reset: arm the boot countdown of the masked envs (after reset_kernel)
+__global__ void arm_boot_kernel(const uint8_t *mask, const uint8_t *starts, int noop_steps, int reset_steps, int max_starts, uint32_t *boot, int B) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= B || (mask && !mask[e])) return;
+  int k = starts ? (int)starts[e] : 0; if (k > max_starts) k = max_starts;
+  boot[e] = (uint32_t)(noop_steps + reset_steps + k) | ((uint32_t)k << 8) | ((uint32_t)reset_steps << 16);
+}
+__global__ void get_booting_kernel(const uint32_t *boot, uint8_t *out, int B) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e < B) out[e] = (uint8_t)(boot[e] & 0xFFu);
 }
 __global__ void fill_kernel(uint8_t *dst, uint8_t v, int B) {
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
@@ -103,7 +115,7 @@ StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   StepParams p;
   p.st = h->d_st; p.ram = h->d_ram; p.cyc = h->d_cyc; p.screen = h->d_screen;
   p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
-  p.actions = actions; p.switches = h->d_switches; p.mask = nullptr; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
+  p.actions = actions; p.switches = h->d_switches; p.mask = nullptr; p.boot = h->d_boot_ctr; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
   p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom;
   p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0;
   return p;
@@ -204,6 +216,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   CU(h, cudaMalloc((void **)&h->d_switches, (size_t)B));
   CU(h, cudaMemset(h->d_switches, 0x3F, (size_t)B));
   CU(h, cudaMalloc((void **)&h->d_boot, 3 * (size_t)B));
+  CU(h, cudaMalloc((void **)&h->d_boot_ctr, sizeof(uint32_t) * B));
   if (!getenv("VCS_NO_SOFT_ALLOC")) {                                                   // soft mode: every entry decodes at run time (vcs_step_soft)
     std::vector<DWord> sl((h->max_rom < 8192 ? 8192 : h->max_rom) + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});
     std::vector<RomMeta> ms(meta); for (auto &m : ms) { m.pad = m.doff; m.doff = 0; }     // pad: offset into the W(T) x ROM table
@@ -294,6 +307,26 @@ int vcs_boot(vcs_t h, const uint8_t *mask_dev, int32_t noop_frames, int32_t rese
       if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_boot launch", ce);
     }
   }
+  return VCS_OK;
+}
+
+int vcs_auto_reset(vcs_t h, const uint8_t *mask_dev, int32_t noop_steps, int32_t reset_steps, const uint8_t *noop_starts_dev,
+                   int32_t max_noop_starts, void *cuda_stream) {
+  if (!h) return VCS_EINVAL;
+  if (noop_steps < 0 || reset_steps < 0 || max_noop_starts < 0 || noop_steps + reset_steps + max_noop_starts > 255)
+    return fail(h, VCS_EINVAL, "vcs_auto_reset: step counts out of range (their sum must be <= 255)");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int rc = vcs_reset(h, mask_dev, cuda_stream); if (rc) return rc;
+  arm_boot_kernel<<<(h->batch + 255) / 256, 256, 0, s>>>(mask_dev, noop_starts_dev, noop_steps, reset_steps, max_noop_starts, h->d_boot_ctr, h->batch);
+  h->launches += 1;
+  CU(h, cudaGetLastError());
+  return VCS_OK;
+}
+int vcs_get_booting(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
+  if (!h || !out_dev) return VCS_EINVAL;
+  get_booting_kernel<<<(h->batch + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(h->d_boot_ctr, out_dev, h->batch);
+  h->launches += 1;
+  CU(h, cudaGetLastError());
   return VCS_OK;
 }
 
@@ -398,7 +431,7 @@ int vcs_destroy(vcs_t h) {
   if (!h) return VCS_EINVAL;
   cudaDeviceSynchronize();
   cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom);
-  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot);
+  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   delete h;
   return VCS_OK;

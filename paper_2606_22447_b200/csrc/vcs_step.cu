@@ -1003,6 +1003,11 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   // ---- a2 action latch (C.11)
   if (live0) {
     uint32_t act = p.actions[ei]; if (act >= 18u) act = 0;
+    uint32_t inb = p.switches[ei];                         // SWCHB input pins
+    {                                                      // vcs_auto_reset: an env that is still booting ignores the agent
+      const uint32_t b = p.boot[ei], c = b & 0xFFu, k = (b >> 8) & 0xFFu, R = b >> 16;     // steps left | NOOP starts | RESET steps
+      if (c) { act = 0; if (c > k && c <= k + R) inb &= ~1u; p.boot[ei] = b - 1u; }
+    }
     //            NOOP FIRE UP RIGHT LEFT DOWN UR UL DR DL UF RF LF DF URF ULF DRF DLF
     const uint32_t up = 0x0C4C4u, down = 0x32320u, left = 0x29290u, right = 0x14948u, fire = 0x3FC02u;
     uint32_t ina = 0xFFu;
@@ -1011,7 +1016,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     if ((left >> act) & 1u) ina &= ~0x40u;
     if ((right >> act) & 1u) ina &= ~0x80u;
     const uint32_t fire0 = (fire >> act) & 1u;
-    const uint32_t inb = p.switches[ei];                   // SWCHB input pins: bits 0, 1, 3, 6, 7 packed into S_INP bits 9..13
+    // the live SWCHB pins (bits 0, 1, 3, 6, 7) travel in S_INP bits 9..13
     T::S(sl, S_INP) = ina | (fire0 << 8) | (((inb & 3u) | ((inb >> 1) & 4u) | ((inb >> 3) & 0x18u)) << 9) | ((uint32_t)tid << 16);
     if ((fl & TF_LATCHEN) && fire0) fl &= ~TF_INPT4_LATCH;
     T::S(sl, S_FL) = fl;

@@ -9,7 +9,7 @@ namespace vcs {
 struct StepParams {
   uint32_t *st; uint32_t *ram; unsigned long long *cyc; uint8_t *screen;
   const uint8_t *rom_blob; const uint2 *drom; const RomMeta *rom_meta; const int32_t *env_rom;
-  const uint8_t *actions; const uint8_t *switches; const uint8_t *mask;   // switches: SWCHB input pins per env; mask: nullptr = every env steps
+  const uint8_t *actions; const uint8_t *switches; const uint8_t *mask; uint32_t *boot;   // switches: SWCHB input pins per env; mask: nullptr = every env steps; boot: per-env boot countdown (vcs_auto_reset)
   int32_t batch, frameskip, y0, max_lines;
   const float *soft_w; const float *soft_tab; float *soft_out; float soft_alpha; int32_t soft_K;   // soft_out != nullptr: SOFT-STE mode (vcs_step_soft)
   int32_t block, rom_smem, regroup; uint32_t max_rom;     // launch shape: envs per block (64/128/256), ROM staged in smem, largest image

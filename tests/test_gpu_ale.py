@@ -97,7 +97,7 @@ def test_ale_vec_env_auto_reset(torch):
     n = 96
     w = make_workload(4, batch=n, n_roms=6)
     env = AleVecEnv(w.roms, w.seeds, w.env_rom, frameskip=4, noop_max=5, boot_noop_frames=6, boot_reset_frames=2,
-                    max_episode_steps=4, start_seed=3)
+                    max_episode_steps=4, start_seed=3, amortised=False)
     o = OracleVCS(w.roms, w.seeds, w.env_rom)
     starts = env.reset().cpu().numpy()
     assert starts.max() <= 5 and len(set(starts.tolist())) > 1
@@ -140,3 +140,78 @@ def test_masked_and_boot_full_batch_launch_shape(torch):
             st = rng.integers(0, 4, w.batch).astype(np.uint8)
             g.boot(dev(torch, bm), 4, 2, dev(torch, st), 3, 4); o.boot(bm[idx], 4, 2, st[idx], 3, 4)
             compare(g, o, "full boot", envs=idx)
+
+
+@pytest.mark.parametrize("batch,n_roms", [(96, 6), (256, 2)])
+def test_auto_reset_amortised_equals_boot_protocol(torch, batch, n_roms):
+    """vcs_auto_reset arms envs whose boot then runs inside the batch's ordinary vcs_step calls; the result must be
+    what the paper's protocol gives when spelled frame by frame (ovcs_boot: 60 single NOOP frames, 4 single RESET
+    frames, k NOOP steps) followed by the agent's actions from the step at which each env became ready."""
+    w = make_workload(4, batch=batch, n_roms=n_roms)
+    g, o = mk(torch, w)
+    acts = w.actions(0, 60)
+    r = np.random.default_rng(batch)
+    for t in range(3):                                           # some history first
+        g.step(dev(torch, acts[t]), 4); o.step(acts[t], 4, threads=NCPU)
+    mask = (r.integers(0, 3, batch) == 0).astype(np.uint8); mask[0] = 1
+    starts = r.integers(0, 36, batch).astype(np.uint8)           # some above the cap of 30
+    g.auto_reset(dev(torch, mask), 15, 1, dev(torch, starts), 30)
+    o.boot(mask, 60, 4, starts, 30, 4)                           # the oracle boots "instantly" ...
+    k = np.minimum(starts, 30).astype(np.int64)
+    want = np.where(mask != 0, 16 + k, 0)
+    assert (g.get_booting().cpu().numpy() == want).all()
+    T = 16 + 30 + 4
+    for t in range(T):                                           # ... and then waits until the GPU env is ready
+        ready = (t >= want).astype(np.uint8)
+        g.step(dev(torch, acts[3 + t]), 4); o.step_masked(acts[3 + t], 4, ready)
+        assert (g.get_booting().cpu().numpy() == np.maximum(want - (t + 1), 0)).all()
+    compare(g, o, "auto_reset")
+    # a second arming while the first envs play on, with a masked step in between (frozen envs do not count down)
+    m2 = (r.integers(0, 4, batch) == 0).astype(np.uint8)
+    g.auto_reset(dev(torch, m2), 2, 1, None, 0); o.boot(m2, 8, 4, None, 0, 4)
+    frozen = (r.integers(0, 2, batch) == 0).astype(np.uint8)
+    g.step_masked(dev(torch, acts[0]), 4, dev(torch, frozen))
+    left = np.where(m2 != 0, 3, 0) - np.where((m2 != 0) & (frozen != 0), 1, 0)
+    assert (g.get_booting().cpu().numpy() == left).all()
+    o.step_masked(acts[0], 4, frozen & (m2 == 0))
+    for t in range(1, 5):
+        a_t = acts[t]
+        g.step(dev(torch, a_t), 4)
+        o.step_masked(a_t, 4, (left == 0).astype(np.uint8))
+        left = np.maximum(left - 1, 0)
+    compare(g, o, "auto_reset second arming")
+    with pytest.raises(RuntimeError):
+        g.auto_reset(None, 200, 50, None, 30)
+
+
+def test_ale_vec_env_amortised_auto_reset(torch):
+    from paper_2606_22447_b200 import AleVecEnv
+    from oracle.ovcs_py import OracleVCS
+    n = 64
+    w = make_workload(4, batch=n, n_roms=4)
+    env = AleVecEnv(w.roms, w.seeds, w.env_rom, frameskip=4, noop_max=3, boot_noop_frames=8, boot_reset_frames=4, start_seed=1)
+    assert env.amortised
+    o = OracleVCS(w.roms, w.seeds, w.env_rom)
+    st = env.reset().cpu().numpy(); o.boot(None, 8, 4, st, 3, 4)
+    acts = w.actions(0, 14)
+    r = SplitMix64(21)
+    wait = np.zeros(n, np.int64)                                  # boot steps each env still owes
+    for t in range(14):
+        done = np.array([r.rnd(9) == 0 for _ in range(n)], np.uint8)
+        play = (wait == 0).astype(np.uint8)
+        m = env.step(dev(torch, acts[t]), dev(torch, done)).cpu().numpy()
+        o.step_masked(acts[t], 4, play)                          # the oracle env waits while the GPU env runs its boot steps
+        wait = np.maximum(wait - 1, 0)
+        assert (m == done).all()
+        if m.any():
+            k = np.minimum(env.last_starts.cpu().numpy(), 3)
+            o.boot(m, 8, 4, k.astype(np.uint8), 3, 4)
+            wait = np.where(m != 0, 3 + k, wait)
+        assert (env.booting().cpu().numpy() == wait).all()
+    for t in range(8):                                           # let every boot finish
+        play = (wait == 0).astype(np.uint8)
+        env.step(dev(torch, acts[t]))
+        o.step_masked(acts[t], 4, play)
+        wait = np.maximum(wait - 1, 0)
+    compare(env.vcs, o, "amortised AleVecEnv")
+    env.close()

@@ -87,3 +87,20 @@ def test_boot_mask_leaves_others_alone_and_equals_manual_sequence():
     m.set_switches(None)
     for k in range(2): m.step_masked(z, 2, mask & (starts > k))
     assert (o.ram() == m.ram()).all() and (o.regs() == m.regs()).all() and (o.screen() == m.screen()).all()
+
+
+def test_boot_frames_equal_boot_steps_when_inputs_change_every_fourth_frame():
+    """60 single NOOP frames + 4 single RESET frames + k NOOP steps (the protocol as ovcs_boot spells it) == 15 + 1 + k
+    env-steps of frameskip 4 with the same inputs: inputs are latched per step and only change at those frame counts.
+    This is the identity the amortised vcs_auto_reset rests on."""
+    import vcs_inputs
+    w = vcs_inputs.make_workload(4, batch=8, n_roms=4)
+    a = OracleVCS(w.roms, w.seeds, w.env_rom); b = OracleVCS(w.roms, w.seeds, w.env_rom)
+    starts = np.array([0, 1, 2, 3, 5, 8, 13, 30], np.uint8)
+    a.boot(None, 60, 4, starts, 30, 4)
+    z = np.zeros(8, np.uint8)
+    b.reset()
+    for t in range(16 + 30):
+        b.set_switches(np.full(8, 0x3E if t == 15 else 0x3F, np.uint8))
+        b.step_masked(z, 4, (t < 16 + starts.astype(np.int64)).astype(np.uint8))
+    assert (a.ram() == b.ram()).all() and (a.regs() == b.regs()).all() and (a.screen() == b.screen()).all()
