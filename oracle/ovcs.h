@@ -68,6 +68,7 @@ int  ovcs_step(ovcs_t *h, const uint8_t *actions /* [batch] */, int32_t frameski
 int  ovcs_step_range(ovcs_t *h, const uint8_t *actions, int32_t frameskip, int32_t lo, int32_t hi);
 /* SURVEY §8(f) NEXT-4 (Table 8): masked step, console switches, the ALE episode start. */
 int  ovcs_step_masked(ovcs_t *h, const uint8_t *actions, int32_t frameskip, const uint8_t *mask /* [batch] or NULL */);
+int  ovcs_step_masked_range(ovcs_t *h, const uint8_t *actions, int32_t frameskip, const uint8_t *mask, int32_t lo, int32_t hi);
 int  ovcs_set_switches(ovcs_t *h, const uint8_t *switches /* [batch] SWCHB pins, NULL = 0x3F */);
 int  ovcs_boot(ovcs_t *h, const uint8_t *mask, int32_t noop_frames, int32_t reset_frames, const uint8_t *noop_starts,
                int32_t max_noop_starts, int32_t frameskip);

@@ -60,6 +60,7 @@ def lib():
         L.ovcs_reset.argtypes = [P, P]
         L.ovcs_step.argtypes = [P, P, C.c_int32]
         L.ovcs_step_masked.argtypes = [P, P, C.c_int32, P]
+        L.ovcs_step_masked_range.argtypes = [P, P, C.c_int32, P, C.c_int32, C.c_int32]
         L.ovcs_set_switches.argtypes = [P, P]
         L.ovcs_boot.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, C.c_int32]
         L.ovcs_step_range.argtypes = [P, P, C.c_int32, C.c_int32, C.c_int32]
@@ -136,9 +137,17 @@ class OracleVCS:
     def _u8(x):
         return None if x is None else np.ascontiguousarray(x, dtype=np.uint8)
 
-    def step_masked(self, actions, frameskip, mask):
+    def step_masked(self, actions, frameskip, mask, threads=1):
         a, m = self._u8(actions), self._u8(mask)
-        assert lib().ovcs_step_masked(self.h, a.ctypes.data, frameskip, None if m is None else m.ctypes.data) == 0
+        mp = None if m is None else m.ctypes.data
+        n = max(1, min(threads, self.batch))
+        if n == 1:
+            assert lib().ovcs_step_masked(self.h, a.ctypes.data, frameskip, mp) == 0
+            return
+        cuts = [self.batch * i // n for i in range(n + 1)]          # envs are independent: one oracle thread per slice
+        with ThreadPoolExecutor(n) as ex:
+            rcs = list(ex.map(lambda i: lib().ovcs_step_masked_range(self.h, a.ctypes.data, frameskip, mp, cuts[i], cuts[i + 1]), range(n)))
+        assert all(rc == 0 for rc in rcs)
 
     def set_switches(self, switches=None):
         s = self._u8(switches)

@@ -52,9 +52,9 @@ def test_masked_step(torch, cfg, batch, n_roms):
         if t == 5: mask[:] = 0
         if t == 6: mask[: batch // 2] = 0
         g.step_masked(dev(torch, acts[t]), w.frameskip, dev(torch, mask))
-        o.step_masked(acts[t], w.frameskip, mask)
+        o.step_masked(acts[t], w.frameskip, mask, threads=NCPU)
         compare(g, o, f"masked cfg{cfg} step {t}")
-    g.step_masked(dev(torch, acts[0]), 2, None); o.step_masked(acts[0], 2, None)
+    g.step_masked(dev(torch, acts[0]), 2, None); o.step_masked(acts[0], 2, None, threads=NCPU)
     compare(g, o, "masked NULL mask")
 
 
@@ -133,7 +133,7 @@ def test_masked_and_boot_full_batch_launch_shape(torch):
     rng = np.random.default_rng(5)
     for t in range(6):
         mask = (rng.integers(0, 4, w.batch) > 0).astype(np.uint8)
-        g.step_masked(dev(torch, acts[t]), 4, dev(torch, mask)); o.step_masked(acts[t][idx], 4, mask[idx])
+        g.step_masked(dev(torch, acts[t]), 4, dev(torch, mask)); o.step_masked(acts[t][idx], 4, mask[idx], threads=NCPU)
         compare(g, o, f"full masked step {t}", envs=idx)
         if t == 2:
             bm = (rng.integers(0, 3, w.batch) == 0).astype(np.uint8)
@@ -163,7 +163,7 @@ def test_auto_reset_amortised_equals_boot_protocol(torch, batch, n_roms):
     T = 16 + 30 + 4
     for t in range(T):                                           # ... and then waits until the GPU env is ready
         ready = (t >= want).astype(np.uint8)
-        g.step(dev(torch, acts[3 + t]), 4); o.step_masked(acts[3 + t], 4, ready)
+        g.step(dev(torch, acts[3 + t]), 4); o.step_masked(acts[3 + t], 4, ready, threads=NCPU)
         assert (g.get_booting().cpu().numpy() == np.maximum(want - (t + 1), 0)).all()
     compare(g, o, "auto_reset")
     # a second arming while the first envs play on, with a masked step in between (frozen envs do not count down)
@@ -173,11 +173,11 @@ def test_auto_reset_amortised_equals_boot_protocol(torch, batch, n_roms):
     g.step_masked(dev(torch, acts[0]), 4, dev(torch, frozen))
     left = np.where(m2 != 0, 3, 0) - np.where((m2 != 0) & (frozen != 0), 1, 0)
     assert (g.get_booting().cpu().numpy() == left).all()
-    o.step_masked(acts[0], 4, frozen & (m2 == 0))
+    o.step_masked(acts[0], 4, frozen & (m2 == 0), threads=NCPU)
     for t in range(1, 5):
         a_t = acts[t]
         g.step(dev(torch, a_t), 4)
-        o.step_masked(a_t, 4, (left == 0).astype(np.uint8))
+        o.step_masked(a_t, 4, (left == 0).astype(np.uint8), threads=NCPU)
         left = np.maximum(left - 1, 0)
     compare(g, o, "auto_reset second arming")
     with pytest.raises(RuntimeError):
@@ -200,7 +200,7 @@ def test_ale_vec_env_amortised_auto_reset(torch):
         done = np.array([r.rnd(9) == 0 for _ in range(n)], np.uint8)
         play = (wait == 0).astype(np.uint8)
         m = env.step(dev(torch, acts[t]), dev(torch, done)).cpu().numpy()
-        o.step_masked(acts[t], 4, play)                          # the oracle env waits while the GPU env runs its boot steps
+        o.step_masked(acts[t], 4, play, threads=NCPU)                          # the oracle env waits while the GPU env runs its boot steps
         wait = np.maximum(wait - 1, 0)
         assert (m == done).all()
         if m.any():
@@ -211,7 +211,7 @@ def test_ale_vec_env_amortised_auto_reset(torch):
     for t in range(8):                                           # let every boot finish
         play = (wait == 0).astype(np.uint8)
         env.step(dev(torch, acts[t]))
-        o.step_masked(acts[t], 4, play)
+        o.step_masked(acts[t], 4, play, threads=NCPU)
         wait = np.maximum(wait - 1, 0)
     compare(env.vcs, o, "amortised AleVecEnv")
     env.close()
