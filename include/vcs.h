@@ -61,7 +61,7 @@ typedef struct {
  * Layout hint (performance only, never results): when every aligned group of 256 (batches >= 32768), 128 or 64
  * consecutive envs shares one ROM, the ROM is staged in shared memory per block and F8 carts regroup their envs by
  * bank inside the block; otherwise ROM bytes come through the read-only cache.  Tuning overrides read here from
- * the environment: VCS_BLOCK=64|128|256, VCS_ROM_GLOBAL, VCS_NO_REGROUP, VCS_NO_SPIN, VCS_NO_FUSE.
+ * the environment: VCS_BLOCK=64|128|256, VCS_ROM_GLOBAL, VCS_NO_REGROUP, VCS_NO_SPIN, VCS_NO_FUSE, VCS_NO_BALANCE.
  * Errors: VCS_EINVAL (NULL/size/range), VCS_EROM (size not 2048/4096/8192/16384/32768), VCS_ECUDA, VCS_ENOMEM. */
 int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms,
                const int32_t *env_rom, const uint64_t *seeds, const vcs_config *cfg);
@@ -142,6 +142,14 @@ int vcs_get_screen_host(vcs_t h, uint8_t *out_host, void *cuda_stream);
 /* Device pointer to the library-owned front screen [batch][210][160] (valid until vcs_destroy; contents
  * change with every vcs_step).  Zero-copy alternative to vcs_get_screen. */
 int vcs_screen_ptr(vcs_t h, const uint8_t **out_dev_ptr);
+
+/* Block placement introspection (performance only).  A step runs ceil(batch / block) thread blocks, all resident at
+ * once; the library records when and on which SM each block of the last plain vcs_step ran and re-assigns env groups
+ * to block indices so that the SMs finish together (VCS_NO_BALANCE in the environment turns it off).
+ * *n_out = number of blocks; if cap >= n: times_host[3 * b + 0..2] = start ns, end ns (GPU global timer), SM id of
+ * block index b in the last plain vcs_step, perm_host[b] = the env group (envs perm*block .. +block-1) block b runs
+ * next.  Either pointer may be NULL.  Synchronises the device. */
+int vcs_block_times(vcs_t h, uint64_t *times_host, int32_t *perm_host, int32_t cap, int32_t *n_out);
 
 /* Number of kernel launches this handle has enqueued so far (bench bookkeeping). */
 int64_t vcs_launch_count(vcs_t h);

@@ -18,7 +18,7 @@ VCS_OK, VCS_EINVAL, VCS_ECUDA, VCS_ENOMEM, VCS_EROM = 0, -1, -2, -3, -4
 _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
 
 EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
-           "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_launch_count",
+           "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_block_times", "vcs_launch_count",
            "vcs_optable", "vcs_issue_peak", "vcs_destroy", "vcs_last_error"]
 
 REGS_DTYPE = np.dtype([("cycles", "<u8"), ("frame", "<u4"), ("pc", "<u2"), ("a", "u1"), ("x", "u1"), ("y", "u1"),
@@ -65,6 +65,7 @@ def load_library() -> C.CDLL:
     for f in ("vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host"):
         getattr(L, f).argtypes = [P, P, P]
     L.vcs_screen_ptr.argtypes = [P, C.POINTER(P)]
+    L.vcs_block_times.argtypes = [P, P, P, C.c_int32, C.POINTER(C.c_int32)]
     L.vcs_launch_count.argtypes = [P]; L.vcs_launch_count.restype = C.c_int64
     L.vcs_optable.argtypes = [P]
     L.vcs_issue_peak.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -221,6 +222,14 @@ class VCS:
     def screen_host(self, out=None, stream=None) -> np.ndarray:
         out = np.empty((self.batch, 210, 160), dtype=np.uint8) if out is None else out
         self._chk(self.L.vcs_get_screen_host(self.h, out.ctypes.data, _stream_ptr(stream)), "vcs_get_screen_host"); return out
+
+    def block_times(self):
+        """(times uint64[n][3] = start ns, end ns, SM id of each block of the last plain step; perm int32[n])."""
+        n = C.c_int32(0)
+        self._chk(self.L.vcs_block_times(self.h, None, None, 0, C.byref(n)), "vcs_block_times")
+        times = np.zeros((n.value, 3), dtype=np.uint64); perm = np.zeros(n.value, dtype=np.int32)
+        self._chk(self.L.vcs_block_times(self.h, times.ctypes.data, perm.ctypes.data, n.value, C.byref(n)), "vcs_block_times")
+        return times, perm
 
     def launch_count(self) -> int:
         return int(self.L.vcs_launch_count(self.h))

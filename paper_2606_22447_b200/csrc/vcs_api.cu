@@ -115,7 +115,7 @@ StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   StepParams p;
   p.st = h->d_st; p.ram = h->d_ram; p.cyc = h->d_cyc; p.screen = h->d_screen;
   p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
-  p.actions = actions; p.switches = h->d_switches; p.mask = nullptr; p.boot = h->d_boot_ctr; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
+  p.actions = actions; p.switches = h->d_switches; p.mask = nullptr; p.boot = h->d_boot_ctr; p.perm = h->d_perm; p.blk_time = nullptr; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
   p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom;
   p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0;
   return p;
@@ -217,6 +217,15 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   CU(h, cudaMemset(h->d_switches, 0x3F, (size_t)B));
   CU(h, cudaMalloc((void **)&h->d_boot, 3 * (size_t)B));
   CU(h, cudaMalloc((void **)&h->d_boot_ctr, sizeof(uint32_t) * B));
+  {                                                   // block placement: identity until the first measurements are in
+    const int nblk = (batch + h->block - 1) / h->block;
+    std::vector<int32_t> id(nblk); for (int i = 0; i < nblk; ++i) id[i] = i;
+    CU(h, cudaMalloc((void **)&h->d_perm, sizeof(int32_t) * nblk));
+    CU(h, cudaMemcpy(h->d_perm, id.data(), sizeof(int32_t) * nblk, cudaMemcpyHostToDevice));
+    CU(h, cudaMalloc((void **)&h->d_blk_time, sizeof(unsigned long long) * 3 * nblk));
+    CU(h, cudaMemset(h->d_blk_time, 0, sizeof(unsigned long long) * 3 * nblk));
+    h->balance = getenv("VCS_NO_BALANCE") ? 0 : 1; h->plain_steps = 0;
+  }
   if (!getenv("VCS_NO_SOFT_ALLOC")) {                                                   // soft mode: every entry decodes at run time (vcs_step_soft)
     std::vector<DWord> sl((h->max_rom < 8192 ? 8192 : h->max_rom) + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});
     std::vector<RomMeta> ms(meta); for (auto &m : ms) { m.pad = m.doff; m.doff = 0; }     // pad: offset into the W(T) x ROM table
@@ -253,9 +262,18 @@ int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_
   if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31))
     return fail(h, VCS_EINVAL, "vcs_step: frameskip out of range");
   StepParams p = params_of(h, actions_dev, frameskip);
+  if (h->balance) p.blk_time = h->d_blk_time;
   cudaError_t ce = launch_step(p, (cudaStream_t)cuda_stream);
   h->launches += 1;
   if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step launch", ce);
+  if (h->balance) {                                   // re-place the blocks from this step's per-block times: early on, then now and again
+    const long long k = ++h->plain_steps;
+    if (k == 2 || k == 4 || k == 8 || k == 16 || k == 32 || (k & 63) == 0) {
+      ce = launch_rebalance(h->d_perm, h->d_blk_time, (h->batch + h->block - 1) / h->block, (cudaStream_t)cuda_stream);
+      h->launches += 1;
+      if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step rebalance launch", ce);
+    }
+  }
   return VCS_OK;
 }
 
@@ -420,6 +438,17 @@ int vcs_get_screen_host(vcs_t h, uint8_t *out_host, void *cuda_stream) {
   return VCS_OK;
 }
 
+int vcs_block_times(vcs_t h, uint64_t *times_host, int32_t *perm_host, int32_t cap, int32_t *n_out) {
+  if (!h || !n_out) return VCS_EINVAL;
+  const int n = (h->batch + h->block - 1) / h->block;
+  *n_out = n;
+  if (cap < n) return (times_host || perm_host) ? VCS_EINVAL : VCS_OK;
+  CU(h, cudaDeviceSynchronize());
+  if (times_host) CU(h, cudaMemcpy(times_host, h->d_blk_time, sizeof(unsigned long long) * 3 * n, cudaMemcpyDeviceToHost));
+  if (perm_host) CU(h, cudaMemcpy(perm_host, h->d_perm, sizeof(int32_t) * n, cudaMemcpyDeviceToHost));
+  return VCS_OK;
+}
+
 int64_t vcs_launch_count(vcs_t h) { return h ? h->launches : -1; }
 
 int vcs_optable(uint16_t *out256) {
@@ -431,7 +460,7 @@ int vcs_destroy(vcs_t h) {
   if (!h) return VCS_EINVAL;
   cudaDeviceSynchronize();
   cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom);
-  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr);
+  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr); cudaFree(h->d_perm); cudaFree(h->d_blk_time);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   delete h;
   return VCS_OK;

@@ -937,7 +937,12 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   uint32_t *s_ctx = smem + S_WORDS * BLOCK;
   constexpr uint32_t ROM_OFF = (S_WORDS * BLOCK + C_WORDS) * 4;          // byte offset of the ROM image in smem
   const int tid = threadIdx.x;
-  const int e0 = blockIdx.x * BLOCK;
+  if (p.blk_time && tid == 0) {                            // placement bookkeeping: when and where this block ran
+    unsigned long long t; uint32_t sm;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
+    p.blk_time[3 * blockIdx.x] = t; p.blk_time[3 * blockIdx.x + 1] = 0; p.blk_time[3 * blockIdx.x + 2] = sm;
+  }
+  const int e0 = (p.perm ? p.perm[blockIdx.x] : (int)blockIdx.x) * BLOCK;   // which group of BLOCK envs this block runs
   const int B = p.batch;
   const int ei = e0 + tid;                                 // the env this thread starts with
   const bool filed = tid < BLOCK;                          // threads of the spare warp start without a file
@@ -1074,6 +1079,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     for (int i = 0; i < 32; ++i) p.ram[i * B + e] = smem[(S_RAM + i) * BLOCK + fs];
     p.cyc[e] += (unsigned long long)s.cyc;
   }
+  if (p.blk_time) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); atomicMax(&p.blk_time[3 * blockIdx.x + 1], t); }
 }
 
 // W(T) x ROM: for every cell o of every bank of every cartridge the relaxed read of eq. (10) on the 4096 x 8 bit
@@ -1101,6 +1107,65 @@ __global__ void soft_table_kernel(const uint8_t *rom_blob, const RomMeta *meta, 
 }
 cudaError_t launch_soft_table(const uint8_t *rom_blob, const RomMeta *meta, int n_roms, const float *w, int K, float *tab, cudaStream_t stream) {
   soft_table_kernel<<<dim3(32768 / 256, n_roms), 256, 0, stream>>>(rom_blob, meta, w, K, tab);
+  return cudaGetLastError();
+}
+
+// Block placement.  All blocks of a step are resident at once (one wave), two 256-env blocks per SM at most, and 256
+// blocks on 148 SMs leave 108 SMs with two blocks and 40 with one; a block is a ROM's envs, and ROMs differ in work per
+// frame, so with blocks placed in env order the step waits for the unluckiest SM (measured: slowest SM 9.3 ms, mean
+// 7.4 ms).  Every plain vcs_step records when and on which SM each block ran; from that, this kernel estimates each
+// group's stand-alone time W (a block that shares its SM runs A = 1.27x slower while its partner is still there:
+// measured 6.3 -> 7.9 ms on 4K carts, 7.4 -> 9.6 ms on F8 carts) and re-assigns groups to block indices for the next
+// launches — the hardware places block indices on SMs the same way every launch: the heaviest groups get the SMs that
+// hold one block, the others are paired heaviest with lightest.  Results do not depend on the placement (envs are
+// independent); only the step time does.  n <= 1024 blocks, at most two per SM; otherwise the placement is left alone.
+__global__ void rebalance_kernel(int32_t *perm, const unsigned long long *blk, int n) {
+  __shared__ float W[1024]; __shared__ int partner[1024]; __shared__ int grp[1024]; __shared__ int slot_of_rank[1024];
+  __shared__ int bad, n_single;
+  const float A = 1.27f;
+  if (threadIdx.x == 0) { bad = 0; n_single = 0; }
+  __syncthreads();
+  for (int s = threadIdx.x; s < n; s += blockDim.x) {
+    grp[s] = perm[s];
+    const unsigned long long sm = blk[3 * s + 2];
+    int p = -1, cnt = 0;
+    for (int j = 0; j < n; ++j) if (j != s && blk[3 * j + 2] == sm) { p = j; ++cnt; }
+    partner[s] = p;
+    if (cnt > 1 || blk[3 * s + 1] <= blk[3 * s]) bad = 1;             // more than two blocks on an SM, or no measurement
+  }
+  __syncthreads();
+  if (bad) return;
+  for (int s = threadIdx.x; s < n; s += blockDim.x) {                  // stand-alone time of the group in slot s
+    const float d = (float)(blk[3 * s + 1] - blk[3 * s]);
+    const int p = partner[s];
+    if (p < 0) W[s] = d;
+    else {
+      const float dp = (float)(blk[3 * p + 1] - blk[3 * p]);
+      const bool lighter = d < dp || (d == dp && s < p);
+      W[s] = lighter ? d / A : d - (A - 1.f) * (dp / A);
+    }
+  }
+  __syncthreads();
+  // slots in placement order: single-SM slots first, then the pairs (first slot = lower index)
+  for (int s = threadIdx.x; s < n; s += blockDim.x) {
+    if (partner[s] < 0) { int r = 0; for (int j = 0; j < s; ++j) r += partner[j] < 0; slot_of_rank[r] = s; atomicAdd(&n_single, 1); }
+  }
+  __syncthreads();
+  const int ns = n_single, np = (n - ns) / 2;
+  for (int s = threadIdx.x; s < n; s += blockDim.x) {
+    const int p = partner[s];
+    if (p > s) { int r = 0; for (int j = 0; j < s; ++j) r += partner[j] > j; slot_of_rank[ns + r] = s; slot_of_rank[ns + 2 * np - 1 - r] = p; }
+  }
+  __syncthreads();
+  for (int s = threadIdx.x; s < n; s += blockDim.x) {                  // rank of the group in slot s by W, heaviest first
+    int r = 0; const float w = W[s];
+    for (int j = 0; j < n; ++j) r += (W[j] > w || (W[j] == w && j < s)) ? 1 : 0;
+    perm[slot_of_rank[r]] = grp[s];       // ranks 0..ns-1: alone; rank ns+q pairs with rank ns+2np-1-q
+  }
+}
+cudaError_t launch_rebalance(int32_t *perm, const unsigned long long *blk_time, int n, cudaStream_t stream) {
+  if (n < 2 || n > 1024) return cudaSuccess;
+  rebalance_kernel<<<1, 256, 0, stream>>>(perm, blk_time, n);
   return cudaGetLastError();
 }
 

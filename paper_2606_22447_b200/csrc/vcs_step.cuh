@@ -9,7 +9,8 @@ namespace vcs {
 struct StepParams {
   uint32_t *st; uint32_t *ram; unsigned long long *cyc; uint8_t *screen;
   const uint8_t *rom_blob; const uint2 *drom; const RomMeta *rom_meta; const int32_t *env_rom;
-  const uint8_t *actions; const uint8_t *switches; const uint8_t *mask; uint32_t *boot;   // switches: SWCHB input pins per env; mask: nullptr = every env steps; boot: per-env boot countdown (vcs_auto_reset)
+  const uint8_t *actions; const uint8_t *switches; const uint8_t *mask; uint32_t *boot;
+  const int32_t *perm; unsigned long long *blk_time;       // block placement (vcs_step.cu, rebalance_kernel): perm[blockIdx] = env group; blk_time[3 * blockIdx] = start ns, end ns, SM id   // switches: SWCHB input pins per env; mask: nullptr = every env steps; boot: per-env boot countdown (vcs_auto_reset)
   int32_t batch, frameskip, y0, max_lines;
   const float *soft_w; const float *soft_tab; float *soft_out; float soft_alpha; int32_t soft_K;   // soft_out != nullptr: SOFT-STE mode (vcs_step_soft)
   int32_t block, rom_smem, regroup; uint32_t max_rom;     // launch shape: envs per block (64/128/256), ROM staged in smem, largest image
@@ -19,6 +20,7 @@ void upload_optable();
 const uint16_t *host_optable();
 cudaError_t launch_step(const StepParams &p, cudaStream_t stream);
 cudaError_t launch_soft_table(const uint8_t *rom_blob, const RomMeta *meta, int n_roms, const float *w, int K, float *tab, cudaStream_t stream);
+cudaError_t launch_rebalance(int32_t *perm, const unsigned long long *blk_time, int n, cudaStream_t stream);
 size_t step_smem_bytes(int block, bool roms, uint32_t max_rom);
 
 }  // namespace vcs
