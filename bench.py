@@ -258,14 +258,14 @@ def main():
     peak_alu, _ = issue_peak(0)                     # alu pipe alone (16 lanes / scheduler / clk)
     peak = peak_mixed
     kms = float(np.mean(kern_ms))
-    # DRAM bytes of one launch from the committed `ncu --set full` capture of this kernel (profiles/r01_v13_full.txt:
+    # DRAM bytes of one launch from the committed `ncu --set full` capture of this kernel (profiles/r01_v14_full.txt:
     # dram__bytes_read.sum + dram__bytes_write.sum); algorithmic bytes are roofline.hbm.algorithmic_bytes_per_launch
-    NCU_DRAM_BYTES = 27.267840e6 + 2.173354e9
+    NCU_DRAM_BYTES = 27.332096e6 + 2.173480e9
     roof = {"bound": "alu", "unit": "thread-instr/s", "peak": peak,
             "peak_basis": "vcs_issue_peak(kind=1): LOP3+IMAD chains on all SMs, measured in this run",
             "peak_alu_pipe_only": peak_alu, "peak_nominal": nominal,
             "kernel": "vcs_step_kernel", "kernel_ms": kms, "traffic": NCU_DRAM_BYTES if B == 65536 else None,
-            "traffic_unit": "DRAM bytes per launch (ncu, profiles/r01_v13_full.txt)"}
+            "traffic_unit": "DRAM bytes per launch (ncu, profiles/r01_v14_full.txt)"}
     if work:
         ops = MODEL_PER_INSTR * work["instr"] + MODEL_PER_SEGMENT * work["tia_writes"] + MODEL_PER_LINE * work["lines"]
         roof.update(achieved=ops * B / (kms * 1e-3), algorithmic_thread_instr_per_env_step=ops, work_per_env_step=work)

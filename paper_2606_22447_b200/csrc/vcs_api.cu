@@ -224,7 +224,11 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
     CU(h, cudaMemcpy(h->d_perm, id.data(), sizeof(int32_t) * nblk, cudaMemcpyHostToDevice));
     CU(h, cudaMalloc((void **)&h->d_blk_time, sizeof(unsigned long long) * 3 * nblk));
     CU(h, cudaMemset(h->d_blk_time, 0, sizeof(unsigned long long) * 3 * nblk));
+    CU(h, cudaMalloc((void **)&h->d_w_avg, sizeof(float) * nblk));
+    CU(h, cudaMemset(h->d_w_avg, 0, sizeof(float) * nblk));
     h->balance = getenv("VCS_NO_BALANCE") ? 0 : 1; h->plain_steps = 0;
+    h->balance_a = 1.27f;                             // measured slowdown of a block that shares its SM
+    if (const char *ev = getenv("VCS_BALANCE_A")) { const float v = (float)atof(ev); if (v >= 1.f && v <= 2.f) h->balance_a = v; }
   }
   if (!getenv("VCS_NO_SOFT_ALLOC")) {                                                   // soft mode: every entry decodes at run time (vcs_step_soft)
     std::vector<DWord> sl((h->max_rom < 8192 ? 8192 : h->max_rom) + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});
@@ -268,8 +272,8 @@ int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_
   if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step launch", ce);
   if (h->balance) {                                   // re-place the blocks from this step's per-block times: early on, then now and again
     const long long k = ++h->plain_steps;
-    if (k == 2 || k == 4 || k == 8 || k == 16 || k == 32 || (k & 63) == 0) {
-      ce = launch_rebalance(h->d_perm, h->d_blk_time, (h->batch + h->block - 1) / h->block, (cudaStream_t)cuda_stream);
+    if ((k >= 2 && k <= 16) || (k & 3) == 0) {            // (the first step after a reset is a short frame)
+      ce = launch_rebalance(h->d_perm, h->d_blk_time, (h->batch + h->block - 1) / h->block, h->balance_a, h->d_w_avg, (cudaStream_t)cuda_stream);
       h->launches += 1;
       if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step rebalance launch", ce);
     }
@@ -460,7 +464,7 @@ int vcs_destroy(vcs_t h) {
   if (!h) return VCS_EINVAL;
   cudaDeviceSynchronize();
   cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom);
-  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr); cudaFree(h->d_perm); cudaFree(h->d_blk_time);
+  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr); cudaFree(h->d_perm); cudaFree(h->d_blk_time); cudaFree(h->d_w_avg);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   delete h;
   return VCS_OK;

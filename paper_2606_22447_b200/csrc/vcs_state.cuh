@@ -92,7 +92,7 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   uint2 *d_drom_soft; RomMeta *d_rom_meta_soft; float *d_soft_w;   // soft mode: an all-H_SLOW decode table (every byte fetched at run time), metas with doff 0, e^{-k/T}
   uint8_t *d_actions_stage;     // for vcs_step_host
   uint8_t *d_switches;          // SWCHB input pins per env (vcs_set_switches; 0x3F after vcs_create)
-  int32_t *d_perm; unsigned long long *d_blk_time; long long plain_steps; int balance;   // block placement (rebalance_kernel in vcs_step.cu)
+  int32_t *d_perm; unsigned long long *d_blk_time; long long plain_steps; int balance; float balance_a; float *d_w_avg;   // block placement (rebalance_kernel in vcs_step.cu)
   uint32_t *d_boot_ctr;         // per env: boot steps left | NOOP starts << 8 | RESET steps << 16 (vcs_auto_reset; 0 = playing)
   uint8_t *d_boot;              // vcs_boot scratch: [batch] NOOP actions, [batch] per-iteration mask, [batch] switches with RESET held
   uint8_t *h_pinned; size_t h_pinned_bytes;

@@ -1119,10 +1119,9 @@ cudaError_t launch_soft_table(const uint8_t *rom_blob, const RomMeta *meta, int 
 // launches — the hardware places block indices on SMs the same way every launch: the heaviest groups get the SMs that
 // hold one block, the others are paired heaviest with lightest.  Results do not depend on the placement (envs are
 // independent); only the step time does.  n <= 1024 blocks, at most two per SM; otherwise the placement is left alone.
-__global__ void rebalance_kernel(int32_t *perm, const unsigned long long *blk, int n) {
+__global__ void rebalance_kernel(int32_t *perm, const unsigned long long *blk, int n, float A, float *w_avg) {
   __shared__ float W[1024]; __shared__ int partner[1024]; __shared__ int grp[1024]; __shared__ int slot_of_rank[1024];
   __shared__ int bad, n_single;
-  const float A = 1.27f;
   if (threadIdx.x == 0) { bad = 0; n_single = 0; }
   __syncthreads();
   for (int s = threadIdx.x; s < n; s += blockDim.x) {
@@ -1144,6 +1143,8 @@ __global__ void rebalance_kernel(int32_t *perm, const unsigned long long *blk, i
       const bool lighter = d < dp || (d == dp && s < p);
       W[s] = lighter ? d / A : d - (A - 1.f) * (dp / A);
     }
+    float &avg = w_avg[grp[s]];                                        // per group, smoothed over the steps measured so far:
+    W[s] = avg = (avg > 0.f) ? 0.7f * avg + 0.3f * W[s] : W[s];        // one step's inputs move a ROM's time by a few per cent
   }
   __syncthreads();
   // slots in placement order: single-SM slots first, then the pairs (first slot = lower index)
@@ -1163,9 +1164,9 @@ __global__ void rebalance_kernel(int32_t *perm, const unsigned long long *blk, i
     perm[slot_of_rank[r]] = grp[s];       // ranks 0..ns-1: alone; rank ns+q pairs with rank ns+2np-1-q
   }
 }
-cudaError_t launch_rebalance(int32_t *perm, const unsigned long long *blk_time, int n, cudaStream_t stream) {
+cudaError_t launch_rebalance(int32_t *perm, const unsigned long long *blk_time, int n, float slowdown, float *w_avg, cudaStream_t stream) {
   if (n < 2 || n > 1024) return cudaSuccess;
-  rebalance_kernel<<<1, 256, 0, stream>>>(perm, blk_time, n);
+  rebalance_kernel<<<1, 256, 0, stream>>>(perm, blk_time, n, slowdown, w_avg);
   return cudaGetLastError();
 }
 

@@ -20,7 +20,7 @@ void upload_optable();
 const uint16_t *host_optable();
 cudaError_t launch_step(const StepParams &p, cudaStream_t stream);
 cudaError_t launch_soft_table(const uint8_t *rom_blob, const RomMeta *meta, int n_roms, const float *w, int K, float *tab, cudaStream_t stream);
-cudaError_t launch_rebalance(int32_t *perm, const unsigned long long *blk_time, int n, cudaStream_t stream);
+cudaError_t launch_rebalance(int32_t *perm, const unsigned long long *blk_time, int n, float slowdown, float *w_avg, cudaStream_t stream);
 size_t step_smem_bytes(int block, bool roms, uint32_t max_rom);
 
 }  // namespace vcs
