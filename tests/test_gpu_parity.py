@@ -381,3 +381,26 @@ def test_full_length_runs(torch, cfg, steps, stride):
             g.step(dacts[t], w.frameskip); o.step(acts[t][idx], w.frameskip, threads=NCPU)
         compare(g, o, f"config{cfg} full length, step {t0 + chunk}", envs=idx)
     assert int(g.regs_host()["frame"].min()) >= steps * w.frameskip
+
+
+def test_block_placement_permutes_groups_not_results(torch):
+    """Measured block placement: after a few plain steps of config 4 at full batch the block -> env-group
+    map is a non-trivial permutation, every block has a time stamp and an SM, at most two blocks share an SM — and the
+    state is what a handle with the placement switched off computes (envs are independent)."""
+    from paper_2606_22447_b200 import VCS
+    w = make_workload(4)
+    acts = torch.from_numpy(w.actions(0, 6)).cuda()
+    g = VCS(w.roms, w.seeds, w.env_rom)
+    os.environ["VCS_NO_BALANCE"] = "1"
+    try:
+        ref = VCS(w.roms, w.seeds, w.env_rom)
+    finally:
+        del os.environ["VCS_NO_BALANCE"]
+    for t in range(6):
+        g.step(acts[t], 4); ref.step(acts[t], 4)
+    times, perm = g.block_times()
+    assert sorted(perm.tolist()) == list(range(256)) and perm.tolist() != list(range(256))
+    assert (times[:, 1] > times[:, 0]).all() and np.bincount(times[:, 2].astype(np.int64)).max() <= 2
+    _, perm0 = ref.block_times()
+    assert perm0.tolist() == list(range(256))
+    assert (g.get_ram() == ref.get_ram()).all() and (g.get_regs() == ref.get_regs()).all() and (g.get_screen() == ref.get_screen()).all()
