@@ -1118,11 +1118,11 @@ cudaError_t launch_soft_table(const uint8_t *rom_blob, const RomMeta *meta, int 
 // measured 6.3 -> 7.9 ms on 4K carts, 7.4 -> 9.6 ms on F8 carts) and re-assigns groups to block indices for the next
 // launches — the hardware places block indices on SMs the same way every launch: the heaviest groups get the SMs that
 // hold one block, the others are paired heaviest with lightest.  Results do not depend on the placement (envs are
-// independent); only the step time does.  n <= 1024 blocks, at most two per SM; otherwise the placement is left alone.
+// independent); only the step time does.  n <= 1024 blocks; with more than two blocks per SM: longest first (below).
 __global__ void rebalance_kernel(int32_t *perm, const unsigned long long *blk, int n, float A, float *w_avg) {
   __shared__ float W[1024]; __shared__ int partner[1024]; __shared__ int grp[1024]; __shared__ int slot_of_rank[1024];
-  __shared__ int bad, n_single;
-  if (threadIdx.x == 0) { bad = 0; n_single = 0; }
+  __shared__ int bad, n_single, crowded;
+  if (threadIdx.x == 0) { bad = 0; n_single = 0; crowded = 0; }
   __syncthreads();
   for (int s = threadIdx.x; s < n; s += blockDim.x) {
     grp[s] = perm[s];
@@ -1130,10 +1130,35 @@ __global__ void rebalance_kernel(int32_t *perm, const unsigned long long *blk, i
     int p = -1, cnt = 0;
     for (int j = 0; j < n; ++j) if (j != s && blk[3 * j + 2] == sm) { p = j; ++cnt; }
     partner[s] = p;
-    if (cnt > 1 || blk[3 * s + 1] <= blk[3 * s]) bad = 1;             // more than two blocks on an SM, or no measurement
+    if (blk[3 * s + 1] <= blk[3 * s]) bad = 1;                        // no measurement
+    else if (cnt > 1) atomicOr(&crowded, 1);                          // more than two blocks ran on that SM
   }
   __syncthreads();
   if (bad) return;
+  if (crowded) {
+    __shared__ unsigned long long t_first, t_last, d_max;
+    if (threadIdx.x == 0) { t_first = ~0ull; t_last = 0; d_max = 0; }
+    __syncthreads();
+    for (int s = threadIdx.x; s < n; s += blockDim.x) {
+      atomicMin(&t_first, blk[3 * s]); atomicMax(&t_last, blk[3 * s]); atomicMax(&d_max, blk[3 * s + 1] - blk[3 * s]);
+    }
+    __syncthreads();
+    if (t_last - t_first < d_max / 4) return;             // one wave of small blocks: every block started at once, leave it alone
+    // More blocks than the SMs hold at once (batches beyond one wave) or small blocks: the hardware hands out block
+    // indices in order as SMs free up, so run the longest blocks first and let the short ones fill the tail.
+    for (int s = threadIdx.x; s < n; s += blockDim.x) {
+      float &avg = w_avg[grp[s]];
+      const float d = (float)(blk[3 * s + 1] - blk[3 * s]);
+      W[s] = avg = (avg > 0.f) ? 0.7f * avg + 0.3f * d : d;
+    }
+    __syncthreads();
+    for (int s = threadIdx.x; s < n; s += blockDim.x) {
+      int r = 0; const float w = W[s];
+      for (int j = 0; j < n; ++j) r += (W[j] > w || (W[j] == w && j < s)) ? 1 : 0;
+      perm[r] = grp[s];
+    }
+    return;
+  }
   for (int s = threadIdx.x; s < n; s += blockDim.x) {                  // stand-alone time of the group in slot s
     const float d = (float)(blk[3 * s + 1] - blk[3 * s]);
     const int p = partner[s];

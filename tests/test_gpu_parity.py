@@ -404,3 +404,20 @@ def test_block_placement_permutes_groups_not_results(torch):
     _, perm0 = ref.block_times()
     assert perm0.tolist() == list(range(256))
     assert (g.get_ram() == ref.get_ram()).all() and (g.get_regs() == ref.get_regs()).all() and (g.get_screen() == ref.get_screen()).all()
+
+
+def test_two_wave_batch_longest_first_placement(torch):
+    """131,072 envs = 512 blocks on 296 block slots: the launch runs in two waves and the placement kernel orders the
+    blocks longest first; a sample of envs against the oracle, and the block order must still be a permutation."""
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    w = make_workload(4, batch=131072, n_roms=256)
+    idx = np.arange(64) * 2048 + (np.arange(64) * 197) % 2048
+    g = VCS(w.roms, w.seeds, w.env_rom)
+    o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx])
+    acts = w.actions(0, 6)
+    for t in range(6):
+        g.step(torch.from_numpy(acts[t]).cuda(), 4); o.step(acts[t][idx], 4, threads=NCPU)
+    compare(g, o, "two waves", envs=idx)
+    _, perm = g.block_times()
+    assert sorted(perm.tolist()) == list(range(512)) and perm.tolist() != list(range(512))
