@@ -273,13 +273,25 @@ def main():
     hbm_bytes = B * (210 * 160 + 2 * (128 + 4 * 15 + 8) + 1)
     roof["hbm"] = {"algorithmic_bytes_per_launch": hbm_bytes, "achieved_gbs": hbm_bytes / (kms * 1e-3) / 1e9,
                    "peak_gbs": peaks.get("hbm_gbs"), "frac": (hbm_bytes / (kms * 1e-3) / 1e9) / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None}
+    placement = None
+    try:                                            # per-SM finishing times of the last step's blocks
+        bt, perm = env.block_times()
+        if len(perm) and (bt[:, 1] > bt[:, 0]).all():
+            t0_ = bt[:, 0].min(); ends = {}
+            for b in range(len(perm)):
+                ends[int(bt[b, 2])] = max(ends.get(int(bt[b, 2]), 0.0), float(bt[b, 1] - t0_) * 1e-6)
+            ev = np.array(list(ends.values()))
+            placement = {"blocks": int(len(perm)), "sms_used": int(len(ev)), "sm_end_ms": {"min": float(ev.min()), "mean": float(ev.mean()), "max": float(ev.max())},
+                         "identity": bool((perm == np.arange(len(perm))).all())}
+    except Exception as ex:                         # diagnostics only
+        placement = {"error": str(ex)}
     line = {"metric": METRIC if B == 65536 else METRIC.replace("65536", str(B)), "value": value, "unit": "env-steps/s", "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "u8" if args.soft_T is None else "u8 + f32 soft reads", "data": "synthetic", "emulated_cycles_per_s": cycles / (total_ms * 1e-3), "frames_per_s": value * FRAMESKIP,
             "config": {"workload": label,
                        "batch_per_gpu": B, "frameskip": FRAMESKIP, "l2": "per-step working set 2.2 GB (screens) > 126 MB L2; no explicit flush",
                        "target_env_steps_per_s": 1e7},
-            "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, "roofline": roof, "cpu_baseline": cpu}
+            "clocks": clocks, "gpu_launches": int(launches), "placement": placement, "e2e": e2e, "roofline": roof, "cpu_baseline": cpu}
     if work:      # the paper's own unit (one step = one CPU instruction), from the oracle's instruction count per env-step
         line["emulated_instructions_per_s"] = value * work["instr"]
     print(json.dumps(line), flush=True)
