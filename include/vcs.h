@@ -61,7 +61,7 @@ typedef struct {
  * Layout hint (performance only, never results): when every aligned group of 256 (batches >= 32768), 128 or 64
  * consecutive envs shares one ROM, the ROM is staged in shared memory per block and F8 carts regroup their envs by
  * bank inside the block; otherwise ROM bytes come through the read-only cache.  Tuning overrides read here from
- * the environment: VCS_BLOCK=64|128|256, VCS_ROM_GLOBAL, VCS_NO_REGROUP, VCS_NO_SPIN, VCS_NO_FUSE, VCS_NO_BALANCE.
+ * the environment: VCS_BLOCK=64|128|256, VCS_ROM_GLOBAL, VCS_NO_REGROUP, VCS_NO_SPIN, VCS_NO_FUSE, VCS_NO_BALANCE, VCS_BALANCE_A=<1..2>.
  * Errors: VCS_EINVAL (NULL/size/range), VCS_EROM (size not 2048/4096/8192/16384/32768), VCS_ECUDA, VCS_ENOMEM. */
 int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms,
                const int32_t *env_rom, const uint64_t *seeds, const vcs_config *cfg);
