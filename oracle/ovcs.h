@@ -94,6 +94,7 @@ float  ovcs_soft_ste(float soft, float hard);
 int  ovcs_set_action(ovcs_t *h, int32_t env, int32_t action);  /* latch pins only (C.11)  */
 int  ovcs_step_instruction(ovcs_t *h, int32_t env);             /* returns frame-end events */
 int  ovcs_tick(ovcs_t *h, int32_t env);                         /* one idle CPU cycle       */
+int  ovcs_tick_trace(ovcs_t *h, int32_t env, int32_t n, uint8_t *timer_out, uint8_t *tflag_out); /* n idle cycles, timer / flag after each */
 int  ovcs_get_debug(ovcs_t *h, int32_t env, ovcs_debug *out);
 int  ovcs_get_back(ovcs_t *h, int32_t env, uint8_t *out /* [210][160] */);
 int  ovcs_set_cpu(ovcs_t *h, int32_t env, int a, int x, int y, int sp, int p, int pc); /* <0 = keep */

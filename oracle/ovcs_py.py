@@ -70,6 +70,7 @@ def lib():
         L.ovcs_set_action.argtypes = [P, C.c_int32, C.c_int32]
         L.ovcs_step_instruction.argtypes = [P, C.c_int32]
         L.ovcs_tick.argtypes = [P, C.c_int32]
+        L.ovcs_tick_trace.argtypes = [P, C.c_int32, C.c_int32, P, P]
         L.ovcs_get_debug.argtypes = [P, C.c_int32, C.POINTER(Debug)]
         L.ovcs_get_back.argtypes = [P, C.c_int32, P]
         L.ovcs_set_cpu.argtypes = [P] + [C.c_int32] * 7
@@ -185,6 +186,10 @@ class OracleVCS:
     def set_action(self, env, action): assert lib().ovcs_set_action(self.h, env, action) == 0
     def step_instruction(self, env=0): return lib().ovcs_step_instruction(self.h, env)
     def tick(self, env=0): assert lib().ovcs_tick(self.h, env) == 0
+    def tick_trace(self, n, env=0):
+        t = np.empty(n, dtype=np.uint8); f = np.empty(n, dtype=np.uint8)
+        assert lib().ovcs_tick_trace(self.h, env, n, t.ctypes.data, f.ctypes.data) == 0
+        return t, f
     def debug(self, env=0):
         d = Debug(); assert lib().ovcs_get_debug(self.h, env, C.byref(d)) == 0; return d
     def back(self, env=0):
