@@ -49,8 +49,7 @@ typedef struct {
   uint16_t pc; uint8_t a, x, y, sp, p;   /* p: bit5 always 1, bit4 always 0                        */
   uint8_t  bank;             /* current cartridge bank                                             */
   uint16_t line; uint8_t cyc_in_line;    /* beam: scanline in frame, cycles % 76                   */
-  uint8_t  status;           /* bit0 halt on an unimplemented (undocumented) opcode, bit1 frame cap was hit,
-                                bit2 bus pattern outside the kernel's modelled set */
+  uint8_t  status;           /* bit0 halt on an unimplemented (undocumented) opcode, bit1 frame cap was hit */
   uint8_t  intim, timint, _pad[6];       /* timer value and TIMINT bit 7, read without side effects */
 } vcs_regs;
 

@@ -58,7 +58,7 @@ enum { OB_PF = 0, OB_BL, OB_P0, OB_P1, OB_M0, OB_M1 };
 enum { CX_M0P1 = 0, CX_M0P0, CX_M1P0, CX_M1P1, CX_P0PF, CX_P0BL, CX_P1PF, CX_P1BL,
        CX_M0PF, CX_M0BL, CX_M1PF, CX_M1BL, CX_BLPF, CX_P0P1, CX_M0M1 };
 
-enum : uint32_t { STATUS_ILLEGAL = 1, STATUS_CAP = 2, STATUS_UNMODELLED = 4 };
+enum : uint32_t { STATUS_ILLEGAL = 1, STATUS_CAP = 2 };
 
 // per-thread shared-memory file (word index; word i of thread t lives at smem[i*BLOCK + t])
 enum SmWord {

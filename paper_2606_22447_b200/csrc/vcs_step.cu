@@ -137,7 +137,11 @@ struct Cpu {
   // ------------------------------------------------------------------ RAM (smem, conflict-free)
   DEV uint32_t ram_rd_off(uint32_t off) const { return reinterpret_cast<const uint8_t *>(smem)[off + sl4]; }
   DEV void ram_wr_off(uint32_t off, uint32_t v) { reinterpret_cast<uint8_t *>(smem)[off + sl4] = (uint8_t)v; }
-  DEV uint32_t ram_rd(uint32_t a) { const uint32_t v = ram_rd_off(((a & 0x7Cu) * BLOCK) | (a & 3u)); if constexpr (SOFT) return soft_ram(a & 0x7Fu, v); else return v; }
+  DEV uint32_t ram_rd(uint32_t a, bool value = true) {
+    const uint32_t v = ram_rd_off(((a & 0x7Cu) * BLOCK) | (a & 3u));
+    if constexpr (SOFT) { if (value) return soft_ram(a & 0x7Fu, v); }
+    return v;
+  }
   DEV void ram_wr(uint32_t a, uint32_t v) { ram_wr_off(((a & 0x7Cu) * BLOCK) | (a & 3u), v); }
 
   // ------------------------------------------------------------------ ROM
@@ -223,25 +227,19 @@ struct Cpu {
     }
   }
 
-  // side-effect-light read used for instruction bytes, zero-page pointers, JMP() vectors and stack
-  // pulls: cartridge (incl. F8 hotspots) or RAM.  Anything else is outside the modelled set (status bit 2).
-  DEV void unmodelled() { status |= STATUS_UNMODELLED; lim = LIM_NOW; }
-  DEV uint32_t lite_rd(uint32_t addr, bool value = true) {
-    const uint32_t a = addr & 0x1FFFu;
-    if (a & 0x1000u) return rom_rd(a, value);
-    if ((a & 0x0280u) == 0x0080u) return ram_rd(a);
-    unmodelled(); return 0;
+  // stack accesses (C.3: $0100 | SP decodes like any other address — RAM for SP >= $80, TIA registers below) k cycles
+  // into the instruction
+  DEV void push(uint32_t v, int k) { bus_write(0x0100u | SP, v, k); SP = (SP - 1u) & 0xFFu; }
+  DEV uint32_t pull(int k) { SP = (SP + 1u) & 0xFFu; return bus_read(0x0100u | SP, k); }
+  // a READ cycle k cycles into the instruction while WSYNC holds RDY (C.4: only read cycles are stalled, so the writes of
+  // a JSR / BRK sequence run through a freshly set latch and the next read idles to the line end)
+  DEV void rdy(int k) {
+    if (!wsync) return;
+    const int32_t n = cyc + k - lstart;
+    if (n < LINE_CYC) cyc += LINE_CYC - n;
+    T::line_end(sl); lstart += LINE_CYC; wsync = false; relim();
   }
-  DEV void push(uint32_t v) {
-    if (SP & 0x80u) ram_wr(SP, v); else unmodelled();
-    SP = (SP - 1u) & 0xFFu;
-  }
-  DEV uint32_t pull() {
-    SP = (SP + 1u) & 0xFFu;
-    if (SP & 0x80u) return ram_rd(SP);
-    unmodelled(); return 0;
-  }
-  // dummy read of an indexed mode's uncorrected address in cycle cyc+k: only INTIM and F8 hotspots react
+  // a read whose value is discarded (C.5 "dummy") in cycle cyc+k: only INTIM and bank hotspots react
   DEV void dummy_rd(uint32_t addr, int k) {
     const uint32_t a = addr & 0x1FFFu;
     if (a & 0x1000u) hotspot(a);
@@ -249,7 +247,7 @@ struct Cpu {
   }
   // lim from (lstart, fstart, wsync, status)
   DEV void relim() {
-    lim = (status & (STATUS_ILLEGAL | STATUS_UNMODELLED)) ? LIM_NOW : wsync ? LIM_WSYNC : min(lstart + LINE_CYC, fstart + cap);
+    lim = (status & STATUS_ILLEGAL) ? LIM_NOW : wsync ? LIM_WSYNC : min(lstart + LINE_CYC, fstart + cap);
   }
   // after a TIA access that reported events; fc = cycle count at which a frame that just ended did so
   DEV void tia_events(uint32_t ev, int32_t fc) {
@@ -264,10 +262,10 @@ struct Cpu {
     if (ev) tia_events(ev, cyc + k + 1);
   }
   // the generic operand read (C.3 decode), k cycles into the instruction
-  DEV uint32_t bus_read(uint32_t addr, int k) {
+  DEV uint32_t bus_read(uint32_t addr, int k, bool value = true) {     // value: the byte is used (soft reads skip discarded ones)
     const uint32_t a = addr & 0x1FFFu;
-    if ((a & 0x1280u) == 0x0080u) return ram_rd(a);
-    if (a & 0x1000u) return rom_rd(a);
+    if ((a & 0x1280u) == 0x0080u) return ram_rd(a, value);
+    if (a & 0x1000u) return rom_rd(a, value);
     if (a & 0x0080u) return riot_read(a, cyc + k);
     const uint32_t r = T::read(sl, a & 0xFu, cyc - lstart + k);
     if (r >> 12) { lstart += LINE_CYC * (int32_t)(r >> 12); wsync = false; relim(); }
@@ -395,7 +393,7 @@ struct Cpu {
       rekey(); relim(); return false;
     }
     if (cyc - lstart >= LINE_CYC) { T::line_end(sl); lstart += LINE_CYC; wsync = false; }     // n == 76 exactly
-    if (status & (STATUS_ILLEGAL | STATUS_UNMODELLED)) {   // halted: idle cycles to the line end / the cap
+    if (status & STATUS_ILLEGAL) {                         // halted: idle cycles to the line end / the cap
       cyc += min(LINE_CYC - (cyc - lstart), cap - (cyc - fstart));
       return false;
     }
@@ -492,17 +490,24 @@ struct Cpu {
     {
       bool slow = false;                                   // run-time decoded
       uint32_t ea = 0, v = 0, wv = 0, op2 = 0, hid;
-      int k = 0, i0 = 0, total = 0;
+      int k = 0, i0 = 0, total = 0, kb = 0;
     dispatch:
       hid = cx & 0x7Fu;
+      kb = -(int)((cx >> DW_CY_SHIFT) & 0xFFu);            // cyc + kb = the instruction's first cycle (cy is already added; 0 for the generic handlers)
       switch (hid) {
         case H_SLOW: {                                     // byte-wise fetch with side effects, run-time decode
+          // the instruction bytes are ordinary bus reads in cycles 0, 1, 2 of the instruction (C.3 / C.5): cartridge,
+          // RAM, TIA (collision latches) or RIOT (an INTIM read clears the underflow flag), whatever PC decodes to
           const uint32_t pc0 = pc();
-          const uint32_t opc = lite_rd(pc0);
+          const uint32_t opc = bus_read(pc0, 0);
           uint32_t g = c_gen[opc];
-          const uint32_t ln = (g >> DW_LEN_SHIFT) & 0xFFu;
+          const uint32_t ln = (g >> DW_LEN_SHIFT) & 0xFFu, gh = g & 0x7Fu;
           uint32_t b1 = 0, b2 = 0;
-          if ((g & 0x7Fu) != H_ILL) { b1 = lite_rd(pc0 + 1u, ln >= 2 && (g & 0x7Fu) != H_BRK); if (ln == 3) b2 = lite_rd(pc0 + 2u); }
+          if (gh != H_ILL) {
+            if (ln == 1 || gh == H_BRK) dummy_rd(pc0 + 1u, 1);             // "R dummy@PC" of the one-byte instructions and of BRK
+            else b1 = bus_read(pc0 + 1u, 1);
+            if (ln == 3 && gh != H_JSR) b2 = bus_read(pc0 + 2u, 2);        // (JSR reads its high byte after the pushes)
+          }
           pl = b1 | (b2 << 8);
           if ((g & 0x7Fu) >= H_BR0 && (g & 0x7Fu) < H_BR0 + 8) {
             const uint32_t next = (pc0 + 2u) & 0xFFFFu, target = (next + (uint32_t)(int32_t)(int8_t)b1) & 0xFFFFu;
@@ -583,14 +588,18 @@ struct Cpu {
         } goto br_taken;
         // ---- control transfers and stack
         case H_JMP: set_pc(pl); goto ctl;
+        // (C.5 sequences; the dummy stack read of JSR / RTS / RTI / PLA / PLP lands in RAM or on a TIA read address: no effect)
         case H_JSR: { const uint32_t ret = (pc() - 1u) & 0xFFFFu;     // address of the 3rd byte
-          push(ret >> 8); push(ret & 0xFFu); rekey(); set_pc(pl); } goto ctl;
-        case H_RTS: { const uint32_t lo = pull(), hi = pull(); const uint32_t r = lo | (hi << 8);
-          rekey(); hotspot(r & 0x1FFFu); set_pc((r + 1u) & 0xFFFFu); } goto ctl;
-        case H_PHA: push(A); rekey(); break;
-        case H_PHP: push(pack_p() | 0x30u); rekey(); break;
-        case H_PLA: A = pull(); zn = A; rekey(); break;
-        case H_PLP: unpack_p(pull()); rekey(); break;
+          push(ret >> 8, kb + 3); push(ret & 0xFFu, kb + 4); rekey();
+          rdy(kb + 5);                                                        // R hi@PC comes after the pushes:
+          if (slow) pl |= bus_read(ret, kb + 5) << 8;                          // they may have set WSYNC, or rewritten that byte
+          set_pc(pl); } goto ctl;
+        case H_RTS: { const uint32_t lo = pull(kb + 3), hi = pull(kb + 4); const uint32_t r = lo | (hi << 8);
+          rekey(); dummy_rd(r, kb + 5); set_pc((r + 1u) & 0xFFFFu); } goto ctl;
+        case H_PHA: push(A, kb + 2); rekey(); break;
+        case H_PHP: push(pack_p() | 0x30u, kb + 2); rekey(); break;
+        case H_PLA: A = pull(kb + 3); zn = A; rekey(); break;
+        case H_PLP: unpack_p(pull(kb + 3)); rekey(); break;
         // ---- absolute read of INTIM / TIMINT (4th cycle)
         case H_RTIM: read_op(cx >> DW_OP2_SHIFT, timer_read(pl, cyc - 1)); break;
         // ---- generic addressing: reads (cyc = first cycle of the instruction; they add `total` themselves)
@@ -601,14 +610,14 @@ struct Cpu {
         case H_R0 + 4: ea = pl; k = 3; goto do_read;
         case H_R0 + 5: case H_R0 + 6: case H_R0 + 8: {
           uint32_t lo, hi;
-          if (hid == H_R0 + 8) { lo = lite_rd(pl & 0xFFu); hi = lite_rd((pl + 1u) & 0xFFu); k = 4; }
+          if (hid == H_R0 + 8) { lo = bus_read(pl & 0xFFu, 2); hi = bus_read((pl + 1u) & 0xFFu, 3); k = 4; }
           else { lo = pl & 0xFFu; hi = pl >> 8; k = 3; }
           const uint32_t t = lo + ((hid == H_R0 + 5) ? X : Y);
           const uint32_t unc = (hi << 8) | (t & 0xFFu);
           ea = (unc + (t & 0x100u)) & 0xFFFFu;
           if (t & 0x100u) { dummy_rd(unc, k); k += 1; }
         } goto do_read;
-        case H_R0 + 7: { const uint32_t z = (pl + X) & 0xFFu; ea = lite_rd(z) | (lite_rd((z + 1u) & 0xFFu) << 8); k = 5; } goto do_read;
+        case H_R0 + 7: { const uint32_t z = (pl + X) & 0xFFu; ea = bus_read(z, 3); ea |= bus_read((z + 1u) & 0xFFu, 4) << 8; k = 5; } goto do_read;
         // ---- generic addressing: stores
         case H_W0 + 0: ea = pl & 0xFFu; k = 2; goto do_write;
         case H_W0 + 1: ea = (pl + X) & 0xFFu; k = 3; goto do_write;
@@ -616,14 +625,14 @@ struct Cpu {
         case H_W0 + 3: ea = pl; k = 3; goto do_write;
         case H_W0 + 4: case H_W0 + 5: case H_W0 + 7: {
           uint32_t lo, hi;
-          if (hid == H_W0 + 7) { lo = lite_rd(pl & 0xFFu); hi = lite_rd((pl + 1u) & 0xFFu); k = 4; }
+          if (hid == H_W0 + 7) { lo = bus_read(pl & 0xFFu, 2); hi = bus_read((pl + 1u) & 0xFFu, 3); k = 4; }
           else { lo = pl & 0xFFu; hi = pl >> 8; k = 3; }
           const uint32_t t = lo + ((hid == H_W0 + 4) ? X : Y);
           const uint32_t unc = (hi << 8) | (t & 0xFFu);
           ea = (unc + (t & 0x100u)) & 0xFFFFu;
           dummy_rd(unc, k); k += 1;
         } goto do_write;
-        case H_W0 + 6: { const uint32_t z = (pl + X) & 0xFFu; ea = lite_rd(z) | (lite_rd((z + 1u) & 0xFFu) << 8); k = 5; } goto do_write;
+        case H_W0 + 6: { const uint32_t z = (pl + X) & 0xFFu; ea = bus_read(z, 3); ea |= bus_read((z + 1u) & 0xFFu, 4) << 8; k = 5; } goto do_write;
         // ---- generic addressing: read-modify-write
         case H_M0 + 0: ea = pl & 0xFFu; k = 2; goto do_rmw;
         case H_M0 + 1: ea = (pl + X) & 0xFFu; k = 3; goto do_rmw;
@@ -631,15 +640,16 @@ struct Cpu {
         case H_M0 + 3: { const uint32_t t = (pl & 0xFFu) + X; const uint32_t unc = (pl & 0xFF00u) | (t & 0xFFu);
           ea = (unc + (t & 0x100u)) & 0xFFFFu; dummy_rd(unc, 3); k = 4; } goto do_rmw;
         // ---- rare
-        case H_JMPI: { const uint32_t l2 = lite_rd(pl), h2 = lite_rd((pl & 0xFF00u) | ((pl + 1u) & 0xFFu));   // no carry into the page
+        case H_JMPI: { const uint32_t l2 = bus_read(pl, kb + 3), h2 = bus_read((pl & 0xFF00u) | ((pl + 1u) & 0xFFu), kb + 4);   // no carry into the page
           set_pc(l2 | (h2 << 8)); } goto ctl;
-        case H_RTI: { unpack_p(pull()); const uint32_t lo = pull(), hi = pull(); rekey(); set_pc(lo | (hi << 8)); } goto ctl;
+        case H_RTI: { unpack_p(pull(kb + 3)); const uint32_t lo = pull(kb + 4), hi = pull(kb + 5); rekey(); set_pc(lo | (hi << 8)); } goto ctl;
         case H_BRK: { const uint32_t ret = pc();             // address of the opcode + 2
-          push(ret >> 8); push(ret & 0xFFu); push(pack_p() | 0x30u); rekey();
-          const uint32_t l2 = lite_rd(0xFFFEu), h2 = lite_rd(0xFFFFu);
+          push(ret >> 8, kb + 2); push(ret & 0xFFu, kb + 3); push(pack_p() | 0x30u, kb + 4); rekey();
+          rdy(kb + 5);
+          const uint32_t l2 = bus_read(0xFFFEu, kb + 5), h2 = bus_read(0xFFFFu, kb + 6);
           set_pc(l2 | (h2 << 8)); fDI |= 4u; } goto ctl;
         default:                                           // H_ILL — C.12: halt for good, PC stays
-          if (!(status & STATUS_UNMODELLED)) status |= STATUS_ILLEGAL;
+          status |= STATUS_ILLEGAL;
           lim = LIM_NOW; goto ctl;
         do_read:
           v = bus_read(ea, k); total = k + 1;
@@ -664,8 +674,8 @@ struct Cpu {
         br_taken:
           if (slow) {                                      // the dummy reads @PC and @(old PCH : new PCL), any target
             const uint32_t next = pc(), target = (next + pl) & 0xFFFFu;
-            hotspot(next & 0x1FFFu);
-            if ((cx >> DW_OP2_SHIFT) == 2u) hotspot(((next & 0xFF00u) | (target & 0xFFu)) & 0x1FFFu);
+            dummy_rd(next, 0);                             // (cyc already counts the two base cycles: this is the third)
+            if ((cx >> DW_OP2_SHIFT) == 2u) dummy_rd((next & 0xFF00u) | (target & 0xFFu), 1);
             set_pc(target);
           } else di += pl;
           cyc += (int32_t)(cx >> DW_OP2_SHIFT);

@@ -159,6 +159,8 @@ def _chaos_rom(seed: int) -> bytes:
                 a.op("LDA", "abx", RIOT["INTIM"] - 0x20 + r.rnd(0x40)); a.op("INX")       # indexed: dummy/real reads around the RIOT
             else:
                 if r.chance(1, 3): a.op("PHA"); a.op("PLA")
+                elif r.chance(1, 4):                              # the stack on TIA registers: pushes are register writes, pulls read latches
+                    a.op("LDX", "imm", r.rnd(0x80)); a.op("TXS"); a.op(r.choice(["PHA", "PHP"])); a.op(r.choice(["PHA", "PLA", "PLP"])); a.op("LDX", "imm", 0xFF); a.op("TXS")
                 else: a.op(r.choice(["NOP", "INX", "DEY", "CLC", "SEC"]))
         a.op("JMP", "abs", "top")
     return hand_rom(build)
@@ -326,13 +328,13 @@ def _undoc_rom(seed: int) -> bytes:
                 if opc in (0xA7, 0xB7): a.byte(opc, 0x80 + r.rnd(0x60))
                 elif opc in (0xAF, 0xBF): t = r.choice([0xF900 + r.rnd(0x1F0), 0x0080 + r.rnd(0x60)]); a.byte(opc, t & 0xFF, t >> 8)
                 else:
-                    if opc == 0xA3: a.op("LDX", "imm", r.rnd(3) * 2)      # (zp,X): keep the pointer cells in RAM (status bit 2)
-                    a.byte(opc, r.choice([0x90, 0x92, 0x94]) if opc == 0xB3 else 0x90)
+                    if opc == 0xA3: a.op("LDX", "imm", r.rnd(256) if r.chance(1, 2) else r.rnd(3) * 2)     # (zp,X): the pointer cells may be anywhere in page 0
+                    a.byte(opc, r.choice([0x90, 0x92, 0x94, r.rnd(256)]) if opc == 0xB3 else 0x90)
             elif k < 11:
                 opc = r.choice([0x87, 0x97, 0x8F, 0x83])
                 if opc in (0x87, 0x97): a.byte(opc, r.choice([0x80 + r.rnd(0x60), TIA_W[r.choice(["COLUBK", "PF1", "GRP0", "COLUPF", "ENAM0"])]]))
                 elif opc == 0x8F: a.byte(opc, 0x80 + r.rnd(0x60), 0x00)
-                else: a.op("LDX", "imm", r.rnd(3) * 2); a.byte(opc, 0x90)                                        # (zp,X) -> pointer at $90/$92/$94
+                else: a.op("LDX", "imm", r.rnd(256) if r.chance(1, 2) else r.rnd(3) * 2); a.byte(opc, 0x90)      # (zp,X) -> pointer at $90/$92/$94 or anywhere
             elif k < 12:
                 if r.chance(1, 2): a.op("SED")
                 a.byte(0xEB, r.rnd(256)); a.op("CLD")
