@@ -166,7 +166,7 @@ inline void hot_class(uint32_t &x, uint32_t &y) {
 inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, int nb, DWord *out) {
   for (uint32_t off = 0; off < 4096; ++off) {
     const uint32_t lead = leader[off] ? DW_LEADER : 0u;
-    if (off >= DW_SLOW_LIMIT) { out[off].x = H_SLOW | lead; out[off].y = 0; continue; }
+    if (off >= DW_SLOW_LIMIT) { out[off].x = (HC_COLD + H_SLOW) | lead; out[off].y = 0; continue; }
     const uint32_t opc = img[off], b1 = img[off + 1], b2 = img[off + 2];
     const uint32_t ent = kOpTable[opc], mode = ent & 15u, op = (ent >> 4) & 63u, kind = ent >> 10;
     uint32_t x = generic_entry(opc);

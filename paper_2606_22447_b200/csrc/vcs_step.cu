@@ -52,10 +52,97 @@ constexpr uint32_t KEY_PARKED = 0xFFFE0000u;         // keys >= this: parked for
 constexpr uint32_t NOSLOT = 0xFFFFFFFFu;             // a thread of the spare warp that holds no environment right now
 constexpr int32_t LIM_WSYNC = LIM_NOW + 1;            // `lim` while WSYNC holds the CPU (and nothing else is pending)
 
+// ---- RIOT: interval timer in closed form and the two I/O ports (C.7).  All of its state lives in the thread's
+// shared-memory file, so these are plain static functions of the file slot.
+template <int BLOCK, int TAG = 0>
+struct Riot {
+  using T = Tia<BLOCK, TAG>;
+  static DEV uint32_t &S(uint32_t sl, int i) { return T::S(sl, i); }
+  // advance the (timer, sub, tflag) state in smem to "after `ticks` cycles of this step" and return it unpacked
+  static DEV void timer_sync(uint32_t sl, int32_t ticks, uint32_t &timer, uint32_t &sub, uint32_t &shift, uint32_t &tflag) {
+    const uint32_t tw = S(sl, S_TMR);
+    timer = tw & 0xFFu; shift = (tw >> 8) & 0xFu; tflag = (tw >> 12) & 1u; sub = tw >> 16;
+    const uint32_t d = (uint32_t)(ticks - (int32_t)S(sl, S_TTICKS));
+    if ((int32_t)d <= 0) return;
+    S(sl, S_TTICKS) = (uint32_t)ticks;
+    const uint32_t mask = (1u << shift) - 1u;
+    if (tflag) { timer = (timer - d) & 0xFFu; sub = (sub + d) & mask; return; }
+    const uint32_t k = (sub + d) >> shift;            // prescaler wraps (decrement events) in d ticks
+    if (k <= timer) { timer -= k; }
+    else {                                            // event number timer+1 is the underflow
+      const uint32_t iu = ((timer + 1u) << shift) - sub;    // tick index (1-based) of the underflow
+      timer = (0xFFu - (d - iu)) & 0xFFu; tflag = 1;
+    }
+    sub = (sub + d) & mask;
+  }
+  static DEV void timer_put(uint32_t sl, uint32_t timer, uint32_t sub, uint32_t shift, uint32_t tflag) { S(sl, S_TMR) = timer | (shift << 8) | (tflag << 12) | (sub << 16); }
+  // INTIM / TIMINT read in cycle index c (tick c happened first)
+  static DEV uint32_t timer_read(uint32_t sl, uint32_t a, int32_t c) {
+    const uint32_t tw = S(sl, S_TMR);
+    const uint32_t d = (uint32_t)(c + 1 - (int32_t)S(sl, S_TTICKS));
+    if (!(tw & 0x1000u) && (int32_t)d > 0) {          // before the underflow nothing has to be written back
+      const uint32_t timer = tw & 0xFFu, k = ((tw >> 16) + d) >> ((tw >> 8) & 0xFu);
+      if (k <= timer) return (a & 1u) ? 0u : timer - k;
+    }
+    uint32_t timer, sub, shift, tflag;
+    timer_sync(sl, c + 1, timer, sub, shift, tflag);
+    if (!(a & 1u)) { timer_put(sl, timer, sub, shift, 0); return timer; }     // INTIM clears the flag
+    timer_put(sl, timer, sub, shift, tflag);
+    return tflag << 7;                                                        // TIMINT
+  }
+  static DEV uint32_t read(uint32_t sl, uint32_t a, int32_t c) {     // access in cycle index c
+    if ((a & 4u) == 0) {
+      const uint32_t ports = S(sl, S_PORTS);
+      const uint32_t ora = byte_of(ports, 0), ddra = byte_of(ports, 1), orb = byte_of(ports, 2), ddrb = byte_of(ports, 3);
+      switch (a & 3u) {
+        case 0: return (ora & ddra) | (S(sl, S_INP) & ~ddra & 0xFFu);
+        case 1: return ddra;
+        case 2: { const uint32_t k = S(sl, S_INP) >> 9;    // console switches (vcs_set_switches), pins 2, 4, 5 not connected
+                  const uint32_t inb = 0x34u | (k & 3u) | ((k & 4u) << 1) | ((k & 0x18u) << 3);
+                  return (orb & ddrb) | (inb & ~ddrb); }
+        default: return ddrb;
+      }
+    }
+    return timer_read(sl, a, c);
+  }
+  static DEV void write(uint32_t sl, uint32_t a, uint32_t v, int32_t c) {
+    if ((a & 4u) == 0) { S(sl, S_PORTS) = set_byte(S(sl, S_PORTS), a & 3u, v); return; }
+    if ((a & 0x14u) == 0x14u) {
+      const uint32_t k = a & 3u;
+      const uint32_t shift = (k == 0) ? 0u : (k == 1) ? 3u : (k == 2) ? 6u : 10u;
+      timer_put(sl, v & 0xFFu, (1u << shift) - 1u, shift, 0); S(sl, S_TTICKS) = (uint32_t)(c + 1);
+    }
+  }
+};
+// Bus accesses that are neither RAM nor cartridge (a = addr & 0x1FFF without A12; c = cycle index in this step, m = cycle
+// in the scanline).  Inline: a call level more on the way to the TIA functions costs them convergence-barrier registers
+// (ptxas then saves / restores B registers with BMOV inside render_visible & co.: measured +20 % instructions there).
+template <int BLOCK, int TAG>
+DEV uint32_t io_read(uint32_t sl, uint32_t a, int32_t c, int m) {       // -> value | line ends performed << 12
+  if (a & 0x0080u) return Riot<BLOCK, TAG>::read(sl, a, c);
+  return Tia<BLOCK, TAG>::read(sl, a & 0xFu, m);
+}
+template <int BLOCK, int TAG>
+DEV uint32_t io_write(uint32_t sl, uint32_t a, uint32_t v, int32_t c, int m) {   // -> TIA events (EV_*)
+  if (a & 0x0080u) { Riot<BLOCK, TAG>::write(sl, a, v, c); return 0; }
+  const uint32_t r = a & 0x3Fu;
+  if (r > 0x2Cu || (r >= 0x15u && r <= 0x1Au) || r == 0x03u) return 0;      // no effect (audio: PAPER.md L205)
+  return Tia<BLOCK, TAG>::write(sl, r, v, m);
+}
+template <int BLOCK, int TAG>
+DEV void io_dummy_intim(uint32_t sl, int32_t ticks) {      // a discarded read of INTIM still clears the underflow flag
+  uint32_t t, s, sh, f; Riot<BLOCK, TAG>::timer_sync(sl, ticks, t, s, sh, f); Riot<BLOCK, TAG>::timer_put(sl, t, s, sh, 0);
+}
+
 // What the inline interpreter loop keeps in registers.  A, X, Y, SP are the four bytes of `axys`, so that "which
 // register" is a byte-permute selector from the decode entry; `fl` holds C, I, D, V at their P-register bits.
 // Everything else of an environment (status, frame start, TIA/RIOT latches, RAM) lives in its shared-memory file
 // and block-uniform values live in the block context; the out-of-line paths below rebuild a full Cpu from both.
+#ifndef VCS_COLD_TAG
+#define VCS_COLD_TAG 2
+#endif
+constexpr int COLD_TAG = VCS_COLD_TAG;               // the copy of the TIA code the compact out-of-line executor calls (vcs_tia.cuh)
+constexpr uint32_t AUX_GENERIC = 2u;                 // Hot::aux after cold_exec: run the entry (wx, wy) on cold_exec_generic
 struct Hot {
   uint32_t axys, fl, zn;               // Z <=> (zn & 0xFF) == 0 ; N <=> (zn & 0x180) != 0
   uint32_t di, pbase;                  // PC = (pbase + di) & 0xFFFF ; di = bank<<12 | PC & 0xFFF
@@ -65,9 +152,9 @@ struct Hot {
   uint32_t aux;                        // return flag of the out-of-line calls
 };
 
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT, int TAG = 0>      // TAG: which copy of the TIA code this Cpu calls (vcs_tia.cuh)
 struct Cpu {
-  using T = Tia<BLOCK>;
+  using T = Tia<BLOCK, TAG>;
   // ---- CPU
   uint32_t A, X, Y, SP;
   uint32_t di, pbase;                  // PC = (pbase + di) & 0xFFFF ; di = bank<<12 | PC & 0xFFF
@@ -170,67 +257,29 @@ struct Cpu {
     return __ldg(dr + di);
   }
 
-  // ------------------------------------------------------------------ RIOT timer, closed form (C.7)
-  // advance the (timer, sub, tflag) state in smem to "after `ticks` cycles of this step" and return it unpacked
-  DEV void timer_sync(int32_t ticks, uint32_t &timer, uint32_t &sub, uint32_t &shift, uint32_t &tflag) {
-    const uint32_t tw = S(S_TMR);
-    timer = tw & 0xFFu; shift = (tw >> 8) & 0xFu; tflag = (tw >> 12) & 1u; sub = tw >> 16;
-    const uint32_t d = (uint32_t)(ticks - (int32_t)S(S_TTICKS));
-    if ((int32_t)d <= 0) return;
-    S(S_TTICKS) = (uint32_t)ticks;
-    const uint32_t mask = (1u << shift) - 1u;
-    if (tflag) { timer = (timer - d) & 0xFFu; sub = (sub + d) & mask; return; }
-    const uint32_t k = (sub + d) >> shift;            // prescaler wraps (decrement events) in d ticks
-    if (k <= timer) { timer -= k; }
-    else {                                            // event number timer+1 is the underflow
-      const uint32_t iu = ((timer + 1u) << shift) - sub;    // tick index (1-based) of the underflow
-      timer = (0xFFu - (d - iu)) & 0xFFu; tflag = 1;
-    }
-    sub = (sub + d) & mask;
-  }
-  DEV void timer_put(uint32_t timer, uint32_t sub, uint32_t shift, uint32_t tflag) { S(S_TMR) = timer | (shift << 8) | (tflag << 12) | (sub << 16); }
-  // INTIM / TIMINT read in cycle index c (tick c happened first)
-  DEV uint32_t timer_read(uint32_t a, int32_t c) {
-    const uint32_t tw = S(S_TMR);
-    const uint32_t d = (uint32_t)(c + 1 - (int32_t)S(S_TTICKS));
-    if (!(tw & 0x1000u) && (int32_t)d > 0) {          // before the underflow nothing has to be written back
-      const uint32_t timer = tw & 0xFFu, k = ((tw >> 16) + d) >> ((tw >> 8) & 0xFu);
-      if (k <= timer) return (a & 1u) ? 0u : timer - k;
-    }
-    uint32_t timer, sub, shift, tflag;
-    timer_sync(c + 1, timer, sub, shift, tflag);
-    if (!(a & 1u)) { timer_put(timer, sub, shift, 0); return timer; }         // INTIM clears the flag
-    timer_put(timer, sub, shift, tflag);
-    return tflag << 7;                                                        // TIMINT
-  }
-  DEV uint32_t riot_read(uint32_t a, int32_t c) {     // access in cycle index c
-    if ((a & 4u) == 0) {
-      const uint32_t ports = S(S_PORTS);
-      const uint32_t ora = byte_of(ports, 0), ddra = byte_of(ports, 1), orb = byte_of(ports, 2), ddrb = byte_of(ports, 3);
-      switch (a & 3u) {
-        case 0: return (ora & ddra) | (S(S_INP) & ~ddra & 0xFFu);
-        case 1: return ddra;
-        case 2: { const uint32_t k = S(S_INP) >> 9;        // console switches (vcs_set_switches), pins 2, 4, 5 not connected
-                  const uint32_t inb = 0x34u | (k & 3u) | ((k & 4u) << 1) | ((k & 0x18u) << 3);
-                  return (orb & ddrb) | (inb & ~ddrb); }
-        default: return ddrb;
-      }
-    }
-    return timer_read(a, c);
-  }
-  DEV void riot_write(uint32_t a, uint32_t v, int32_t c) {
-    if ((a & 4u) == 0) { S(S_PORTS) = set_byte(S(S_PORTS), a & 3u, v); return; }
-    if ((a & 0x14u) == 0x14u) {
-      const uint32_t k = a & 3u;
-      const uint32_t shift = (k == 0) ? 0u : (k == 1) ? 3u : (k == 2) ? 6u : 10u;
-      timer_put(v & 0xFFu, (1u << shift) - 1u, shift, 0); S(S_TTICKS) = (uint32_t)(c + 1);
-    }
-  }
+  // ------------------------------------------------------------------ RIOT (struct Riot above)
+  using R = Riot<BLOCK, TAG>;
+  DEV void timer_sync(int32_t ticks, uint32_t &timer, uint32_t &sub, uint32_t &shift, uint32_t &tflag) { R::timer_sync(sl, ticks, timer, sub, shift, tflag); }
+  DEV uint32_t timer_read(uint32_t a, int32_t c) { return R::timer_read(sl, a, c); }
 
   // stack accesses (C.3: $0100 | SP decodes like any other address — RAM for SP >= $80, TIA registers below) k cycles
   // into the instruction
-  DEV void push(uint32_t v, int k) { bus_write(0x0100u | SP, v, k); SP = (SP - 1u) & 0xFFu; }
-  DEV uint32_t pull(int k) { SP = (SP + 1u) & 0xFFu; return bus_read(0x0100u | SP, k); }
+  // GEN = false is the compact form of the common case (the whole access stays in RAM; exec_one<false> bails out to
+  // exec_one<true> before it touches anything when that does not hold)
+  template <bool GEN> DEV void push(uint32_t v, int k) {
+    if constexpr (GEN) bus_write(0x0100u | SP, v, k); else ram_wr(SP, v);
+    SP = (SP - 1u) & 0xFFu;
+  }
+  template <bool GEN> DEV uint32_t pull(int k) {
+    SP = (SP + 1u) & 0xFFu;
+    if constexpr (GEN) return bus_read(0x0100u | SP, k); else return ram_rd(SP);
+  }
+  // pointer / vector / instruction bytes: cartridge or RAM in the compact form, anything in the generic one
+  template <bool GEN> DEV uint32_t rd8(uint32_t addr, int k, bool value = true) {
+    if constexpr (GEN) return bus_read(addr, k, value);
+    else { const uint32_t a = addr & 0x1FFFu; return (a & 0x1000u) ? rom_rd(a, value) : ram_rd(a, value); }
+  }
+  static DEV bool ram_or_rom(uint32_t addr) { return (addr & 0x1000u) || (addr & 0x0280u) == 0x0080u; }
   // a READ cycle k cycles into the instruction while WSYNC holds RDY (C.4: only read cycles are stalled, so the writes of
   // a JSR / BRK sequence run through a freshly set latch and the next read idles to the line end)
   DEV void rdy(int k) {
@@ -243,7 +292,7 @@ struct Cpu {
   DEV void dummy_rd(uint32_t addr, int k) {
     const uint32_t a = addr & 0x1FFFu;
     if (a & 0x1000u) hotspot(a);
-    else if ((a & 0x0285u) == 0x0284u) { uint32_t t, s, sh, f; timer_sync(cyc + k + 1, t, s, sh, f); timer_put(t, s, sh, 0); }
+    else if ((a & 0x0285u) == 0x0284u) io_dummy_intim<BLOCK, TAG>(sl, cyc + k + 1);
   }
   // lim from (lstart, fstart, wsync, status)
   DEV void relim() {
@@ -256,18 +305,12 @@ struct Cpu {
     if (ev & EV_FRAME) { fdone += 1; fstart = fc; rekey(); }
     relim();
   }
-  // generic handlers: a TIA write k cycles into the instruction (cyc = its first cycle)
-  DEV void tia_write(uint32_t r, uint32_t v, int k) {
-    const uint32_t ev = T::write(sl, r, v, cyc - lstart + k);
-    if (ev) tia_events(ev, cyc + k + 1);
-  }
   // the generic operand read (C.3 decode), k cycles into the instruction
   DEV uint32_t bus_read(uint32_t addr, int k, bool value = true) {     // value: the byte is used (soft reads skip discarded ones)
     const uint32_t a = addr & 0x1FFFu;
     if ((a & 0x1280u) == 0x0080u) return ram_rd(a, value);
     if (a & 0x1000u) return rom_rd(a, value);
-    if (a & 0x0080u) return riot_read(a, cyc + k);
-    const uint32_t r = T::read(sl, a & 0xFu, cyc - lstart + k);
+    const uint32_t r = io_read<BLOCK, TAG>(sl, a, cyc + k, cyc - lstart + k);
     if (r >> 12) { lstart += LINE_CYC * (int32_t)(r >> 12); wsync = false; relim(); }
     return r & 0xFFu;
   }
@@ -275,10 +318,8 @@ struct Cpu {
     const uint32_t a = addr & 0x1FFFu;
     if ((a & 0x1280u) == 0x0080u) { ram_wr(a, v); return; }
     if (a & 0x1000u) { hotspot(a); return; }
-    if (a & 0x0080u) { riot_write(a, v, cyc + k); return; }
-    const uint32_t r = a & 0x3Fu;
-    if (r > 0x2Cu || (r >= 0x15u && r <= 0x1Au) || r == 0x03u) return;      // no effect (audio: PAPER.md L205)
-    tia_write(r, v, k);
+    const uint32_t ev = io_write<BLOCK, TAG>(sl, a, v, cyc + k, cyc - lstart + k);
+    if (ev) tia_events(ev, cyc + k + 1);
   }
   // ---------------------------------------------------------------- SOFT-STE mode (include/vcs.h vcs_step_soft; eq. 8-10)
   DEV void soft_note(int k, float soft_v, float hard, float ste) {
@@ -401,7 +442,8 @@ struct Cpu {
       cyc = lstart + LINE_CYC; T::line_end(sl); lstart = cyc; wsync = false;
     }
     relim();
-    return cyc < lim;                                      // (the cap can fall on the line start reached by WSYNC)
+    return true;       // (when the cap falls on the line start reached by WSYNC the instruction still runs: the stall is part of
+                       //  its first read cycle, C.4, and the cap is looked at on instruction boundaries only, C.10)
   }
 
   // ---------------------------------------------------------------- block-wide regroup (F8 divergence)
@@ -486,7 +528,12 @@ struct Cpu {
   // ---------------------------------------------------------------- the out-of-line executor: ONE instruction
   // Runs the entry (cx, pl) in the vcs_decode.cuh Hid numbering; di and cyc have already been advanced by the
   // entry's length and base cycles.  Leaves w = the entry at the new (bank, PC): the caller re-schedules.
-  DEV void exec_one(uint32_t cx, uint32_t pl) {
+  // GEN = false: the compact executor for the common case — code in cartridge space, stack and pointer cells in RAM.
+  // It returns true, having changed nothing but this Cpu's registers, when the instruction needs an access outside that
+  // (stack on TIA registers, pointer / vector bytes or code in TIA / RIOT / RAM space): the caller then drops this Cpu
+  // and runs the instruction again on exec_one<true>, where every access goes through the generic bus code.
+  template <bool GEN>
+  DEV bool exec_one(uint32_t cx, uint32_t pl) {
     {
       bool slow = false;                                   // run-time decoded
       uint32_t ea = 0, v = 0, wv = 0, op2 = 0, hid;
@@ -499,14 +546,15 @@ struct Cpu {
           // the instruction bytes are ordinary bus reads in cycles 0, 1, 2 of the instruction (C.3 / C.5): cartridge,
           // RAM, TIA (collision latches) or RIOT (an INTIM read clears the underflow flag), whatever PC decodes to
           const uint32_t pc0 = pc();
-          const uint32_t opc = bus_read(pc0, 0);
+          if constexpr (!GEN) { if (((pc0 & 0x1000u) == 0) | (((pc0 + 2u) & 0x1000u) == 0)) return true; }
+          const uint32_t opc = rd8<GEN>(pc0, 0);
           uint32_t g = c_gen[opc];
           const uint32_t ln = (g >> DW_LEN_SHIFT) & 0xFFu, gh = g & 0x7Fu;
           uint32_t b1 = 0, b2 = 0;
           if (gh != H_ILL) {
             if (ln == 1 || gh == H_BRK) dummy_rd(pc0 + 1u, 1);             // "R dummy@PC" of the one-byte instructions and of BRK
-            else b1 = bus_read(pc0 + 1u, 1);
-            if (ln == 3 && gh != H_JSR) b2 = bus_read(pc0 + 2u, 2);        // (JSR reads its high byte after the pushes)
+            else b1 = rd8<GEN>(pc0 + 1u, 1);
+            if (ln == 3 && !(GEN && gh == H_JSR)) b2 = rd8<GEN>(pc0 + 2u, 2);   // (a generic JSR reads its high byte after the pushes)
           }
           pl = b1 | (b2 << 8);
           if ((g & 0x7Fu) >= H_BR0 && (g & 0x7Fu) < H_BR0 + 8) {
@@ -590,16 +638,20 @@ struct Cpu {
         case H_JMP: set_pc(pl); goto ctl;
         // (C.5 sequences; the dummy stack read of JSR / RTS / RTI / PLA / PLP lands in RAM or on a TIA read address: no effect)
         case H_JSR: { const uint32_t ret = (pc() - 1u) & 0xFFFFu;     // address of the 3rd byte
-          push(ret >> 8, kb + 3); push(ret & 0xFFu, kb + 4); rekey();
-          rdy(kb + 5);                                                        // R hi@PC comes after the pushes:
-          if (slow) pl |= bus_read(ret, kb + 5) << 8;                          // they may have set WSYNC, or rewritten that byte
+          if constexpr (!GEN) { if (SP < 0x81u) return true; }
+          push<GEN>(ret >> 8, kb + 3); push<GEN>(ret & 0xFFu, kb + 4); rekey();
+          if constexpr (GEN) {
+            rdy(kb + 5);                                                      // R hi@PC comes after the pushes:
+            if (slow) pl |= bus_read(ret, kb + 5) << 8;                        // they may have set WSYNC, or rewritten that byte
+          }
           set_pc(pl); } goto ctl;
-        case H_RTS: { const uint32_t lo = pull(kb + 3), hi = pull(kb + 4); const uint32_t r = lo | (hi << 8);
+        case H_RTS: { if constexpr (!GEN) { if (SP - 0x7Fu > 0xFDu - 0x7Fu) return true; }      // pulls from SP+1, SP+2
+          const uint32_t lo = pull<GEN>(kb + 3), hi = pull<GEN>(kb + 4); const uint32_t r = lo | (hi << 8);
           rekey(); dummy_rd(r, kb + 5); set_pc((r + 1u) & 0xFFFFu); } goto ctl;
-        case H_PHA: push(A, kb + 2); rekey(); break;
-        case H_PHP: push(pack_p() | 0x30u, kb + 2); rekey(); break;
-        case H_PLA: A = pull(kb + 3); zn = A; rekey(); break;
-        case H_PLP: unpack_p(pull(kb + 3)); rekey(); break;
+        case H_PHA: if constexpr (!GEN) { if (SP < 0x80u) return true; } push<GEN>(A, kb + 2); rekey(); break;
+        case H_PHP: if constexpr (!GEN) { if (SP < 0x80u) return true; } push<GEN>(pack_p() | 0x30u, kb + 2); rekey(); break;
+        case H_PLA: if constexpr (!GEN) { if (SP - 0x7Fu > 0xFEu - 0x7Fu) return true; } A = pull<GEN>(kb + 3); zn = A; rekey(); break;
+        case H_PLP: if constexpr (!GEN) { if (SP - 0x7Fu > 0xFEu - 0x7Fu) return true; } unpack_p(pull<GEN>(kb + 3)); rekey(); break;
         // ---- absolute read of INTIM / TIMINT (4th cycle)
         case H_RTIM: read_op(cx >> DW_OP2_SHIFT, timer_read(pl, cyc - 1)); break;
         // ---- generic addressing: reads (cyc = first cycle of the instruction; they add `total` themselves)
@@ -610,14 +662,16 @@ struct Cpu {
         case H_R0 + 4: ea = pl; k = 3; goto do_read;
         case H_R0 + 5: case H_R0 + 6: case H_R0 + 8: {
           uint32_t lo, hi;
-          if (hid == H_R0 + 8) { lo = bus_read(pl & 0xFFu, 2); hi = bus_read((pl + 1u) & 0xFFu, 3); k = 4; }
+          if (hid == H_R0 + 8) { if constexpr (!GEN) { if ((pl & 0xFFu) - 0x80u > 0x7Eu) return true; }       // pointer cells pl, pl+1 in RAM
+                                 lo = rd8<GEN>(pl & 0xFFu, 2); hi = rd8<GEN>((pl + 1u) & 0xFFu, 3); k = 4; }
           else { lo = pl & 0xFFu; hi = pl >> 8; k = 3; }
           const uint32_t t = lo + ((hid == H_R0 + 5) ? X : Y);
           const uint32_t unc = (hi << 8) | (t & 0xFFu);
           ea = (unc + (t & 0x100u)) & 0xFFFFu;
           if (t & 0x100u) { dummy_rd(unc, k); k += 1; }
         } goto do_read;
-        case H_R0 + 7: { const uint32_t z = (pl + X) & 0xFFu; ea = bus_read(z, 3); ea |= bus_read((z + 1u) & 0xFFu, 4) << 8; k = 5; } goto do_read;
+        case H_R0 + 7: { const uint32_t z = (pl + X) & 0xFFu; if constexpr (!GEN) { if (z - 0x80u > 0x7Eu) return true; }
+          ea = rd8<GEN>(z, 3); ea |= rd8<GEN>((z + 1u) & 0xFFu, 4) << 8; k = 5; } goto do_read;
         // ---- generic addressing: stores
         case H_W0 + 0: ea = pl & 0xFFu; k = 2; goto do_write;
         case H_W0 + 1: ea = (pl + X) & 0xFFu; k = 3; goto do_write;
@@ -625,14 +679,16 @@ struct Cpu {
         case H_W0 + 3: ea = pl; k = 3; goto do_write;
         case H_W0 + 4: case H_W0 + 5: case H_W0 + 7: {
           uint32_t lo, hi;
-          if (hid == H_W0 + 7) { lo = bus_read(pl & 0xFFu, 2); hi = bus_read((pl + 1u) & 0xFFu, 3); k = 4; }
+          if (hid == H_W0 + 7) { if constexpr (!GEN) { if ((pl & 0xFFu) - 0x80u > 0x7Eu) return true; }
+                                 lo = rd8<GEN>(pl & 0xFFu, 2); hi = rd8<GEN>((pl + 1u) & 0xFFu, 3); k = 4; }
           else { lo = pl & 0xFFu; hi = pl >> 8; k = 3; }
           const uint32_t t = lo + ((hid == H_W0 + 4) ? X : Y);
           const uint32_t unc = (hi << 8) | (t & 0xFFu);
           ea = (unc + (t & 0x100u)) & 0xFFFFu;
           dummy_rd(unc, k); k += 1;
         } goto do_write;
-        case H_W0 + 6: { const uint32_t z = (pl + X) & 0xFFu; ea = bus_read(z, 3); ea |= bus_read((z + 1u) & 0xFFu, 4) << 8; k = 5; } goto do_write;
+        case H_W0 + 6: { const uint32_t z = (pl + X) & 0xFFu; if constexpr (!GEN) { if (z - 0x80u > 0x7Eu) return true; }
+          ea = rd8<GEN>(z, 3); ea |= rd8<GEN>((z + 1u) & 0xFFu, 4) << 8; k = 5; } goto do_write;
         // ---- generic addressing: read-modify-write
         case H_M0 + 0: ea = pl & 0xFFu; k = 2; goto do_rmw;
         case H_M0 + 1: ea = (pl + X) & 0xFFu; k = 3; goto do_rmw;
@@ -640,13 +696,17 @@ struct Cpu {
         case H_M0 + 3: { const uint32_t t = (pl & 0xFFu) + X; const uint32_t unc = (pl & 0xFF00u) | (t & 0xFFu);
           ea = (unc + (t & 0x100u)) & 0xFFFFu; dummy_rd(unc, 3); k = 4; } goto do_rmw;
         // ---- rare
-        case H_JMPI: { const uint32_t l2 = bus_read(pl, kb + 3), h2 = bus_read((pl & 0xFF00u) | ((pl + 1u) & 0xFFu), kb + 4);   // no carry into the page
+        case H_JMPI: { const uint32_t p2 = (pl & 0xFF00u) | ((pl + 1u) & 0xFFu);                  // no carry into the page
+          if constexpr (!GEN) { if (!ram_or_rom(pl) || !ram_or_rom(p2)) return true; }
+          const uint32_t l2 = rd8<GEN>(pl, kb + 3), h2 = rd8<GEN>(p2, kb + 4);
           set_pc(l2 | (h2 << 8)); } goto ctl;
-        case H_RTI: { unpack_p(pull(kb + 3)); const uint32_t lo = pull(kb + 4), hi = pull(kb + 5); rekey(); set_pc(lo | (hi << 8)); } goto ctl;
+        case H_RTI: { if constexpr (!GEN) { if (SP - 0x7Fu > 0xFCu - 0x7Fu) return true; }       // pulls from SP+1 .. SP+3
+          unpack_p(pull<GEN>(kb + 3)); const uint32_t lo = pull<GEN>(kb + 4), hi = pull<GEN>(kb + 5); rekey(); set_pc(lo | (hi << 8)); } goto ctl;
         case H_BRK: { const uint32_t ret = pc();             // address of the opcode + 2
-          push(ret >> 8, kb + 2); push(ret & 0xFFu, kb + 3); push(pack_p() | 0x30u, kb + 4); rekey();
-          rdy(kb + 5);
-          const uint32_t l2 = bus_read(0xFFFEu, kb + 5), h2 = bus_read(0xFFFFu, kb + 6);
+          if constexpr (!GEN) { if (SP < 0x82u) return true; }
+          push<GEN>(ret >> 8, kb + 2); push<GEN>(ret & 0xFFu, kb + 3); push<GEN>(pack_p() | 0x30u, kb + 4); rekey();
+          if constexpr (GEN) rdy(kb + 5);
+          const uint32_t l2 = rom_rd(0x1FFEu), h2 = rom_rd(0x1FFFu);          // ($FFFE / $FFFF: always the cartridge)
           set_pc(l2 | (h2 << 8)); fDI |= 4u; } goto ctl;
         default:                                           // H_ILL — C.12: halt for good, PC stays
           status |= STATUS_ILLEGAL;
@@ -689,6 +749,7 @@ struct Cpu {
     ctl:                                                   // every path ends here: refetch at the new (bank, PC)
       park &= ~4u;
       w = fetch();
+      return false;
   }
 };
 
@@ -769,9 +830,19 @@ DEV uint32_t rmw(Hot &h, uint32_t o, uint32_t s) {
 // back: the struct copy through the stack is only paid on these (rare) calls, and the instruction cache keeps the
 // inline loop below to itself.
 template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
+__device__ __noinline__ Hot cold_exec_generic(Hot h, uint32_t sl, uint32_t cx, uint32_t pl) {   // one instruction, any bus pattern
+  Cpu<BLOCK, ROMS, THREADS, SOFT, SOFT ? 0 : 1> c; c.load(h, sl);     // (its own copy of the TIA code: see vcs_tia.cuh, TAG)
+  c.template exec_one<true>((cx & 0xFFFFFF80u) | ((cx & 0x7Fu) - HC_COLD), pl);
+  return c.store();
+}
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 __device__ __noinline__ Hot cold_exec(Hot h, uint32_t sl, uint32_t cx, uint32_t pl) {       // one instruction
-  Cpu<BLOCK, ROMS, THREADS, SOFT> c; c.load(h, sl);
-  c.exec_one((cx & 0xFFFFFF80u) | ((cx & 0x7Fu) - HC_COLD), pl);
+  if constexpr (SOFT) return cold_exec_generic<BLOCK, ROMS, THREADS, SOFT>(h, sl, cx, pl);   // (soft reads are counted: no second try)
+  Cpu<BLOCK, ROMS, THREADS, SOFT, COLD_TAG> c; c.load(h, sl);
+  // a bus pattern outside the compact executor's: nothing of `c` is stored; the kernel's scheduling loop runs the
+  // instruction again on cold_exec_generic (from there, not from here: the generic code calls into the TIA too, and the
+  // TIA functions pay for every call level above them)
+  if (c.template exec_one<false>((cx & 0xFFFFFF80u) | ((cx & 0x7Fu) - HC_COLD), pl)) { h.aux = AUX_GENERIC; return h; }
   return c.store();
 }
 template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
@@ -791,12 +862,7 @@ __device__ __noinline__ Hot cold_events(Hot h, uint32_t sl, uint32_t ev) {      
 }
 template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 __device__ __noinline__ uint32_t cold_timer_read(uint32_t sl, uint32_t a, int32_t c) {       // INTIM / TIMINT around the underflow
-  Cpu<BLOCK, ROMS, THREADS, SOFT> cp; cp.sl = sl; cp.sl4 = 4u * sl;
-  uint32_t timer, sub, shift, tflag;
-  cp.timer_sync(c + 1, timer, sub, shift, tflag);
-  if (!(a & 1u)) { cp.timer_put(timer, sub, shift, 0); return timer; }
-  cp.timer_put(timer, sub, shift, tflag);
-  return tflag << 7;
+  return Riot<BLOCK, 0>::timer_read(sl, a, c);
 }
 
 // WSYNC released at the end of the line (a12), the common way a line ends: returns the new `lim`, or LIM_NOW when
@@ -1057,6 +1123,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
       const uint32_t mk = __reduce_min_sync(0xFFFFFFFFu, key);
       if (mk >= KEY_PARKED) break;                         // every lane is parked or has finished the step
       if (key == mk) run_block<BLOCK, ROMS, THREADS, SOFT>(h, dr, cur);
+      if (h.aux == AUX_GENERIC) h = cold_exec_generic<BLOCK, ROMS, THREADS, SOFT>(h, cur, h.wx, h.wy);   // (a rare bus pattern: see cold_exec)
     }
     if (!regroups) break;
     if (!__syncthreads_or(h.keyhi == KEY_PARKED)) break;   // nobody left to run in this block

@@ -86,7 +86,11 @@ inline void tia_desc_table(uint32_t *t) {
 }
 __constant__ uint32_t c_tia_desc[64];
 
-template <int BLOCK>
+// TAG tells copies of this code apart: the kernel's inline interpreter loop uses TAG 0, the out-of-line executors their
+// own (vcs_step.cu).  Same source, same results — but ptxas hands out convergence-barrier registers over the whole call
+// graph, and a hot function that is also reachable from a deeply nested rare path pays for it on every call (BMOV
+// saves / restores inside render_visible & co.); with a copy per caller the hot copy is compiled for the hot path alone.
+template <int BLOCK, int TAG = 0>
 struct Tia {
   static DEV uint32_t &S(uint32_t sl, int i) { return smem[i * BLOCK + sl]; }
   static DEV uint32_t ctx(int i) { return smem[S_WORDS * BLOCK + i]; }

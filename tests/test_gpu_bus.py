@@ -172,6 +172,39 @@ def test_code_running_from_ram_tia_and_riot_space(torch):
     _run(torch, bytes(rom), 36, 10, seed=41, max_lines=130)
 
 
+def test_code_in_the_last_16_bytes_of_a_bank_and_opcode_fetches_on_f8_hotspots(torch):
+    """The CPU runs through $FFF0-$FFFB: the opcode fetch at $FFF8 selects bank 0 (and returns ITS byte), the dummy read
+    of that one-byte instruction at $FFF9 selects bank 1 again, the fetch at $FFF9 executes bank 1's byte; the JMP at
+    $FFFA takes its high byte from the reset vector ($00) and lands in a RAM stub."""
+    def build(a):
+        a.org(0xF000); a.op("SEI"); a.op("CLD"); a.op("LDX", "imm", 0xFF); a.op("TXS")
+        for i, b in enumerate((0x4C, 0x00, 0xF1)): a.op("LDA", "imm", b); a.op("STA", "zp", 0x80 + i)    # RAM stub: JMP $F100
+        def body(a):
+            a.op("INC", "zp", 0x90); a.op("LDY", "zp", 0x90); a.op("JMP", "abs", 0xFFF0)
+            a.label("after")
+        _frame(a, body)
+        a.org(0xF100); a.op("STX", "zp", 0x91); a.op("STY", "zp", 0x92); a.op("JMP", "abs", "after")
+        a.org(0xFFF0)
+        for _ in range(6): a.op("NOP")
+        a.op("LDX", "imm", 0x11)                                                                         # $FFF6
+        a.byte(0xCA, 0xC8)                                                                               # $FFF8 DEX, $FFF9 INY (bank 1's bytes)
+        a.byte(0x4C, 0x80)                                                                               # $FFFA JMP $0080 (high byte = $FFFC = $00)
+    b1 = bytearray(hand_rom(build)); b0 = bytearray(b1)
+    b0[0xFF8] = 0xE8; b0[0xFF9] = 0x88                                                                   # bank 0: INX, DEY
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    roms = [bytes(b0 + b1), bytes(b1)]                                                                   # the F8 cart and the same code as a plain 4K cart
+    seeds = env_seeds(77, 64); env_rom = (np.arange(64) % 2).astype(np.int32)
+    g, o = VCS(roms, seeds, env_rom, max_lines=120), OracleVCS(roms, seeds, env_rom, max_lines=120)
+    for t in range(5):
+        a = np.zeros(64, np.uint8)
+        g.step(torch.from_numpy(a).cuda(), 2); o.step(a, 2, threads=NCPU)
+        _compare(g, o, f"bank end step {t}")
+    ram = g.ram_host()
+    assert (ram[0::2, 0x11] == 0x12).all() and (ram[1::2, 0x11] == 0x10).all()                          # F8: INX from bank 0; 4K: DEX
+    assert not (g.regs_host()["status"] & 1).any()
+
+
 def _soup_rom(seed: int) -> bytes:
     """Random instruction soup with the stack pointer, the pointer cells and the jump vectors anywhere: TXS with random X,
     pushes / pulls / JSR / RTS / BRK at any SP, every indirect mode with any zero-page cell, JMP () through any page,
