@@ -12,8 +12,15 @@
  *   - "host" pointers are ordinary CPU memory, "device" pointers are CUDA device memory of the GPU that
  *     was current when vcs_create ran.  No torch types cross this boundary.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  vcs_reset,
- *     vcs_step and vcs_get_* only enqueue work on that stream and return; ordering is stream ordering.
- *     vcs_create / vcs_destroy synchronise the device.
+ *     vcs_step* and vcs_get_* only enqueue work on that stream and return; ordering is stream ordering.
+ *     The only calls that wait for the GPU are vcs_create / vcs_destroy (whole device), the *_host conveniences
+ *     (their own copies), vcs_block_times, vcs_issue_peak, and vcs_step_soft when the temperature CHANGES (it waits
+ *     for its own previous upload of the weight table from the handle's pinned buffer, long since finished).
+ *   - One stream per handle: all calls on a handle must be issued on one stream, or be ordered by the caller (events)
+ *     as if they were.  The library keeps per-handle device state between calls (environment state, the block
+ *     placement of the next step, the soft-mode tables) and orders its own work by that stream alone.
+ *   - One device per handle: the CUDA device that was current in vcs_create must be current in every later call on
+ *     that handle (VCS_EINVAL otherwise; vcs_destroy switches to it itself).
  *   - The library owns all per-environment state and the front screen buffer.  The caller owns the
  *     action buffer and every output buffer.  roms / env_rom / seeds are copied by vcs_create.
  *   - There is no CPU fallback: without a CUDA device vcs_create returns VCS_ECUDA.
@@ -36,11 +43,26 @@ enum { VCS_OK = 0, VCS_EINVAL = -1, VCS_ECUDA = -2, VCS_ENOMEM = -3, VCS_EROM = 
  * that holds one does not stage ROMs in shared memory and does not regroup F8 blocks: slower, same results). */
 typedef struct { const uint8_t *data; uint32_t size; } vcs_rom;
 
-/* y0: scanline shown as screen row 0 (default 34, must be >= 2);  max_lines: frame cap in scanlines
- * (default 320) — a frame that has not ended by a VSYNC 1->0 write after max_lines*76 CPU cycles is
- * ended at the next instruction boundary;  f8_start_bank: bank selected at reset for
- * 8 KB images (default 1);  flags: reserved, must be 0. */
+/* y0: scanline shown as screen row 0 (default 34);  max_lines: frame cap in scanlines (default 320, 1..65535) — a
+ * frame that has not ended by a VSYNC 1->0 write after max_lines*76 CPU cycles is ended at the next instruction
+ * boundary;  f8_start_bank: bank selected at reset for 8 KB images (default 1);  flags: VCS_F_* below.
+ * y0 must be >= 2.  Why: the scanline in progress when a frame ends becomes line 0 of the next frame (C.10), and a
+ * step returns right after the instruction that ended its last frame — so the pixels of line 0 (and the first cycles
+ * of line 1, when that instruction runs over the line end) are drawn before the call that will finish THEIR frame has
+ * begun.  The kernel keeps no back buffer between calls (rows go straight to the front screen in the call that
+ * completes the frame), so those two lines are never shown; every console kernel spends them in VSYNC anyway. */
 typedef struct { int32_t y0, max_lines, f8_start_bank; uint32_t flags; } vcs_config;
+/* vcs_config.flags — launch-shape and decode switches.  PERFORMANCE ONLY: a handle computes the same bytes with any
+ * combination (tests/test_gpu_flags.py steps every one of them against the default).  0 = the library's own choice. */
+enum {
+  VCS_F_NO_SPIN    = 1u << 0,   /* run timer wait loops poll by poll instead of in closed form                 */
+  VCS_F_NO_FUSE    = 1u << 1,   /* no fused "LDx #imm ; STx <TIA register>" decode entries                     */
+  VCS_F_NO_REGROUP = 1u << 2,   /* F8 blocks do not re-sort their envs by bank at hotspot accesses             */
+  VCS_F_ROM_GLOBAL = 1u << 3,   /* cartridge bytes through the read-only cache instead of shared memory        */
+  VCS_F_NO_BALANCE = 1u << 4,   /* blocks run env groups in env order (no measured placement)    */
+  VCS_F_BLOCK_64   = 1u << 8, VCS_F_BLOCK_128 = 2u << 8, VCS_F_BLOCK_256 = 3u << 8, VCS_F_BLOCK_MASK = 3u << 8,  /* envs per block */
+  VCS_F_ALL = 0x31Fu
+};
 
 /* 32 bytes per environment, little-endian. */
 typedef struct {
@@ -59,9 +81,9 @@ typedef struct {
  * On return every env is in its reset state (C.2) and the screens are zero.
  * Layout hint (performance only, never results): when every aligned group of 256 (batches >= 32768), 128 or 64
  * consecutive envs shares one ROM, the ROM is staged in shared memory per block and F8 carts regroup their envs by
- * bank inside the block; otherwise ROM bytes come through the read-only cache.  Tuning overrides read here from
- * the environment: VCS_BLOCK=64|128|256, VCS_ROM_GLOBAL, VCS_NO_REGROUP, VCS_NO_SPIN, VCS_NO_FUSE, VCS_NO_BALANCE, VCS_BALANCE_A=<1..2>.
- * Errors: VCS_EINVAL (NULL/size/range), VCS_EROM (size not 2048/4096/8192/16384/32768), VCS_ECUDA, VCS_ENOMEM. */
+ * bank inside the block; otherwise ROM bytes come through the read-only cache.  cfg->flags (VCS_F_*) overrides these
+ * choices; the library reads nothing from the process environment.
+ * Errors: VCS_EINVAL (NULL/size/range/unknown flag), VCS_EROM (size not 2048/4096/8192/16384/32768), VCS_ECUDA, VCS_ENOMEM. */
 int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms,
                const int32_t *env_rom, const uint64_t *seeds, const vcs_config *cfg);
 
@@ -144,7 +166,8 @@ int vcs_screen_ptr(vcs_t h, const uint8_t **out_dev_ptr);
 
 /* Block placement introspection (performance only).  A step runs ceil(batch / block) thread blocks, all resident at
  * once; the library records when and on which SM each block of the last plain vcs_step ran and re-assigns env groups
- * to block indices so that the SMs finish together (VCS_NO_BALANCE in the environment turns it off).
+ * to block indices so that the SMs finish together (VCS_F_NO_BALANCE turns it off; handles with more
+ * than 1024 blocks — batches above 262,144 — keep env order).
  * *n_out = number of blocks; if cap >= n: times_host[3 * b + 0..2] = start ns, end ns (GPU global timer), SM id of
  * block index b in the last plain vcs_step, perm_host[b] = the env group (envs perm*block .. +block-1) block b runs
  * next.  Either pointer may be NULL.  Synchronises the device. */

@@ -56,11 +56,14 @@ class AleVecEnv:
         game logic) and those that hit max_episode_steps.  Returns the uint8[batch] mask of the envs that were re-booted
         (their observation is the first one of the new episode)."""
         t = self.torch
+        # an env that is still running its (amortised) boot ignores the agent in this step: the step does not count
+        # towards its episode, and a `done` the caller computed from its RAM meanwhile does not re-arm it
+        playing = (self.vcs.get_booting() == 0) if self.amortised else None
         self.vcs.step(actions, self.frameskip)
-        self.episode_steps += 1
+        self.episode_steps += 1 if playing is None else playing.to(self.episode_steps.dtype)
         over = None
         if done is not None:
-            over = done != 0
+            over = (done != 0) if playing is None else ((done != 0) & playing)
         if self.max_episode_steps is not None:
             trunc = self.episode_steps >= int(self.max_episode_steps)
             over = trunc if over is None else (over | trunc)

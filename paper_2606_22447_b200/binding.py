@@ -15,6 +15,9 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_PKG, "libvcsb200.so")
 
 VCS_OK, VCS_EINVAL, VCS_ECUDA, VCS_ENOMEM, VCS_EROM = 0, -1, -2, -3, -4
+# vcs_config.flags (include/vcs.h): performance only, never results
+VCS_F_NO_SPIN, VCS_F_NO_FUSE, VCS_F_NO_REGROUP, VCS_F_ROM_GLOBAL, VCS_F_NO_BALANCE = 1, 2, 4, 8, 16
+VCS_F_BLOCK_64, VCS_F_BLOCK_128, VCS_F_BLOCK_256 = 1 << 8, 2 << 8, 3 << 8
 _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
 
 EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
@@ -100,7 +103,7 @@ def _stream_ptr(stream) -> int | None:
 class VCS:
     """A batch of consoles on the current CUDA device (vcs_create ... vcs_destroy)."""
 
-    def __init__(self, roms, seeds, env_rom=None, y0=34, max_lines=320, f8_start_bank=1):
+    def __init__(self, roms, seeds, env_rom=None, y0=34, max_lines=320, f8_start_bank=1, flags=0):
         import torch
         if not torch.cuda.is_available():
             raise VcsError("no CUDA device: libvcsb200 has no CPU fallback")
@@ -113,7 +116,7 @@ class VCS:
         for i, b in enumerate(bufs):
             arr[i].data = C.cast(b, C.POINTER(C.c_uint8)); arr[i].size = len(b)
         er = None if env_rom is None else np.ascontiguousarray(env_rom, dtype=np.int32)
-        cfg = VcsConfig(y0, max_lines, f8_start_bank, 0)
+        cfg = VcsConfig(y0, max_lines, f8_start_bank, int(flags))
         self.h = C.c_void_p()
         rc = L.vcs_create(C.byref(self.h), self.batch, arr, len(roms), None if er is None else er.ctypes.data,
                           seeds.ctypes.data, C.byref(cfg))

@@ -26,6 +26,13 @@ int fail(Handle *h, int code, const char *what, cudaError_t ce = cudaSuccess) {
   return code;
 }
 #define CU(h, call) do { cudaError_t ce_ = (call); if (ce_ != cudaSuccess) return fail(h, VCS_ECUDA, #call, ce_); } while (0)
+// every entry point that touches device memory: the handle's GPU must be the current one (its pointers belong to it)
+int wrong_device(Handle *h) {
+  int d = -1;
+  if (cudaGetDevice(&d) != cudaSuccess || d != h->device) return fail(h, VCS_EINVAL, "the handle was created on another CUDA device than the current one");
+  return VCS_OK;
+}
+#define DEV_OK(h) do { if (!(h)) return VCS_EINVAL; if (int rc_ = wrong_device(h)) return rc_; } while (0)
 
 __device__ unsigned long long splitmix64(unsigned long long &s) {
   s += 0x9E3779B97F4A7C15ull;
@@ -148,13 +155,14 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   if (env_rom) for (int i = 0; i < batch; ++i) if (env_rom[i] < 0 || env_rom[i] >= n_roms) return VCS_EINVAL;
   vcs_config c = {34, 320, 1, 0};
   if (cfg) c = *cfg;
-  if (c.y0 < 2 || c.max_lines < 1 || c.max_lines > 65535 || c.flags != 0) return VCS_EINVAL;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return VCS_ECUDA;     // no CPU fallback
+  if (c.y0 < 2 || c.max_lines < 1 || c.max_lines > 65535 || (c.flags & ~(uint32_t)VCS_F_ALL) != 0) return VCS_EINVAL;
+  const uint32_t fblock = c.flags & VCS_F_BLOCK_MASK;
+  int ndev = 0, dev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || cudaGetDevice(&dev) != cudaSuccess) return VCS_ECUDA;     // no CPU fallback
   vcs_s *h = new (std::nothrow) vcs_s();
   if (!h) return VCS_ENOMEM;
   memset(static_cast<Handle *>(h), 0, sizeof(Handle));
-  h->batch = batch; h->n_roms = n_roms; h->y0 = c.y0; h->max_lines = c.max_lines; h->f8_start_bank = c.f8_start_bank;
+  h->batch = batch; h->n_roms = n_roms; h->y0 = c.y0; h->max_lines = c.max_lines; h->f8_start_bank = c.f8_start_bank; h->device = dev;
   *out = h;                                           // so that the caller can read vcs_last_error and destroy
 
   std::vector<RomMeta> meta(n_roms);
@@ -167,17 +175,17 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   for (int r = 0; r < n_roms; ++r) memcpy(hb.data() + meta[r].offset, roms[r].data, roms[r].size);
   std::vector<int32_t> er(batch, 0);
   if (env_rom) memcpy(er.data(), env_rom, sizeof(int32_t) * batch);
-  // launch shape: envs per block (VCS_BLOCK=64|128|256 overrides), and whether every block maps to one ROM so
+  // launch shape: envs per block (cfg.flags VCS_F_BLOCK_* overrides), and whether every block maps to one ROM so
   // that the ROM can be staged in shared memory (otherwise the kernel reads it through the read-only path)
   int want = (batch >= 32768) ? 256 : 128;           // big batches: 256 envs per block (measured 8 % faster on config 4: fewer, larger regroup domains)
-  if (const char *ev = getenv("VCS_BLOCK")) { const int v = atoi(ev); if (v == 64 || v == 128 || v == 256) want = v; }
+  if (fblock) want = (fblock == VCS_F_BLOCK_64) ? 64 : (fblock == VCS_F_BLOCK_128) ? 128 : 256;
   h->max_rom = 0;
   for (int r = 0; r < n_roms; ++r) if (roms[r].size > h->max_rom) h->max_rom = roms[r].size;
   auto uniform = [&](int blk) { for (int i = 0; i < batch; ++i) if (er[i] != er[i - i % blk]) return false; return true; };
   h->block = want; h->rom_smem = 0;
   for (int blk = want; blk >= 64; blk >>= 1) if (uniform(blk)) { h->block = blk; h->rom_smem = 1; break; }
-  if (getenv("VCS_ROM_GLOBAL") || h->max_rom > 8192) h->rom_smem = 0;     // F6 / F4 images stay in global memory (read-only path)
-  h->regroup = getenv("VCS_NO_REGROUP") ? 0 : 1;
+  if ((c.flags & VCS_F_ROM_GLOBAL) || h->max_rom > 8192) h->rom_smem = 0;     // F6 / F4 images stay in global memory (read-only path)
+  h->regroup = (c.flags & VCS_F_NO_REGROUP) ? 0 : 1;
   // pre-decode every byte offset of every bank once (vcs_decode.cuh); the words depend on the launch shape
   // (zero-page RAM operands are stored as shared-memory offsets)
   std::vector<DWord> dw(dwords + 8, DWord{0, 0});
@@ -192,8 +200,8 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
           else memcpy(img.data(), roms[r].data + 4096 * b, 4096);
           if (pass == 0) mark_leaders(img.data(), leader.data());
           else { decode_bank(img.data(), leader.data(), h->block, nb, dw.data() + meta[r].doff + 4096 * b);
-                 if (!getenv("VCS_NO_SPIN")) mark_spins(img.data(), dw.data() + meta[r].doff + 4096 * b);
-                 if (!getenv("VCS_NO_FUSE")) fuse_ld_st(dw.data() + meta[r].doff + 4096 * b); }
+                 if (!(c.flags & VCS_F_NO_SPIN)) mark_spins(img.data(), dw.data() + meta[r].doff + 4096 * b);
+                 if (!(c.flags & VCS_F_NO_FUSE)) fuse_ld_st(dw.data() + meta[r].doff + 4096 * b); }
         }
     }
   }
@@ -226,11 +234,10 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
     CU(h, cudaMemset(h->d_blk_time, 0, sizeof(unsigned long long) * 3 * nblk));
     CU(h, cudaMalloc((void **)&h->d_w_avg, sizeof(float) * nblk));
     CU(h, cudaMemset(h->d_w_avg, 0, sizeof(float) * nblk));
-    h->balance = getenv("VCS_NO_BALANCE") ? 0 : 1; h->plain_steps = 0;
+    h->balance = (c.flags & VCS_F_NO_BALANCE) ? 0 : 1; h->plain_steps = 0;
     h->balance_a = 1.27f;                             // measured slowdown of a block that shares its SM
-    if (const char *ev = getenv("VCS_BALANCE_A")) { const float v = (float)atof(ev); if (v >= 1.f && v <= 2.f) h->balance_a = v; }
   }
-  if (!getenv("VCS_NO_SOFT_ALLOC")) {                                                   // soft mode: every entry decodes at run time (vcs_step_soft)
+  {                                                                                     // soft mode: every entry decodes at run time (vcs_step_soft)
     std::vector<DWord> sl((h->max_rom < 8192 ? 8192 : h->max_rom) + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});
     std::vector<RomMeta> ms(meta); for (auto &m : ms) { m.pad = m.doff; m.doff = 0; }     // pad: offset into the W(T) x ROM table
     h->soft_tab_n = dwords; h->soft_tab_T = -1.f;
@@ -240,6 +247,8 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
     CU(h, cudaMalloc((void **)&h->d_rom_meta_soft, sizeof(RomMeta) * n_roms));
     CU(h, cudaMemcpy(h->d_rom_meta_soft, ms.data(), sizeof(RomMeta) * n_roms, cudaMemcpyHostToDevice));
     CU(h, cudaMalloc((void **)&h->d_soft_w, sizeof(float) * 1024));
+    CU(h, cudaMallocHost((void **)&h->h_soft_w, sizeof(float) * 1024));
+    CU(h, cudaEventCreateWithFlags(&h->soft_w_done, cudaEventDisableTiming));
   }
   upload_optable();
   CU(h, cudaGetLastError());
@@ -250,7 +259,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
 }
 
 int vcs_reset(vcs_t h, const uint8_t *mask_dev, void *cuda_stream) {
-  if (!h) return VCS_EINVAL;
+  DEV_OK(h);
   cudaStream_t s = (cudaStream_t)cuda_stream;
   StepParams p = params_of(h, nullptr, 1);
   reset_kernel<<<(h->batch + 127) / 128, 128, 0, s>>>(p, h->d_seeds, mask_dev, h->f8_start_bank);
@@ -261,7 +270,7 @@ int vcs_reset(vcs_t h, const uint8_t *mask_dev, void *cuda_stream) {
 }
 
 int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_stream) {
-  if (!h) return VCS_EINVAL;
+  DEV_OK(h);
   if (!actions_dev) return fail(h, VCS_EINVAL, "vcs_step: actions_dev is NULL");
   if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31))
     return fail(h, VCS_EINVAL, "vcs_step: frameskip out of range");
@@ -282,7 +291,7 @@ int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_
 }
 
 int vcs_step_masked(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, const uint8_t *mask_dev, void *cuda_stream) {
-  if (!h) return VCS_EINVAL;
+  DEV_OK(h);
   if (!actions_dev) return fail(h, VCS_EINVAL, "vcs_step_masked: actions_dev is NULL");
   if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31))
     return fail(h, VCS_EINVAL, "vcs_step_masked: frameskip out of range");
@@ -295,7 +304,7 @@ int vcs_step_masked(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, cons
 }
 
 int vcs_set_switches(vcs_t h, const uint8_t *switches_dev, void *cuda_stream) {
-  if (!h) return VCS_EINVAL;
+  DEV_OK(h);
   cudaStream_t s = (cudaStream_t)cuda_stream;
   if (switches_dev) CU(h, cudaMemcpyAsync(h->d_switches, switches_dev, (size_t)h->batch, cudaMemcpyDeviceToDevice, s));
   else { fill_kernel<<<(h->batch + 255) / 256, 256, 0, s>>>(h->d_switches, 0x3F, h->batch); h->launches += 1; CU(h, cudaGetLastError()); }
@@ -304,7 +313,7 @@ int vcs_set_switches(vcs_t h, const uint8_t *switches_dev, void *cuda_stream) {
 
 int vcs_boot(vcs_t h, const uint8_t *mask_dev, int32_t noop_frames, int32_t reset_frames, const uint8_t *noop_starts_dev,
              int32_t max_noop_starts, int32_t frameskip, void *cuda_stream) {
-  if (!h) return VCS_EINVAL;
+  DEV_OK(h);
   if (noop_frames < 0 || reset_frames < 0 || max_noop_starts < 0 || max_noop_starts > 255 || noop_frames > 100000 || reset_frames > 100000)
     return fail(h, VCS_EINVAL, "vcs_boot: frame counts out of range");
   if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31)) return fail(h, VCS_EINVAL, "vcs_boot: frameskip out of range");
@@ -334,7 +343,7 @@ int vcs_boot(vcs_t h, const uint8_t *mask_dev, int32_t noop_frames, int32_t rese
 
 int vcs_auto_reset(vcs_t h, const uint8_t *mask_dev, int32_t noop_steps, int32_t reset_steps, const uint8_t *noop_starts_dev,
                    int32_t max_noop_starts, void *cuda_stream) {
-  if (!h) return VCS_EINVAL;
+  DEV_OK(h);
   if (noop_steps < 0 || reset_steps < 0 || max_noop_starts < 0 || noop_steps + reset_steps + max_noop_starts > 255)
     return fail(h, VCS_EINVAL, "vcs_auto_reset: step counts out of range (their sum must be <= 255)");
   cudaStream_t s = (cudaStream_t)cuda_stream;
@@ -345,7 +354,7 @@ int vcs_auto_reset(vcs_t h, const uint8_t *mask_dev, int32_t noop_steps, int32_t
   return VCS_OK;
 }
 int vcs_get_booting(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
-  if (!h || !out_dev) return VCS_EINVAL;
+  DEV_OK(h); if (!out_dev) return VCS_EINVAL;
   get_booting_kernel<<<(h->batch + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(h->d_boot_ctr, out_dev, h->batch);
   h->launches += 1;
   CU(h, cudaGetLastError());
@@ -353,26 +362,27 @@ int vcs_get_booting(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
 }
 
 int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float T, float alpha, float *soft_out_dev, void *cuda_stream) {
-  if (!h) return VCS_EINVAL;
+  DEV_OK(h);
   if (!actions_dev || !soft_out_dev) return fail(h, VCS_EINVAL, "vcs_step_soft: NULL buffer");
   if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31)) return fail(h, VCS_EINVAL, "vcs_step_soft: frameskip out of range");
   if (!(T > 0.f) || T > 60.f || !(alpha == alpha) || alpha > 1e30f || alpha < -1e30f) return fail(h, VCS_EINVAL, "vcs_step_soft: T or alpha out of range");
   cudaStream_t s = (cudaStream_t)cuda_stream;
-  int K = (int)ceil(17.0 * (double)T); if (K < 1) K = 1; if (K > 1023) K = 1023;
-  float w[1024];
-  for (int k = 0; k <= K; ++k) w[k] = (float)exp(-(double)k / (double)T);
-  CU(h, cudaMemcpyAsync(h->d_soft_w, w, sizeof(float) * (K + 1), cudaMemcpyHostToDevice, s));
-  CU(h, cudaStreamSynchronize(s));                     // (w is on this stack frame)
-  if (h->soft_tab_T != T) {                            // W(T) x ROM once per temperature
+  if (h->soft_tab_T != T) {                            // a new temperature: e^{-k/T} and W(T) x ROM, once
+    int K = (int)ceil(17.0 * (double)T); if (K < 1) K = 1; if (K > 1023) K = 1023;
+    CU(h, cudaEventSynchronize(h->soft_w_done));       // (the previous upload from the handle's pinned buffer; long since done)
+    for (int k = 0; k <= K; ++k) h->h_soft_w[k] = (float)exp(-(double)k / (double)T);
+    CU(h, cudaMemcpyAsync(h->d_soft_w, h->h_soft_w, sizeof(float) * (K + 1), cudaMemcpyHostToDevice, s));
+    CU(h, cudaEventRecord(h->soft_w_done, s));
     cudaError_t ce0 = launch_soft_table(h->d_rom_blob, h->d_rom_meta_soft, h->n_roms, h->d_soft_w, K, h->d_soft_tab, s);
     h->launches += 1;
     if (ce0 != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_soft table launch", ce0);
-    h->soft_tab_T = T;
+    h->soft_tab_T = T; h->soft_K = K;
   }
   CU(h, cudaMemsetAsync(soft_out_dev, 0, sizeof(float) * 8 * (size_t)h->batch, s));
   StepParams p = params_of(h, actions_dev, frameskip);
   p.drom = h->d_drom_soft; p.rom_meta = h->d_rom_meta_soft;
-  p.soft_w = h->d_soft_w; p.soft_tab = h->d_soft_tab; p.soft_out = soft_out_dev; p.soft_alpha = alpha; p.soft_K = K;
+  p.perm = nullptr;                                    // the soft kernel has its own launch shape (128 envs per block): blocks in env order
+  p.soft_w = h->d_soft_w; p.soft_tab = h->d_soft_tab; p.soft_out = soft_out_dev; p.soft_alpha = alpha; p.soft_K = h->soft_K;
   cudaError_t ce = launch_step(p, s);
   h->launches += 1;
   if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_soft launch", ce);
@@ -380,7 +390,7 @@ int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float 
 }
 
 int vcs_get_ram(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
-  if (!h || !out_dev) return VCS_EINVAL;
+  DEV_OK(h); if (!out_dev) return VCS_EINVAL;
   const long long n = 32ll * h->batch;
   get_ram_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(h->d_ram, reinterpret_cast<uint32_t *>(out_dev), h->batch);
   h->launches += 1;
@@ -388,14 +398,14 @@ int vcs_get_ram(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
   return VCS_OK;
 }
 int vcs_get_regs(vcs_t h, vcs_regs *out_dev, void *cuda_stream) {
-  if (!h || !out_dev) return VCS_EINVAL;
+  DEV_OK(h); if (!out_dev) return VCS_EINVAL;
   get_regs_kernel<<<(h->batch + 127) / 128, 128, 0, (cudaStream_t)cuda_stream>>>(h->d_st, h->d_cyc, reinterpret_cast<uint4 *>(out_dev), h->batch);
   h->launches += 1;
   CU(h, cudaGetLastError());
   return VCS_OK;
 }
 int vcs_get_screen(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
-  if (!h || !out_dev) return VCS_EINVAL;
+  DEV_OK(h); if (!out_dev) return VCS_EINVAL;
   CU(h, cudaMemcpyAsync(out_dev, h->d_screen, (size_t)SCR_W * SCR_H * h->batch, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
   return VCS_OK;
 }
@@ -405,7 +415,7 @@ int vcs_screen_ptr(vcs_t h, const uint8_t **out_dev_ptr) {
 }
 
 int vcs_step_host(vcs_t h, const uint8_t *actions_host, int32_t frameskip, void *cuda_stream) {
-  if (!h || !actions_host) return VCS_EINVAL;
+  DEV_OK(h); if (!actions_host) return VCS_EINVAL;
   int rc = ensure_stage(h, (size_t)h->batch * 128); if (rc) return rc;
   cudaStream_t s = (cudaStream_t)cuda_stream;
   memcpy(h->h_pinned, actions_host, h->batch);
@@ -415,7 +425,7 @@ int vcs_step_host(vcs_t h, const uint8_t *actions_host, int32_t frameskip, void 
   return VCS_OK;
 }
 int vcs_get_ram_host(vcs_t h, uint8_t *out_host, void *cuda_stream) {
-  if (!h || !out_host) return VCS_EINVAL;
+  DEV_OK(h); if (!out_host) return VCS_EINVAL;
   int rc = ensure_stage(h, (size_t)h->batch * 128); if (rc) return rc;
   cudaStream_t s = (cudaStream_t)cuda_stream;
   rc = vcs_get_ram(h, h->d_actions_stage, cuda_stream); if (rc) return rc;
@@ -425,7 +435,7 @@ int vcs_get_ram_host(vcs_t h, uint8_t *out_host, void *cuda_stream) {
   return VCS_OK;
 }
 int vcs_get_regs_host(vcs_t h, vcs_regs *out_host, void *cuda_stream) {
-  if (!h || !out_host) return VCS_EINVAL;
+  DEV_OK(h); if (!out_host) return VCS_EINVAL;
   int rc = ensure_stage(h, (size_t)h->batch * 128); if (rc) return rc;
   cudaStream_t s = (cudaStream_t)cuda_stream;
   rc = vcs_get_regs(h, reinterpret_cast<vcs_regs *>(h->d_actions_stage), cuda_stream); if (rc) return rc;
@@ -435,7 +445,7 @@ int vcs_get_regs_host(vcs_t h, vcs_regs *out_host, void *cuda_stream) {
   return VCS_OK;
 }
 int vcs_get_screen_host(vcs_t h, uint8_t *out_host, void *cuda_stream) {
-  if (!h || !out_host) return VCS_EINVAL;
+  DEV_OK(h); if (!out_host) return VCS_EINVAL;
   cudaStream_t s = (cudaStream_t)cuda_stream;
   CU(h, cudaMemcpyAsync(out_host, h->d_screen, (size_t)SCR_W * SCR_H * h->batch, cudaMemcpyDeviceToHost, s));
   CU(h, cudaStreamSynchronize(s));
@@ -443,7 +453,7 @@ int vcs_get_screen_host(vcs_t h, uint8_t *out_host, void *cuda_stream) {
 }
 
 int vcs_block_times(vcs_t h, uint64_t *times_host, int32_t *perm_host, int32_t cap, int32_t *n_out) {
-  if (!h || !n_out) return VCS_EINVAL;
+  DEV_OK(h); if (!n_out) return VCS_EINVAL;
   const int n = (h->batch + h->block - 1) / h->block;
   *n_out = n;
   if (cap < n) return (times_host || perm_host) ? VCS_EINVAL : VCS_OK;
@@ -462,10 +472,15 @@ int vcs_optable(uint16_t *out256) {
 
 int vcs_destroy(vcs_t h) {
   if (!h) return VCS_EINVAL;
+  int cur = -1; cudaGetDevice(&cur);
+  if (cur != h->device) cudaSetDevice(h->device);     // free on the handle's own device, then give the caller's back
   cudaDeviceSynchronize();
   cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom);
   cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr); cudaFree(h->d_perm); cudaFree(h->d_blk_time); cudaFree(h->d_w_avg);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
+  if (h->h_soft_w) cudaFreeHost(h->h_soft_w);
+  if (h->soft_w_done) cudaEventDestroy(h->soft_w_done);
+  if (cur >= 0 && cur != h->device) cudaSetDevice(cur);
   delete h;
   return VCS_OK;
 }

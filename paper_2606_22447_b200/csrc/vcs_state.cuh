@@ -88,6 +88,8 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   int32_t y0, max_lines, f8_start_bank;
   uint32_t *d_st; uint32_t *d_ram; unsigned long long *d_cyc; uint8_t *d_screen;
   uint8_t *d_rom_blob; uint2 *d_drom; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
+  int device;                   // the CUDA device every pointer below belongs to
+  float *h_soft_w; cudaEvent_t soft_w_done; int soft_K;            // soft mode: pinned e^{-k/T} staging buffer, its upload, window of the cached temperature
   float *d_soft_tab; float soft_tab_T; size_t soft_tab_n;          // W(T) x ROM: the relaxed read of every ROM cell at the cached temperature
   uint2 *d_drom_soft; RomMeta *d_rom_meta_soft; float *d_soft_w;   // soft mode: an all-H_SLOW decode table (every byte fetched at run time), metas with doff 0, e^{-k/T}
   uint8_t *d_actions_stage;     // for vcs_step_host

@@ -1279,11 +1279,12 @@ size_t step_smem_bytes(int block, bool roms, uint32_t max_rom) {
 template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
 static cudaError_t launch_one(const StepParams &p, cudaStream_t stream) {
   const size_t smem_bytes = step_smem_bytes(BLOCK, ROMS, p.max_rom);
-  static size_t configured = 0;
-  if (configured < smem_bytes) {
+  static size_t configured[64] = {0};                   // per device: the attribute belongs to the (function, device) pair
+  int dev = 0; cudaGetDevice(&dev);
+  if (dev < 0 || dev >= 64 || configured[dev] < smem_bytes) {
     cudaError_t e = cudaFuncSetAttribute(vcs_step_kernel<BLOCK, ROMS, THREADS, SOFT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
-    configured = smem_bytes;
+    if (dev >= 0 && dev < 64) configured[dev] = smem_bytes;
   }
   const int grid = (p.batch + BLOCK - 1) / BLOCK;
   vcs_step_kernel<BLOCK, ROMS, THREADS, SOFT><<<grid, THREADS, smem_bytes, stream>>>(p);

@@ -202,7 +202,7 @@ def test_ale_vec_env_amortised_auto_reset(torch):
         m = env.step(dev(torch, acts[t]), dev(torch, done)).cpu().numpy()
         o.step_masked(acts[t], 4, play, threads=NCPU)                          # the oracle env waits while the GPU env runs its boot steps
         wait = np.maximum(wait - 1, 0)
-        assert (m == done).all()
+        assert (m == (done & play)).all()                        # a `done` for an env that is still booting is ignored
         if m.any():
             k = np.minimum(env.last_starts.cpu().numpy(), 3)
             o.boot(m, 8, 4, k.astype(np.uint8), 3, 4)
@@ -215,3 +215,29 @@ def test_ale_vec_env_amortised_auto_reset(torch):
         wait = np.maximum(wait - 1, 0)
     compare(env.vcs, o, "amortised AleVecEnv")
     env.close()
+
+
+def test_ale_vec_env_truncates_at_the_same_agent_step_in_both_modes(torch):
+    """max_episode_steps counts AGENT steps: the boot steps an amortised re-boot spends inside the batch's steps do not
+    count, so both modes end every episode after the same number of steps in which the env followed the agent."""
+    from paper_2606_22447_b200 import AleVecEnv
+    n = 48
+    w = make_workload(2, batch=n)
+    acts = w.actions(0, 40)
+    played = {}
+    for amortised in (False, True):
+        env = AleVecEnv(w.roms, w.seeds, w.env_rom, frameskip=4, noop_max=2, boot_noop_frames=8, boot_reset_frames=4,
+                        max_episode_steps=5, start_seed=3, amortised=amortised)
+        env.reset()
+        agent_steps = np.zeros(n, np.int64); lengths = [[] for _ in range(n)]
+        for t in range(40):
+            play = (env.booting().cpu().numpy() == 0) if amortised else np.ones(n, bool)
+            m = env.step(dev(torch, acts[t])).cpu().numpy()
+            agent_steps += play
+            for e in np.nonzero(m)[0]:
+                lengths[e].append(int(agent_steps[e])); agent_steps[e] = 0
+        played[amortised] = lengths
+        env.close()
+    for e in range(n):
+        assert played[False][e] and all(v == 5 for v in played[False][e]), (e, played[False][e])
+        assert played[True][e] and all(v == 5 for v in played[True][e]), (e, played[True][e])

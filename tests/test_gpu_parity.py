@@ -392,12 +392,9 @@ def test_block_placement_permutes_groups_not_results(torch):
     from paper_2606_22447_b200 import VCS
     w = make_workload(4)
     acts = torch.from_numpy(w.actions(0, 6)).cuda()
+    from paper_2606_22447_b200.binding import VCS_F_NO_BALANCE
     g = VCS(w.roms, w.seeds, w.env_rom)
-    os.environ["VCS_NO_BALANCE"] = "1"
-    try:
-        ref = VCS(w.roms, w.seeds, w.env_rom)
-    finally:
-        del os.environ["VCS_NO_BALANCE"]
+    ref = VCS(w.roms, w.seeds, w.env_rom, flags=VCS_F_NO_BALANCE)
     for t in range(6):
         g.step(acts[t], 4); ref.step(acts[t], 4)
     times, perm = g.block_times()

@@ -53,8 +53,8 @@ def test_soft_three_way(torch, cfg, kw, T, alpha):
 
 def test_config5_soft_forward_equals_hard(torch):
     """BASELINE config 5: batch 4096 on config 2's ROM, 200 steps of frameskip 4 at T in {0.1, 1, 10}; forward
-    RAM / regs / screen of soft mode == hard mode, every env, tolerance 0 (checked every 20 steps and at the end;
-    a sample of 16 envs is also checked against the oracle's hard mode at the end)."""
+    RAM / regs / screen of soft mode == hard mode, every env, tolerance 0 (checked every 20 steps and at the end), and
+    == the oracle's hard mode on a 64-env sample at the same checkpoints."""
     from paper_2606_22447_b200 import VCS
     from oracle.ovcs_py import OracleVCS
     w = make_workload(2, batch=4096)
@@ -63,24 +63,54 @@ def test_config5_soft_forward_equals_hard(torch):
     acts = torch.from_numpy(acts_host).cuda()
     g = VCS(w.roms, w.seeds, w.env_rom)
     softs = {T: VCS(w.roms, w.seeds, w.env_rom) for T in (0.1, 1.0, 10.0)}
+    idx = np.arange(64) * 64 + (np.arange(64) * 7) % 64
+    o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx])
     out = torch.empty((4096, 8), dtype=torch.float32, device="cuda")
     bad = torch.zeros((), dtype=torch.float32, device="cuda")
     for t in range(steps):
         g.step(acts[t], 4)
+        o.step(acts_host[t][idx], 4, threads=NCPU)
         for T, gs in softs.items():
             gs.step_soft(acts[t], 4, T, 6.0, out=out)
             bad += out[:, 6].sum()
         if t % 20 == 19 or t == steps - 1:
+            oregs = o.regs()
             for T, gs in softs.items():
                 same_state(gs, g, f"config5 T={T} step {t}")
+                assert (gs.ram_host()[idx] == o.ram()).all() and (gs.screen_host()[idx] == o.screen()).all(), f"T={T} step {t} vs oracle"
+                assert all((gs.regs_host()[idx][f] == oregs[f]).all() for f in oregs.dtype.names), f"T={T} step {t} regs vs oracle"
     assert float(bad.item()) == 0.0
-    idx = np.arange(16) * 256 + 7
+
+
+def test_soft_at_other_launch_shapes(torch):
+    """The soft kernel always runs 128 envs per block in env order, whatever shape and block placement the handle's
+    hard steps use: a 32,768-env handle (256-env blocks) and a handle with 64-env blocks whose placement has been
+    re-computed by a few plain steps must both step soft == hard, every env."""
+    from paper_2606_22447_b200 import VCS
+    from paper_2606_22447_b200.binding import VCS_F_BLOCK_64
+    from oracle.ovcs_py import OracleVCS
+    w = make_workload(2, batch=32768)
+    acts_host = w.actions(0, 4); acts = torch.from_numpy(acts_host).cuda()
+    g, gs = VCS(w.roms, w.seeds, w.env_rom), VCS(w.roms, w.seeds, w.env_rom)
+    idx = np.arange(32) * 1024 + (np.arange(32) * 37) % 1024
     o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx])
-    for t in range(steps):
-        o.step(acts_host[t][idx], 4, threads=NCPU)
-    gs = softs[10.0]
+    for t in range(4):
+        g.step(acts[t], 4); o.step(acts_host[t][idx], 4, threads=NCPU)
+        if t < 2: gs.step(acts[t], 4)
+        else: gs.step_soft(acts[t], 4, 1.0, 6.0)
+    same_state(gs, g, "soft at batch 32768")
     assert (gs.ram_host()[idx] == o.ram()).all() and (gs.screen_host()[idx] == o.screen()).all()
-    assert all((gs.regs_host()[idx][f] == o.regs()[f]).all() for f in o.regs().dtype.names)
+    g.close(); gs.close()
+    w = make_workload(4, batch=512, n_roms=8)                                # 64 envs per ROM
+    acts = torch.from_numpy(w.actions(0, 8)).cuda()
+    g, gs = VCS(w.roms, w.seeds, w.env_rom, flags=VCS_F_BLOCK_64), VCS(w.roms, w.seeds, w.env_rom, flags=VCS_F_BLOCK_64)
+    for t in range(8):
+        g.step(acts[t], 4)
+        if t < 6: gs.step(acts[t], 4)                                         # plain steps 2.. re-place the blocks
+        else: gs.step_soft(acts[t], 4, 10.0, 2.0)
+    _, perm = gs.block_times()
+    assert sorted(perm.tolist()) == list(range(8))
+    same_state(gs, g, "soft after a re-placement with 64-env blocks")
 
 
 def test_soft_argument_checks(torch):
