@@ -54,6 +54,33 @@ def oracle_sample(w, n_envs: int, steps: int, threads: int):
                 sample=f"{n_envs} envs (one per {w.batch // n_envs} of {w.name}'s batch, spread over its ROMs) x {steps} env-steps of frameskip 4")
 
 
+KERNEL_DRAM = os.path.join(ROOT, "profiles", "r02_kernel_dram.txt")
+
+
+def csrc_hash() -> str:
+    """sha256 over the kernel sources (what an ncu capture has to have been taken from to describe this build)"""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2606_22447_b200", "csrc")
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode()); h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def kernel_dram_traffic(batch: int):
+    """(bytes per launch | None, where it comes from): the committed ncu capture, if it matches batch and sources"""
+    try:
+        kv = dict(l.strip().split("=", 1) for l in open(KERNEL_DRAM) if "=" in l and not l.startswith("#"))
+    except OSError:
+        return None, "no capture committed"
+    if int(kv.get("batch", -1)) != batch:
+        return None, f"{os.path.relpath(KERNEL_DRAM, ROOT)} is for batch {kv.get('batch')}"
+    if kv.get("csrc_sha256_16") != csrc_hash():
+        return None, f"{os.path.relpath(KERNEL_DRAM, ROOT)} was captured from other kernel sources ({kv.get('csrc_sha256_16')} != {csrc_hash()}): stale"
+    return float(kv["dram_bytes_read"]) + float(kv["dram_bytes_write"]), f"{os.path.relpath(KERNEL_DRAM, ROOT)} (ncu --set full, same kernel sources {kv['csrc_sha256_16']})"
+
+
 class ClockSampler(threading.Thread):
     FIELDS = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
@@ -123,8 +150,8 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=120)      # ~1 s of timed steps: long enough for the clock sampler
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--batch", type=int, default=65536, help="envs per GPU (default: BASELINE config 4)")
     ap.add_argument("--workload", type=int, default=4, choices=[2, 3, 4],
@@ -246,9 +273,12 @@ def main():
     if not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
         s = oracle_sample(make_workload(args.workload), 32 * cores, 24, cores)       # ~10-20 s of wall clock on the box's cores
+        s1 = oracle_sample(make_workload(args.workload), 64, 16, 1)                  # the same oracle on ONE core (~4 s)
         work = s["work"]
         cpu = {"value": s["value"], "unit": "env-steps/s", "cores": cores, "kind": "oracle", "sample": s["sample"],
-               "emulated_cycles_per_s": s["cycles_per_s"], "seconds": s["seconds"]}
+               "emulated_cycles_per_s": s["cycles_per_s"], "seconds": s["seconds"],
+               "one_core": {"value": s1["value"], "unit": "env-steps/s", "cores": 1, "emulated_cycles_per_s": s1["cycles_per_s"],
+                            "seconds": s1["seconds"], "sample": s1["sample"]}}
     # ---- roofline: integer-issue bound.  peak = 148 SM x 4 schedulers x 32 lanes x SM clock (1 warp-instruction
     # per scheduler per clock); achieved = SURVEY §8(d)'s lower-bound work model x envs / kernel time.
     sm_mhz = clocks.get("sm_mhz") or peaks.get("sm_max_mhz") or 1965.0
@@ -258,14 +288,16 @@ def main():
     peak_alu, _ = issue_peak(0)                     # alu pipe alone (16 lanes / scheduler / clk)
     peak = peak_mixed
     kms = float(np.mean(kern_ms))
-    # DRAM bytes of one launch from the committed `ncu --set full` capture of this kernel (profiles/r01_v14_full.txt:
-    # dram__bytes_read.sum + dram__bytes_write.sum); algorithmic bytes are roofline.hbm.algorithmic_bytes_per_launch
-    NCU_DRAM_BYTES = 27.332096e6 + 2.173480e9
+    # DRAM bytes of one launch: from the committed `ncu --set full` capture (profiles/KERNEL_DRAM) — used only when that
+    # capture was taken from the kernel sources this run was built from (hash of csrc/), else null
+    traffic, traffic_note = kernel_dram_traffic(B)
     roof = {"bound": "alu", "unit": "thread-instr/s", "peak": peak,
             "peak_basis": "vcs_issue_peak(kind=1): LOP3+IMAD chains on all SMs, measured in this run",
             "peak_alu_pipe_only": peak_alu, "peak_nominal": nominal,
-            "kernel": "vcs_step_kernel", "kernel_ms": kms, "traffic": NCU_DRAM_BYTES if B == 65536 else None,
-            "traffic_unit": "DRAM bytes per launch (ncu, profiles/r01_v14_full.txt)"}
+            "kernel": "vcs_step_kernel", "kernel_ms": kms, "traffic": traffic,
+            "traffic_unit": "DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)", "traffic_source": traffic_note,
+            "achieved_basis": "modelled: SURVEY 8(d) lower-bound work model (40 / 6502 instruction + 80 / TIA write + 40 / scanline) x counts "
+                              "from the oracle's instrumentation in this run; the executed counters are in profiles/"}
     if work:
         ops = MODEL_PER_INSTR * work["instr"] + MODEL_PER_SEGMENT * work["tia_writes"] + MODEL_PER_LINE * work["lines"]
         roof.update(achieved=ops * B / (kms * 1e-3), algorithmic_thread_instr_per_env_step=ops, work_per_env_step=work)

@@ -55,6 +55,13 @@ DEV uint32_t spread8(uint32_t b) {
 
 enum : uint32_t { EV_FRAME = 1u, EV_WSYNC = 2u, EV_CROSS = 16u };   // EV_CROSS * (line ends performed)
 
+// 16 bytes of a screen row -> HBM: one st.global.v4 (SASS STG.E.128), streaming (.cs: the kernel never reads a row
+// back and a step's 2.2 GB of rows would only evict what it does re-use from L2).  Rows are 160 B = 10 such stores;
+// 33,600 B per env and 160 B per row keep every row 16-byte aligned (the screen base comes from cudaMalloc).
+DEV void st_row16(uint4 *p, uint4 v) {
+  asm volatile("st.global.cs.v4.b32 [%0], {%1, %2, %3, %4};" ::"l"(__cvta_generic_to_global(p)), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
 // ---- descriptors of the plain VALUE registers (SURVEY C.8 write effects that are "store a masked field"): the write
 // path handles them with one piece of code instead of one switch case each (the hot code must stay small: icache).
 //   bits 2:0 kind (0 special, 1 field store into a packed word, 2 flag) ; 5:3 word - S_COLU ; 10:6 bit shift of the
@@ -216,7 +223,7 @@ struct Tia {
     uint4 *dst = reinterpret_cast<uint4 *>(row_ptr(sl, r));
     if (fl & TF_VBLANK) {
 #pragma unroll
-      for (int q = 0; q < 10; ++q) dst[q] = make_uint4(0, 0, 0, 0);
+      for (int q = 0; q < 10; ++q) st_row16(dst + q, make_uint4(0, 0, 0, 0));
       return;
     }
     const uint32_t colu = S(sl, S_COLU);
@@ -229,7 +236,7 @@ struct Tia {
         const uint32_t s0 = spread8(a) | (spread8(b) << 1), s1 = spread8(a >> 8) | (spread8(b >> 8) << 1);
         uint4 v = make_uint4(__byte_perm(colu, 0, s0), __byte_perm(colu, 0, s0 >> 16), __byte_perm(colu, 0, s1), __byte_perm(colu, 0, s1 >> 16));
         if (w == 0 && h == 0 && (fl & TF_HMBLANK)) { v.x = 0; v.y = 0; }
-        dst[2 * w + h] = v;
+        st_row16(dst + 2 * w + h, v);
       }
     }
   }
@@ -291,10 +298,11 @@ struct Tia {
         if (max(x, px) < SCR_W) paint_range(sl, r, max(x, px), SCR_W, fl, true);
       }
       const uint4 z = make_uint4(0, 0, 0, 0);                      // rows the beam never reached in this frame
+#pragma unroll 1
       for (int rr = max(r + 1, 0); rr < SCR_H; ++rr) {
         uint4 *dst = reinterpret_cast<uint4 *>(row_ptr(sl, rr));
 #pragma unroll
-        for (int q = 0; q < 10; ++q) dst[q] = z;
+        for (int q = 0; q < 10; ++q) st_row16(dst + q, z);
       }
     }
     const uint32_t fd = S(sl, S_FDONE) + 1;
