@@ -60,8 +60,9 @@ enum {
   VCS_F_NO_REGROUP = 1u << 2,   /* F8 blocks do not re-sort their envs by bank at hotspot accesses             */
   VCS_F_ROM_GLOBAL = 1u << 3,   /* cartridge bytes through the read-only cache instead of shared memory        */
   VCS_F_NO_BALANCE = 1u << 4,   /* blocks run env groups in env order (no measured placement)    */
+  VCS_F_NO_PROMOTE = 1u << 5,   /* indexed / indirect / stack instructions always run in the out-of-line executor */
   VCS_F_BLOCK_64   = 1u << 8, VCS_F_BLOCK_128 = 2u << 8, VCS_F_BLOCK_256 = 3u << 8, VCS_F_BLOCK_MASK = 3u << 8,  /* envs per block */
-  VCS_F_ALL = 0x31Fu
+  VCS_F_ALL = 0x33Fu
 };
 
 /* 32 bytes per environment, little-endian. */

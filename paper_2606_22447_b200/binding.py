@@ -16,7 +16,7 @@ _SO = os.path.join(_PKG, "libvcsb200.so")
 
 VCS_OK, VCS_EINVAL, VCS_ECUDA, VCS_ENOMEM, VCS_EROM = 0, -1, -2, -3, -4
 # vcs_config.flags (include/vcs.h): performance only, never results
-VCS_F_NO_SPIN, VCS_F_NO_FUSE, VCS_F_NO_REGROUP, VCS_F_ROM_GLOBAL, VCS_F_NO_BALANCE = 1, 2, 4, 8, 16
+VCS_F_NO_SPIN, VCS_F_NO_FUSE, VCS_F_NO_REGROUP, VCS_F_ROM_GLOBAL, VCS_F_NO_BALANCE, VCS_F_NO_PROMOTE = 1, 2, 4, 8, 16, 32
 VCS_F_BLOCK_64, VCS_F_BLOCK_128, VCS_F_BLOCK_256 = 1 << 8, 2 << 8, 3 << 8
 _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
 

@@ -199,7 +199,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
           if (roms[r].size == 2048) { memcpy(img.data(), roms[r].data, 2048); memcpy(img.data() + 2048, roms[r].data, 2048); }
           else memcpy(img.data(), roms[r].data + 4096 * b, 4096);
           if (pass == 0) mark_leaders(img.data(), leader.data());
-          else { decode_bank(img.data(), leader.data(), h->block, nb, dw.data() + meta[r].doff + 4096 * b);
+          else { decode_bank(img.data(), leader.data(), h->block, nb, dw.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE));
                  if (!(c.flags & VCS_F_NO_SPIN)) mark_spins(img.data(), dw.data() + meta[r].doff + 4096 * b);
                  if (!(c.flags & VCS_F_NO_FUSE)) fuse_ld_st(dw.data() + meta[r].doff + 4096 * b); }
         }

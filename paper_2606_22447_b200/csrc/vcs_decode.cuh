@@ -118,11 +118,27 @@ enum HotClass : uint32_t {
   HC_SPIN = 16,      // LDA INTIM ; BNE *-3  /  BIT TIMINT ; BPL *-3 : the timer wait loop, fast-forwarded (aux = 0 / 1 ; y = the poll's own entry .x)
   HC_LDST = 17,      // LDx #imm ; STx <TIA register> as one entry: y = imm | (register | source index << 6) << 8 | insert selector << 16 ;
                      // aux = 1 when the store is absolute ; cy / len cover both instructions
-  HC_COLD = 18       // + Hid: executed by the out-of-line executor
+  // Indexed / indirect accesses and stack instructions whose bus accesses all turn out, at run time, to be RAM cells or
+  // plain cartridge bytes (no TIA / RIOT register, no bank hotspot).  The inline loop checks that first and otherwise
+  // hands the instruction, untouched, to the out-of-line executor under its generic handler id.
+  HC_IDX_RD = 18,    // zp,X zp,Y abs,X abs,Y reads: y = base | index extract selector << 16 ; aux = read op | zp-indexed << 7
+  HC_IZY_RD = 19,    // (zp),Y reads, pointer cells in RAM: y = smem byte offset of cell zp | of cell zp+1 << 15 ; aux = read op
+  HC_IZX_RD = 20,    // (zp,X) reads: y = zp ; aux = read op
+  HC_IDX_ST = 21,    // zp,X zp,Y abs,X abs,Y stores into RAM: y = base | index extract selector << 16 ; aux = source (0 A, 1 X, 2 Y) | zp-indexed << 7
+  HC_IZY_ST = 22,    // (zp),Y stores: y as HC_IZY_RD ; aux = source
+  HC_IZX_ST = 23,    // (zp,X) stores: y = zp ; aux = source
+  HC_JSR = 24,       // y = target
+  HC_RTS = 25,
+  HC_STACK = 26,     // aux = 0 PHA, 1 PHP, 2 PLA, 3 PLP
+  HC_ST_RIOT = 27,   // absolute store to a RIOT register (ports, timer): y = address | extract selector << 16
+  HC_COLD = 28       // + Hid: executed by the out-of-line executor
 };
 static_assert(HC_COLD + H_COUNT <= 128, "hid is 7 bits");
 
-inline void hot_class(uint32_t &x, uint32_t &y) {
+// smem byte offset of RAM cell `a` (any address that decodes to RAM) in a file of `block` interleaved words
+inline uint32_t ram_cell_offset(uint32_t a, int block) { return ((a & 0x7Cu) * (uint32_t)block) | (a & 3u); }
+
+inline void hot_class(uint32_t &x, uint32_t &y, int block, bool promote) {
   const uint32_t hid = x & 0x7Fu, rest = x & 0x00FFFF00u;                  // cy and len stay
   static const uint32_t ins[4] = {0x3214u, 0x3240u, 0x3410u, 0x4210u};     // prmt(axys, v, sel): v -> A, X, Y, SP
   auto ext = [](uint32_t i) { return 0x4440u | i; };                       // prmt(axys, 0, sel): zero-extended byte i
@@ -156,6 +172,33 @@ inline void hot_class(uint32_t &x, uint32_t &y) {
   }
   else if (hid == H_JMP) mk(HC_JMP, 0);
   else if (hid == H_RTIM) mk(HC_RTIM, x >> DW_OP2_SHIFT);
+  else if (promote && (hid == H_R0 + 2 || hid == H_R0 + 3 || hid == H_R0 + 5 || hid == H_R0 + 6) && (x >> DW_OP2_SHIFT) <= 11u) {
+    const bool zpm = hid < H_R0 + 4, useX = (hid == H_R0 + 2 || hid == H_R0 + 5);              // ZPX ZPY ABX ABY reads
+    y = (y & 0xFFFFu) | (ext(useX ? 1u : 2u) << 16);
+    x = HC_IDX_RD | (4u << DW_CY_SHIFT) | (x & 0x00FF0000u) | (((x >> DW_OP2_SHIFT) | (zpm ? 0x80u : 0u)) << DW_OP2_SHIFT);
+  }
+  else if (promote && (hid == H_W0 + 1 || hid == H_W0 + 2 || hid == H_W0 + 4 || hid == H_W0 + 5) && (x >> DW_OP2_SHIFT) <= 2u) {
+    const bool zpm = hid < H_W0 + 3, useX = (hid == H_W0 + 1 || hid == H_W0 + 4);              // ZPX ZPY ABX ABY stores
+    y = (y & 0xFFFFu) | (ext(useX ? 1u : 2u) << 16);
+    x = HC_IDX_ST | ((zpm ? 4u : 5u) << DW_CY_SHIFT) | (x & 0x00FF0000u) | (((x >> DW_OP2_SHIFT) | (zpm ? 0x80u : 0u)) << DW_OP2_SHIFT);
+  }
+  else if (promote && (hid == H_R0 + 8 || hid == H_W0 + 7) && (y & 0xFFu) >= 0x80u && (y & 0xFFu) <= 0xFEu &&
+           (x >> DW_OP2_SHIFT) <= (hid == H_R0 + 8 ? 11u : 2u)) {                                // (zp),Y with both pointer cells in RAM
+    const uint32_t z = y & 0xFFu;
+    y = ram_cell_offset(z, block) | (ram_cell_offset(z + 1u, block) << 15);
+    x = (hid == H_R0 + 8 ? (uint32_t)HC_IZY_RD | (5u << DW_CY_SHIFT) : (uint32_t)HC_IZY_ST | (6u << DW_CY_SHIFT)) | (x & 0xFFFF0000u);
+  }
+  else if (promote && (hid == H_R0 + 7 || hid == H_W0 + 6) && (x >> DW_OP2_SHIFT) <= (hid == H_R0 + 7 ? 11u : 2u)) {    // (zp,X)
+    y &= 0xFFu;
+    x = (hid == H_R0 + 7 ? (uint32_t)HC_IZX_RD : (uint32_t)HC_IZX_ST) | (6u << DW_CY_SHIFT) | (x & 0xFFFF0000u);
+  }
+  else if (promote && hid == H_JSR) mk(HC_JSR, 0);
+  else if (promote && hid == H_RTS) mk(HC_RTS, 0);
+  else if (promote && hid >= H_PHA && hid <= H_PLP) mk(HC_STACK, hid - H_PHA);
+  else if (promote && hid == H_W0 + 3 && (x >> DW_OP2_SHIFT) <= 2u && (y & 0x1280u) == 0x0280u) {                      // STx abs -> RIOT
+    y = (y & 0x1FFFu) | (ext(x >> DW_OP2_SHIFT) << 16);
+    x = HC_ST_RIOT | (4u << DW_CY_SHIFT) | (x & 0x00FF0000u);
+  }
   else x += HC_COLD;                                                       // (hid + HC_COLD stays below 128)
   const uint32_t hc = x & 0x7Fu;
   x |= (hc == HC_ST_TIA) ? DW_F_STTIA : (hc == HC_LD_IMM) ? DW_F_LDIMM : (hc == HC_BR) ? DW_F_BR : 0u;
@@ -163,7 +206,7 @@ inline void hot_class(uint32_t &x, uint32_t &y) {
 
 // One bank image (4096 bytes; 2 KB carts are passed mirrored) -> 4096 decode entries.  `leader` is the bank-
 // independent leader bitmap (4096 flags) filled by mark_leaders() for every bank of the cartridge first.
-inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, int nb, DWord *out) {
+inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, int nb, DWord *out, bool promote = true) {
   for (uint32_t off = 0; off < 4096; ++off) {
     const uint32_t lead = leader[off] ? DW_LEADER : 0u;
     if (off >= DW_SLOW_LIMIT) { out[off].x = (HC_COLD + H_SLOW) | lead; out[off].y = 0; continue; }
@@ -212,7 +255,7 @@ inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, in
       }
     }
     if ((x & 0x7Fu) == H_SLOW) { out[off].x = (HC_COLD + H_SLOW) | lead; out[off].y = 0; }
-    else { hot_class(x, payload); out[off].x = x | lead; out[off].y = payload; }
+    else { hot_class(x, payload, block, promote); out[off].x = x | lead; out[off].y = payload; }
   }
 }
 

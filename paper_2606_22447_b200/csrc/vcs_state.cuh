@@ -79,7 +79,10 @@ static_assert(S_STATUS == 58, "file layout");
 // per-block context, in words after the thread files (block-uniform values the out-of-line paths need)
 enum CtxWord { C_SCREEN_LO = 0, C_SCREEN_HI, C_Y0, C_FRAMESKIP, C_BATCH, C_ENV0, C_CAP, C_ROMOFF, C_REGROUP,
                C_META_LO, C_META_HI, C_BLOB_LO, C_BLOB_HI, C_DROM_LO, C_DROM_HI,
-               C_SOFT_OUT_LO, C_SOFT_OUT_HI, C_SOFT_W_LO, C_SOFT_W_HI, C_SOFT_K, C_SOFT_ALPHA, C_SOFT_TAB_LO, C_SOFT_TAB_HI, C_WORDS = 24 };
+               C_SOFT_OUT_LO, C_SOFT_OUT_HI, C_SOFT_W_LO, C_SOFT_W_HI, C_SOFT_K, C_SOFT_ALPHA, C_SOFT_TAB_LO, C_SOFT_TAB_HI,
+               C_HS,           // bank hotspots of the block's ROM (ROM staged in smem: one ROM per block): first address | count << 16
+               C_WORDS = 24 };
+static_assert(C_HS < C_WORDS, "context layout");
 
 struct RomMeta { uint32_t offset; uint32_t size; uint32_t doff; uint32_t pad; };   // byte offset into the ROM blob, size, word offset into the decode blob
 

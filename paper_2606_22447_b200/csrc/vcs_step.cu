@@ -876,6 +876,20 @@ __device__ __noinline__ int32_t wsync_line(uint32_t sl, int32_t cyc, int32_t lst
   return lstart + 2 * LINE_CYC;
 }
 
+// is `addr` a RAM cell or a plain byte of the (shared-memory staged) cartridge?  hs = first hotspot | count << 16
+template <bool ROMS>
+DEV bool plain_addr(uint32_t addr, uint32_t hs) {
+  const uint32_t a = addr & 0x1FFFu;
+  if ((a & 0x1280u) == 0x0080u) return true;
+  if constexpr (ROMS) return (a & 0x1000u) && (a - (hs & 0xFFFFu)) >= (hs >> 16);
+  else return false;                                       // (ROM in global memory: left to the out-of-line executor)
+}
+template <int BLOCK, bool ROMS>
+DEV uint32_t rom_byte_hot(uint32_t off) {                  // byte `off` (bank << 12 | offset) of the block's staged ROM
+  if constexpr (ROMS) return reinterpret_cast<const uint8_t *>(smem)[(S_WORDS * BLOCK + C_WORDS) * 4 + off];
+  else return 0;
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // The inline interpreter loop: instructions of this lane's min-key group until the next scheduling point.
 template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
@@ -890,6 +904,7 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
       else { h = cold_pre<BLOCK, ROMS, THREADS, SOFT>(h, sl); if (!h.aux) return; }
     }
     uint32_t cx = h.wx, pl = h.wy;                         // the entry being executed
+    const int32_t cyc0 = h.cyc;                            // its first cycle
     h.di += (cx >> DW_LEN_SHIFT) & 0xFFu;
     uint2 wn = __ldg(dr + h.di);                           // sequential prefetch
     h.cyc += (int32_t)((cx >> DW_CY_SHIFT) & 0xFu);
@@ -976,6 +991,93 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
       aux = cx >> DW_OP2_SHIFT;
         } goto do_rtim;
         case HC_JMP: { const uint32_t nd = (h.di & 0x7000u) | (pl & 0xFFFu); h.pbase = pl - nd; h.di = nd; } goto ctl;
+        // ---- indexed / indirect accesses and the stack, as long as every bus access of the instruction is a RAM cell
+        // or a plain cartridge byte (C.5 sequences; their dummy cycles then have no effect).  Anything else — TIA / RIOT
+        // registers, bank hotspots, stack or pointer cells outside RAM — goes to the out-of-line executor untouched.
+        case HC_IDX_RD: case HC_IDX_ST: case HC_IZY_RD: case HC_IZY_ST: case HC_IZX_RD: case HC_IZX_ST: {
+          const bool store = cls >= HC_IDX_ST;
+          const uint32_t hs = T::ctx(C_HS);
+          uint32_t ea, gid;                                // effective address ; the generic handler id of this instruction
+          bool ok = true;
+          if (cls == HC_IDX_RD || cls == HC_IDX_ST) {
+            const uint32_t idx = __byte_perm(h.axys, 0u, pl >> 16), base = pl & 0xFFFFu, useX = ((pl >> 16) & 3u) == 1u;
+            if (aux & 0x80u) { ea = (base + idx) & 0xFFu; gid = (store ? H_W0 + 2u : H_R0 + 3u) - useX; }
+            else {
+              const uint32_t t = (base & 0xFFu) + idx, unc = (base & 0xFF00u) | (t & 0xFFu);
+              ea = (unc + (t & 0x100u)) & 0xFFFFu; gid = (store ? H_W0 + 5u : H_R0 + 6u) - useX;
+              if (store || (t & 0x100u)) ok = plain_addr<ROMS>(unc, hs);        // the discarded read at the uncorrected address
+              if (!store) h.cyc += (int32_t)(t >> 8);                            // page crossed: one more cycle
+            }
+            aux &= 0x7Fu;
+          } else {
+            const bool izy = cls == HC_IZY_RD || cls == HC_IZY_ST;
+            uint32_t lo, hi, iy = 0;
+            if (izy) { lo = ramb[pl & 0x7FFFu]; hi = ramb[pl >> 15]; iy = (h.axys >> 16) & 0xFFu; gid = store ? H_W0 + 7u : H_R0 + 8u; }
+            else {
+              const uint32_t z = (pl + ((h.axys >> 8) & 0xFFu)) & 0xFFu; gid = store ? H_W0 + 6u : H_R0 + 7u;
+              ok = z - 0x80u <= 0x7Eu;                                           // both pointer cells in RAM
+              lo = ramb[((z & 0x7Cu) * BLOCK) | (z & 3u)]; hi = ramb[(((z + 1u) & 0x7Cu) * BLOCK) | ((z + 1u) & 3u)];
+            }
+            const uint32_t t = lo + iy, unc = (hi << 8) | (t & 0xFFu);
+            ea = (unc + (t & 0x100u)) & 0xFFFFu;
+            if (izy && (store || (t & 0x100u))) ok = ok && plain_addr<ROMS>(unc, hs);     // (zp),Y: the discarded read at the uncorrected address
+            if (izy && !store) h.cyc += (int32_t)(t >> 8);                                 // page crossed: one more cycle
+          }
+          const bool in_ram = (ea & 0x1280u) == 0x0080u;
+          ok = ok && (store ? in_ram : plain_addr<ROMS>(ea, hs));
+          if (!ok) {                                       // not this simple: the generic handler, from the instruction's first cycle
+            h.cyc = cyc0;
+            uint32_t gpl = pl & 0xFFFFu;
+            if (cls == HC_IZY_RD || cls == HC_IZY_ST) { const uint32_t o = pl & 0x7FFFu; gpl = 0x80u | ((o / BLOCK) & 0x7Cu) | (o & 3u); }
+            else if (cls == HC_IZX_RD || cls == HC_IZX_ST) gpl = pl & 0xFFu;
+            h.wx = (HC_COLD + gid) | (cx & 0x00FF0000u) | (aux << DW_OP2_SHIFT); h.wy = gpl;   // (kept in h: cold_exec may pass it on, AUX_GENERIC)
+            h = cold_exec<BLOCK, ROMS, THREADS, SOFT>(h, sl, h.wx, h.wy);
+            return;
+          }
+          const uint32_t ro = ((ea & 0x7Cu) * BLOCK) | (ea & 3u);
+          if (store) { ramb[ro] = (uint8_t)__byte_perm(h.axys, 0u, 0x4440u | aux); break; }
+          v = in_ram ? (uint32_t)ramb[ro] : rom_byte_hot<BLOCK, ROMS>((h.di & 0x7000u) + (ea & 0xFFFu));
+        } goto do_alu;
+        case HC_JSR: case HC_RTS: case HC_STACK: {
+          const uint32_t sp = h.axys >> 24;
+          uint32_t nsp, target;
+          auto cell = [&](uint32_t a) -> uint8_t & { return ramb[((a & 0x7Cu) * BLOCK) | (a & 3u)]; };
+          if (cls == HC_JSR) {
+            if (sp < 0x81u) goto generic_stack;
+            const uint32_t ret = (h.pbase + h.di - 1u) & 0xFFFFu;               // address of the instruction's third byte
+            cell(sp) = (uint8_t)(ret >> 8); cell(sp - 1u) = (uint8_t)ret; nsp = sp - 2u; target = pl;
+          } else if (cls == HC_RTS) {
+            if (sp - 0x7Fu > 0xFDu - 0x7Fu) goto generic_stack;
+            const uint32_t r = (uint32_t)cell(sp + 1u) | ((uint32_t)cell(sp + 2u) << 8);
+            if (!((r & 0x1000u) && plain_addr<ROMS>(r, T::ctx(C_HS)))) goto generic_stack;   // the discarded read at the pulled address
+            nsp = sp + 2u; target = (r + 1u) & 0xFFFFu;
+          } else if (aux < 2u) {                           // PHA / PHP
+            if (sp < 0x80u) goto generic_stack;
+            cell(sp) = aux ? (uint8_t)((h.fl & 0x4Du) | 0x30u | ((h.zn & 0x180u) ? 0x80u : 0u) | ((h.zn & 0xFFu) ? 0u : 2u)) : (uint8_t)h.axys;
+            nsp = (sp - 1u) & 0xFFu; target = 0x10000u;
+          } else {                                         // PLA / PLP
+            if (sp - 0x7Fu > 0xFEu - 0x7Fu) goto generic_stack;
+            v = cell(sp + 1u); nsp = sp + 1u; target = 0x10000u;
+            if (aux == 2u) { h.axys = __byte_perm(h.axys, v, 0x3214u); h.zn = v; }
+            else { h.fl = v & 0x4Du; h.zn = ((v & 0x80u) << 1) | ((v & 2u) ? 0u : 1u); }
+          }
+          h.axys = (h.axys & 0x00FFFFFFu) | (nsp << 24);
+          if (h.keyhi < KEY_PARKED) h.keyhi = (h.keyhi & ~(0xFFu << 19)) | (nsp << 19);          // SP is part of the scheduling key
+          if (target < 0x10000u) { const uint32_t nd = (h.di & 0x7000u) | (target & 0xFFFu); h.pbase = target - nd; h.di = nd; goto ctl; }
+          break;
+        generic_stack:
+          h.wx = (HC_COLD + (cls == HC_JSR ? (uint32_t)H_JSR : cls == HC_RTS ? (uint32_t)H_RTS : H_PHA + aux)) | (cx & 0x00FFFF00u);
+          h = cold_exec<BLOCK, ROMS, THREADS, SOFT>(h, sl, h.wx, pl);
+          return;
+        }
+        case HC_ST_RIOT: {                                 // STx abs to a RIOT register: the write is the instruction's 4th cycle
+          v = __byte_perm(h.axys, 0u, pl >> 16);
+          if ((pl & 4u) == 0) { const uint32_t sh = 8u * (pl & 3u); T::S(sl, S_PORTS) = (T::S(sl, S_PORTS) & ~(0xFFu << sh)) | (v << sh); }
+          else if ((pl & 0x14u) == 0x14u) {
+            const uint32_t k = pl & 3u, shift = (0x0A630u >> (4u * k)) & 0xFu;                 // 0, 3, 6, 10
+            T::S(sl, S_TMR) = v | (shift << 8) | (((1u << shift) - 1u) << 16); T::S(sl, S_TTICKS) = (uint32_t)h.cyc;
+          }
+        } break;
         default:                                           // everything else: out of line, then re-schedule
           h = cold_exec<BLOCK, ROMS, THREADS, SOFT>(h, sl, cx, pl);
           return;
@@ -1032,6 +1134,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     s_ctx[C_Y0] = (uint32_t)p.y0; s_ctx[C_FRAMESKIP] = (uint32_t)p.frameskip; s_ctx[C_BATCH] = (uint32_t)B; s_ctx[C_ENV0] = (uint32_t)e0;
     s_ctx[C_CAP] = (uint32_t)(p.max_lines * LINE_CYC); s_ctx[C_ROMOFF] = ROM_OFF;
     s_ctx[C_REGROUP] = (ROMS && rm.size == 8192 && p.regroup) ? 1u : 0u;
+    { const uint32_t n = (rm.size >> 12) < 2u ? 0u : (rm.size >> 12); s_ctx[C_HS] = ((n == 8u) ? 0x1FF4u : 0x1FFAu - n) | (n << 16); }
     auto put = [&](int lo, const void *q) { const unsigned long long v = reinterpret_cast<unsigned long long>(q); s_ctx[lo] = (uint32_t)v; s_ctx[lo + 1] = (uint32_t)(v >> 32); };
     put(C_META_LO, p.rom_meta); put(C_BLOB_LO, p.rom_blob); put(C_DROM_LO, p.drom);
     put(C_SOFT_OUT_LO, p.soft_out); put(C_SOFT_W_LO, p.soft_w); put(C_SOFT_TAB_LO, p.soft_tab); s_ctx[C_SOFT_K] = (uint32_t)p.soft_K; s_ctx[C_SOFT_ALPHA] = __float_as_uint(p.soft_alpha);

@@ -21,9 +21,9 @@ def torch():
 def _flags():
     from paper_2606_22447_b200 import binding as B
     return [("no_spin", B.VCS_F_NO_SPIN), ("no_fuse", B.VCS_F_NO_FUSE), ("no_regroup", B.VCS_F_NO_REGROUP),
-            ("rom_global", B.VCS_F_ROM_GLOBAL), ("no_balance", B.VCS_F_NO_BALANCE), ("block64", B.VCS_F_BLOCK_64),
+            ("rom_global", B.VCS_F_ROM_GLOBAL), ("no_balance", B.VCS_F_NO_BALANCE), ("no_promote", B.VCS_F_NO_PROMOTE), ("block64", B.VCS_F_BLOCK_64),
             ("block128", B.VCS_F_BLOCK_128), ("block256", B.VCS_F_BLOCK_256),
-            ("all_off+block64", B.VCS_F_NO_SPIN | B.VCS_F_NO_FUSE | B.VCS_F_NO_REGROUP | B.VCS_F_ROM_GLOBAL | B.VCS_F_NO_BALANCE | B.VCS_F_BLOCK_64),
+            ("all_off+block64", B.VCS_F_NO_SPIN | B.VCS_F_NO_FUSE | B.VCS_F_NO_REGROUP | B.VCS_F_ROM_GLOBAL | B.VCS_F_NO_BALANCE | B.VCS_F_NO_PROMOTE | B.VCS_F_BLOCK_64),
             ("rom_global+block256", B.VCS_F_ROM_GLOBAL | B.VCS_F_BLOCK_256)]
 
 
