@@ -865,15 +865,16 @@ __device__ __noinline__ uint32_t cold_timer_read(uint32_t sl, uint32_t a, int32_
   return Riot<BLOCK, 0>::timer_read(sl, a, c);
 }
 
-// WSYNC released at the end of the line (a12), the common way a line ends: returns the new `lim`, or LIM_NOW when
-// the case is not the plain one (instruction ran over the line end, frame cap in reach) and cold_pre must decide.
+// The common ways a line ends — WSYNC released at the end of the line (a12: ws), or the code simply ran into the next
+// line: returns the new `lim`, or LIM_NOW when the case is not the plain one (a stalled instruction that had already
+// run over the line end, the frame cap in reach or reached) and cold_pre must decide.
 template <int BLOCK>
-__device__ __noinline__ int32_t wsync_line(uint32_t sl, int32_t cyc, int32_t lstart) {
+__device__ __noinline__ int32_t line_step(uint32_t sl, int32_t cyc, int32_t lstart, bool ws) {
   using T = Tia<BLOCK>;
   const int32_t fcap = (int32_t)T::S(sl, S_FSTART) + (int32_t)T::ctx(C_CAP);
-  if (cyc - lstart > LINE_CYC || lstart + 2 * LINE_CYC >= fcap) return LIM_NOW;
+  if (ws ? (cyc - lstart > LINE_CYC || lstart + 2 * LINE_CYC >= fcap) : (cyc - lstart < LINE_CYC || cyc >= fcap)) return LIM_NOW;
   T::line_end(sl);
-  return lstart + 2 * LINE_CYC;
+  return min(lstart + 2 * LINE_CYC, fcap);
 }
 
 // is `addr` a RAM cell or a plain byte of the (shared-memory staged) cartridge?  hs = first hotspot | count << 16
@@ -899,8 +900,9 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
   for (;;) {
     if (h.cyc >= h.lim) {
       int32_t nl = LIM_NOW;
-      if (h.lim == LIM_WSYNC) nl = wsync_line<BLOCK>(sl, h.cyc, h.lstart);
-      if (nl != LIM_NOW) { h.lstart += LINE_CYC; h.cyc = h.lstart; h.lim = nl; }
+      const bool ws = h.lim == LIM_WSYNC;
+      if (h.lim != LIM_NOW) nl = line_step<BLOCK>(sl, h.cyc, h.lstart, ws);
+      if (nl != LIM_NOW) { h.lstart += LINE_CYC; if (ws) h.cyc = h.lstart; h.lim = nl; }
       else { h = cold_pre<BLOCK, ROMS, THREADS, SOFT>(h, sl); if (!h.aux) return; }
     }
     uint32_t cx = h.wx, pl = h.wy;                         // the entry being executed

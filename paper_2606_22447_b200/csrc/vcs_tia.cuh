@@ -170,7 +170,7 @@ struct Tia {
     if (fl & TF_DIRTY_ALL) { rebuild(sl, fl); fl &= ~TF_DIRTY_ALL; S(sl, S_FL) = fl; }
     const bool vis = (fl & TF_ROWVIS) != 0;
     const uint32_t ctrl = S(sl, S_PF) >> 24;
-    uint32_t a0 = 0, a1 = 0, a2 = 0, a3 = 0, a4 = 0, a5 = 0, a6 = 0, a7 = 0, a8 = 0, a9 = 0, a10 = 0, a11 = 0, a12 = 0, a13 = 0, a14 = 0;
+    uint32_t a0 = 0, a1 = 0, a2 = 0, a3 = 0, a4 = 0, a5 = 0, a6 = 0, a7 = 0, a8 = 0, a9 = 0, a10 = 0, a11 = 0, a12 = 0, a13 = 0, a14 = 0, any2 = 0;
     const int w1 = (x1 - 1) >> 5;
 #pragma unroll 1
     for (int w = x0 >> 5; w <= w1; ++w) {
@@ -181,8 +181,13 @@ struct Tia {
       const uint32_t *o = &smem[(S_OBJ + w) * BLOCK + sl];
       const uint32_t PF = o[0] & act, BL = o[5 * BLOCK] & act, P0 = o[10 * BLOCK] & act, P1 = o[15 * BLOCK] & act,
                      M0 = o[20 * BLOCK] & act, M1 = o[25 * BLOCK] & act;
-      a0 |= M0 & P1; a1 |= M0 & P0; a2 |= M1 & P0; a3 |= M1 & P1; a4 |= P0 & PF; a5 |= P0 & BL; a6 |= P1 & PF; a7 |= P1 & BL;
-      a8 |= M0 & PF; a9 |= M0 & BL; a10 |= M1 & PF; a11 |= M1 & BL; a12 |= BL & PF; a13 |= P0 & P1; a14 |= M0 & M1;
+      uint32_t ones = PF | BL, twos = PF & BL;                    // pixels where two or more objects are lit: no such pixel
+      twos |= ones & P0; ones |= P0; twos |= ones & P1; ones |= P1; twos |= ones & M0; ones |= M0; twos |= ones & M1;   // in the word, no pair to look at
+      if (twos) {
+        any2 = 1;
+        a0 |= M0 & P1; a1 |= M0 & P0; a2 |= M1 & P0; a3 |= M1 & P1; a4 |= P0 & PF; a5 |= P0 & BL; a6 |= P1 & PF; a7 |= P1 & BL;
+        a8 |= M0 & PF; a9 |= M0 & BL; a10 |= M1 & PF; a11 |= M1 & BL; a12 |= BL & PF; a13 |= P0 & P1; a14 |= M0 & M1;
+      }
       if (vis) {                                                   // priority -> colour index 0 P0, 1 P1, 2 PF, 3 BK
         uint32_t o0 = P0 | M0, o1 = P1 | M1, e0, e1, ef;
         const uint32_t of = PF | BL;
@@ -200,6 +205,7 @@ struct Tia {
         pl[5 * BLOCK] = (pl[5 * BLOCK] & ~rm) | ((ef | eb) & rm);
       }
     }
+    if (!any2) return;
     uint32_t c = 0;
     c |= a0 ? 1u << CX_M0P1 : 0; c |= a1 ? 1u << CX_M0P0 : 0; c |= a2 ? 1u << CX_M1P0 : 0; c |= a3 ? 1u << CX_M1P1 : 0;
     c |= a4 ? 1u << CX_P0PF : 0; c |= a5 ? 1u << CX_P0BL : 0; c |= a6 ? 1u << CX_P1PF : 0; c |= a7 ? 1u << CX_P1BL : 0;
