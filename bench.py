@@ -109,6 +109,37 @@ class ClockSampler(threading.Thread):
                 "power_w_max": max(float(r[2]) for r in self.rows), "samples": len(self.rows)}
 
 
+def run_paper_axis(args):
+    """Instructions per second of 3,000-instruction rollouts over the batch size (the axis of PAPER.md Table 7)."""
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    from paper_2606_22447_b200 import VCS
+    from vcs_inputs import make_workload
+    torch.cuda.set_device(0)
+    rows = []
+    for n in (1, 16, 64, 256, 1024, 4096, 16384, 65536):
+        w = make_workload(2, batch=n)
+        env = VCS(w.roms, w.seeds, w.env_rom)
+        acts = torch.from_numpy(w.actions(0, 16)).cuda()
+        for t in range(3):
+            env.step_instructions(acts[t], 3000)                   # warm-up rollouts
+        torch.cuda.synchronize()
+        reps = 10
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(reps + 1)]
+        ev[0].record()
+        for t in range(reps):
+            env.step_instructions(acts[3 + t], 3000); ev[t + 1].record()
+        torch.cuda.synchronize()
+        ms = np.array([ev[i].elapsed_time(ev[i + 1]) for i in range(reps)])
+        rows.append({"N": n, "ms_per_rollout_mean": float(ms.mean()), "ms_sd": float(ms.std()),
+                     "instructions_per_s": n * 3000 / (float(ms.mean()) * 1e-3)})
+        env.close()
+    print(json.dumps({"metric": "emulated CPU instructions/s, 3,000-instruction rollouts (PAPER.md Table 7 axis)", "unit": "instructions/s",
+                      "mode": "hard (integer) mode, vcs_step_instructions; the paper's rows are float32 soft mode on a GTX 1080 Ti with the Pong ROM",
+                      "workload": "config 2: N envs sharing one seeded 4K ROM, per-env random actions", "rows": rows}), flush=True)
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -159,6 +190,9 @@ def main():
                          "axis of the paper's Table 7, SURVEY §8(f) NEXT-2)")
     ap.add_argument("--soft-T", type=float, default=None,
                     help="run vcs_step_soft (SOFT-STE forward, BASELINE config 5: --workload 2 --batch 4096) at this temperature")
+    ap.add_argument("--paper-axis", action="store_true",
+                    help="the paper's own throughput axis (PAPER.md Table 7, L566-576; L582 one step = one CPU instruction): "
+                         "3,000-instruction rollouts (vcs_step_instructions) of one shared 4K ROM at N in {1, 16, ..., 65536}; prints a table line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -166,6 +200,8 @@ def main():
         args.no_e2e = True
     if args.impl == "reference":
         return run_reference(args)
+    if args.paper_axis:
+        return run_paper_axis(args)
 
     import torch
     import torch.distributed as dist

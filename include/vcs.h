@@ -103,6 +103,16 @@ int vcs_step(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, void *cuda_
  * episode starts; errors as vcs_step. */
 int vcs_step_masked(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, const uint8_t *mask_dev, void *cuda_stream);
 
+/* The paper's own step unit ("one step = one CPU instruction"; Table 8 "rollout length 3,000 CPU
+ * instructions"): latch the actions as vcs_step does, then execute exactly n_instr whole
+ * instructions per env (1 <= n_instr <= 1,000,000).  Frames end on the way as they would in vcs_step (VSYNC 1->0 or the
+ * cap; a frame end at the cap is not an instruction) and are counted in vcs_regs.frame; a halted env (status bit 0)
+ * spends one idle CPU cycle per instruction.  CPU, RAM, RIOT and TIA state (collision latches, positions, beam) after
+ * the call are those of the oracle after the same n_instr single-instruction steps.  The FRONT SCREEN IS NOT UPDATED:
+ * rows are produced by vcs_step only, and the first frame a following vcs_step completes may lack the rows this call
+ * ran through (with frameskip >= 2 the frame vcs_step shows lies wholly inside that call).  Errors as vcs_step. */
+int vcs_step_instructions(vcs_t h, const uint8_t *actions_dev, int32_t n_instr, void *cuda_stream);
+
 /* Console switches (SURVEY.md §8(f) NEXT-4 "console switches as inputs"; C.7 port B): switches_dev[e] (DEVICE
  * uint8[batch], copied) is the level of the SWCHB input pins of env e — bit 0 RESET and bit 1 SELECT (0 = pressed),
  * bit 3 colour (1) / b&w (0), bits 6 / 7 difficulty P0 / P1; pins 2, 4 and 5 are not connected and always read 1.

@@ -72,6 +72,8 @@ int  ovcs_step_masked_range(ovcs_t *h, const uint8_t *actions, int32_t frameskip
 int  ovcs_set_switches(ovcs_t *h, const uint8_t *switches /* [batch] SWCHB pins, NULL = 0x3F */);
 int  ovcs_boot(ovcs_t *h, const uint8_t *mask, int32_t noop_frames, int32_t reset_frames, const uint8_t *noop_starts,
                int32_t max_noop_starts, int32_t frameskip);
+/* the paper's step unit: latch the actions, then n_instr single-instruction steps (ovcs_step_instruction) per env of [lo,hi) */
+int  ovcs_step_instructions_range(ovcs_t *h, const uint8_t *actions, int32_t n_instr, int32_t lo, int32_t hi);
 int  ovcs_get_ram(ovcs_t *h, uint8_t *out /* [batch][128] */);
 int  ovcs_get_regs(ovcs_t *h, ovcs_regs *out /* [batch] */);
 int  ovcs_get_screen(ovcs_t *h, uint8_t *out /* [batch][210][160] */);

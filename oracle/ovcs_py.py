@@ -64,6 +64,7 @@ def lib():
         L.ovcs_set_switches.argtypes = [P, P]
         L.ovcs_boot.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, C.c_int32]
         L.ovcs_step_range.argtypes = [P, P, C.c_int32, C.c_int32, C.c_int32]
+        L.ovcs_step_instructions_range.argtypes = [P, P, C.c_int32, C.c_int32, C.c_int32]
         for f in ("ovcs_get_ram", "ovcs_get_regs", "ovcs_get_screen"):
             getattr(L, f).argtypes = [P, P]
         L.ovcs_destroy.argtypes = [P]
@@ -132,6 +133,16 @@ class OracleVCS:
         cuts = [self.batch * i // n for i in range(n + 1)]
         with ThreadPoolExecutor(n) as ex:
             rcs = list(ex.map(lambda i: lib().ovcs_step_range(self.h, a.ctypes.data, frameskip, cuts[i], cuts[i + 1]), range(n)))
+        assert all(rc == 0 for rc in rcs)
+
+    def step_instructions(self, actions, n_instr, threads=1):
+        """latch the actions, then n_instr single-instruction steps per env (the paper's step unit)"""
+        a = np.ascontiguousarray(actions, dtype=np.uint8)
+        assert a.shape == (self.batch,)
+        n = max(1, min(threads, self.batch))
+        cuts = [self.batch * i // n for i in range(n + 1)]
+        with ThreadPoolExecutor(n) as ex:
+            rcs = list(ex.map(lambda i: lib().ovcs_step_instructions_range(self.h, a.ctypes.data, int(n_instr), cuts[i], cuts[i + 1]), range(n)))
         assert all(rc == 0 for rc in rcs)
 
     @staticmethod

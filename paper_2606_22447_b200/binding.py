@@ -20,7 +20,7 @@ VCS_F_NO_SPIN, VCS_F_NO_FUSE, VCS_F_NO_REGROUP, VCS_F_ROM_GLOBAL, VCS_F_NO_BALAN
 VCS_F_BLOCK_64, VCS_F_BLOCK_128, VCS_F_BLOCK_256 = 1 << 8, 2 << 8, 3 << 8
 _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
 
-EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
+EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_instructions", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
            "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_block_times", "vcs_launch_count",
            "vcs_optable", "vcs_issue_peak", "vcs_destroy", "vcs_last_error"]
 
@@ -59,6 +59,7 @@ def load_library() -> C.CDLL:
     L.vcs_reset.argtypes = [P, P, P]
     L.vcs_step.argtypes = [P, P, C.c_int32, P]
     L.vcs_step_host.argtypes = [P, P, C.c_int32, P]
+    L.vcs_step_instructions.argtypes = [P, P, C.c_int32, P]
     L.vcs_step_masked.argtypes = [P, P, C.c_int32, P, P]
     L.vcs_set_switches.argtypes = [P, P, P]
     L.vcs_boot.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, C.c_int32, P]
@@ -152,6 +153,11 @@ class VCS:
     def step(self, actions, frameskip=4, stream=None):
         assert actions.is_cuda and actions.dtype == self.torch.uint8 and actions.numel() == self.batch and actions.is_contiguous()
         self._chk(self.L.vcs_step(self.h, actions.data_ptr(), int(frameskip), _stream_ptr(stream)), "vcs_step")
+
+    def step_instructions(self, actions, n_instr, stream=None):
+        """vcs_step_instructions: exactly n_instr CPU instructions per env (the paper's step unit); the screen is not updated."""
+        assert actions.is_cuda and actions.dtype == self.torch.uint8 and actions.numel() == self.batch and actions.is_contiguous()
+        self._chk(self.L.vcs_step_instructions(self.h, actions.data_ptr(), int(n_instr), _stream_ptr(stream)), "vcs_step_instructions")
 
     def _u8(self, x, what):
         if x is None:

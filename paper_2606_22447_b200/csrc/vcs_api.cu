@@ -124,7 +124,7 @@ StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
   p.actions = actions; p.switches = h->d_switches; p.mask = nullptr; p.boot = h->d_boot_ctr; p.perm = h->d_perm; p.blk_time = nullptr; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
   p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom;
-  p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0;
+  p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0; p.n_instr = 0;
   return p;
 }
 
@@ -188,7 +188,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   h->regroup = (c.flags & VCS_F_NO_REGROUP) ? 0 : 1;
   // pre-decode every byte offset of every bank once (vcs_decode.cuh); the words depend on the launch shape
   // (zero-page RAM operands are stored as shared-memory offsets)
-  std::vector<DWord> dw(dwords + 8, DWord{0, 0});
+  std::vector<DWord> dw(dwords + 8, DWord{0, 0}), dwp(dwords + 8, DWord{0, 0});      // dwp: the plain table of vcs_step_instructions
   {
     std::vector<uint8_t> img(4096 + 4, 0), leader(4096);
     for (int r = 0; r < n_roms; ++r) {
@@ -201,7 +201,8 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
           if (pass == 0) mark_leaders(img.data(), leader.data());
           else { decode_bank(img.data(), leader.data(), h->block, nb, dw.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE));
                  if (!(c.flags & VCS_F_NO_SPIN)) mark_spins(img.data(), dw.data() + meta[r].doff + 4096 * b);
-                 if (!(c.flags & VCS_F_NO_FUSE)) fuse_ld_st(dw.data() + meta[r].doff + 4096 * b); }
+                 if (!(c.flags & VCS_F_NO_FUSE)) fuse_ld_st(dw.data() + meta[r].doff + 4096 * b);
+                 decode_bank(img.data(), leader.data(), 128, nb, dwp.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE)); }
         }
     }
   }
@@ -214,6 +215,8 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   CU(h, cudaMalloc((void **)&h->d_rom_blob, blob));
   CU(h, cudaMalloc((void **)&h->d_drom, sizeof(DWord) * dw.size()));
   CU(h, cudaMemcpy(h->d_drom, dw.data(), sizeof(DWord) * dw.size(), cudaMemcpyHostToDevice));
+  CU(h, cudaMalloc((void **)&h->d_drom_plain, sizeof(DWord) * dwp.size()));
+  CU(h, cudaMemcpy(h->d_drom_plain, dwp.data(), sizeof(DWord) * dwp.size(), cudaMemcpyHostToDevice));
   CU(h, cudaMalloc((void **)&h->d_rom_meta, sizeof(RomMeta) * n_roms));
   CU(h, cudaMalloc((void **)&h->d_env_rom, sizeof(int32_t) * B));
   CU(h, cudaMalloc((void **)&h->d_seeds, sizeof(unsigned long long) * B));
@@ -300,6 +303,18 @@ int vcs_step_masked(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, cons
   cudaError_t ce = launch_step(p, (cudaStream_t)cuda_stream);
   h->launches += 1;
   if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_masked launch", ce);
+  return VCS_OK;
+}
+
+int vcs_step_instructions(vcs_t h, const uint8_t *actions_dev, int32_t n_instr, void *cuda_stream) {
+  DEV_OK(h);
+  if (!actions_dev) return fail(h, VCS_EINVAL, "vcs_step_instructions: actions_dev is NULL");
+  if (n_instr < 1 || n_instr > 1000000) return fail(h, VCS_EINVAL, "vcs_step_instructions: n_instr out of range (1 .. 1,000,000)");
+  StepParams p = params_of(h, actions_dev, 0x7FFFFFF0);   // (no frame count ends this step, and no frame of it is the "last" one)
+  p.n_instr = n_instr; p.drom = h->d_drom_plain; p.perm = nullptr; p.regroup = 0;
+  cudaError_t ce = launch_step(p, (cudaStream_t)cuda_stream);
+  h->launches += 1;
+  if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_instructions launch", ce);
   return VCS_OK;
 }
 
@@ -475,7 +490,7 @@ int vcs_destroy(vcs_t h) {
   int cur = -1; cudaGetDevice(&cur);
   if (cur != h->device) cudaSetDevice(h->device);     // free on the handle's own device, then give the caller's back
   cudaDeviceSynchronize();
-  cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom);
+  cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom); cudaFree(h->d_drom_plain);
   cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr); cudaFree(h->d_perm); cudaFree(h->d_blk_time); cudaFree(h->d_w_avg);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   if (h->h_soft_w) cudaFreeHost(h->h_soft_w);

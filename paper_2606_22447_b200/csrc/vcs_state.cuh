@@ -64,6 +64,7 @@ enum : uint32_t { STATUS_ILLEGAL = 1, STATUS_CAP = 2 };
 enum SmWord {
   S_RAM = 0,                       // 32 words: the 128 RAM bytes
   S_PLANE = 32,                    // 10 words: colour-index bit planes of the scanline in progress (i0[5], i1[5])
+  S_BUDGET = 32,                   // vcs_step_instructions only (it keeps no rows, so the planes are free): instructions left to run
   S_COLU = 42, S_PF, S_GRP, S_NUSIZ, S_POS, S_POS2,   // TIA registers, packed as the W_* words (S_POS2 without rx)
   S_CX, S_FL, S_RX, S_PX,          // collision latches, flags, clocks rendered, pixels painted of the current line
   S_LINE, S_FDONE,                 // scanline in frame, frames completed in this step
@@ -94,6 +95,7 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   int device;                   // the CUDA device every pointer below belongs to
   float *h_soft_w; cudaEvent_t soft_w_done; int soft_K;            // soft mode: pinned e^{-k/T} staging buffer, its upload, window of the cached temperature
   float *d_soft_tab; float soft_tab_T; size_t soft_tab_n;          // W(T) x ROM: the relaxed read of every ROM cell at the cached temperature
+  uint2 *d_drom_plain;          // vcs_step_instructions: a decode table for 128-env blocks without fused / closed-form entries (one entry = one instruction)
   uint2 *d_drom_soft; RomMeta *d_rom_meta_soft; float *d_soft_w;   // soft mode: an all-H_SLOW decode table (every byte fetched at run time), metas with doff 0, e^{-k/T}
   uint8_t *d_actions_stage;     // for vcs_step_host
   uint8_t *d_switches;          // SWCHB input pins per env (vcs_set_switches; 0x3F after vcs_create)

@@ -427,6 +427,9 @@ struct Cpu {
   // ---------------------------------------------------------------- the checks ahead of an instruction (C.4, C.10)
   // entered when cyc >= lim.  Returns false when no instruction may run now (a frame ended at the cap, or
   // the CPU is halted and idled): the lane goes back to the scheduling point.
+  // COUNT (vcs_step_instructions): the lane runs on an instruction budget (smem word S_BUDGET); a halted CPU spends one
+  // idle cycle per unit of it, as the oracle's single-instruction step does.
+  template <bool COUNT = false>
   DEV bool slow_pre() {
     if (cyc - lstart > LINE_CYC) { T::line_end(sl); lstart += LINE_CYC; wsync = false; }     // the previous instruction ran over the line end
     if (cyc - fstart >= cap) {                             // frame cap at the instruction boundary
@@ -435,7 +438,9 @@ struct Cpu {
     }
     if (cyc - lstart >= LINE_CYC) { T::line_end(sl); lstart += LINE_CYC; wsync = false; }     // n == 76 exactly
     if (status & STATUS_ILLEGAL) {                         // halted: idle cycles to the line end / the cap
-      cyc += min(LINE_CYC - (cyc - lstart), cap - (cyc - fstart));
+      int32_t m = min(LINE_CYC - (cyc - lstart), cap - (cyc - fstart));
+      if constexpr (COUNT) { m = min(m, (int32_t)S(S_BUDGET)); S(S_BUDGET) -= (uint32_t)m; }
+      cyc += m;
       return false;
     }
     if (wsync) {                                           // a12: RDY holds the CPU until the line ends
@@ -845,10 +850,10 @@ __device__ __noinline__ Hot cold_exec(Hot h, uint32_t sl, uint32_t cx, uint32_t 
   if (c.template exec_one<false>((cx & 0xFFFFFF80u) | ((cx & 0x7Fu) - HC_COLD), pl)) { h.aux = AUX_GENERIC; return h; }
   return c.store();
 }
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT, bool COUNT = false>
 __device__ __noinline__ Hot cold_pre(Hot h, uint32_t sl) {                                   // cyc >= lim: line end, WSYNC, cap, halt
   Cpu<BLOCK, ROMS, THREADS, SOFT> c; c.template load<false>(h, sl);
-  const bool ok = c.slow_pre();
+  const bool ok = c.template slow_pre<COUNT>();
   Hot r = c.store(); r.aux = ok ? 1u : 0u;
   return r;
 }
@@ -893,18 +898,20 @@ DEV uint32_t rom_byte_hot(uint32_t off) {                  // byte `off` (bank <
 
 // ---------------------------------------------------------------------------------------------------------------
 // The inline interpreter loop: instructions of this lane's min-key group until the next scheduling point.
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT, bool COUNT = false>
 DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
   using T = Tia<BLOCK>;
   uint8_t *const ramb = reinterpret_cast<uint8_t *>(smem) + 4u * sl;
   for (;;) {
+    if constexpr (COUNT) { if (T::S(sl, S_BUDGET) == 0) { h.keyhi = 0xFFFFFFFFu; return; } }   // the budget is spent: this lane is done
     if (h.cyc >= h.lim) {
       int32_t nl = LIM_NOW;
       const bool ws = h.lim == LIM_WSYNC;
       if (h.lim != LIM_NOW) nl = line_step<BLOCK>(sl, h.cyc, h.lstart, ws);
       if (nl != LIM_NOW) { h.lstart += LINE_CYC; if (ws) h.cyc = h.lstart; h.lim = nl; }
-      else { h = cold_pre<BLOCK, ROMS, THREADS, SOFT>(h, sl); if (!h.aux) return; }
+      else { h = cold_pre<BLOCK, ROMS, THREADS, SOFT, COUNT>(h, sl); if (!h.aux) return; }
     }
+    if constexpr (COUNT) T::S(sl, S_BUDGET) -= 1u;         // (a frame end at the cap or an idle cycle above is not an instruction)
     uint32_t cx = h.wx, pl = h.wy;                         // the entry being executed
     const int32_t cyc0 = h.cyc;                            // its first cycle
     h.di += (cx >> DW_LEN_SHIFT) & 0xFFu;
@@ -1110,7 +1117,7 @@ DEV void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile("{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @!p bra WAIT_%=;\n}" ::"r"(bar), "r"(parity) : "memory");
 }
 
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT, bool COUNT = false>
 __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepParams p) {
   using T = Tia<BLOCK>;
   __shared__ __align__(8) unsigned long long s_bar;
@@ -1172,6 +1179,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     T::S(sl, S_PX) = 0; T::S(sl, S_FDONE) = 0;
     for (int i = 0; i < 32; ++i) smem[(S_RAM + i) * BLOCK + tid] = p.ram[i * B + ei];
     for (int i = 0; i < 10; ++i) smem[(S_PLANE + i) * BLOCK + tid] = 0;
+    if constexpr (COUNT) T::S(sl, S_BUDGET) = (uint32_t)p.n_instr;        // (no row is kept in this mode: the planes are free)
     if (p.frameskip == 1) { fl |= TF_STORING; if ((T::S(sl, S_LINE) - (uint32_t)p.y0) < (uint32_t)SCR_H) fl |= TF_ROWVIS; }
   } else {
     s.A = s.X = s.Y = s.SP = 0; s.unpack_p(0x24); s.status = 0; s.fstart = 0;
@@ -1227,7 +1235,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
       const uint32_t key = h.keyhi | ((h.pbase + h.di) & 0xFFFFu);
       const uint32_t mk = __reduce_min_sync(0xFFFFFFFFu, key);
       if (mk >= KEY_PARKED) break;                         // every lane is parked or has finished the step
-      if (key == mk) run_block<BLOCK, ROMS, THREADS, SOFT>(h, dr, cur);
+      if (key == mk) run_block<BLOCK, ROMS, THREADS, SOFT, COUNT>(h, dr, cur);
       if (h.aux == AUX_GENERIC) h = cold_exec_generic<BLOCK, ROMS, THREADS, SOFT>(h, cur, h.wx, h.wy);   // (a rare bus pattern: see cold_exec)
     }
     if (!regroups) break;
@@ -1381,22 +1389,24 @@ size_t step_smem_bytes(int block, bool roms, uint32_t max_rom) {
   return (size_t)(S_WORDS * block + C_WORDS) * 4 + (roms ? (max_rom < 4096 ? 4096 : max_rom) + 16 : 0);
 }
 
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
+template <int BLOCK, bool ROMS, int THREADS, bool SOFT, bool COUNT = false>
 static cudaError_t launch_one(const StepParams &p, cudaStream_t stream) {
   const size_t smem_bytes = step_smem_bytes(BLOCK, ROMS, p.max_rom);
   static size_t configured[64] = {0};                   // per device: the attribute belongs to the (function, device) pair
   int dev = 0; cudaGetDevice(&dev);
   if (dev < 0 || dev >= 64 || configured[dev] < smem_bytes) {
-    cudaError_t e = cudaFuncSetAttribute(vcs_step_kernel<BLOCK, ROMS, THREADS, SOFT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    cudaError_t e = cudaFuncSetAttribute(vcs_step_kernel<BLOCK, ROMS, THREADS, SOFT, COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
     if (dev >= 0 && dev < 64) configured[dev] = smem_bytes;
   }
   const int grid = (p.batch + BLOCK - 1) / BLOCK;
-  vcs_step_kernel<BLOCK, ROMS, THREADS, SOFT><<<grid, THREADS, smem_bytes, stream>>>(p);
+  vcs_step_kernel<BLOCK, ROMS, THREADS, SOFT, COUNT><<<grid, THREADS, smem_bytes, stream>>>(p);
   return cudaGetLastError();
 }
 
 cudaError_t launch_step(const StepParams &p, cudaStream_t stream) {
+  if (p.n_instr > 0)                                       // vcs_step_instructions: one variant (128 envs per block, ROM through the read-only path)
+    return launch_one<128, false, 128, false, true>(p, stream);
   if (p.soft_out)                                          // SOFT-STE mode: one variant (ROM through the read-only path, no regroup)
     return launch_one<128, false, 128, true>(p, stream);
   if (p.rom_smem && p.regroup && p.max_rom == 8192) {      // F8 carts present: one spare warp per block for the regroup

@@ -14,6 +14,7 @@ struct StepParams {
   int32_t batch, frameskip, y0, max_lines;
   const float *soft_w; const float *soft_tab; float *soft_out; float soft_alpha; int32_t soft_K;   // soft_out != nullptr: SOFT-STE mode (vcs_step_soft)
   int32_t block, rom_smem, regroup; uint32_t max_rom;     // launch shape: envs per block (64/128/256), ROM staged in smem, largest image
+  int32_t n_instr;                                        // > 0: vcs_step_instructions — run this many instructions per env instead of `frameskip` frames
 };
 
 void upload_optable();

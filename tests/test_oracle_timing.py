@@ -160,3 +160,19 @@ def test_halted_env_idles_to_the_cap():
     o = oracle_for(build, max_lines=50)
     o.step(np.zeros(1, np.uint8), 3)
     r = regs(o); assert r["status"] == 3 and r["frame"] == 3 and r["pc"] == 0xF000 and r["cycles"] == 3 * 3800
+
+
+def test_step_instructions_is_n_single_instruction_steps():
+    """SURVEY §8(f) NEXT-2 / PAPER.md L582: n instructions of a NOP sled are 2n cycles and n bytes of PC; a WSYNC stall
+    belongs to the instruction that follows it; the call latches the action first."""
+    def build(a):
+        a.org(0xF000)
+        for _ in range(20): a.op("NOP")
+        a.op("STA", "zp", TIA_W["WSYNC"]); a.op("LDA", "abs", RIOT["SWCHA"]); a.op("STA", "zp", 0x80)
+    o = oracle_for(build)
+    o.step_instructions(np.array([3], np.uint8), 7)                  # RIGHT
+    r = regs(o); assert r["cycles"] == 14 and r["pc"] == 0xF007
+    o.step_instructions(np.array([3], np.uint8), 14)                 # 13 NOPs + STA WSYNC (3 cycles, written in cycle 42)
+    r = regs(o); assert r["cycles"] == 14 + 26 + 3 and r["pc"] == 0xF016
+    o.step_instructions(np.array([3], np.uint8), 2)                  # LDA SWCHA waits for the line end first: 76 + 4, then STA 3
+    r = regs(o); assert r["cycles"] == 76 + 4 + 3 and o.ram()[0][0] == 0x7F
