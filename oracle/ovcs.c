@@ -32,6 +32,10 @@ typedef struct {
   uint8_t inpt4_latch, inpt5_latch, fire0;
   /* cart */
   const uint8_t *rom; uint32_t rom_size; uint8_t bank;
+  uint8_t kind;                  /* OVCS_MAP_* (never BY_SIZE) */
+  uint8_t sc_ram[128];           /* Superchip RAM */
+  uint8_t seg[3];                /* E0: slices shown at $1000, $1400, $1800 */
+  uint8_t fe_pending;            /* FE: the previous access was to $01FE */
   uint64_t seed;
   uint64_t n_instr, n_tia_writes;    /* instrumentation only (bench work model); never read by the model */
   uint8_t *back, *front;
@@ -52,18 +56,36 @@ uint64_t ovcs_splitmix64(uint64_t *s) {
 }
 
 /* ------------------------------------------------------------- C.9 cartridge */
-static void cart_hotspot(env_t *e, uint16_t a) {          /* any bus access, a = addr&0x1FFF */
-  if (e->rom_size == 8192) { if (a == 0x1FF8) e->bank = 0; else if (a == 0x1FF9) e->bank = 1; }
-  /* SURVEY §8(f) NEXT-3, PAPER.md L69 / L469 (F6, F4 among the implemented formats) [D]: the same scheme with more
-   * banks — F6 (16 KB): $1FF6..$1FF9 select banks 0..3;  F4 (32 KB): $1FF4..$1FFB select banks 0..7. */
-  if (e->rom_size == 16384 && a >= 0x1FF6 && a <= 0x1FF9) e->bank = (uint8_t)(a - 0x1FF6);
-  if (e->rom_size == 32768 && a >= 0x1FF4 && a <= 0x1FFB) e->bank = (uint8_t)(a - 0x1FF4);
+static int cart_banks(const env_t *e) {          /* 4 KB banks switched by hotspots (0 = none) */
+  switch (e->kind) { case OVCS_MAP_F8: case OVCS_MAP_F8SC: return 2; case OVCS_MAP_F6: case OVCS_MAP_F6SC: return 4;
+                     case OVCS_MAP_F4: case OVCS_MAP_F4SC: return 8; default: return 0; }
+}
+static int cart_has_sc(const env_t *e) { return e->kind == OVCS_MAP_F8SC || e->kind == OVCS_MAP_F6SC || e->kind == OVCS_MAP_F4SC; }
+static void cart_hotspot(env_t *e, uint16_t a) {          /* any bus access, a = addr&0x1FFF with A12 set */
+  /* F8: $1FF8/9 -> bank 0/1 [D]; F6 (16 KB): $1FF6..$1FF9 -> banks 0..3; F4 (32 KB): $1FF4..$1FFB -> banks 0..7
+   * (PAPER.md L61, L69, L469); the Superchip variants switch the same way */
+  int nb = cart_banks(e);
+  if (nb) { uint16_t lo = (uint16_t)(nb == 8 ? 0x1FF4 : 0x1FFA - nb); if (a >= lo && a < lo + nb) e->bank = (uint8_t)(a - lo); }
+  /* E0 [D]: $1FE0-7 choose the slice of the $1000 window, $1FE8-F of $1400, $1FF0-7 of $1800 */
+  if (e->kind == OVCS_MAP_E0 && a >= 0x1FE0 && a <= 0x1FF7) e->seg[(a - 0x1FE0) >> 3] = (uint8_t)(a & 7);
 }
 static uint8_t cart_peek(const env_t *e, uint16_t a) {
   uint32_t o = a & 0x0FFF;
-  if (e->rom_size == 2048) return e->rom[o & 0x7FF];
-  if (e->rom_size == 4096) return e->rom[o];
-  return e->rom[(uint32_t)e->bank * 4096u + o];
+  if (cart_has_sc(e) && o < 0x100) return e->sc_ram[o & 0x7F];   /* read port $1080-$10FF; a read of the write port sees the cell too, unchanged [R] */
+  if (e->kind == OVCS_MAP_2K) return e->rom[o & 0x7FF];
+  if (e->kind == OVCS_MAP_4K) return e->rom[o];
+  if (e->kind == OVCS_MAP_E0) { uint32_t w = o >> 10, slice = (w == 3) ? 7u : e->seg[w]; return e->rom[slice * 1024u + (o & 0x3FF)]; }
+  return e->rom[(uint32_t)e->bank * 4096u + o];                   /* F8 / F6 / F4 (+SC), FE */
+}
+static void cart_poke(env_t *e, uint16_t a, uint8_t v) {          /* a write cycle in cartridge space (after the hotspot check) */
+  if (cart_has_sc(e) && (a & 0x0F80) == 0) e->sc_ram[a & 0x7F] = v;   /* write port $1000-$107F [D] */
+}
+/* FE [D]: the board watches the bus for $01FE (the stack cell JSR / RTS touch last / first); the data of the access that
+ * FOLLOWS it carries the high byte of the new PC, and its bit 5 tells the $F000 page (bank 0) from the $D000 page (bank 1) */
+static void fe_snoop(env_t *e, uint16_t a, uint8_t data) {
+  if (e->kind != OVCS_MAP_FE) return;
+  if (e->fe_pending) { e->bank = (data & 0x20) ? 0 : 1; e->fe_pending = 0; }
+  if (a == 0x01FE) e->fe_pending = 1;
 }
 
 /* ------------------------------------------------------------------ C.7 RIOT */
@@ -278,24 +300,27 @@ static uint8_t soft_ram(ctx_t *c, int cell, uint8_t v) { return osoft_ram_read((
 
 /* C.3 address decode + the access itself (post-tick) */
 static uint8_t bus_read(ctx_t *c, uint16_t addr) {
-  env_t *e = c->e; uint16_t a = addr & 0x1FFF;
+  env_t *e = c->e; uint16_t a = addr & 0x1FFF; uint8_t v;
   while (e->wsync && (e->cyc % LINE_CYC) != 0) tick(c);   /* RDY halts read cycles only [D] */
   tick(c);
   const int dummy = c->dummy; c->dummy = 0;                /* set by DUMMY_READ: a cycle whose value is discarded */
-  if (a & 0x1000) { cart_hotspot(e, a); uint8_t v = cart_peek(e, a); return (c->soft && !dummy) ? soft_rom(c, a, v) : v; }
-  if ((a & 0x0080) == 0) return tia_read(e, a);
-  if ((a & 0x0200) == 0) { uint8_t v = e->ram[a & 0x7F]; return (c->soft && !dummy) ? soft_ram(c, a & 0x7F, v) : v; }
-  return riot_read(e, a);
+  if (a & 0x1000) { cart_hotspot(e, a); v = cart_peek(e, a); if (c->soft && !dummy && !(cart_has_sc(e) && (a & 0xF00) == 0)) v = soft_rom(c, a, v); }
+  else if ((a & 0x0080) == 0) v = tia_read(e, a);
+  else if ((a & 0x0200) == 0) { v = e->ram[a & 0x7F]; if (c->soft && !dummy) v = soft_ram(c, a & 0x7F, v); }
+  else v = riot_read(e, a);
+  fe_snoop(e, a, v);
+  return v;
 }
 #define DUMMY_READ(c, addr) ((c)->dummy = 1, (void)bus_read((c), (addr)))
 static void bus_write(ctx_t *c, uint16_t addr, uint8_t v) {
   env_t *e = c->e; uint16_t a = addr & 0x1FFF;
   tick(c);
   int n = (int)((e->cyc - 1) % LINE_CYC);
-  if (a & 0x1000) { cart_hotspot(e, a); return; }
-  if ((a & 0x0080) == 0) { e->n_tia_writes++; tia_write(e, a, v, n); return; }
-  if ((a & 0x0200) == 0) { e->ram[a & 0x7F] = v; return; }
-  riot_write(e, a, v);
+  if (a & 0x1000) { cart_hotspot(e, a); cart_poke(e, a, v); }
+  else if ((a & 0x0080) == 0) { e->n_tia_writes++; tia_write(e, a, v, n); }
+  else if ((a & 0x0200) == 0) e->ram[a & 0x7F] = v;
+  else riot_write(e, a, v);
+  fe_snoop(e, a, v);
 }
 
 #include "ovcs_cpu.inc"   /* C.5/C.6: the 6507 */

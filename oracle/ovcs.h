@@ -31,7 +31,21 @@ extern "C" {
 
 typedef struct ovcs_s ovcs_t;
 
-typedef struct { const uint8_t *data; uint32_t size; /* 2048 | 4096 | 8192 (F8) | 16384 (F6) | 32768 (F4) */ } ovcs_rom;
+/* Cartridge formats ("cartridge mappers", L469: 2K, 4K, F8, F6, F4, F8SC, F6SC, F4SC, E0, FE; SURVEY C.9 and
+ * §8(f) NEXT-3; behaviour per the public documentation of these boards [D], power-up states [R], R15-R17):
+ *   2K / 4K        no switching (2K mirrored)
+ *   F8 / F6 / F4   2 / 4 / 8 banks of 4 KB; any access to $1FF8-9 / $1FF6-9 / $1FF4-B selects the bank before data returns
+ *   ..SC           the same plus 128 bytes of cartridge RAM in every bank: write port $1000-$107F, read port $1080-$10FF
+ *   E0             eight 1 KB slices; windows $1000 / $1400 / $1800 show the slice chosen by any access to
+ *                  $1FE0-7 / $1FE8-F / $1FF0-7, window $1C00 always shows slice 7
+ *   FE             two 4 KB banks; the access after one to $01FE selects the bank from bit 5 of its data (1: bank 0)
+ * OVCS_MAP_BY_SIZE picks 2K / 4K / F8 / F6 / F4 from the image size. */
+enum { OVCS_MAP_BY_SIZE = 0, OVCS_MAP_2K, OVCS_MAP_4K, OVCS_MAP_F8, OVCS_MAP_F6, OVCS_MAP_F4, OVCS_MAP_F8SC, OVCS_MAP_F6SC, OVCS_MAP_F4SC,
+       OVCS_MAP_E0, OVCS_MAP_FE, OVCS_MAP_COUNT };
+typedef struct { const uint8_t *data; uint32_t size; /* 2048 | 4096 | 8192 | 16384 | 32768 */ uint32_t mapper; /* OVCS_MAP_* */ } ovcs_rom;
+/* content-based format guess from size and image bytes (PAPER.md L69 / L469 "mapper auto-detected"; the rules are this
+ * build's reading R17 in DESIGN.md): returns OVCS_MAP_2K .. OVCS_MAP_FE, or -1 for a size no format has */
+int  ovcs_detect_mapper(const uint8_t *data, uint32_t size);
 typedef struct { int32_t y0, max_lines, f8_start_bank; uint32_t flags; } ovcs_config;
 
 /* Same 32-byte record as include/vcs.h's vcs_regs; retyped, not shared. */
@@ -42,7 +56,7 @@ typedef struct {
   uint8_t bank;
   uint16_t line; uint8_t cyc_in_line;
   uint8_t status;            /* bit0 illegal-opcode halt, bit1 frame cap was hit */
-  uint8_t intim, timint, pad[6];
+  uint8_t intim, timint, pad[6];   /* pad[0]: E0 — slice in the $1800 window (bank = slice@$1000 | slice@$1400 << 3); FE — 1 while an access to $01FE awaits its successor */
 } ovcs_regs;
 
 /* Debug view of the TIA/RIOT latches, for the hand-program pins (tests only). */
@@ -75,6 +89,7 @@ int  ovcs_boot(ovcs_t *h, const uint8_t *mask, int32_t noop_frames, int32_t rese
 /* the paper's step unit: latch the actions, then n_instr single-instruction steps (ovcs_step_instruction) per env of [lo,hi) */
 int  ovcs_step_instructions_range(ovcs_t *h, const uint8_t *actions, int32_t n_instr, int32_t lo, int32_t hi);
 int  ovcs_get_ram(ovcs_t *h, uint8_t *out /* [batch][128] */);
+int  ovcs_get_cart_ram(ovcs_t *h, uint8_t *out /* [batch][128]: the Superchip RAM (zeros for carts without) */);
 int  ovcs_get_regs(ovcs_t *h, ovcs_regs *out /* [batch] */);
 int  ovcs_get_screen(ovcs_t *h, uint8_t *out /* [batch][210][160] */);
 int  ovcs_destroy(ovcs_t *h);

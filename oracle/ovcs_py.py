@@ -27,7 +27,10 @@ def build(force: bool = False) -> str:
 
 
 class Rom(C.Structure):
-    _fields_ = [("data", C.POINTER(C.c_uint8)), ("size", C.c_uint32)]
+    _fields_ = [("data", C.POINTER(C.c_uint8)), ("size", C.c_uint32), ("mapper", C.c_uint32)]
+
+
+MAPPERS = {"": 0, "2K": 1, "4K": 2, "F8": 3, "F6": 4, "F4": 5, "F8SC": 6, "F6SC": 7, "F4SC": 8, "E0": 9, "FE": 10}   # OVCS_MAP_*
 
 
 class Config(C.Structure):
@@ -65,7 +68,8 @@ def lib():
         L.ovcs_boot.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, C.c_int32]
         L.ovcs_step_range.argtypes = [P, P, C.c_int32, C.c_int32, C.c_int32]
         L.ovcs_step_instructions_range.argtypes = [P, P, C.c_int32, C.c_int32, C.c_int32]
-        for f in ("ovcs_get_ram", "ovcs_get_regs", "ovcs_get_screen"):
+        L.ovcs_detect_mapper.argtypes = [P, C.c_uint32]
+        for f in ("ovcs_get_ram", "ovcs_get_regs", "ovcs_get_screen", "ovcs_get_cart_ram"):
             getattr(L, f).argtypes = [P, P]
         L.ovcs_destroy.argtypes = [P]
         L.ovcs_set_action.argtypes = [P, C.c_int32, C.c_int32]
@@ -92,7 +96,7 @@ def lib():
 class OracleVCS:
     """Host-side batch of oracle consoles with the same surface as the CUDA binding."""
 
-    def __init__(self, roms, seeds, env_rom=None, batch=None, y0=34, max_lines=320, f8_start_bank=1):
+    def __init__(self, roms, seeds, env_rom=None, batch=None, y0=34, max_lines=320, f8_start_bank=1, mappers=None):
         L = lib()
         seeds = np.ascontiguousarray(seeds, dtype=np.uint64)
         self.batch = int(batch if batch is not None else len(seeds))
@@ -100,6 +104,7 @@ class OracleVCS:
         arr = (Rom * len(roms))()
         for i, b in enumerate(self._rom_bufs):
             arr[i].data = C.cast(b, C.POINTER(C.c_uint8)); arr[i].size = len(b)
+            arr[i].mapper = 0 if mappers is None else (MAPPERS[mappers[i]] if isinstance(mappers[i], str) else int(mappers[i]))
         er = None if env_rom is None else np.ascontiguousarray(env_rom, dtype=np.int32)
         cfg = Config(y0, max_lines, f8_start_bank, 0)
         self.h = C.c_void_p()
@@ -187,6 +192,9 @@ class OracleVCS:
     def ram(self):
         out = np.empty((self.batch, 128), dtype=np.uint8); assert lib().ovcs_get_ram(self.h, out.ctypes.data) == 0; return out
 
+    def cart_ram(self):
+        out = np.empty((self.batch, 128), dtype=np.uint8); assert lib().ovcs_get_cart_ram(self.h, out.ctypes.data) == 0; return out
+
     def regs(self):
         out = np.empty(self.batch, dtype=REGS_DTYPE); assert lib().ovcs_get_regs(self.h, out.ctypes.data) == 0; return out
 
@@ -207,3 +215,10 @@ class OracleVCS:
         out = np.empty((210, 160), dtype=np.uint8); assert lib().ovcs_get_back(self.h, env, out.ctypes.data) == 0; return out
     def set_cpu(self, env=0, a=-1, x=-1, y=-1, sp=-1, p=-1, pc=-1): assert lib().ovcs_set_cpu(self.h, env, a, x, y, sp, p, pc) == 0
     def poke_ram(self, env, idx, value): assert lib().ovcs_poke_ram(self.h, env, idx, value) == 0
+
+
+def detect_mapper(image: bytes) -> str:
+    """ovcs_detect_mapper as a format name ('' when no format has that size)"""
+    buf = (C.c_uint8 * len(image)).from_buffer_copy(bytes(image))
+    k = lib().ovcs_detect_mapper(C.cast(buf, C.c_void_p), len(image))
+    return {v: n for n, v in MAPPERS.items()}.get(k, "") if k > 0 else ""
