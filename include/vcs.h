@@ -36,12 +36,29 @@ typedef struct vcs_s *vcs_t;
 
 enum { VCS_OK = 0, VCS_EINVAL = -1, VCS_ECUDA = -2, VCS_ENOMEM = -3, VCS_EROM = -4 };
 
-/* One cartridge image (host memory).  size 2048 (2K, mirrored), 4096 (4K), 8192 (F8: any bus access to
- * $1FF8/$1FF9 selects bank 0/1 — SURVEY C.9; "writes to special addresses swap which 4KB ROM page
- * is visible"), 16384 (F6: $1FF6..$1FF9 select banks 0..3) or 32768 (F4: $1FF4..$1FFB select banks 0..7) — PAPER.md
- * L69 / L469, SURVEY §8(f) NEXT-3.  F6 / F4 images power up in bank 0 and are read from global memory (a handle
- * that holds one does not stage ROMs in shared memory and does not regroup F8 blocks: slower, same results). */
-typedef struct { const uint8_t *data; uint32_t size; } vcs_rom;
+/* Cartridge formats ("cartridge mappers", L469: 2K, 4K, F8, F6, F4, F8SC, F6SC, F4SC, E0, FE; SURVEY C.9,
+ * §8(f) NEXT-3; behaviour per the public descriptions of these boards, power-up states are readings R15 / R16 of DESIGN.md):
+ *   2K / 4K        no switching (2K mirrored)
+ *   F8 / F6 / F4   8 / 16 / 32 KB in 4 KB banks; ANY bus access to $1FF8-9 / $1FF6-9 / $1FF4-B selects the bank before the
+ *                  access returns data ("writes to special addresses swap which 4KB ROM page is visible")
+ *   ..SC           the same plus 128 bytes of cartridge (Superchip) RAM in every bank: write port $1000-$107F, read port
+ *                  $1080-$10FF; power-on contents = draws 17-32 of the env's seed stream
+ *   E0             8 KB in 1 KB slices; the windows at $1000 / $1400 / $1800 show the slice chosen by any access to
+ *                  $1FE0-7 / $1FE8-F / $1FF0-7 (power-up: 4, 5, 6), the window at $1C00 always shows slice 7
+ *   FE             8 KB in two banks; the bus access that FOLLOWS one to $01FE selects the bank from bit 5 of its data
+ *                  (1: bank 0 = the $F000 page, 0: bank 1 = the $D000 page); power-up bank 0
+ * VCS_MAP_BY_SIZE (0) takes 2K / 4K / F8 / F6 / F4 from the image size.  F6 / F4 (+SC) images are read from global
+ * memory; Superchip, E0 and FE carts run their out-of-line instructions on the generic executor (slower, same results)
+ * and are not available to vcs_step_soft. */
+enum { VCS_MAP_BY_SIZE = 0, VCS_MAP_2K, VCS_MAP_4K, VCS_MAP_F8, VCS_MAP_F6, VCS_MAP_F4, VCS_MAP_F8SC, VCS_MAP_F6SC, VCS_MAP_F4SC,
+       VCS_MAP_E0, VCS_MAP_FE };
+/* One cartridge image (host memory): size 2048 / 4096 / 8192 / 16384 / 32768 and its format (VCS_MAP_*). */
+typedef struct { const uint8_t *data; uint32_t size; uint32_t mapper; } vcs_rom;
+/* Content-based format guess (PAPER.md L69 / L469 "mapper auto-detected by the ports"; the rules are this build's reading
+ * R17): the size fixes the family; an image whose banks all start with 256 equal bytes is a Superchip one;
+ * among 8 KB images, E0 / FE are told from F8 by the absolute operands of their code ($1FE0-$1FF7 accesses, JSR / JMP into
+ * the $D000 page).  HOST call, no GPU needed.  Returns VCS_MAP_2K .. VCS_MAP_FE, VCS_EROM for a size no format has. */
+int vcs_detect_mapper(const uint8_t *data_host, uint32_t size);
 
 /* y0: scanline shown as screen row 0 (default 34);  max_lines: frame cap in scanlines (default 320, 1..65535) — a
  * frame that has not ended by a VSYNC 1->0 write after max_lines*76 CPU cycles is ended at the next instruction
@@ -73,7 +90,9 @@ typedef struct {
   uint8_t  bank;             /* current cartridge bank                                             */
   uint16_t line; uint8_t cyc_in_line;    /* beam: scanline in frame, cycles % 76                   */
   uint8_t  status;           /* bit0 halt on an unimplemented (undocumented) opcode, bit1 frame cap was hit */
-  uint8_t  intim, timint, _pad[6];       /* timer value and TIMINT bit 7, read without side effects */
+  uint8_t  intim, timint, _pad[6];       /* timer value and TIMINT bit 7, read without side effects.  _pad[0]: E0 — slice shown
+                                            at $1800 (`bank` = slice at $1000 | slice at $1400 << 3); FE — 1 while an access to $01FE
+                                            awaits its successor; 0 otherwise */
 } vcs_regs;
 
 /* Create `batch` consoles.  roms[n_roms], env_rom[batch] (index into roms; NULL = all 0) and
@@ -84,7 +103,7 @@ typedef struct {
  * consecutive envs shares one ROM, the ROM is staged in shared memory per block and F8 carts regroup their envs by
  * bank inside the block; otherwise ROM bytes come through the read-only cache.  cfg->flags (VCS_F_*) overrides these
  * choices; the library reads nothing from the process environment.
- * Errors: VCS_EINVAL (NULL/size/range/unknown flag), VCS_EROM (size not 2048/4096/8192/16384/32768), VCS_ECUDA, VCS_ENOMEM. */
+ * Errors: VCS_EINVAL (NULL/size/range/unknown flag), VCS_EROM (no such format, or the size is not the format's), VCS_ECUDA, VCS_ENOMEM. */
 int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms,
                const int32_t *env_rom, const uint64_t *seeds, const vcs_config *cfg);
 
@@ -162,6 +181,7 @@ int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float 
 /* Copies into caller-owned DEVICE buffers. */
 int vcs_get_ram(vcs_t h, uint8_t *out_dev /* [batch][128] */, void *cuda_stream);
 int vcs_get_regs(vcs_t h, vcs_regs *out_dev /* [batch] */, void *cuda_stream);
+int vcs_get_cart_ram(vcs_t h, uint8_t *out_dev /* [batch][128]: Superchip RAM, zeros for carts without */, void *cuda_stream);
 int vcs_get_screen(vcs_t h, uint8_t *out_dev /* [batch][210][160] */, void *cuda_stream);
 
 /* Convenience for hosts without their own device buffers: vcs_step / vcs_get_* with HOST pointers.

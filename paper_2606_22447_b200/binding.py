@@ -20,7 +20,7 @@ VCS_F_NO_SPIN, VCS_F_NO_FUSE, VCS_F_NO_REGROUP, VCS_F_ROM_GLOBAL, VCS_F_NO_BALAN
 VCS_F_BLOCK_64, VCS_F_BLOCK_128, VCS_F_BLOCK_256 = 1 << 8, 2 << 8, 3 << 8
 _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
 
-EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_instructions", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_step_host",
+EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_instructions", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_cart_ram", "vcs_get_screen", "vcs_detect_mapper", "vcs_step_host",
            "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_block_times", "vcs_launch_count",
            "vcs_optable", "vcs_issue_peak", "vcs_destroy", "vcs_last_error"]
 
@@ -31,7 +31,10 @@ assert REGS_DTYPE.itemsize == 32
 
 
 class VcsRom(C.Structure):
-    _fields_ = [("data", C.POINTER(C.c_uint8)), ("size", C.c_uint32)]
+    _fields_ = [("data", C.POINTER(C.c_uint8)), ("size", C.c_uint32), ("mapper", C.c_uint32)]
+
+
+MAPPERS = {"": 0, "2K": 1, "4K": 2, "F8": 3, "F6": 4, "F4": 5, "F8SC": 6, "F6SC": 7, "F4SC": 8, "E0": 9, "FE": 10}   # VCS_MAP_*
 
 
 class VcsConfig(C.Structure):
@@ -66,7 +69,8 @@ def load_library() -> C.CDLL:
     L.vcs_auto_reset.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, P]
     L.vcs_get_booting.argtypes = [P, P, P]
     L.vcs_step_soft.argtypes = [P, P, C.c_int32, C.c_float, C.c_float, P, P]
-    for f in ("vcs_get_ram", "vcs_get_regs", "vcs_get_screen", "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host"):
+    L.vcs_detect_mapper.argtypes = [P, C.c_uint32]
+    for f in ("vcs_get_ram", "vcs_get_regs", "vcs_get_cart_ram", "vcs_get_screen", "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host"):
         getattr(L, f).argtypes = [P, P, P]
     L.vcs_screen_ptr.argtypes = [P, C.POINTER(P)]
     L.vcs_block_times.argtypes = [P, P, P, C.c_int32, C.POINTER(C.c_int32)]
@@ -77,6 +81,13 @@ def load_library() -> C.CDLL:
     L.vcs_last_error.argtypes = [P]; L.vcs_last_error.restype = C.c_char_p
     _lib = L
     return L
+
+
+def detect_mapper(image: bytes) -> str:
+    """vcs_detect_mapper as a format name (host call; '' when no format has that size)"""
+    buf = (C.c_uint8 * len(image)).from_buffer_copy(bytes(image))
+    k = load_library().vcs_detect_mapper(C.cast(buf, C.c_void_p), len(image))
+    return {v: n for n, v in MAPPERS.items()}.get(k, "") if k > 0 else ""
 
 
 def optable() -> np.ndarray:
@@ -104,7 +115,7 @@ def _stream_ptr(stream) -> int | None:
 class VCS:
     """A batch of consoles on the current CUDA device (vcs_create ... vcs_destroy)."""
 
-    def __init__(self, roms, seeds, env_rom=None, y0=34, max_lines=320, f8_start_bank=1, flags=0):
+    def __init__(self, roms, seeds, env_rom=None, y0=34, max_lines=320, f8_start_bank=1, flags=0, mappers=None):
         import torch
         if not torch.cuda.is_available():
             raise VcsError("no CUDA device: libvcsb200 has no CPU fallback")
@@ -116,6 +127,7 @@ class VCS:
         arr = (VcsRom * len(roms))()
         for i, b in enumerate(bufs):
             arr[i].data = C.cast(b, C.POINTER(C.c_uint8)); arr[i].size = len(b)
+            arr[i].mapper = 0 if mappers is None else (MAPPERS[mappers[i]] if isinstance(mappers[i], str) else int(mappers[i]))
         er = None if env_rom is None else np.ascontiguousarray(env_rom, dtype=np.int32)
         cfg = VcsConfig(y0, max_lines, f8_start_bank, int(flags))
         self.h = C.c_void_p()
@@ -204,6 +216,11 @@ class VCS:
         t = self.torch
         out = t.empty((self.batch, 128), dtype=t.uint8, device=self.device) if out is None else out
         self._chk(self.L.vcs_get_ram(self.h, out.data_ptr(), _stream_ptr(stream)), "vcs_get_ram"); return out
+
+    def get_cart_ram(self, out=None, stream=None):
+        t = self.torch
+        out = t.empty((self.batch, 128), dtype=t.uint8, device=self.device) if out is None else out
+        self._chk(self.L.vcs_get_cart_ram(self.h, out.data_ptr(), _stream_ptr(stream)), "vcs_get_cart_ram"); return out
 
     def get_regs(self, out=None, stream=None):
         t = self.torch

@@ -49,15 +49,17 @@ __global__ void reset_kernel(StepParams p, const unsigned long long *seeds, cons
   const int B = p.batch;
   const RomMeta rm = p.rom_meta[p.env_rom[e]];
   const uint8_t *rom = p.rom_blob + rm.offset;
-  const uint32_t bank = (rm.size == 8192) ? (uint32_t)(f8_start_bank & 1) : 0u;      // F6 / F4 power up in bank 0 (reading R15)
+  const uint32_t bank = (rm.kind == MK_F8 || rm.kind == MK_F8SC) ? (uint32_t)(f8_start_bank & 1) : 0u;      // F6 / F4 / FE power up in bank 0 (readings R15, R16)
   const uint32_t mask_a = (rm.size == 2048) ? 0x7FFu : 0xFFFu;
-  const uint32_t pc = rom[(bank << 12) + (0xFFCu & mask_a)] | ((uint32_t)rom[(bank << 12) + (0xFFDu & mask_a)] << 8);
+  const uint32_t vbank = (rm.kind == MK_E0) ? 1u : bank;                             // E0: $1FFC lies in the fixed window = slice 7 = the image's last KB
+  const uint32_t pc = rom[(vbank << 12) + (0xFFCu & mask_a)] | ((uint32_t)rom[(vbank << 12) + (0xFFDu & mask_a)] << 8);
   for (int w = 0; w < ST_WORDS; ++w) p.st[w * B + e] = 0;
   p.st[W_AXYS * B + e] = 0xFDu << 24;
   p.st[W_PC * B + e] = pc | (0x24u << 16);
   p.st[W_BEAM * B + e] = bank << 24;
   p.st[W_TIMER * B + e] = 0xFFu | (10u << 8);
   p.st[W_FLAGS * B + e] = TF_INPT4_LATCH | TF_INPT5_LATCH;
+  p.st[W_CART * B + e] = (rm.kind == MK_E0) ? (4u | (5u << 3) | (6u << 6)) : 0u;      // E0 power-up slices [R] (R16)
   p.cyc[e] = 0;
   p.boot[e] = 0;
   unsigned long long s = seeds[e];
@@ -65,6 +67,14 @@ __global__ void reset_kernel(StepParams p, const unsigned long long *seeds, cons
     unsigned long long z = splitmix64(s);
     p.ram[(2 * k) * B + e] = (uint32_t)z;
     p.ram[(2 * k + 1) * B + e] = (uint32_t)(z >> 32);
+  }
+  if (p.sc_ram) {                                      // Superchip RAM: the next 16 draws (its power-on contents must come from the seed)
+    const bool sc = rm.hs & HS_SC;
+    for (int k = 0; k < 16; ++k) {
+      unsigned long long z = splitmix64(s);
+      p.sc_ram[(2 * k) * B + e] = sc ? (uint32_t)z : 0u;
+      p.sc_ram[(2 * k + 1) * B + e] = sc ? (uint32_t)(z >> 32) : 0u;
+    }
   }
 }
 __global__ void clear_screen_kernel(uint8_t *screen, const uint8_t *mask) {
@@ -103,24 +113,43 @@ __global__ void get_ram_kernel(const uint32_t *ram, uint32_t *out, int B) {
   const int e = (int)(idx >> 5), i = (int)(idx & 31);
   out[idx] = ram[(size_t)i * B + e];
 }
-__global__ void get_regs_kernel(const uint32_t *st, const unsigned long long *cyc, uint4 *out, int B) {
+__global__ void get_regs_kernel(const uint32_t *st, const unsigned long long *cyc, uint4 *out, int B, const RomMeta *meta, const int32_t *env_rom) {
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= B) return;
+  const uint32_t kind = meta[env_rom[e]].kind, cart = st[W_CART * B + e];
   const uint32_t axys = st[W_AXYS * B + e], pcw = st[W_PC * B + e], beam = st[W_BEAM * B + e], tm = st[W_TIMER * B + e];
   const unsigned long long c = cyc[e];
   uint4 lo, hi;
   lo.x = (uint32_t)c; lo.y = (uint32_t)(c >> 32); lo.z = st[W_FRAME * B + e];
   lo.w = (pcw & 0xFFFFu) | ((axys & 0xFFu) << 16) | (((axys >> 8) & 0xFFu) << 24);                 // pc, a, x
-  hi.x = ((axys >> 16) & 0xFFu) | ((axys >> 24) << 8) | (((pcw >> 16) & 0xFFu) << 16) | ((beam >> 24) << 24);   // y, sp, p, bank
+  const uint32_t bank = (kind == MK_E0) ? (cart & 0x3Fu) : (beam >> 24);          // E0: slice at $1000 | slice at $1400 << 3
+  hi.x = ((axys >> 16) & 0xFFu) | ((axys >> 24) << 8) | (((pcw >> 16) & 0xFFu) << 16) | (bank << 24);   // y, sp, p, bank
   hi.y = ((beam >> 8) & 0xFFFFu) | (((beam & 0xFFu) % LINE_CYC) << 16) | ((pcw >> 24) << 24);                    // line, cyc_in_line, status
-  hi.z = (tm & 0xFFu) | ((((tm >> 12) & 1u) << 7) << 8);                                            // intim, timint
+  const uint32_t pad0 = (kind == MK_E0) ? (cart >> 6) & 7u : (kind == MK_FE) ? (cart >> 9) & 1u : 0u;   // E0: slice at $1800 ; FE: pending bit
+  hi.z = (tm & 0xFFu) | ((((tm >> 12) & 1u) << 7) << 8) | (pad0 << 16);                             // intim, timint, _pad[0]
   hi.w = 0;
   out[2 * e] = lo; out[2 * e + 1] = hi;
 }
 
+// the format of an image: the caller's choice when its size fits that format, else (VCS_MAP_BY_SIZE) the plain format of the size
+int map_kind(uint32_t size, uint32_t mapper) {
+  static_assert((int)VCS_MAP_2K == (int)MK_2K && (int)VCS_MAP_F8 == (int)MK_F8 && (int)VCS_MAP_F4SC == (int)MK_F4SC && (int)VCS_MAP_E0 == (int)MK_E0 &&
+                (int)VCS_MAP_FE == (int)MK_FE, "format numbers");
+  if (mapper == VCS_MAP_BY_SIZE)
+    return size == 2048 ? (int)MK_2K : size == 4096 ? (int)MK_4K : size == 8192 ? (int)MK_F8 : size == 16384 ? (int)MK_F6 : size == 32768 ? (int)MK_F4 : -1;
+  uint32_t want = 0;
+  switch (mapper) {
+    case VCS_MAP_2K: want = 2048; break;  case VCS_MAP_4K: want = 4096; break;
+    case VCS_MAP_F8: case VCS_MAP_F8SC: case VCS_MAP_E0: case VCS_MAP_FE: want = 8192; break;
+    case VCS_MAP_F6: case VCS_MAP_F6SC: want = 16384; break;  case VCS_MAP_F4: case VCS_MAP_F4SC: want = 32768; break;
+    default: return -1;
+  }
+  return want == size ? (int)mapper : -1;
+}
+
 StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   StepParams p;
-  p.st = h->d_st; p.ram = h->d_ram; p.cyc = h->d_cyc; p.screen = h->d_screen;
+  p.st = h->d_st; p.ram = h->d_ram; p.cyc = h->d_cyc; p.screen = h->d_screen; p.sc_ram = h->d_sc_ram;
   p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
   p.actions = actions; p.switches = h->d_switches; p.mask = nullptr; p.boot = h->d_boot_ctr; p.perm = h->d_perm; p.blk_time = nullptr; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
   p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom;
@@ -150,7 +179,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   if (batch < 1 || !roms || n_roms < 1 || !seeds) return VCS_EINVAL;
   for (int r = 0; r < n_roms; ++r) {
     if (!roms[r].data) return VCS_EINVAL;
-    if (roms[r].size != 2048 && roms[r].size != 4096 && roms[r].size != 8192 && roms[r].size != 16384 && roms[r].size != 32768) return VCS_EROM;
+    if (map_kind(roms[r].size, roms[r].mapper) < 0) return VCS_EROM;
   }
   if (env_rom) for (int i = 0; i < batch; ++i) if (env_rom[i] < 0 || env_rom[i] >= n_roms) return VCS_EINVAL;
   vcs_config c = {34, 320, 1, 0};
@@ -167,8 +196,14 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
 
   std::vector<RomMeta> meta(n_roms);
   size_t blob = 0, dwords = 0;
+  bool any_sc = false, any_special = false;
   for (int r = 0; r < n_roms; ++r) {
     meta[r].offset = (uint32_t)blob; meta[r].size = roms[r].size; meta[r].doff = (uint32_t)dwords; meta[r].pad = 0;
+    const uint32_t kind = (uint32_t)map_kind(roms[r].size, roms[r].mapper);
+    const uint32_t nbk = (kind == MK_F8 || kind == MK_F8SC) ? 2u : (kind == MK_F6 || kind == MK_F6SC) ? 4u : (kind == MK_F4 || kind == MK_F4SC) ? 8u : 0u;
+    meta[r].kind = kind;
+    meta[r].hs = (nbk ? (((nbk == 8u) ? 0x1FF4u : 0x1FFAu - nbk) | (nbk << 16)) : 0u) | ((kind >= MK_F8SC && kind <= MK_F4SC) ? HS_SC : 0u);
+    any_sc = any_sc || (meta[r].hs & HS_SC); any_special = any_special || kind >= MK_F8SC;
     blob += roms[r].size; dwords += (roms[r].size < 4096) ? 4096 : roms[r].size;
   }
   std::vector<uint8_t> hb(blob);
@@ -193,16 +228,21 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
     std::vector<uint8_t> img(4096 + 4, 0), leader(4096);
     for (int r = 0; r < n_roms; ++r) {
       const int nb = (roms[r].size < 4096) ? 1 : (int)(roms[r].size / 4096);
+      if (meta[r].kind == MK_E0 || meta[r].kind == MK_FE) {         // 1 KB windows / a bank that follows the data bus: every byte decodes at run time
+        for (size_t i = 0; i < (size_t)nb * 4096; ++i) { dw[meta[r].doff + i] = DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0}; dwp[meta[r].doff + i] = dw[meta[r].doff + i]; }
+        continue;
+      }
+      const bool sc = (meta[r].hs & HS_SC) != 0;
       std::fill(leader.begin(), leader.end(), 0);
       for (int pass = 0; pass < 2; ++pass)
         for (int b = 0; b < nb; ++b) {
           if (roms[r].size == 2048) { memcpy(img.data(), roms[r].data, 2048); memcpy(img.data() + 2048, roms[r].data, 2048); }
           else memcpy(img.data(), roms[r].data + 4096 * b, 4096);
           if (pass == 0) mark_leaders(img.data(), leader.data());
-          else { decode_bank(img.data(), leader.data(), h->block, nb, dw.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE));
+          else { decode_bank(img.data(), leader.data(), h->block, nb, dw.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE), sc);
                  if (!(c.flags & VCS_F_NO_SPIN)) mark_spins(img.data(), dw.data() + meta[r].doff + 4096 * b);
                  if (!(c.flags & VCS_F_NO_FUSE)) fuse_ld_st(dw.data() + meta[r].doff + 4096 * b);
-                 decode_bank(img.data(), leader.data(), 128, nb, dwp.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE)); }
+                 decode_bank(img.data(), leader.data(), 128, nb, dwp.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE), sc); }
         }
     }
   }
@@ -212,6 +252,8 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   CU(h, cudaMalloc((void **)&h->d_ram, sizeof(uint32_t) * 32 * B));
   CU(h, cudaMalloc((void **)&h->d_cyc, sizeof(unsigned long long) * B));
   CU(h, cudaMalloc((void **)&h->d_screen, (size_t)SCR_W * SCR_H * B));
+  if (any_sc) CU(h, cudaMalloc((void **)&h->d_sc_ram, sizeof(uint32_t) * 32 * B));
+  h->special_carts = any_special ? 1 : 0;
   CU(h, cudaMalloc((void **)&h->d_rom_blob, blob));
   CU(h, cudaMalloc((void **)&h->d_drom, sizeof(DWord) * dw.size()));
   CU(h, cudaMemcpy(h->d_drom, dw.data(), sizeof(DWord) * dw.size(), cudaMemcpyHostToDevice));
@@ -381,6 +423,7 @@ int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float 
   if (!actions_dev || !soft_out_dev) return fail(h, VCS_EINVAL, "vcs_step_soft: NULL buffer");
   if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31)) return fail(h, VCS_EINVAL, "vcs_step_soft: frameskip out of range");
   if (!(T > 0.f) || T > 60.f || !(alpha == alpha) || alpha > 1e30f || alpha < -1e30f) return fail(h, VCS_EINVAL, "vcs_step_soft: T or alpha out of range");
+  if (h->special_carts) return fail(h, VCS_EINVAL, "vcs_step_soft: Superchip / E0 / FE cartridges run in hard mode only");
   cudaStream_t s = (cudaStream_t)cuda_stream;
   if (h->soft_tab_T != T) {                            // a new temperature: e^{-k/T} and W(T) x ROM, once
     int K = (int)ceil(17.0 * (double)T); if (K < 1) K = 1; if (K > 1023) K = 1023;
@@ -412,9 +455,18 @@ int vcs_get_ram(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
   CU(h, cudaGetLastError());
   return VCS_OK;
 }
+int vcs_get_cart_ram(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
+  DEV_OK(h); if (!out_dev) return VCS_EINVAL;
+  if (!h->d_sc_ram) { CU(h, cudaMemsetAsync(out_dev, 0, (size_t)128 * h->batch, (cudaStream_t)cuda_stream)); return VCS_OK; }
+  const long long n = 32ll * h->batch;
+  get_ram_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(h->d_sc_ram, reinterpret_cast<uint32_t *>(out_dev), h->batch);
+  h->launches += 1;
+  CU(h, cudaGetLastError());
+  return VCS_OK;
+}
 int vcs_get_regs(vcs_t h, vcs_regs *out_dev, void *cuda_stream) {
   DEV_OK(h); if (!out_dev) return VCS_EINVAL;
-  get_regs_kernel<<<(h->batch + 127) / 128, 128, 0, (cudaStream_t)cuda_stream>>>(h->d_st, h->d_cyc, reinterpret_cast<uint4 *>(out_dev), h->batch);
+  get_regs_kernel<<<(h->batch + 127) / 128, 128, 0, (cudaStream_t)cuda_stream>>>(h->d_st, h->d_cyc, reinterpret_cast<uint4 *>(out_dev), h->batch, h->d_rom_meta, h->d_env_rom);
   h->launches += 1;
   CU(h, cudaGetLastError());
   return VCS_OK;
@@ -480,6 +532,34 @@ int vcs_block_times(vcs_t h, uint64_t *times_host, int32_t *perm_host, int32_t c
 
 int64_t vcs_launch_count(vcs_t h) { return h ? h->launches : -1; }
 
+// Format guess from size and content (reading R17).  Host only.
+int vcs_detect_mapper(const uint8_t *data, uint32_t size) {
+  if (!data) return VCS_EINVAL;
+  if (size == 2048) return VCS_MAP_2K;
+  if (size == 4096) return VCS_MAP_4K;
+  if (size != 8192 && size != 16384 && size != 32768) return VCS_EROM;
+  bool filler = true;                                   // Superchip: every bank starts with 256 equal bytes (its RAM ports sit there)
+  for (uint32_t bank = 0; bank < size / 4096 && filler; ++bank) {
+    const uint8_t *b = data + 4096 * bank;
+    for (int i = 255; i > 0; --i) if (b[i] != b[0]) { filler = false; break; }
+  }
+  if (size == 16384) return filler ? VCS_MAP_F6SC : VCS_MAP_F6;
+  if (size == 32768) return filler ? VCS_MAP_F4SC : VCS_MAP_F4;
+  if (filler) return VCS_MAP_F8SC;
+  int n_f8 = 0, n_e0 = 0, n_fe = 0;                     // what the code's absolute operands point at
+  for (uint32_t i = 0; i + 2 < size; ++i) {
+    const uint32_t op = data[i], target = data[i + 1] | ((uint32_t)data[i + 2] << 8), low5 = op & 0x1Fu;
+    if (op == 0x20 || op == 0x4C) { if ((target & 0xF000u) == 0xD000u) ++n_fe; continue; }       // JSR / JMP into the $D000 page
+    if (op == 0x6C || low5 < 0x0C || low5 > 0x0E) continue;                                      // columns xC, xD, xE hold the absolute modes
+    const uint32_t a = target & 0x1FFFu;
+    if (a == 0x1FF8u || a == 0x1FF9u) ++n_f8;
+    else if (a >= 0x1FE0u && a <= 0x1FF7u) ++n_e0;
+  }
+  if (n_e0 >= 2 && n_e0 > n_f8) return VCS_MAP_E0;
+  if (n_fe >= 2 && n_f8 == 0) return VCS_MAP_FE;
+  return VCS_MAP_F8;
+}
+
 int vcs_optable(uint16_t *out256) {
   if (!out256) return VCS_EINVAL;
   memcpy(out256, host_optable(), 512); return VCS_OK;
@@ -490,7 +570,7 @@ int vcs_destroy(vcs_t h) {
   int cur = -1; cudaGetDevice(&cur);
   if (cur != h->device) cudaSetDevice(h->device);     // free on the handle's own device, then give the caller's back
   cudaDeviceSynchronize();
-  cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom); cudaFree(h->d_drom_plain);
+  cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_sc_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom); cudaFree(h->d_drom_plain);
   cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr); cudaFree(h->d_perm); cudaFree(h->d_blk_time); cudaFree(h->d_w_avg);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   if (h->h_soft_w) cudaFreeHost(h->h_soft_w);

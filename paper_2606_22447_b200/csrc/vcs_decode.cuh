@@ -206,10 +206,12 @@ inline void hot_class(uint32_t &x, uint32_t &y, int block, bool promote) {
 
 // One bank image (4096 bytes; 2 KB carts are passed mirrored) -> 4096 decode entries.  `leader` is the bank-
 // independent leader bitmap (4096 flags) filled by mark_leaders() for every bank of the cartridge first.
-inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, int nb, DWord *out, bool promote = true) {
+// sc: a Superchip cart — the first 256 bytes of the bank are RAM ports, not ROM: no instruction there is pre-decoded and
+// no operand there is folded into an immediate
+inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, int nb, DWord *out, bool promote = true, bool sc = false) {
   for (uint32_t off = 0; off < 4096; ++off) {
     const uint32_t lead = leader[off] ? DW_LEADER : 0u;
-    if (off >= DW_SLOW_LIMIT) { out[off].x = (HC_COLD + H_SLOW) | lead; out[off].y = 0; continue; }
+    if (off >= DW_SLOW_LIMIT || (sc && off < 0x100u)) { out[off].x = (HC_COLD + H_SLOW) | lead; out[off].y = 0; continue; }
     const uint32_t opc = img[off], b1 = img[off + 1], b2 = img[off + 2];
     const uint32_t ent = kOpTable[opc], mode = ent & 15u, op = (ent >> 4) & 63u, kind = ent >> 10;
     uint32_t x = generic_entry(opc);
@@ -238,7 +240,7 @@ inline void decode_bank(const uint8_t *img, const uint8_t *leader, int block, in
       else if (ab && rd_std && (a13 & 0x1284u) == 0x0284u) {       // INTIM / TIMINT
         x = dw_x(H_RTIM, 4, 3, op - OP_LDA); payload = a13;
       }
-      else if (ab && rd_std && op != OP_BIT && (a13 & 0x1000u) && !is_hotspot(a13, nb)) {   // a fixed ROM byte
+      else if (ab && rd_std && op != OP_BIT && (a13 & 0x1000u) && !is_hotspot(a13, nb) && !(sc && (a13 & 0x0F00u) == 0)) {   // a fixed ROM byte
         x = dw_x(H_IMM0 + (op - OP_LDA), 4, 3, 0); payload = img[a13 & 0xFFFu];                        // of this bank
       }
       else if (mode == MD_REL) {

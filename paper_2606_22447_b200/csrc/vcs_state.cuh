@@ -33,8 +33,12 @@ enum StWord {
   W_POS2,       // posBL | HMBL<<8 | rx<<16 (colour clocks of the current line already rendered, 0..228)
   W_FLAGS,      // TIA / input flag bits, see TF_* (only the bits below TF_DIRTY0 are architectural)
   W_CX,         // 15 collision latches
+  W_CART,       // E0: slice shown at $1000 | at $1400 << 3 | at $1800 << 6 ; FE: bit 9 = the previous access was to $01FE
   ST_WORDS
 };
+// cartridge formats (the numbers are include/vcs.h's VCS_MAP_*)
+enum MapKind : uint32_t { MK_2K = 1, MK_4K, MK_F8, MK_F6, MK_F4, MK_F8SC, MK_F6SC, MK_F4SC, MK_E0, MK_FE };
+constexpr uint32_t HS_SC = 1u << 31;       // RomMeta::hs / C_HS: the first 256 bytes of every bank are the Superchip RAM ports
 
 // W_FLAGS bits
 enum : uint32_t {
@@ -71,26 +75,31 @@ enum SmWord {
   S_PORTS, S_INP,                  // RIOT port latches; ina | fire0<<8 | switches (5 pins)<<9 | (env index inside the block)<<16
   S_TMR, S_TTICKS,                 // timer state packed as W_TIMER, valid after S_TTICKS cycles of this step
   S_STATUS, S_FSTART,              // status bits | ROM index << 8; value of the step's cycle count at which the current frame began
-  S_OBJ = 60,                      // 30 words: cached 160-bit line masks of PF, BL, P0, P1, M0, M1 (5 words each);
+  S_CART,                          // W_CART: E0 window slices, FE's pending bit
+  S_OBJ = 61,                      // 30 words: cached 160-bit line masks of PF, BL, P0, P1, M0, M1 (5 words each);
                                    //           a derived cache — also the scratch area of a regroup (vcs_step.cu)
-  S_WORDS = 90,
+  S_WORDS = 91,
   S_MOVED = S_OBJ + 8              // a regroup moves words [0, S_MOVED): the state proper + 8 words of saved CPU registers
 };
-static_assert(S_STATUS == 58, "file layout");
+static_assert(S_STATUS == 58 && S_CART == 60, "file layout");
 // per-block context, in words after the thread files (block-uniform values the out-of-line paths need)
 enum CtxWord { C_SCREEN_LO = 0, C_SCREEN_HI, C_Y0, C_FRAMESKIP, C_BATCH, C_ENV0, C_CAP, C_ROMOFF, C_REGROUP,
                C_META_LO, C_META_HI, C_BLOB_LO, C_BLOB_HI, C_DROM_LO, C_DROM_HI,
                C_SOFT_OUT_LO, C_SOFT_OUT_HI, C_SOFT_W_LO, C_SOFT_W_HI, C_SOFT_K, C_SOFT_ALPHA, C_SOFT_TAB_LO, C_SOFT_TAB_HI,
-               C_HS,           // bank hotspots of the block's ROM (ROM staged in smem: one ROM per block): first address | count << 16
-               C_WORDS = 24 };
+               C_HS,           // bank hotspots of the block's ROM (ROM staged in smem: one ROM per block): first address | count << 16 | HS_SC
+               C_SCRAM_LO, C_SCRAM_HI,     // Superchip RAM of all envs, [32][batch] words like `ram` (nullptr when no cart has it)
+               C_WORDS = 28 };         // (a multiple of 4: the ROM image staged behind the context is a 16-byte aligned bulk-copy target)
+static_assert(C_WORDS % 4 == 0 && C_SCRAM_HI < C_WORDS, "context layout");
 static_assert(C_HS < C_WORDS, "context layout");
 
-struct RomMeta { uint32_t offset; uint32_t size; uint32_t doff; uint32_t pad; };   // byte offset into the ROM blob, size, word offset into the decode blob
+struct RomMeta { uint32_t offset; uint32_t size; uint32_t doff; uint32_t pad;      // byte offset into the ROM blob, size, word offset into the decode blob
+                 uint32_t kind; uint32_t hs; };                                      // MapKind ; first hotspot | count << 16 | HS_SC (F8 / F6 / F4 families)
 
 struct Handle {                 // host-side bookkeeping behind vcs_t
   int32_t batch, n_roms;
   int32_t y0, max_lines, f8_start_bank;
   uint32_t *d_st; uint32_t *d_ram; unsigned long long *d_cyc; uint8_t *d_screen;
+  uint32_t *d_sc_ram;           // Superchip RAM [32][batch] (only when a cart has it)
   uint8_t *d_rom_blob; uint2 *d_drom; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
   int device;                   // the CUDA device every pointer below belongs to
   float *h_soft_w; cudaEvent_t soft_w_done; int soft_K;            // soft mode: pinned e^{-k/T} staging buffer, its upload, window of the cached temperature
@@ -103,6 +112,7 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   uint32_t *d_boot_ctr;         // per env: boot steps left | NOOP starts << 8 | RESET steps << 16 (vcs_auto_reset; 0 = playing)
   uint8_t *d_boot;              // vcs_boot scratch: [batch] NOOP actions, [batch] per-iteration mask, [batch] switches with RESET held
   uint8_t *h_pinned; size_t h_pinned_bytes;
+  int special_carts;            // some cart is Superchip / E0 / FE (hard mode only)
   int block;                    // threads (= envs) per block of the interpreter kernel
   int regroup;                  // F8 blocks re-sort their envs across threads at bank-hotspot accesses
   int rom_smem;                 // every block maps to a single ROM: it is staged in shared memory

@@ -172,6 +172,7 @@ struct Cpu {
   bool wsync;         // mirror of TF_WSYNC
   // ---- cart
   uint32_t hs_lo, hs_n, rom_mask;      // bank hotspots: hs_n addresses from hs_lo (F8 $1FF8 x2, F6 $1FF6 x4, F4 $1FF4 x8); hs_n 0 = none
+  uint32_t kind;      // MapKind of this env's cartridge
   uint32_t park;      // bit0: this block regroups its envs at bank-hotspot accesses; bit1: this lane is parked for a
                       // regroup; bit2: a bank hotspot was accessed by the instruction in flight
   uint32_t rom_off;   // ROMS: byte offset of the ROM image inside smem
@@ -197,14 +198,14 @@ struct Cpu {
     if constexpr (CART) {                                  // (the line-end / event paths never touch the cartridge)
       auto ptr = [](int lo) { return (unsigned long long)T::ctx(lo) | ((unsigned long long)T::ctx(lo + 1) << 32); };
       const RomMeta rm = reinterpret_cast<const RomMeta *>(ptr(C_META_LO))[romid];
-      hs_n = rm.size >> 12; if (hs_n < 2u) hs_n = 0; hs_lo = (hs_n == 8u) ? 0x1FF4u : 0x1FFAu - hs_n; rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
+      hs_n = (rm.hs >> 16) & 0xFFu; hs_lo = rm.hs & 0xFFFFu; kind = rm.kind; rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
       rom_g = reinterpret_cast<const uint8_t *>(ptr(C_BLOB_LO)) + rm.offset;
       dr = reinterpret_cast<const uint2 *>(ptr(C_DROM_LO)) + rm.doff;
       if constexpr (SOFT) {
         soft = reinterpret_cast<float *>(ptr(C_SOFT_OUT_LO)) + 8 * (size_t)(T::ctx(C_ENV0) + (S(S_INP) >> 16));
         soft_tab = reinterpret_cast<const float *>(ptr(C_SOFT_TAB_LO)) + rm.pad;
       } else { soft = nullptr; soft_tab = nullptr; }
-    } else { hs_n = 0; hs_lo = 0; rom_mask = 0xFFFu; rom_g = nullptr; dr = nullptr; soft = nullptr; soft_tab = nullptr; }
+    } else { hs_n = 0; hs_lo = 0; kind = MK_4K; rom_mask = 0xFFFu; rom_g = nullptr; dr = nullptr; soft = nullptr; soft_tab = nullptr; }
     park = T::ctx(C_REGROUP) | ((keyhi == KEY_PARKED) ? 2u : 0u);
   }
   DEV Hot store() const {
@@ -237,7 +238,30 @@ struct Cpu {
     else return __ldg(rom_g + off);
   }
   // any access to a hotspot ($1FF8/$1FF9 on F8 carts) selects the bank; in a block that regroups it also parks the lane (park bit 1)
+  // --- formats only the generic executor (TAG 1) runs: Superchip RAM ports, E0's 1 KB windows, FE (include/vcs.h)
+  DEV uint8_t *sc_cell(uint32_t cell) const {              // byte `cell` of this env's Superchip RAM ([32][batch] words in global memory)
+    uint32_t *base = reinterpret_cast<uint32_t *>((unsigned long long)T::ctx(C_SCRAM_LO) | ((unsigned long long)T::ctx(C_SCRAM_HI) << 32));
+    return reinterpret_cast<uint8_t *>(base + (size_t)(cell >> 2) * T::ctx(C_BATCH) + (T::ctx(C_ENV0) + (S(S_INP) >> 16))) + (cell & 3u);
+  }
+  DEV bool has_sc() const { return kind - MK_F8SC <= MK_F4SC - MK_F8SC; }
+  DEV void fe_snoop(uint32_t a, uint32_t data) {           // FE: the access after one to $01FE selects the bank from bit 5 of its data
+    if (kind != MK_FE) return;
+    uint32_t c = S(S_CART);
+    if (c & 0x200u) {
+      const uint32_t nd = (di & 0xFFFu) | ((data & 0x20u) ? 0u : 0x1000u);
+      pbase += di - nd; di = nd; rekey();
+      c &= ~0x200u;
+    }
+    if (a == 0x01FEu) c |= 0x200u;
+    S(S_CART) = c;
+  }
   DEV void hotspot(uint32_t a) {
+    if constexpr (TAG == 1) {
+      if (kind == MK_E0) {                                 // $1FE0-7 / $1FE8-F / $1FF0-7: slice of the window at $1000 / $1400 / $1800
+        if (a - 0x1FE0u < 0x18u) { const uint32_t sh = 3u * ((a - 0x1FE0u) >> 3); S(S_CART) = (S(S_CART) & ~(7u << sh)) | ((a & 7u) << sh); }
+        return;
+      }
+    }
     if (a - hs_lo < hs_n) {
       const uint32_t nd = (di & 0xFFFu) | ((a - hs_lo) << 12);
       pbase += di - nd; di = nd;                     // PC is unchanged
@@ -247,6 +271,10 @@ struct Cpu {
   }
   DEV uint32_t rom_rd(uint32_t a, bool value = true) {   // a = addr & 0x1FFF with A12 set; value: the byte is used (not a dummy cycle)
     hotspot(a);
+    if constexpr (TAG == 1) {
+      if (has_sc() && (a & 0x0F00u) == 0) return *sc_cell(a & 0x7Fu);          // read port (a read of the write port sees the cell too)
+      if (kind == MK_E0) { const uint32_t w = (a >> 10) & 3u, slice = (w == 3u) ? 7u : (S(S_CART) >> (3u * w)) & 7u; return rom_byte(slice * 1024u + (a & 0x3FFu)); }
+    }
     const uint32_t v = rom_byte((di & 0x7000u) + (a & rom_mask));
     if constexpr (SOFT) { if (value) return soft_rom(a & 0xFFFu, v); }
     return v;
@@ -290,6 +318,7 @@ struct Cpu {
   }
   // a read whose value is discarded (C.5 "dummy") in cycle cyc+k: only INTIM and bank hotspots react
   DEV void dummy_rd(uint32_t addr, int k) {
+    if constexpr (TAG == 1) { if (kind == MK_FE) { (void)bus_read(addr, k, false); return; } }     // (FE watches every cycle's address and data)
     const uint32_t a = addr & 0x1FFFu;
     if (a & 0x1000u) hotspot(a);
     else if ((a & 0x0285u) == 0x0284u) io_dummy_intim<BLOCK, TAG>(sl, cyc + k + 1);
@@ -306,20 +335,25 @@ struct Cpu {
     relim();
   }
   // the generic operand read (C.3 decode), k cycles into the instruction
-  DEV uint32_t bus_read(uint32_t addr, int k, bool value = true) {     // value: the byte is used (soft reads skip discarded ones)
-    const uint32_t a = addr & 0x1FFFu;
+  DEV uint32_t bus_read0(uint32_t a, int k, bool value) {
     if ((a & 0x1280u) == 0x0080u) return ram_rd(a, value);
     if (a & 0x1000u) return rom_rd(a, value);
     const uint32_t r = io_read<BLOCK, TAG>(sl, a, cyc + k, cyc - lstart + k);
     if (r >> 12) { lstart += LINE_CYC * (int32_t)(r >> 12); wsync = false; relim(); }
     return r & 0xFFu;
   }
+  DEV uint32_t bus_read(uint32_t addr, int k, bool value = true) {     // value: the byte is used (soft reads skip discarded ones)
+    const uint32_t a = addr & 0x1FFFu;
+    const uint32_t v = bus_read0(a, k, value);
+    if constexpr (TAG == 1) fe_snoop(a, v);
+    return v;
+  }
   DEV void bus_write(uint32_t addr, uint32_t v, int k) {
     const uint32_t a = addr & 0x1FFFu;
-    if ((a & 0x1280u) == 0x0080u) { ram_wr(a, v); return; }
-    if (a & 0x1000u) { hotspot(a); return; }
-    const uint32_t ev = io_write<BLOCK, TAG>(sl, a, v, cyc + k, cyc - lstart + k);
-    if (ev) tia_events(ev, cyc + k + 1);
+    if ((a & 0x1280u) == 0x0080u) ram_wr(a, v);
+    else if (a & 0x1000u) { hotspot(a); if constexpr (TAG == 1) { if (has_sc() && (a & 0x0F80u) == 0) *sc_cell(a & 0x7Fu) = (uint8_t)v; } }   // Superchip write port
+    else { const uint32_t ev = io_write<BLOCK, TAG>(sl, a, v, cyc + k, cyc - lstart + k); if (ev) tia_events(ev, cyc + k + 1); }
+    if constexpr (TAG == 1) fe_snoop(a, v);
   }
   // ---------------------------------------------------------------- SOFT-STE mode (include/vcs.h vcs_step_soft; eq. 8-10)
   DEV void soft_note(int k, float soft_v, float hard, float ste) {
@@ -475,7 +509,7 @@ struct Cpu {
 #pragma unroll 4
       for (int j = 0; j < BLOCK; ++j) { const uint32_t kj = keys[j]; rank += (kj < skey || (kj == skey && (uint32_t)j < sl)) ? 1u : 0u; }
     }
-    constexpr int NB = 17;
+    constexpr int NB = 23;
     static_assert(S_MOVED % NB == 0, "batching");
 #pragma unroll 1
     for (int base = 0; base < S_MOVED; base += NB) {
@@ -543,6 +577,7 @@ struct Cpu {
       bool slow = false;                                   // run-time decoded
       uint32_t ea = 0, v = 0, wv = 0, op2 = 0, hid;
       int k = 0, i0 = 0, total = 0, kb = 0;
+      if constexpr (!GEN) { if (kind >= MK_F8SC) return true; }          // Superchip / E0 / FE carts: the generic executor knows their ports
     dispatch:
       hid = cx & 0x7Fu;
       kb = -(int)((cx >> DW_CY_SHIFT) & 0xFFu);            // cyc + kb = the instruction's first cycle (cy is already added; 0 for the generic handlers)
@@ -644,6 +679,7 @@ struct Cpu {
         // (C.5 sequences; the dummy stack read of JSR / RTS / RTI / PLA / PLP lands in RAM or on a TIA read address: no effect)
         case H_JSR: { const uint32_t ret = (pc() - 1u) & 0xFFFFu;     // address of the 3rd byte
           if constexpr (!GEN) { if (SP < 0x81u) return true; }
+          if constexpr (GEN) dummy_rd(0x0100u | SP, kb + 2);
           push<GEN>(ret >> 8, kb + 3); push<GEN>(ret & 0xFFu, kb + 4); rekey();
           if constexpr (GEN) {
             rdy(kb + 5);                                                      // R hi@PC comes after the pushes:
@@ -651,19 +687,22 @@ struct Cpu {
           }
           set_pc(pl); } goto ctl;
         case H_RTS: { if constexpr (!GEN) { if (SP - 0x7Fu > 0xFDu - 0x7Fu) return true; }      // pulls from SP+1, SP+2
+          if constexpr (GEN) dummy_rd(0x0100u | SP, kb + 2);
           const uint32_t lo = pull<GEN>(kb + 3), hi = pull<GEN>(kb + 4); const uint32_t r = lo | (hi << 8);
           rekey(); dummy_rd(r, kb + 5); set_pc((r + 1u) & 0xFFFFu); } goto ctl;
         case H_PHA: if constexpr (!GEN) { if (SP < 0x80u) return true; } push<GEN>(A, kb + 2); rekey(); break;
         case H_PHP: if constexpr (!GEN) { if (SP < 0x80u) return true; } push<GEN>(pack_p() | 0x30u, kb + 2); rekey(); break;
-        case H_PLA: if constexpr (!GEN) { if (SP - 0x7Fu > 0xFEu - 0x7Fu) return true; } A = pull<GEN>(kb + 3); zn = A; rekey(); break;
-        case H_PLP: if constexpr (!GEN) { if (SP - 0x7Fu > 0xFEu - 0x7Fu) return true; } unpack_p(pull<GEN>(kb + 3)); rekey(); break;
+        case H_PLA: if constexpr (!GEN) { if (SP - 0x7Fu > 0xFEu - 0x7Fu) return true; } if constexpr (GEN) dummy_rd(0x0100u | SP, kb + 2);
+                    A = pull<GEN>(kb + 3); zn = A; rekey(); break;
+        case H_PLP: if constexpr (!GEN) { if (SP - 0x7Fu > 0xFEu - 0x7Fu) return true; } if constexpr (GEN) dummy_rd(0x0100u | SP, kb + 2);
+                    unpack_p(pull<GEN>(kb + 3)); rekey(); break;
         // ---- absolute read of INTIM / TIMINT (4th cycle)
         case H_RTIM: read_op(cx >> DW_OP2_SHIFT, timer_read(pl, cyc - 1)); break;
         // ---- generic addressing: reads (cyc = first cycle of the instruction; they add `total` themselves)
         case H_R0 + 0: v = pl & 0xFFu; total = 2; goto do_read_op;
         case H_R0 + 1: ea = pl & 0xFFu; k = 2; goto do_read;
-        case H_R0 + 2: ea = (pl + X) & 0xFFu; k = 3; goto do_read;
-        case H_R0 + 3: ea = (pl + Y) & 0xFFu; k = 3; goto do_read;
+        case H_R0 + 2: if constexpr (GEN) dummy_rd(pl & 0xFFu, 2); ea = (pl + X) & 0xFFu; k = 3; goto do_read;      // (R dummy@zp)
+        case H_R0 + 3: if constexpr (GEN) dummy_rd(pl & 0xFFu, 2); ea = (pl + Y) & 0xFFu; k = 3; goto do_read;
         case H_R0 + 4: ea = pl; k = 3; goto do_read;
         case H_R0 + 5: case H_R0 + 6: case H_R0 + 8: {
           uint32_t lo, hi;
@@ -676,11 +715,12 @@ struct Cpu {
           if (t & 0x100u) { dummy_rd(unc, k); k += 1; }
         } goto do_read;
         case H_R0 + 7: { const uint32_t z = (pl + X) & 0xFFu; if constexpr (!GEN) { if (z - 0x80u > 0x7Eu) return true; }
+          if constexpr (GEN) dummy_rd(pl & 0xFFu, 2);
           ea = rd8<GEN>(z, 3); ea |= rd8<GEN>((z + 1u) & 0xFFu, 4) << 8; k = 5; } goto do_read;
         // ---- generic addressing: stores
         case H_W0 + 0: ea = pl & 0xFFu; k = 2; goto do_write;
-        case H_W0 + 1: ea = (pl + X) & 0xFFu; k = 3; goto do_write;
-        case H_W0 + 2: ea = (pl + Y) & 0xFFu; k = 3; goto do_write;
+        case H_W0 + 1: if constexpr (GEN) dummy_rd(pl & 0xFFu, 2); ea = (pl + X) & 0xFFu; k = 3; goto do_write;
+        case H_W0 + 2: if constexpr (GEN) dummy_rd(pl & 0xFFu, 2); ea = (pl + Y) & 0xFFu; k = 3; goto do_write;
         case H_W0 + 3: ea = pl; k = 3; goto do_write;
         case H_W0 + 4: case H_W0 + 5: case H_W0 + 7: {
           uint32_t lo, hi;
@@ -693,10 +733,11 @@ struct Cpu {
           dummy_rd(unc, k); k += 1;
         } goto do_write;
         case H_W0 + 6: { const uint32_t z = (pl + X) & 0xFFu; if constexpr (!GEN) { if (z - 0x80u > 0x7Eu) return true; }
+          if constexpr (GEN) dummy_rd(pl & 0xFFu, 2);
           ea = rd8<GEN>(z, 3); ea |= rd8<GEN>((z + 1u) & 0xFFu, 4) << 8; k = 5; } goto do_write;
         // ---- generic addressing: read-modify-write
         case H_M0 + 0: ea = pl & 0xFFu; k = 2; goto do_rmw;
-        case H_M0 + 1: ea = (pl + X) & 0xFFu; k = 3; goto do_rmw;
+        case H_M0 + 1: if constexpr (GEN) dummy_rd(pl & 0xFFu, 2); ea = (pl + X) & 0xFFu; k = 3; goto do_rmw;
         case H_M0 + 2: ea = pl; k = 3; goto do_rmw;
         case H_M0 + 3: { const uint32_t t = (pl & 0xFFu) + X; const uint32_t unc = (pl & 0xFF00u) | (t & 0xFFu);
           ea = (unc + (t & 0x100u)) & 0xFFFFu; dummy_rd(unc, 3); k = 4; } goto do_rmw;
@@ -706,12 +747,13 @@ struct Cpu {
           const uint32_t l2 = rd8<GEN>(pl, kb + 3), h2 = rd8<GEN>(p2, kb + 4);
           set_pc(l2 | (h2 << 8)); } goto ctl;
         case H_RTI: { if constexpr (!GEN) { if (SP - 0x7Fu > 0xFCu - 0x7Fu) return true; }       // pulls from SP+1 .. SP+3
+          if constexpr (GEN) dummy_rd(0x0100u | SP, kb + 2);
           unpack_p(pull<GEN>(kb + 3)); const uint32_t lo = pull<GEN>(kb + 4), hi = pull<GEN>(kb + 5); rekey(); set_pc(lo | (hi << 8)); } goto ctl;
         case H_BRK: { const uint32_t ret = pc();             // address of the opcode + 2
           if constexpr (!GEN) { if (SP < 0x82u) return true; }
           push<GEN>(ret >> 8, kb + 2); push<GEN>(ret & 0xFFu, kb + 3); push<GEN>(pack_p() | 0x30u, kb + 4); rekey();
           if constexpr (GEN) rdy(kb + 5);
-          const uint32_t l2 = rom_rd(0x1FFEu), h2 = rom_rd(0x1FFFu);          // ($FFFE / $FFFF: always the cartridge)
+          const uint32_t l2 = rd8<GEN>(0xFFFEu, kb + 5), h2 = rd8<GEN>(0xFFFFu, kb + 6);       // ($FFFE / $FFFF: always the cartridge)
           set_pc(l2 | (h2 << 8)); fDI |= 4u; } goto ctl;
         default:                                           // H_ILL — C.12: halt for good, PC stays
           status |= STATUS_ILLEGAL;
@@ -887,7 +929,7 @@ template <bool ROMS>
 DEV bool plain_addr(uint32_t addr, uint32_t hs) {
   const uint32_t a = addr & 0x1FFFu;
   if ((a & 0x1280u) == 0x0080u) return true;
-  if constexpr (ROMS) return (a & 0x1000u) && (a - (hs & 0xFFFFu)) >= (hs >> 16);
+  if constexpr (ROMS) return (a & 0x1000u) && (a - (hs & 0xFFFFu)) >= ((hs >> 16) & 0xFFu) && !((hs & HS_SC) && (a & 0x0F00u) == 0);
   else return false;                                       // (ROM in global memory: left to the out-of-line executor)
 }
 template <int BLOCK, bool ROMS>
@@ -1142,8 +1184,9 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     s_ctx[C_SCREEN_LO] = (uint32_t)scr; s_ctx[C_SCREEN_HI] = (uint32_t)(scr >> 32);
     s_ctx[C_Y0] = (uint32_t)p.y0; s_ctx[C_FRAMESKIP] = (uint32_t)p.frameskip; s_ctx[C_BATCH] = (uint32_t)B; s_ctx[C_ENV0] = (uint32_t)e0;
     s_ctx[C_CAP] = (uint32_t)(p.max_lines * LINE_CYC); s_ctx[C_ROMOFF] = ROM_OFF;
-    s_ctx[C_REGROUP] = (ROMS && rm.size == 8192 && p.regroup) ? 1u : 0u;
-    { const uint32_t n = (rm.size >> 12) < 2u ? 0u : (rm.size >> 12); s_ctx[C_HS] = ((n == 8u) ? 0x1FF4u : 0x1FFAu - n) | (n << 16); }
+    s_ctx[C_REGROUP] = (ROMS && rm.kind == MK_F8 && p.regroup) ? 1u : 0u;
+    s_ctx[C_HS] = rm.hs;
+    { const unsigned long long v = reinterpret_cast<unsigned long long>(p.sc_ram); s_ctx[C_SCRAM_LO] = (uint32_t)v; s_ctx[C_SCRAM_HI] = (uint32_t)(v >> 32); }
     auto put = [&](int lo, const void *q) { const unsigned long long v = reinterpret_cast<unsigned long long>(q); s_ctx[lo] = (uint32_t)v; s_ctx[lo + 1] = (uint32_t)(v >> 32); };
     put(C_META_LO, p.rom_meta); put(C_BLOB_LO, p.rom_blob); put(C_DROM_LO, p.drom);
     put(C_SOFT_OUT_LO, p.soft_out); put(C_SOFT_W_LO, p.soft_w); put(C_SOFT_TAB_LO, p.soft_tab); s_ctx[C_SOFT_K] = (uint32_t)p.soft_K; s_ctx[C_SOFT_ALPHA] = __float_as_uint(p.soft_alpha);
@@ -1175,7 +1218,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     T::S(sl, S_PORTS) = p.st[W_PORTS * B + ei];
     T::S(sl, S_COLU) = p.st[W_COLU * B + ei]; T::S(sl, S_PF) = p.st[W_PF * B + ei]; T::S(sl, S_GRP) = p.st[W_GRP * B + ei]; T::S(sl, S_NUSIZ) = p.st[W_NUSIZ * B + ei];
     T::S(sl, S_POS) = p.st[W_POS * B + ei]; w = p.st[W_POS2 * B + ei]; T::S(sl, S_POS2) = w & 0xFFFF; T::S(sl, S_RX) = w >> 16;
-    fl = (p.st[W_FLAGS * B + ei] & TF_ARCH_MASK) | TF_DIRTY_ALL; T::S(sl, S_CX) = p.st[W_CX * B + ei];
+    fl = (p.st[W_FLAGS * B + ei] & TF_ARCH_MASK) | TF_DIRTY_ALL; T::S(sl, S_CX) = p.st[W_CX * B + ei]; T::S(sl, S_CART) = p.st[W_CART * B + ei];
     T::S(sl, S_PX) = 0; T::S(sl, S_FDONE) = 0;
     for (int i = 0; i < 32; ++i) smem[(S_RAM + i) * BLOCK + tid] = p.ram[i * B + ei];
     for (int i = 0; i < 10; ++i) smem[(S_PLANE + i) * BLOCK + tid] = 0;
@@ -1189,8 +1232,8 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   s.fskip = (uint32_t)p.frameskip;
   s.cyc = 0; s.lstart = -(int32_t)n0; s.fdone = live0 ? 0u : s.fskip; s.romid = romid;
   s.cap = p.max_lines * LINE_CYC;
-  s.hs_n = rm.size >> 12; if (s.hs_n < 2u) s.hs_n = 0; s.hs_lo = (s.hs_n == 8u) ? 0x1FF4u : 0x1FFAu - s.hs_n;
-  const bool regroups = ROMS && rm.size == 8192 && p.regroup;      // block-uniform
+  s.hs_n = (rm.hs >> 16) & 0xFFu; s.hs_lo = rm.hs & 0xFFFFu; s.kind = rm.kind;
+  const bool regroups = ROMS && rm.kind == MK_F8 && p.regroup;      // block-uniform
   s.park = regroups ? 1u : 0u;
   s.rom_off = ROM_OFF; s.rom_g = p.rom_blob + rm.offset; s.dr = p.drom + rm.doff; 
   s.rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
@@ -1265,7 +1308,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     p.st[W_PORTS * B + e] = T::S(fs, S_PORTS);
     p.st[W_COLU * B + e] = T::S(fs, S_COLU); p.st[W_PF * B + e] = T::S(fs, S_PF); p.st[W_GRP * B + e] = T::S(fs, S_GRP); p.st[W_NUSIZ * B + e] = T::S(fs, S_NUSIZ);
     p.st[W_POS * B + e] = T::S(fs, S_POS); p.st[W_POS2 * B + e] = (T::S(fs, S_POS2) & 0xFFFF) | (T::S(fs, S_RX) << 16);
-    p.st[W_FLAGS * B + e] = T::S(fs, S_FL) & TF_ARCH_MASK; p.st[W_CX * B + e] = T::S(fs, S_CX);
+    p.st[W_FLAGS * B + e] = T::S(fs, S_FL) & TF_ARCH_MASK; p.st[W_CX * B + e] = T::S(fs, S_CX); p.st[W_CART * B + e] = T::S(fs, S_CART);
     for (int i = 0; i < 32; ++i) p.ram[i * B + e] = smem[(S_RAM + i) * BLOCK + fs];
     p.cyc[e] += (unsigned long long)s.cyc;
   }

@@ -7,7 +7,7 @@ namespace vcs {
 
 
 struct StepParams {
-  uint32_t *st; uint32_t *ram; unsigned long long *cyc; uint8_t *screen;
+  uint32_t *st; uint32_t *ram; unsigned long long *cyc; uint8_t *screen; uint32_t *sc_ram;
   const uint8_t *rom_blob; const uint2 *drom; const RomMeta *rom_meta; const int32_t *env_rom;
   const uint8_t *actions; const uint8_t *switches; const uint8_t *mask; uint32_t *boot;
   const int32_t *perm; unsigned long long *blk_time;       // block placement (vcs_step.cu, rebalance_kernel): perm[blockIdx] = env group; blk_time[3 * blockIdx] = start ns, end ns, SM id   // switches: SWCHB input pins per env; mask: nullptr = every env steps; boot: per-env boot countdown (vcs_auto_reset)

@@ -16,7 +16,8 @@ NCPU = os.cpu_count() or 1
 def pair(roms, seeds, env_rom=None, **kw):
     from paper_2606_22447_b200 import VCS
     from oracle.ovcs_py import OracleVCS
-    return VCS(roms, seeds, env_rom, **kw), OracleVCS(roms, seeds, env_rom, **kw)
+    okw = {k: v for k, v in kw.items() if k != "flags"}
+    return VCS(roms, seeds, env_rom, **kw), OracleVCS(roms, seeds, env_rom, **okw)
 
 
 def run(torch, roms, env_rom, steps, tag, frameskip=4):
@@ -75,3 +76,85 @@ def test_soft_mode_on_f6(torch):
         a = np.array([r.rnd(18) for _ in range(n)], np.uint8)
         g.step_soft(torch.from_numpy(a).cuda(), 2, 1.0, 4.0); o.step(a, 2, threads=NCPU)     # Theorem 1/3: soft forward == hard
         compare(g, o, f"soft f6 step {t}")
+
+
+# ---------------------------------------------------------------------------------------------- Superchip, E0, FE
+from vcs_inputs import superchip_rom, e0_rom, fe_rom
+
+
+def compare_cart_ram(g, o, tag):
+    assert (g.get_cart_ram().cpu().numpy() == o.cart_ram()).all(), f"{tag}: Superchip RAM differs"
+
+
+def run_kinds(torch, roms, kinds, env_rom, steps, tag, **kw):
+    n = len(env_rom)
+    g, o = pair(roms, env_seeds(37, n), np.asarray(env_rom, np.int32), mappers=kinds, **kw)
+    r = SplitMix64(99 + n)
+    compare(g, o, f"{tag} reset"); compare_cart_ram(g, o, f"{tag} reset")
+    for t in range(steps):
+        a = np.array([r.rnd(18) for _ in range(n)], np.uint8)
+        fs = 1 + t % 3
+        g.step(torch.from_numpy(a).cuda(), fs); o.step(a, fs, threads=NCPU)
+        compare(g, o, f"{tag} step {t}"); compare_cart_ram(g, o, f"{tag} step {t}")
+    regs = g.regs_host()
+    g.close(); o.close()
+    return regs
+
+
+@pytest.mark.parametrize("kind", ["F8SC", "F6SC", "F4SC"])
+def test_superchip_carts(torch, kind):
+    regs = run_kinds(torch, [superchip_rom(kind, 21), superchip_rom(kind, 22)], [kind, kind], [e // 72 for e in range(144)], 8, kind, max_lines=200)
+    assert (regs["status"] == 0).all() and len(set(regs["bank"].tolist())) > 1
+
+
+def test_e0_carts(torch):
+    regs = run_kinds(torch, [e0_rom(31), e0_rom(32)], ["E0", "E0"], [e // 72 for e in range(144)], 8, "E0", max_lines=200)
+    assert (regs["status"] == 0).all() and len(set(zip(regs["bank"].tolist(), regs["pad"][:, 0].tolist()))) > 4
+
+
+def test_fe_carts(torch):
+    regs = run_kinds(torch, [fe_rom(41), fe_rom(42)], ["FE", "FE"], [e // 72 for e in range(144)], 8, "FE", max_lines=200)
+    assert (regs["status"] == 0).all()
+
+
+def test_all_ten_formats_in_one_batch(torch):
+    """every lane of a warp on a cartridge of another format, the Superchip program also run as a plain F8 image (no RAM there)"""
+    roms = [make_rom(7, FEATURES[1]), make_rom(8, FEATURES["4a"]), make_rom(9, FEATURES["4b"]), make_rom(10, FEATURES["f6"]), make_rom(11, FEATURES["f4"]),
+            superchip_rom("F8SC", 51), superchip_rom("F6SC", 52), superchip_rom("F4SC", 53), e0_rom(54), fe_rom(55), superchip_rom("F8SC", 51)]
+    kinds = ["2K", "4K", "F8", "F6", "F4", "F8SC", "F6SC", "F4SC", "E0", "FE", "F8"]
+    run_kinds(torch, roms, kinds, [(e * 5) % 11 for e in range(165)], 8, "ten formats", max_lines=220)
+
+
+def test_special_formats_instruction_steps_and_blocks(torch):
+    """the same carts in 256-env blocks that share a ROM (staged in shared memory), and stepped by instructions"""
+    from paper_2606_22447_b200.binding import VCS_F_BLOCK_256
+    roms = [superchip_rom("F8SC", 61), e0_rom(62), fe_rom(63)]; kinds = ["F8SC", "E0", "FE"]
+    env_rom = [e // 256 for e in range(768)]
+    from paper_2606_22447_b200 import VCS
+    from oracle.ovcs_py import OracleVCS
+    seeds = env_seeds(5, 768)
+    g = VCS(roms, seeds, np.asarray(env_rom, np.int32), mappers=kinds, max_lines=200, flags=VCS_F_BLOCK_256)
+    o = OracleVCS(roms, seeds, np.asarray(env_rom, np.int32), mappers=kinds, max_lines=200)
+    r = SplitMix64(3)
+    for t in range(4):
+        a = np.array([r.rnd(18) for _ in range(768)], np.uint8)
+        g.step(torch.from_numpy(a).cuda(), 2); o.step(a, 2, threads=NCPU)
+        compare(g, o, f"special blocks step {t}"); compare_cart_ram(g, o, f"special blocks step {t}")
+    for n in (1, 13, 700):
+        a = np.array([r.rnd(18) for _ in range(768)], np.uint8)
+        g.step_instructions(torch.from_numpy(a).cuda(), n); o.step_instructions(a, n, threads=NCPU)
+        gr, orr = g.regs_host(), o.regs()
+        for f in gr.dtype.names:
+            assert (gr[f] == orr[f]).all(), f"instructions {n}: regs.{f}"
+        assert (g.ram_host() == o.ram()).all(); compare_cart_ram(g, o, f"instructions {n}")
+
+
+def test_format_errors(torch):
+    from paper_2606_22447_b200 import VCS, VcsError
+    with pytest.raises(VcsError):
+        VCS([bytes(4096)], env_seeds(1, 4), mappers=["E0"])                         # E0 is an 8 KB format
+    with pytest.raises(VcsError):
+        VCS([bytes(8192)], env_seeds(1, 4), mappers=[77])
+    g = VCS([e0_rom(1)], env_seeds(1, 4), mappers=["E0"])
+    with pytest.raises(VcsError):
+        g.step_soft(torch.zeros(4, dtype=torch.uint8, device="cuda"), 1, 1.0, 4.0)   # hard mode only
