@@ -13,6 +13,9 @@
 #include "vcs_decode.cuh"
 
 using namespace vcs;
+#ifndef VCS_BALANCE_A
+#define VCS_BALANCE_A 1.27f         // measured slowdown of a block that shares its SM
+#endif
 
 struct vcs_s : Handle {};
 
@@ -280,7 +283,7 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
     CU(h, cudaMalloc((void **)&h->d_w_avg, sizeof(float) * nblk));
     CU(h, cudaMemset(h->d_w_avg, 0, sizeof(float) * nblk));
     h->balance = (c.flags & VCS_F_NO_BALANCE) ? 0 : 1; h->plain_steps = 0;
-    h->balance_a = 1.27f;                             // measured slowdown of a block that shares its SM
+    h->balance_a = VCS_BALANCE_A;                             // measured slowdown of a block that shares its SM
   }
   {                                                                                     // soft mode: every entry decodes at run time (vcs_step_soft)
     std::vector<DWord> sl((h->max_rom < 8192 ? 8192 : h->max_rom) + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});

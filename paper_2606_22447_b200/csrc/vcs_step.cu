@@ -1139,11 +1139,14 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
     alu(h, aux, v);
   seq:                                                     // sequential successor
     h.wx = wn.x; h.wy = wn.y;
-    if (!(wn.x & DW_LEADER)) continue;
+    // a leader is where another lane of the warp may be waiting: re-form the group — unless all 32 lanes are in this
+    // group already (nobody can be waiting; which lanes run together never changes results, only the time they take)
+    if (!(wn.x & DW_LEADER) || __activemask() == 0xFFFFFFFFu) continue;
     return;
   ctl:                                                     // taken branch / jump: fetch at the new PC, re-schedule
     if (!((h.pbase + h.di) & 0x1000u)) { h.wx = HC_COLD + H_SLOW; h.wy = 0; }
     else { const uint2 t = __ldg(dr + h.di); h.wx = t.x; h.wy = t.y; }
+    if (__activemask() == 0xFFFFFFFFu) continue;           // (the whole warp took it together)
     return;
   }
 }
