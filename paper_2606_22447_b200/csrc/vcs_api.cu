@@ -156,7 +156,7 @@ StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
   p.actions = actions; p.switches = h->d_switches; p.mask = nullptr; p.boot = h->d_boot_ctr; p.perm = h->d_perm; p.blk_time = nullptr; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
   p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom;
-  p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0; p.n_instr = 0;
+  p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_ent = nullptr; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0; p.n_instr = 0;
   return p;
 }
 
@@ -226,13 +226,13 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   h->regroup = (c.flags & VCS_F_NO_REGROUP) ? 0 : 1;
   // pre-decode every byte offset of every bank once (vcs_decode.cuh); the words depend on the launch shape
   // (zero-page RAM operands are stored as shared-memory offsets)
-  std::vector<DWord> dw(dwords + 8, DWord{0, 0}), dwp(dwords + 8, DWord{0, 0});      // dwp: the plain table of vcs_step_instructions
+  std::vector<DWord> dw(dwords + 8, DWord{0, 0}), dwp(dwords + 8, DWord{0, 0}), dws(dwords + 8, DWord{0, 0});   // dwp: the plain table of vcs_step_instructions; dws: soft mode's
   {
     std::vector<uint8_t> img(4096 + 4, 0), leader(4096);
     for (int r = 0; r < n_roms; ++r) {
       const int nb = (roms[r].size < 4096) ? 1 : (int)(roms[r].size / 4096);
       if (meta[r].kind == MK_E0 || meta[r].kind == MK_FE) {         // 1 KB windows / a bank that follows the data bus: every byte decodes at run time
-        for (size_t i = 0; i < (size_t)nb * 4096; ++i) { dw[meta[r].doff + i] = DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0}; dwp[meta[r].doff + i] = dw[meta[r].doff + i]; }
+        for (size_t i = 0; i < (size_t)nb * 4096; ++i) { dw[meta[r].doff + i] = DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0}; dwp[meta[r].doff + i] = dw[meta[r].doff + i]; dws[meta[r].doff + i] = dw[meta[r].doff + i]; }
         continue;
       }
       const bool sc = (meta[r].hs & HS_SC) != 0;
@@ -245,7 +245,8 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
           else { decode_bank(img.data(), leader.data(), h->block, nb, dw.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE), sc);
                  if (!(c.flags & VCS_F_NO_SPIN)) mark_spins(img.data(), dw.data() + meta[r].doff + 4096 * b);
                  if (!(c.flags & VCS_F_NO_FUSE)) fuse_ld_st(dw.data() + meta[r].doff + 4096 * b);
-                 decode_bank(img.data(), leader.data(), 128, nb, dwp.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE), sc); }
+                 decode_bank(img.data(), leader.data(), 128, nb, dwp.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE), sc);
+                 decode_bank(img.data(), leader.data(), 128, nb, dws.data() + meta[r].doff + 4096 * b, !(c.flags & VCS_F_NO_PROMOTE), sc); }
         }
     }
   }
@@ -285,17 +286,17 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
     h->balance = (c.flags & VCS_F_NO_BALANCE) ? 0 : 1; h->plain_steps = 0;
     h->balance_a = VCS_BALANCE_A;                             // measured slowdown of a block that shares its SM
   }
-  {                                                                                     // soft mode: every entry decodes at run time (vcs_step_soft)
-    std::vector<DWord> sl((h->max_rom < 8192 ? 8192 : h->max_rom) + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});
-    std::vector<RomMeta> ms(meta); for (auto &m : ms) { m.pad = m.doff; m.doff = 0; }     // pad: offset into the W(T) x ROM table
+  {                                                   // soft mode (vcs_step_soft): its own decode table (128-env blocks, one entry per instruction);
+    std::vector<RomMeta> ms(meta); for (auto &m : ms) m.pad = m.doff;     // pad: offset into the W(T) x ROM table
     h->soft_tab_n = dwords; h->soft_tab_T = -1.f;
     CU(h, cudaMalloc((void **)&h->d_soft_tab, sizeof(float) * (dwords + 8)));
-    CU(h, cudaMalloc((void **)&h->d_drom_soft, sizeof(DWord) * sl.size()));
-    CU(h, cudaMemcpy(h->d_drom_soft, sl.data(), sizeof(DWord) * sl.size(), cudaMemcpyHostToDevice));
+    CU(h, cudaMalloc((void **)&h->d_soft_ent, sizeof(float4) * (dwords + 8)));
+    CU(h, cudaMalloc((void **)&h->d_drom_soft, sizeof(DWord) * dws.size()));
+    CU(h, cudaMemcpy(h->d_drom_soft, dws.data(), sizeof(DWord) * dws.size(), cudaMemcpyHostToDevice));
     CU(h, cudaMalloc((void **)&h->d_rom_meta_soft, sizeof(RomMeta) * n_roms));
     CU(h, cudaMemcpy(h->d_rom_meta_soft, ms.data(), sizeof(RomMeta) * n_roms, cudaMemcpyHostToDevice));
-    CU(h, cudaMalloc((void **)&h->d_soft_w, sizeof(float) * 1024));
-    CU(h, cudaMallocHost((void **)&h->h_soft_w, sizeof(float) * 1024));
+    CU(h, cudaMalloc((void **)&h->d_soft_w, sizeof(float) * SOFT_W_WORDS));
+    CU(h, cudaMallocHost((void **)&h->h_soft_w, sizeof(float) * SOFT_W_WORDS));
     CU(h, cudaEventCreateWithFlags(&h->soft_w_done, cudaEventDisableTiming));
   }
   upload_optable();
@@ -431,19 +432,24 @@ int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float 
   if (h->soft_tab_T != T) {                            // a new temperature: e^{-k/T} and W(T) x ROM, once
     int K = (int)ceil(17.0 * (double)T); if (K < 1) K = 1; if (K > 1023) K = 1023;
     CU(h, cudaEventSynchronize(h->soft_w_done));       // (the previous upload from the handle's pinned buffer; long since done)
-    for (int k = 0; k <= K; ++k) h->h_soft_w[k] = (float)exp(-(double)k / (double)T);
-    CU(h, cudaMemcpyAsync(h->d_soft_w, h->h_soft_w, sizeof(float) * (K + 1), cudaMemcpyHostToDevice, s));
+    for (int k = 0; k < SOFT_W_N; ++k) h->h_soft_w[k] = k <= K ? (float)exp(-(double)k / (double)T) : 0.f;
+    double cw = 0.0;                                   // normaliser of a RAM-tape window reaching n cells to one side (soft_ram_read)
+    for (int n = 0; n < 128; ++n) { if (n <= K) cw += exp(-(double)n / (double)T); h->h_soft_w[SOFT_CW + n] = (float)cw; }
+    CU(h, cudaMemcpyAsync(h->d_soft_w, h->h_soft_w, sizeof(float) * SOFT_W_WORDS, cudaMemcpyHostToDevice, s));
     CU(h, cudaEventRecord(h->soft_w_done, s));
     cudaError_t ce0 = launch_soft_table(h->d_rom_blob, h->d_rom_meta_soft, h->n_roms, h->d_soft_w, K, h->d_soft_tab, s);
     h->launches += 1;
     if (ce0 != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_soft table launch", ce0);
+    ce0 = launch_soft_entries(h->d_rom_blob, h->d_rom_meta_soft, h->n_roms, h->d_drom_soft, h->d_soft_tab, h->d_soft_ent, s);
+    h->launches += 1;
+    if (ce0 != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_soft entry-table launch", ce0);
     h->soft_tab_T = T; h->soft_K = K;
   }
   CU(h, cudaMemsetAsync(soft_out_dev, 0, sizeof(float) * 8 * (size_t)h->batch, s));
   StepParams p = params_of(h, actions_dev, frameskip);
   p.drom = h->d_drom_soft; p.rom_meta = h->d_rom_meta_soft;
   p.perm = nullptr;                                    // the soft kernel has its own launch shape (128 envs per block): blocks in env order
-  p.soft_w = h->d_soft_w; p.soft_tab = h->d_soft_tab; p.soft_out = soft_out_dev; p.soft_alpha = alpha; p.soft_K = h->soft_K;
+  p.soft_w = h->d_soft_w; p.soft_tab = h->d_soft_tab; p.soft_ent = h->d_soft_ent; p.soft_out = soft_out_dev; p.soft_alpha = alpha; p.soft_K = h->soft_K;
   cudaError_t ce = launch_step(p, s);
   h->launches += 1;
   if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_soft launch", ce);
@@ -574,7 +580,7 @@ int vcs_destroy(vcs_t h) {
   if (cur != h->device) cudaSetDevice(h->device);     // free on the handle's own device, then give the caller's back
   cudaDeviceSynchronize();
   cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_sc_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom); cudaFree(h->d_drom_plain);
-  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr); cudaFree(h->d_perm); cudaFree(h->d_blk_time); cudaFree(h->d_w_avg);
+  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_soft_ent); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr); cudaFree(h->d_perm); cudaFree(h->d_blk_time); cudaFree(h->d_w_avg);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   if (h->h_soft_w) cudaFreeHost(h->h_soft_w);
   if (h->soft_w_done) cudaEventDestroy(h->soft_w_done);

@@ -103,9 +103,10 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   uint8_t *d_rom_blob; uint2 *d_drom; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
   int device;                   // the CUDA device every pointer below belongs to
   float *h_soft_w; cudaEvent_t soft_w_done; int soft_K;            // soft mode: pinned e^{-k/T} staging buffer, its upload, window of the cached temperature
+  float4 *d_soft_ent;           // soft mode: per decode entry of d_drom_soft, the soft sums of the instruction's own bytes at the cached temperature
   float *d_soft_tab; float soft_tab_T; size_t soft_tab_n;          // W(T) x ROM: the relaxed read of every ROM cell at the cached temperature
   uint2 *d_drom_plain;          // vcs_step_instructions: a decode table for 128-env blocks without fused / closed-form entries (one entry = one instruction)
-  uint2 *d_drom_soft; RomMeta *d_rom_meta_soft; float *d_soft_w;   // soft mode: an all-H_SLOW decode table (every byte fetched at run time), metas with doff 0, e^{-k/T}
+  uint2 *d_drom_soft; RomMeta *d_rom_meta_soft; float *d_soft_w;   // soft mode: a decode table for 128-env blocks, one entry per instruction, indexed / stack instructions out of line; metas with pad = doff; e^{-k/T}
   uint8_t *d_actions_stage;     // for vcs_step_host
   uint8_t *d_switches;          // SWCHB input pins per env (vcs_set_switches; 0x3F after vcs_create)
   int32_t *d_perm; unsigned long long *d_blk_time; long long plain_steps; int balance; float balance_a; float *d_w_avg;   // block placement (rebalance_kernel in vcs_step.cu)

@@ -134,6 +134,65 @@ DEV void io_dummy_intim(uint32_t sl, int32_t ticks) {      // a discarded read o
   uint32_t t, s, sh, f; Riot<BLOCK, TAG>::timer_sync(sl, ticks, t, s, sh, f); Riot<BLOCK, TAG>::timer_put(sl, t, s, sh, 0);
 }
 
+// ---- SOFT-STE mode (vcs_step_soft; eq. (8)-(10), reading R14): per-env sums in shared memory behind the block
+// context (the soft kernel stages no ROM): word k of env slot sl at SOFT_ACC + k * BLOCK + sl, k = sum of soft ROM reads,
+// of soft RAM reads, of branch gates, the three counts, STE/hard mismatches, max |soft - hard|.
+template <int BLOCK> DEV float &soft_acc(uint32_t sl, int k) { return reinterpret_cast<float *>(smem)[S_WORDS * BLOCK + C_WORDS + k * BLOCK + sl]; }
+template <int BLOCK> DEV void soft_note(uint32_t sl, int k, float soft_v, float hard, float ste) {
+  soft_acc<BLOCK>(sl, k) += soft_v; soft_acc<BLOCK>(sl, 3 + k) += 1.f;
+  if (rintf(ste) != hard) soft_acc<BLOCK>(sl, 6) += 1.f;
+  if (k < 2) soft_acc<BLOCK>(sl, 7) = fmaxf(soft_acc<BLOCK>(sl, 7), fabsf(soft_v - hard));
+}
+// eq. (10) on the 128-cell RAM tape, window |k| <= K clipped to the tape, then STE + round (one copy: the inline loop and
+// the out-of-line executor both read RAM through it in soft mode).  The weights are e^{-|k|/T} = q^|k|, so each side of
+// the window is a Horner chain from its far end towards the cell, taken a RAM word (4 cells) at a time: the four cells
+// of a word combine off the critical path and the running sum advances by one multiply-add (x q^4) per word; no weight
+// loads.  The normaliser comes from the cumulative table cw[n] = sum_{j<=n} e^{-j/T} (host, in double): den = cw[nl] +
+// cw[nr] - 1.  `hard` is ram[cell].
+template <int BLOCK>
+__device__ __noinline__ uint32_t soft_ram_read(uint32_t sl, uint32_t cell, uint32_t hard) {
+  using T = Tia<BLOCK>;
+  const int K = (int)T::ctx(C_SOFT_K);
+  const float *wt = reinterpret_cast<const float *>((unsigned long long)T::ctx(C_SOFT_W_LO) | ((unsigned long long)T::ctx(C_SOFT_W_HI) << 32));
+  const uint32_t *ramw = smem + sl;                        // RAM word i of this env at ramw[i * BLOCK], cell 4 i + j in byte j
+  const float q = __ldg(wt + 1), q4 = (q * q) * (q * q);
+  const int c = (int)cell, nl = min(K, c), nr = min(K, 127 - c), a = c - nl, b = c + nr, wc = c >> 2, m = c & 3;
+  const uint32_t keep_a = 0xFFFFFFFFu << (8 * (a & 3)), keep_b = 0xFFFFFFFFu >> (8 * (3 - (b & 3)));   // cells of the edge words inside [a, b]
+  auto f = [](uint32_t x, int j) { return (float)((x >> (8 * j)) & 0xFFu); };
+  float L = 0.f, R = 0.f;                                  // L: sum_{j < 4 wc} q^(4 wc - 1 - j) ram[j];  R: sum_{j >= 4 wc + 4} q^(j - 4 wc - 4) ram[j]
+#pragma unroll 2
+  for (int w = a >> 2; w < wc; ++w) {
+    uint32_t x = ramw[w * BLOCK]; if (w == (a >> 2)) x &= keep_a;
+    L = fmaf(L, q4, fmaf(fmaf(fmaf(f(x, 0), q, f(x, 1)), q, f(x, 2)), q, f(x, 3)));
+  }
+#pragma unroll 2
+  for (int w = b >> 2; w > wc; --w) {
+    uint32_t x = ramw[w * BLOCK]; if (w == (b >> 2)) x &= keep_b;
+    R = fmaf(R, q4, fmaf(fmaf(fmaf(f(x, 3), q, f(x, 2)), q, f(x, 1)), q, f(x, 0)));
+  }
+  uint32_t x = ramw[wc * BLOCK];                           // the cell's own word: up to 3 more cells on either side
+  if ((a >> 2) == wc) x &= keep_a;
+  if ((b >> 2) == wc) x &= keep_b;
+  if (m > 0) L = fmaf(L, q, f(x, 0));
+  if (m > 1) L = fmaf(L, q, f(x, 1));
+  if (m > 2) L = fmaf(L, q, f(x, 2));
+  if (m < 3) R = fmaf(R, q, f(x, 3));
+  if (m < 2) R = fmaf(R, q, f(x, 2));
+  if (m < 1) R = fmaf(R, q, f(x, 1));
+  const float h = (float)hard;
+  const float sv = (h + (L + R) * q) / (__ldg(wt + SOFT_CW + nl) + __ldg(wt + SOFT_CW + nr) - 1.f), ste = sv + (h - sv);
+  soft_note<BLOCK>(sl, 1, sv, h, ste);
+  return (uint32_t)(int)rintf(ste) & 0xFFu;
+}
+// eq. (8) + STE for a conditional branch: f = the flag tested, sense = +1 branch-if-set / -1 branch-if-clear
+template <int BLOCK>
+__device__ __noinline__ void soft_branch_note(uint32_t sl, uint32_t f, float sense, float delta, bool taken, float pc_nb) {
+  const float z = sense * (2.f * (float)f - 1.f), alpha = __uint_as_float(Tia<BLOCK>::ctx(C_SOFT_ALPHA));
+  const float g = 1.f / (1.f + expf(-alpha * z));
+  const float pc_soft = pc_nb + g * delta, pc_hard = pc_nb + (taken ? delta : 0.f);
+  soft_note<BLOCK>(sl, 2, g, pc_hard, pc_soft + (pc_hard - pc_soft));
+}
+
 // What the inline interpreter loop keeps in registers.  A, X, Y, SP are the four bytes of `axys`, so that "which
 // register" is a byte-permute selector from the decode entry; `fl` holds C, I, D, V at their P-register bits.
 // Everything else of an environment (status, frame start, TIA/RIOT latches, RAM) lives in its shared-memory file
@@ -180,8 +239,7 @@ struct Cpu {
   const uint2 *dr;         // decode entries of this env's ROM (4096 per bank)
   uint2 w;            // decode entry at (bank, PC) — valid at every scheduling point
   uint32_t sl, sl4;   // this thread's file slot (word i of the file lives at smem[i*BLOCK + sl]) and 4*sl
-  float *soft;        // SOFT-STE mode (vcs_step_soft): this env's 8 output sums, else nullptr
-  const float *soft_tab;   // ... and the relaxed read of every cell of this env's ROM (4096 per bank)
+  const float *soft_tab;   // SOFT-STE mode (vcs_step_soft): the relaxed read of every cell of this env's ROM (4096 per bank), else nullptr
 
   DEV uint32_t &S(int i) const { return T::S(sl, i); }
 
@@ -201,11 +259,9 @@ struct Cpu {
       hs_n = (rm.hs >> 16) & 0xFFu; hs_lo = rm.hs & 0xFFFFu; kind = rm.kind; rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
       rom_g = reinterpret_cast<const uint8_t *>(ptr(C_BLOB_LO)) + rm.offset;
       dr = reinterpret_cast<const uint2 *>(ptr(C_DROM_LO)) + rm.doff;
-      if constexpr (SOFT) {
-        soft = reinterpret_cast<float *>(ptr(C_SOFT_OUT_LO)) + 8 * (size_t)(T::ctx(C_ENV0) + (S(S_INP) >> 16));
-        soft_tab = reinterpret_cast<const float *>(ptr(C_SOFT_TAB_LO)) + rm.pad;
-      } else { soft = nullptr; soft_tab = nullptr; }
-    } else { hs_n = 0; hs_lo = 0; kind = MK_4K; rom_mask = 0xFFFu; rom_g = nullptr; dr = nullptr; soft = nullptr; soft_tab = nullptr; }
+      if constexpr (SOFT) soft_tab = reinterpret_cast<const float *>(ptr(C_SOFT_TAB_LO)) + rm.pad;
+      else soft_tab = nullptr;
+    } else { hs_n = 0; hs_lo = 0; kind = MK_4K; rom_mask = 0xFFFu; rom_g = nullptr; dr = nullptr; soft_tab = nullptr; }
     park = T::ctx(C_REGROUP) | ((keyhi == KEY_PARKED) ? 2u : 0u);
   }
   DEV Hot store() const {
@@ -356,38 +412,16 @@ struct Cpu {
     if constexpr (TAG == 1) fe_snoop(a, v);
   }
   // ---------------------------------------------------------------- SOFT-STE mode (include/vcs.h vcs_step_soft; eq. 8-10)
-  DEV void soft_note(int k, float soft_v, float hard, float ste) {
-    soft[k] += soft_v; soft[3 + k] += 1.f;
-    if (rintf(ste) != hard) soft[6] += 1.f;
-    if (k < 2) soft[7] = fmaxf(soft[7], fabsf(soft_v - hard));
-  }
   DEV uint32_t soft_rom(uint32_t o, uint32_t hard) {       // eq. (10) on the 4096 x 8 bit tensor of the visible bank, then STE + round
     // the ROM is constant, so W(T) x ROM is computed once per temperature (soft_table_kernel): a fetch is one lookup
     const float sv = __ldg(soft_tab + (di & 0x7000u) + o);
     const float h = (float)hard, ste = sv + (h - sv);      // eq. (9), forward
-    soft_note(0, sv, h, ste);
+    soft_note<BLOCK>(sl, 0, sv, h, ste);
     return (uint32_t)(int)rintf(ste) & 0xFFu;
   }
-  DEV uint32_t soft_ram(uint32_t cell, uint32_t hard) {    // eq. (10) on the 128-cell RAM tape
-    const int K = (int)T::ctx(C_SOFT_K);
-    const float *wt = reinterpret_cast<const float *>((unsigned long long)T::ctx(C_SOFT_W_LO) | ((unsigned long long)T::ctx(C_SOFT_W_HI) << 32));
-    float num = 0, den = 0;
-    const int lo = max(-K, -(int)cell), hi = min(K, 127 - (int)cell);
-#pragma unroll 1
-    for (int k = lo; k <= hi; ++k) {
-      const float w = __ldg(wt + abs(k));
-      const uint32_t c = (uint32_t)((int)cell + k);
-      num += w * (float)ram_rd_off(((c & 0x7Cu) * BLOCK) | (c & 3u)); den += w;
-    }
-    const float sv = num / den, h = (float)hard, ste = sv + (h - sv);
-    soft_note(1, sv, h, ste);
-    return (uint32_t)(int)rintf(ste) & 0xFFu;
-  }
-  DEV void soft_branch(uint32_t f, float sense, float delta, bool taken) {   // eq. (8) + STE; the PC itself is set by the hard path
-    const float z = sense * (2.f * (float)f - 1.f), alpha = __uint_as_float(T::ctx(C_SOFT_ALPHA));
-    const float g = 1.f / (1.f + expf(-alpha * z));
-    const float pc_nb = (float)pc(), pc_soft = pc_nb + g * delta, pc_hard = pc_nb + (taken ? delta : 0.f);
-    soft_note(2, g, pc_hard, pc_soft + (pc_hard - pc_soft));
+  DEV uint32_t soft_ram(uint32_t cell, uint32_t hard) { return soft_ram_read<BLOCK>(sl, cell, hard); }
+  DEV void soft_branch(uint32_t f, float sense, float delta, bool taken) {   // the PC itself is set by the hard path (R14)
+    soft_branch_note<BLOCK>(sl, f, sense, delta, taken, (float)pc());
   }
   DEV uint32_t pack_p() const {
     return ((zn & 0x180u) ? 0x80u : 0u) | (fV << 6) | 0x20u | fDI | (((zn & 0xFFu) == 0) ? 2u : 0u) | fC;
@@ -932,6 +966,7 @@ DEV bool plain_addr(uint32_t addr, uint32_t hs) {
   if constexpr (ROMS) return (a & 0x1000u) && (a - (hs & 0xFFFFu)) >= ((hs >> 16) & 0xFFu) && !((hs & HS_SC) && (a & 0x0F00u) == 0);
   else return false;                                       // (ROM in global memory: left to the out-of-line executor)
 }
+template <int BLOCK> DEV uint32_t cell_of(uint32_t off) { return ((off / BLOCK) & 0x7Cu) | (off & 3u); }   // RAM cell of a smem byte offset
 template <int BLOCK, bool ROMS>
 DEV uint32_t rom_byte_hot(uint32_t off) {                  // byte `off` (bank << 12 | offset) of the block's staged ROM
   if constexpr (ROMS) return reinterpret_cast<const uint8_t *>(smem)[(S_WORDS * BLOCK + C_WORDS) * 4 + off];
@@ -940,10 +975,14 @@ DEV uint32_t rom_byte_hot(uint32_t off) {                  // byte `off` (bank <
 
 // ---------------------------------------------------------------------------------------------------------------
 // The inline interpreter loop: instructions of this lane's min-key group until the next scheduling point.
+// SOFT: `se` = per decode entry {sum of the soft values of the instruction's own bytes, their count, their largest
+// |soft - hard|, STE mismatches among them} (soft_entry_kernel); data reads of RAM and branches are noted where they run.
 template <int BLOCK, bool ROMS, int THREADS, bool SOFT, bool COUNT = false>
-DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
+DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl, const float4 *se = nullptr, const float *stab = nullptr) {
   using T = Tia<BLOCK>;
   uint8_t *const ramb = reinterpret_cast<uint8_t *>(smem) + 4u * sl;
+  auto soft_cell = [&](uint32_t a, uint32_t hard) -> uint32_t {          // SOFT: a value read of RAM cell a & 0x7F (else the byte as it is)
+    if constexpr (SOFT) return soft_ram_read<BLOCK>(sl, a & 0x7Fu, hard); else return hard; };
   for (;;) {
     if constexpr (COUNT) { if (T::S(sl, S_BUDGET) == 0) { h.keyhi = 0xFFFFFFFFu; return; } }   // the budget is spent: this lane is done
     if (h.cyc >= h.lim) {
@@ -956,6 +995,11 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
     if constexpr (COUNT) T::S(sl, S_BUDGET) -= 1u;         // (a frame end at the cap or an idle cycle above is not an instruction)
     uint32_t cx = h.wx, pl = h.wy;                         // the entry being executed
     const int32_t cyc0 = h.cyc;                            // its first cycle
+    if constexpr (SOFT) { if ((cx & 0x7Fu) != HC_COLD + H_SLOW) {     // the instruction's own bytes, pre-summed (one decoded at run time — code in RAM
+      const float4 e = __ldg(se + h.di);                             // included, whose di aliases a ROM entry — notes its bytes as it fetches them)
+      soft_acc<BLOCK>(sl, 0) += e.x; soft_acc<BLOCK>(sl, 3) += e.y; soft_acc<BLOCK>(sl, 6) += e.w;
+      soft_acc<BLOCK>(sl, 7) = fmaxf(soft_acc<BLOCK>(sl, 7), e.z);
+    } }
     h.di += (cx >> DW_LEN_SHIFT) & 0xFFu;
     uint2 wn = __ldg(dr + h.di);                           // sequential prefetch
     h.cyc += (int32_t)((cx >> DW_CY_SHIFT) & 0xFu);
@@ -985,7 +1029,9 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
     else if (cx & DW_F_LDIMM) { h.axys = __byte_perm(h.axys, pl, pl >> 16); h.zn = pl & 0xFFu; }
     else if (cx & DW_F_BR) {
       const uint32_t t = (h.fl & 0x41u) | ((h.zn & 0x180u) ? 0x80u : 0u) | ((h.zn & 0xFFu) ? 0u : 2u);
-      if (((t >> (aux & 7u)) & 1u) == ((aux >> 3) & 1u)) { h.di += pl; h.cyc += (int32_t)(aux >> 4); goto ctl; }
+      const bool taken = ((t >> (aux & 7u)) & 1u) == ((aux >> 3) & 1u);
+      if constexpr (SOFT) soft_branch_note<BLOCK>(sl, (t >> (aux & 7u)) & 1u, (aux & 8u) ? 1.f : -1.f, (float)(int32_t)pl, taken, (float)((h.pbase + h.di) & 0xFFFFu));
+      if (taken) { h.di += pl; h.cyc += (int32_t)(aux >> 4); goto ctl; }
     }
     else if (cls == HC_RTIM) {                             // absolute read of INTIM / TIMINT in the 4th cycle
     do_rtim:
@@ -1000,7 +1046,8 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
       v = (__byte_perm(h.axys, 0u, pl) + aux) & 0xFFu;
       h.axys = __byte_perm(h.axys, v, pl >> 16); h.zn = v;
     }
-    else if (cls == HC_LD_RAM) { v = ramb[pl & 0xFFFFu]; h.axys = __byte_perm(h.axys, v, pl >> 16); h.zn = v; }
+    else if (cls == HC_LD_RAM) { v = ramb[pl & 0xFFFFu]; if constexpr (SOFT) v = soft_ram_read<BLOCK>(sl, cell_of<BLOCK>(pl & 0xFFFFu), v);
+                                 h.axys = __byte_perm(h.axys, v, pl >> 16); h.zn = v; }
     else {
       switch (cls) {
         case HC_ST_RAM: ramb[pl & 0xFFFFu] = (uint8_t)__byte_perm(h.axys, 0u, pl >> 16); break;
@@ -1010,8 +1057,9 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
           else if (h.keyhi < KEY_PARKED) h.keyhi = (h.keyhi & ~(0xFFu << 19)) | (v << 19);      // TXS: SP is part of the key
           break;
         case HC_ALU_IMM: v = pl; goto do_alu;
-        case HC_ALU_RAM: v = ramb[pl]; goto do_alu;
-        case HC_RMW_RAM: v = rmw(h, aux, ramb[pl]); ramb[pl] = (uint8_t)v; break;
+        case HC_ALU_RAM: v = ramb[pl]; if constexpr (SOFT) v = soft_ram_read<BLOCK>(sl, cell_of<BLOCK>(pl), v); goto do_alu;
+        case HC_RMW_RAM: v = ramb[pl]; if constexpr (SOFT) v = soft_ram_read<BLOCK>(sl, cell_of<BLOCK>(pl), v);
+                         v = rmw(h, aux, v); ramb[pl] = (uint8_t)v; break;
         case HC_ACC: v = rmw(h, aux, h.axys & 0xFFu); h.axys = __byte_perm(h.axys, v, 0x3214u); break;
         case HC_FLAG: h.fl = (h.fl & ~pl) | (pl >> 16); break;
         case HC_NOP: break;
@@ -1086,8 +1134,19 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
             return;
           }
           const uint32_t ro = ((ea & 0x7Cu) * BLOCK) | (ea & 3u);
+          if constexpr (SOFT) {                            // the pointer bytes are value reads of RAM (their hard values formed ea)
+            if (cls == HC_IZY_RD || cls == HC_IZY_ST) { const uint32_t o = pl & 0x7FFFu, z = ((o / BLOCK) & 0x7Cu) | (o & 3u);
+                                                        soft_cell(z, ramb[o]); soft_cell(z + 1u, ramb[pl >> 15]); }
+            else if (cls == HC_IZX_RD || cls == HC_IZX_ST) { const uint32_t z = (pl + ((h.axys >> 8) & 0xFFu)) & 0xFFu;
+                                                             soft_cell(z, ramb[((z & 0x7Cu) * BLOCK) | (z & 3u)]); soft_cell(z + 1u, ramb[(((z + 1u) & 0x7Cu) * BLOCK) | ((z + 1u) & 3u)]); }
+          }
           if (store) { ramb[ro] = (uint8_t)__byte_perm(h.axys, 0u, 0x4440u | aux); break; }
-          v = in_ram ? (uint32_t)ramb[ro] : rom_byte_hot<BLOCK, ROMS>((h.di & 0x7000u) + (ea & 0xFFFu));
+          if (in_ram) v = soft_cell(ea, ramb[ro]);
+          else {
+            v = rom_byte_hot<BLOCK, ROMS>((h.di & 0x7000u) + (ea & 0xFFFu));
+            if constexpr (SOFT) { const float sv = __ldg(stab + (h.di & 0x7000u) + (ea & 0xFFFu)), hv = (float)v, ste = sv + (hv - sv);
+                                  soft_note<BLOCK>(sl, 0, sv, hv, ste); v = (uint32_t)(int)rintf(ste) & 0xFFu; }
+          }
         } goto do_alu;
         case HC_JSR: case HC_RTS: case HC_STACK: {
           const uint32_t sp = h.axys >> 24;
@@ -1101,6 +1160,7 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
             if (sp - 0x7Fu > 0xFDu - 0x7Fu) goto generic_stack;
             const uint32_t r = (uint32_t)cell(sp + 1u) | ((uint32_t)cell(sp + 2u) << 8);
             if (!((r & 0x1000u) && plain_addr<ROMS>(r, T::ctx(C_HS)))) goto generic_stack;   // the discarded read at the pulled address
+            if constexpr (SOFT) { soft_cell(sp + 1u, r & 0xFFu); soft_cell(sp + 2u, r >> 8); }
             nsp = sp + 2u; target = (r + 1u) & 0xFFFFu;
           } else if (aux < 2u) {                           // PHA / PHP
             if (sp < 0x80u) goto generic_stack;
@@ -1108,7 +1168,7 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl) {
             nsp = (sp - 1u) & 0xFFu; target = 0x10000u;
           } else {                                         // PLA / PLP
             if (sp - 0x7Fu > 0xFEu - 0x7Fu) goto generic_stack;
-            v = cell(sp + 1u); nsp = sp + 1u; target = 0x10000u;
+            v = soft_cell(sp + 1u, cell(sp + 1u)); nsp = sp + 1u; target = 0x10000u;
             if (aux == 2u) { h.axys = __byte_perm(h.axys, v, 0x3214u); h.zn = v; }
             else { h.fl = v & 0x4Du; h.zn = ((v & 0x80u) << 1) | ((v & 2u) ? 0u : 1u); }
           }
@@ -1270,6 +1330,9 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   else { h.axys = h.fl = h.zn = h.di = h.pbase = 0; h.cyc = h.lstart = 0; h.lim = LIM_NOW; h.wx = HC_COLD + H_SLOW; h.wy = 0; h.aux = 0; }
   h.keyhi = s.keyhi;
   const uint2 *const dr = s.dr;
+  const float4 *const se = SOFT ? p.soft_ent + rm.doff : nullptr;
+  const float *const stab = SOFT ? p.soft_tab + rm.pad : nullptr;
+  if constexpr (SOFT) { if (filed) { for (int k = 0; k < 8; ++k) soft_acc<BLOCK>(sl, k) = 0.f; } }
   uint32_t cur = sl;                                       // the file this thread runs (changes at a regroup)
 
   // ---- the hot loop: whole instructions until `frameskip` frame-end events (C.10), min-key lanes first.
@@ -1281,7 +1344,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
       const uint32_t key = h.keyhi | ((h.pbase + h.di) & 0xFFFFu);
       const uint32_t mk = __reduce_min_sync(0xFFFFFFFFu, key);
       if (mk >= KEY_PARKED) break;                         // every lane is parked or has finished the step
-      if (key == mk) run_block<BLOCK, ROMS, THREADS, SOFT, COUNT>(h, dr, cur);
+      if (key == mk) run_block<BLOCK, ROMS, THREADS, SOFT, COUNT>(h, dr, cur, se, stab);
       if (h.aux == AUX_GENERIC) h = cold_exec_generic<BLOCK, ROMS, THREADS, SOFT>(h, cur, h.wx, h.wy);   // (a rare bus pattern: see cold_exec)
     }
     if (!regroups) break;
@@ -1314,6 +1377,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     p.st[W_FLAGS * B + e] = T::S(fs, S_FL) & TF_ARCH_MASK; p.st[W_CX * B + e] = T::S(fs, S_CX); p.st[W_CART * B + e] = T::S(fs, S_CART);
     for (int i = 0; i < 32; ++i) p.ram[i * B + e] = smem[(S_RAM + i) * BLOCK + fs];
     p.cyc[e] += (unsigned long long)s.cyc;
+    if constexpr (SOFT) { for (int k = 0; k < 8; ++k) p.soft_out[8 * (size_t)e + k] = soft_acc<BLOCK>(fs, k); }
   }
   if (p.blk_time) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); atomicMax(&p.blk_time[3 * blockIdx.x + 1], t); }
 }
@@ -1343,6 +1407,35 @@ __global__ void soft_table_kernel(const uint8_t *rom_blob, const RomMeta *meta, 
 }
 cudaError_t launch_soft_table(const uint8_t *rom_blob, const RomMeta *meta, int n_roms, const float *w, int K, float *tab, cudaStream_t stream) {
   soft_table_kernel<<<dim3(32768 / 256, n_roms), 256, 0, stream>>>(rom_blob, meta, w, K, tab);
+  return cudaGetLastError();
+}
+
+// Per decode entry of the soft table: what fetching that instruction's own bytes adds to the soft sums (each byte is a
+// value read of the ROM tensor: eq. (10) from W(T) x ROM, then STE + round) — {sum, count, max |soft - hard|, mismatches}.
+// One-byte instructions and BRK read their second byte as a discarded cycle; an absolute load folded into an immediate
+// also reads its ROM operand; entries decoded at run time fetch (and note) their bytes themselves.
+__global__ void soft_entry_kernel(const uint8_t *rom_blob, const RomMeta *meta, const uint2 *drom, const float *tab, float4 *ent) {
+  const RomMeta rm = meta[blockIdx.y];
+  const int nb = max(1, (int)(rm.size >> 12));
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;            // bank * 4096 + o
+  if (idx >= nb * 4096) return;
+  const uint32_t bank = (uint32_t)idx >> 12, o = idx & 0xFFF, mask = (rm.size == 2048) ? 0x7FFu : 0xFFFu;
+  const uint8_t *img = rom_blob + rm.offset + bank * 4096;
+  const float *t = tab + rm.pad + bank * 4096;
+  const uint2 e = drom[rm.doff + idx];
+  const uint32_t cls = e.x & 0x7Fu, len = (e.x >> DW_LEN_SHIFT) & 0xFFu;
+  float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
+  auto add = [&](uint32_t off) { const float sv = t[off & 0xFFFu], h = (float)img[off & mask];
+                                 r.x += sv; r.y += 1.f; r.z = fmaxf(r.z, fabsf(sv - h)); if (rintf(sv + (h - sv)) != h) r.w += 1.f; };
+  if (cls != HC_COLD + H_SLOW) {
+    const uint32_t n = (cls == HC_COLD + H_ILL) ? 1u : (cls == HC_COLD + H_BRK) ? 1u : len;
+    for (uint32_t i = 0; i < n; ++i) add(o + i);
+    if ((cls == HC_LD_IMM || cls == HC_ALU_IMM) && len == 3u) add((uint32_t)img[(o + 1) & mask] | ((uint32_t)img[(o + 2) & mask] << 8));   // folded ROM operand
+  }
+  ent[rm.doff + idx] = r;
+}
+cudaError_t launch_soft_entries(const uint8_t *rom_blob, const RomMeta *meta, int n_roms, const uint2 *drom, const float *tab, float4 *ent, cudaStream_t stream) {
+  soft_entry_kernel<<<dim3(32768 / 256, n_roms), 256, 0, stream>>>(rom_blob, meta, drom, tab, ent);
   return cudaGetLastError();
 }
 
@@ -1431,13 +1524,13 @@ cudaError_t launch_rebalance(int32_t *perm, const unsigned long long *blk_time, 
   return cudaGetLastError();
 }
 
-size_t step_smem_bytes(int block, bool roms, uint32_t max_rom) {
-  return (size_t)(S_WORDS * block + C_WORDS) * 4 + (roms ? (max_rom < 4096 ? 4096 : max_rom) + 16 : 0);
+size_t step_smem_bytes(int block, bool roms, uint32_t max_rom, bool soft) {
+  return (size_t)(S_WORDS * block + C_WORDS) * 4 + (roms ? (max_rom < 4096 ? 4096 : max_rom) + 16 : 0) + (soft ? (size_t)8 * block * 4 : 0);
 }
 
 template <int BLOCK, bool ROMS, int THREADS, bool SOFT, bool COUNT = false>
 static cudaError_t launch_one(const StepParams &p, cudaStream_t stream) {
-  const size_t smem_bytes = step_smem_bytes(BLOCK, ROMS, p.max_rom);
+  const size_t smem_bytes = step_smem_bytes(BLOCK, ROMS, p.max_rom, SOFT);
   static size_t configured[64] = {0};                   // per device: the attribute belongs to the (function, device) pair
   int dev = 0; cudaGetDevice(&dev);
   if (dev < 0 || dev >= 64 || configured[dev] < smem_bytes) {
