@@ -172,18 +172,21 @@ struct Tia {
     const uint32_t ctrl = S(sl, S_PF) >> 24;
     uint32_t a0 = 0, a1 = 0, a2 = 0, a3 = 0, a4 = 0, a5 = 0, a6 = 0, a7 = 0, a8 = 0, a9 = 0, a10 = 0, a11 = 0, a12 = 0, a13 = 0, a14 = 0, any2 = 0;
     const int w1 = (x1 - 1) >> 5;
+    const uint32_t m_last = 0xFFFFFFFFu >> (31 - ((x1 - 1) & 31));           // pixels of the last word before x1
+    uint32_t m = 0xFFFFFFFFu << (x0 & 31);                                     // pixels of the word in hand inside [x0, x1): the first word starts at x0
+    uint32_t comb = ((fl & TF_HMBLANK) && x0 < 32) ? ~0xFFu : 0xFFFFFFFFu;     // HMOVE comb: x 0..7 black, no collisions (word 0 only)
 #pragma unroll 1
     for (int w = x0 >> 5; w <= w1; ++w) {
-      const int lo = max(x0 - 32 * w, 0), hi = min(x1 - 32 * w, 32);
-      const uint32_t rm = (hi >= 32 ? 0xFFFFFFFFu : ((1u << hi) - 1u)) & ~((1u << lo) - 1u);
-      uint32_t act = rm;
-      if ((fl & TF_HMBLANK) && w == 0) act &= ~0xFFu;             // HMOVE comb: x 0..7 black, no collisions
+      const uint32_t rm = (w == w1) ? (m & m_last) : m;
+      const uint32_t act = rm & comb;
+      m = 0xFFFFFFFFu; comb = 0xFFFFFFFFu;
       const uint32_t *o = &smem[(S_OBJ + w) * BLOCK + sl];
       const uint32_t PF = o[0] & act, BL = o[5 * BLOCK] & act, P0 = o[10 * BLOCK] & act, P1 = o[15 * BLOCK] & act,
                      M0 = o[20 * BLOCK] & act, M1 = o[25 * BLOCK] & act;
-      uint32_t ones = PF | BL, twos = PF & BL;                    // pixels where two or more objects are lit: no such pixel
-      twos |= ones & P0; ones |= P0; twos |= ones & P1; ones |= P1; twos |= ones & M0; ones |= M0; twos |= ones & M1;   // in the word, no pair to look at
-      if (twos) {
+      // pixels where two or more objects are lit (no such pixel in the word: no pair to look at): two carry-save adders
+      // over three masks each (sum = xor, carry = majority), then carry | carry | sum & sum
+      const uint32_t s1 = PF ^ BL ^ P0, c1 = (PF & BL) | (P0 & (PF | BL)), s2 = P1 ^ M0 ^ M1, c2 = (P1 & M0) | (M1 & (P1 | M0));
+      if (c1 | c2 | (s1 & s2)) {
         any2 = 1;
         a0 |= M0 & P1; a1 |= M0 & P0; a2 |= M1 & P0; a3 |= M1 & P1; a4 |= P0 & PF; a5 |= P0 & BL; a6 |= P1 & PF; a7 |= P1 & BL;
         a8 |= M0 & PF; a9 |= M0 & BL; a10 |= M1 & PF; a11 |= M1 & BL; a12 |= BL & PF; a13 |= P0 & P1; a14 |= M0 & M1;
