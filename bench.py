@@ -35,7 +35,7 @@ def oracle_sample(w, n_envs: int, steps: int, threads: int):
     """Time the oracle, as it stands, on `n_envs` envs (spread over the ROMs) for `steps` env-steps."""
     from oracle.ovcs_py import OracleVCS
     idx = (np.arange(n_envs) * (w.batch // n_envs) + (np.arange(n_envs) * 37) % max(1, w.batch // n_envs)).astype(np.int64)
-    o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx])
+    o = OracleVCS(w.roms, w.seeds[idx], w.env_rom[idx], mappers=getattr(w, "mappers", None))
     acts = w.actions(0, steps + 1)
     o.step(acts[0][idx], FRAMESKIP, threads=threads)                    # untimed: first (short) frame, page-in
     c0 = o.regs()["cycles"].astype(np.int64).sum()
@@ -188,6 +188,9 @@ def main():
     ap.add_argument("--workload", type=int, default=4, choices=[2, 3, 4],
                     help="BASELINE config the envs run (default 4, the headline; 2/3 = one shared 4K ROM: the single-game "
                          "axis of the paper's Table 7, SURVEY §8(f) NEXT-2)")
+    ap.add_argument("--cart", default=None, choices=["4K", "F8", "F6", "F4", "F8SC", "F6SC", "F4SC", "E0", "FE"],
+                    help="with --workload 2: every env runs one seeded cartridge of this format instead of config 2's 4K ROM "
+                         "(timing of the other bank-switching schemes, DESIGN.md section 10)")
     ap.add_argument("--soft-T", type=float, default=None,
                     help="run vcs_step_soft (SOFT-STE forward, BASELINE config 5: --workload 2 --batch 4096) at this temperature")
     ap.add_argument("--paper-axis", action="store_true",
@@ -223,10 +226,20 @@ def main():
     label = {4: f"config4: {B} envs/GPU, {n_roms} seeded ROMs (half 4K, half 8K F8), uniform random actions, frameskip 4",
              2: f"config2: {B} envs/GPU sharing one seeded 4K ROM, uniform random actions, frameskip 4",
              3: f"config3: {B} envs/GPU sharing one seeded 4K ROM (indexed/indirect, stack, BCD, timers), sticky actions, frameskip 4"}[args.workload]
+    mappers = None
+    if args.cart is not None:
+        if args.workload != 2:
+            raise SystemExit("--cart goes with --workload 2")
+        from vcs_inputs import FEATURES, make_rom, superchip_rom, e0_rom, fe_rom
+        gen = {"4K": lambda: make_rom(4242, FEATURES["4a"]), "F8": lambda: make_rom(4242, FEATURES["4b"]), "F6": lambda: make_rom(4242, FEATURES["f6"]),
+               "F4": lambda: make_rom(4242, FEATURES["f4"]), "F8SC": lambda: superchip_rom("F8SC", 4242), "F6SC": lambda: superchip_rom("F6SC", 4242),
+               "F4SC": lambda: superchip_rom("F4SC", 4242), "E0": lambda: e0_rom(4242), "FE": lambda: fe_rom(4242)}[args.cart]
+        w.roms = [gen()]; mappers = [args.cart]; w.mappers = mappers
+        label = f"{B} envs/GPU sharing one seeded {args.cart} cartridge ({len(w.roms[0])} bytes), uniform random actions, frameskip 4"
     if world > 1:                                   # every rank its own env seeds / action streams (same ROM set)
         from paper_2606_22447_b200.shard import rank_seeds
         w.seeds = rank_seeds(w.seeds, rank); w._act_seeds = rank_seeds(w._act_seeds, rank)
-    env = VCS(w.roms, w.seeds, w.env_rom)
+    env = VCS(w.roms, w.seeds, w.env_rom, mappers=mappers)
     acts_host = w.actions(0, W + K)
     acts = torch.from_numpy(acts_host).cuda()
     stream = torch.cuda.current_stream()

@@ -155,7 +155,7 @@ StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   p.st = h->d_st; p.ram = h->d_ram; p.cyc = h->d_cyc; p.screen = h->d_screen; p.sc_ram = h->d_sc_ram;
   p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
   p.actions = actions; p.switches = h->d_switches; p.mask = nullptr; p.boot = h->d_boot_ctr; p.perm = h->d_perm; p.blk_time = nullptr; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
-  p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom;
+  p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom; p.rom_staged = h->rom_staged; p.banked = h->banked;
   p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_ent = nullptr; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0; p.n_instr = 0;
   return p;
 }
@@ -222,7 +222,10 @@ int vcs_create(vcs_t *out, int32_t batch, const vcs_rom *roms, int32_t n_roms, c
   auto uniform = [&](int blk) { for (int i = 0; i < batch; ++i) if (er[i] != er[i - i % blk]) return false; return true; };
   h->block = want; h->rom_smem = 0;
   for (int blk = want; blk >= 64; blk >>= 1) if (uniform(blk)) { h->block = blk; h->rom_smem = 1; break; }
-  if ((c.flags & VCS_F_ROM_GLOBAL) || h->max_rom > 8192) h->rom_smem = 0;     // F6 / F4 images stay in global memory (read-only path)
+  if (c.flags & VCS_F_ROM_GLOBAL) h->rom_smem = 0;
+  h->rom_staged = h->rom_smem && h->max_rom <= 8192;       // 16 / 32 KB images stay in global memory (read-only path): two blocks per SM must fit
+  h->banked = 0;
+  for (int r = 0; r < n_roms; ++r) if (meta[r].kind >= MK_F8 && meta[r].kind <= MK_F4SC) h->banked = 1;
   h->regroup = (c.flags & VCS_F_NO_REGROUP) ? 0 : 1;
   // pre-decode every byte offset of every bank once (vcs_decode.cuh); the words depend on the launch shape
   // (zero-page RAM operands are stored as shared-memory offsets)

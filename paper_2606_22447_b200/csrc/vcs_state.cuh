@@ -88,8 +88,9 @@ enum CtxWord { C_SCREEN_LO = 0, C_SCREEN_HI, C_Y0, C_FRAMESKIP, C_BATCH, C_ENV0,
                C_SOFT_OUT_LO, C_SOFT_OUT_HI, C_SOFT_W_LO, C_SOFT_W_HI, C_SOFT_K, C_SOFT_ALPHA, C_SOFT_TAB_LO, C_SOFT_TAB_HI,
                C_HS,           // bank hotspots of the block's ROM (ROM staged in smem: one ROM per block): first address | count << 16 | HS_SC
                C_SCRAM_LO, C_SCRAM_HI,     // Superchip RAM of all envs, [32][batch] words like `ram` (nullptr when no cart has it)
+               C_ROMG_LO, C_ROMG_HI,       // the block's ROM image in global memory (one ROM per block; read there when it is not staged, C_ROMOFF then = offset mask)
                C_WORDS = 28 };         // (a multiple of 4: the ROM image staged behind the context is a 16-byte aligned bulk-copy target)
-static_assert(C_WORDS % 4 == 0 && C_SCRAM_HI < C_WORDS, "context layout");
+static_assert(C_WORDS % 4 == 0 && C_ROMG_HI < C_WORDS, "context layout");
 static_assert(C_HS < C_WORDS, "context layout");
 
 struct RomMeta { uint32_t offset; uint32_t size; uint32_t doff; uint32_t pad;      // byte offset into the ROM blob, size, word offset into the decode blob
@@ -116,7 +117,9 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   int special_carts;            // some cart is Superchip / E0 / FE (hard mode only)
   int block;                    // threads (= envs) per block of the interpreter kernel
   int regroup;                  // F8 blocks re-sort their envs across threads at bank-hotspot accesses
-  int rom_smem;                 // every block maps to a single ROM: it is staged in shared memory
+  int rom_smem;                 // every block maps to a single ROM (the ROMS kernel variants: hot-path ROM reads, regroup)
+  int rom_staged;               // ... and the images are small enough (<= 8 KB) to be staged in shared memory
+  int banked;                   // some cartridge is an F8 / F6 / F4 (with or without Superchip RAM): its blocks regroup at bank switches (spare warp)
   uint32_t max_rom;             // largest ROM image
   long long launches;
   char err[256];

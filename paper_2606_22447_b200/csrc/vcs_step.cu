@@ -211,7 +211,7 @@ struct Hot {
   uint32_t aux;                        // return flag of the out-of-line calls
 };
 
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT, int TAG = 0>      // TAG: which copy of the TIA code this Cpu calls (vcs_tia.cuh)
+template <int BLOCK, int ROMS, int THREADS, bool SOFT, int TAG = 0>      // TAG: which copy of the TIA code this Cpu calls (vcs_tia.cuh)
 struct Cpu {
   using T = Tia<BLOCK, TAG>;
   // ---- CPU
@@ -234,8 +234,8 @@ struct Cpu {
   uint32_t kind;      // MapKind of this env's cartridge
   uint32_t park;      // bit0: this block regroups its envs at bank-hotspot accesses; bit1: this lane is parked for a
                       // regroup; bit2: a bank hotspot was accessed by the instruction in flight
-  uint32_t rom_off;   // ROMS: byte offset of the ROM image inside smem
-  const uint8_t *rom_g;    // !ROMS: the image in global memory
+  uint32_t rom_off;   // ROMS == 1: byte offset of the ROM image inside smem
+  const uint8_t *rom_g;    // ROMS != 1: the image in global memory
   const uint2 *dr;         // decode entries of this env's ROM (4096 per bank)
   uint2 w;            // decode entry at (bank, PC) — valid at every scheduling point
   uint32_t sl, sl4;   // this thread's file slot (word i of the file lives at smem[i*BLOCK + sl]) and 4*sl
@@ -256,7 +256,7 @@ struct Cpu {
     if constexpr (CART) {                                  // (the line-end / event paths never touch the cartridge)
       auto ptr = [](int lo) { return (unsigned long long)T::ctx(lo) | ((unsigned long long)T::ctx(lo + 1) << 32); };
       const RomMeta rm = reinterpret_cast<const RomMeta *>(ptr(C_META_LO))[romid];
-      hs_n = (rm.hs >> 16) & 0xFFu; hs_lo = rm.hs & 0xFFFFu; kind = rm.kind; rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
+      hs_n = (rm.hs >> 16) & 0xFFu; hs_lo = rm.hs & 0xFFFFu; kind = rm.kind; rom_mask = (rm.size == 2048 && ROMS != 1) ? 0x7FFu : 0xFFFu;
       rom_g = reinterpret_cast<const uint8_t *>(ptr(C_BLOB_LO)) + rm.offset;
       dr = reinterpret_cast<const uint2 *>(ptr(C_DROM_LO)) + rm.doff;
       if constexpr (SOFT) soft_tab = reinterpret_cast<const float *>(ptr(C_SOFT_TAB_LO)) + rm.pad;
@@ -290,7 +290,7 @@ struct Cpu {
 
   // ------------------------------------------------------------------ ROM
   DEV uint32_t rom_byte(uint32_t off) const {
-    if constexpr (ROMS) return reinterpret_cast<const uint8_t *>(smem)[rom_off + off];
+    if constexpr (ROMS == 1) return reinterpret_cast<const uint8_t *>(smem)[rom_off + off];
     else return __ldg(rom_g + off);
   }
   // any access to a hotspot ($1FF8/$1FF9 on F8 carts) selects the bank; in a block that regroups it also parks the lane (park bit 1)
@@ -533,7 +533,7 @@ struct Cpu {
       S(S_OBJ + 1) = PC | (pack_p() << 16) | (status << 24);
       S(S_OBJ + 2) = (uint32_t)cyc; S(S_OBJ + 3) = (uint32_t)lstart; S(S_OBJ + 4) = (uint32_t)fstart;
       S(S_OBJ + 5) = fdone | (bank << 8) | ((wsync ? 1u : 0u) << 16);
-      skey = (fdone >= fskip) ? 0xFFFFFFFFu : (min(fdone, 63u) << 25) | (bank << 24) | (SP << 16) | PC;
+      skey = (fdone >= fskip) ? 0xFFFFFFFFu : (min(fdone, 30u) << 27) | (bank << 24) | (SP << 16) | PC;    // (bank: 3 bits, F4 has eight)
       S(S_OBJ + 6) = skey;
     }
     __syncthreads();
@@ -563,7 +563,20 @@ struct Cpu {
     // its own and everything else is packed behind it from the next warp boundary on, so that no warp mixes the two
     // banks; slots inside a warp stay consecutive, hence bank-conflict free.
     uint32_t ns = threadIdx.x;
-    if constexpr (THREADS != BLOCK) {
+    if constexpr (THREADS != BLOCK && ROMS == 2) {
+      // F6 / F4 (four / eight banks): files stay in sorted order, and every (frames done, bank) class starts at a warp
+      // boundary for as long as the spare warp's 32 lanes of padding last
+      uint32_t pos = 0, slack = THREADS - BLOCK, prev = keys[0] >> 24;
+      ns = NOSLOT;
+#pragma unroll 4
+      for (int j = 0; j < BLOCK; ++j) {
+        const uint32_t c = keys[j] >> 24;
+        if (c != prev) { const uint32_t pad = (32u - (pos & 31u)) & 31u; if (pad <= slack) { pos += pad; slack -= pad; } prev = c; }
+        if (pos == threadIdx.x) ns = (uint32_t)j;
+        ++pos;
+      }
+      __syncthreads();                                     // (as below)
+    } else if constexpr (THREADS != BLOCK) {
       const uint32_t c0 = keys[0] >> 24;
       uint32_t n0 = 0;
 #pragma unroll 4
@@ -588,7 +601,7 @@ struct Cpu {
       r = S(S_OBJ + 1); const uint32_t npc = r & 0xFFFFu; unpack_p((r >> 16) & 0xFFu); status = r >> 24;
       cyc = (int32_t)S(S_OBJ + 2); lstart = (int32_t)S(S_OBJ + 3); fstart = (int32_t)S(S_OBJ + 4);
       r = S(S_OBJ + 5); fdone = r & 0xFFu; wsync = ((r >> 16) & 1u) != 0;
-      di = (((r >> 8) & 1u) << 12) | (npc & 0xFFFu); pbase = npc - di;
+      di = (((r >> 8) & 7u) << 12) | (npc & 0xFFFu); pbase = npc - di;
       S(S_FL) |= TF_DIRTY_ALL;                             // the object-mask cache was the scratch area
       rekey(); relim();
       w = fetch();
@@ -910,13 +923,13 @@ DEV uint32_t rmw(Hot &h, uint32_t o, uint32_t s) {
 // Out-of-line paths.  Each takes the Hot registers by value, rebuilds a Cpu, does its work and hands the registers
 // back: the struct copy through the stack is only paid on these (rare) calls, and the instruction cache keeps the
 // inline loop below to itself.
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
+template <int BLOCK, int ROMS, int THREADS, bool SOFT>
 __device__ __noinline__ Hot cold_exec_generic(Hot h, uint32_t sl, uint32_t cx, uint32_t pl) {   // one instruction, any bus pattern
   Cpu<BLOCK, ROMS, THREADS, SOFT, SOFT ? 0 : 1> c; c.load(h, sl);     // (its own copy of the TIA code: see vcs_tia.cuh, TAG)
   c.template exec_one<true>((cx & 0xFFFFFF80u) | ((cx & 0x7Fu) - HC_COLD), pl);
   return c.store();
 }
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
+template <int BLOCK, int ROMS, int THREADS, bool SOFT>
 __device__ __noinline__ Hot cold_exec(Hot h, uint32_t sl, uint32_t cx, uint32_t pl) {       // one instruction
   if constexpr (SOFT) return cold_exec_generic<BLOCK, ROMS, THREADS, SOFT>(h, sl, cx, pl);   // (soft reads are counted: no second try)
   Cpu<BLOCK, ROMS, THREADS, SOFT, COLD_TAG> c; c.load(h, sl);
@@ -926,14 +939,14 @@ __device__ __noinline__ Hot cold_exec(Hot h, uint32_t sl, uint32_t cx, uint32_t 
   if (c.template exec_one<false>((cx & 0xFFFFFF80u) | ((cx & 0x7Fu) - HC_COLD), pl)) { h.aux = AUX_GENERIC; return h; }
   return c.store();
 }
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT, bool COUNT = false>
+template <int BLOCK, int ROMS, int THREADS, bool SOFT, bool COUNT = false>
 __device__ __noinline__ Hot cold_pre(Hot h, uint32_t sl) {                                   // cyc >= lim: line end, WSYNC, cap, halt
   Cpu<BLOCK, ROMS, THREADS, SOFT> c; c.template load<false>(h, sl);
   const bool ok = c.template slow_pre<COUNT>();
   Hot r = c.store(); r.aux = ok ? 1u : 0u;
   return r;
 }
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
+template <int BLOCK, int ROMS, int THREADS, bool SOFT>
 __device__ __noinline__ Hot cold_events(Hot h, uint32_t sl, uint32_t ev) {                   // a TIA write crossed a line / ended a frame
   Cpu<BLOCK, ROMS, THREADS, SOFT> c; c.template load<false>(h, sl);
   if (ev & EV_FRAME) c.fdone -= 1;                          // (S_FDONE, loaded above, already counts the frame that just ended)
@@ -941,7 +954,7 @@ __device__ __noinline__ Hot cold_events(Hot h, uint32_t sl, uint32_t ev) {      
   Hot r = c.store(); r.aux = (ev & EV_FRAME) ? 1u : 0u;
   return r;
 }
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT>
+template <int BLOCK, int ROMS, int THREADS, bool SOFT>
 __device__ __noinline__ uint32_t cold_timer_read(uint32_t sl, uint32_t a, int32_t c) {       // INTIM / TIMINT around the underflow
   return Riot<BLOCK, 0>::timer_read(sl, a, c);
 }
@@ -959,7 +972,7 @@ __device__ __noinline__ int32_t line_step(uint32_t sl, int32_t cyc, int32_t lsta
 }
 
 // is `addr` a RAM cell or a plain byte of the (shared-memory staged) cartridge?  hs = first hotspot | count << 16
-template <bool ROMS>
+template <int ROMS>
 DEV bool plain_addr(uint32_t addr, uint32_t hs) {
   const uint32_t a = addr & 0x1FFFu;
   if ((a & 0x1280u) == 0x0080u) return true;
@@ -967,9 +980,11 @@ DEV bool plain_addr(uint32_t addr, uint32_t hs) {
   else return false;                                       // (ROM in global memory: left to the out-of-line executor)
 }
 template <int BLOCK> DEV uint32_t cell_of(uint32_t off) { return ((off / BLOCK) & 0x7Cu) | (off & 3u); }   // RAM cell of a smem byte offset
-template <int BLOCK, bool ROMS>
-DEV uint32_t rom_byte_hot(uint32_t off) {                  // byte `off` (bank << 12 | offset) of the block's staged ROM
-  if constexpr (ROMS) return reinterpret_cast<const uint8_t *>(smem)[(S_WORDS * BLOCK + C_WORDS) * 4 + off];
+template <int BLOCK, int ROMS>
+DEV uint32_t rom_byte_hot(uint32_t off) {                  // byte `off` (bank << 12 | offset) of the block's ROM: staged, or (ROMS == 2) in global memory
+  if constexpr (ROMS == 1) return reinterpret_cast<const uint8_t *>(smem)[(S_WORDS * BLOCK + C_WORDS) * 4 + off];
+  else if constexpr (ROMS == 2)                            // (C_ROMOFF then holds the mask of the image's byte offsets: a 2 KB image has no mirror there)
+    return __ldg(reinterpret_cast<const uint8_t *>((unsigned long long)Tia<BLOCK>::ctx(C_ROMG_LO) | ((unsigned long long)Tia<BLOCK>::ctx(C_ROMG_HI) << 32)) + (off & Tia<BLOCK>::ctx(C_ROMOFF)));
   else return 0;
 }
 
@@ -977,7 +992,7 @@ DEV uint32_t rom_byte_hot(uint32_t off) {                  // byte `off` (bank <
 // The inline interpreter loop: instructions of this lane's min-key group until the next scheduling point.
 // SOFT: `se` = per decode entry {sum of the soft values of the instruction's own bytes, their count, their largest
 // |soft - hard|, STE mismatches among them} (soft_entry_kernel); data reads of RAM and branches are noted where they run.
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT, bool COUNT = false>
+template <int BLOCK, int ROMS, int THREADS, bool SOFT, bool COUNT = false>
 DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl, const float4 *se = nullptr, const float *stab = nullptr) {
   using T = Tia<BLOCK>;
   uint8_t *const ramb = reinterpret_cast<uint8_t *>(smem) + 4u * sl;
@@ -1226,7 +1241,7 @@ DEV void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile("{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @!p bra WAIT_%=;\n}" ::"r"(bar), "r"(parity) : "memory");
 }
 
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT, bool COUNT = false>
+template <int BLOCK, int ROMS, int THREADS, bool SOFT, bool COUNT = false>
 __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepParams p) {
   using T = Tia<BLOCK>;
   __shared__ __align__(8) unsigned long long s_bar;
@@ -1250,17 +1265,17 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     const unsigned long long scr = reinterpret_cast<unsigned long long>(p.screen);
     s_ctx[C_SCREEN_LO] = (uint32_t)scr; s_ctx[C_SCREEN_HI] = (uint32_t)(scr >> 32);
     s_ctx[C_Y0] = (uint32_t)p.y0; s_ctx[C_FRAMESKIP] = (uint32_t)p.frameskip; s_ctx[C_BATCH] = (uint32_t)B; s_ctx[C_ENV0] = (uint32_t)e0;
-    s_ctx[C_CAP] = (uint32_t)(p.max_lines * LINE_CYC); s_ctx[C_ROMOFF] = ROM_OFF;
-    s_ctx[C_REGROUP] = (ROMS && rm.kind == MK_F8 && p.regroup) ? 1u : 0u;
+    s_ctx[C_CAP] = (uint32_t)(p.max_lines * LINE_CYC); s_ctx[C_ROMOFF] = (ROMS == 2) ? ((rm.size == 2048) ? 0x7FFu : 0xFFFFFFFFu) : ROM_OFF;
+    s_ctx[C_REGROUP] = (ROMS && rm.kind >= MK_F8 && rm.kind <= MK_F4SC && p.regroup) ? 1u : 0u;
     s_ctx[C_HS] = rm.hs;
     { const unsigned long long v = reinterpret_cast<unsigned long long>(p.sc_ram); s_ctx[C_SCRAM_LO] = (uint32_t)v; s_ctx[C_SCRAM_HI] = (uint32_t)(v >> 32); }
     auto put = [&](int lo, const void *q) { const unsigned long long v = reinterpret_cast<unsigned long long>(q); s_ctx[lo] = (uint32_t)v; s_ctx[lo + 1] = (uint32_t)(v >> 32); };
-    put(C_META_LO, p.rom_meta); put(C_BLOB_LO, p.rom_blob); put(C_DROM_LO, p.drom);
+    put(C_META_LO, p.rom_meta); put(C_BLOB_LO, p.rom_blob); put(C_DROM_LO, p.drom); put(C_ROMG_LO, p.rom_blob + rm.offset);
     put(C_SOFT_OUT_LO, p.soft_out); put(C_SOFT_W_LO, p.soft_w); put(C_SOFT_TAB_LO, p.soft_tab); s_ctx[C_SOFT_K] = (uint32_t)p.soft_K; s_ctx[C_SOFT_ALPHA] = __float_as_uint(p.soft_alpha);
-    if constexpr (ROMS) { mbar_init(smem_u32(&s_bar), 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+    if constexpr (ROMS == 1) { mbar_init(smem_u32(&s_bar), 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
   }
   __syncthreads();
-  if constexpr (ROMS) {                                    // a3: stage the block's ROM (2 KB images twice: the mirror)
+  if constexpr (ROMS == 1) {                               // a3: stage the block's ROM (2 KB images twice: the mirror)
     if (tid == 0) {
       const uint32_t bar = smem_u32(&s_bar), dst = smem_u32(smem) + ROM_OFF;
       const uint8_t *src = p.rom_blob + rm.offset;
@@ -1300,10 +1315,10 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   s.cyc = 0; s.lstart = -(int32_t)n0; s.fdone = live0 ? 0u : s.fskip; s.romid = romid;
   s.cap = p.max_lines * LINE_CYC;
   s.hs_n = (rm.hs >> 16) & 0xFFu; s.hs_lo = rm.hs & 0xFFFFu; s.kind = rm.kind;
-  const bool regroups = ROMS && rm.kind == MK_F8 && p.regroup;      // block-uniform
+  const bool regroups = ROMS && rm.kind >= MK_F8 && rm.kind <= MK_F4SC && p.regroup;    // block-uniform
   s.park = regroups ? 1u : 0u;
   s.rom_off = ROM_OFF; s.rom_g = p.rom_blob + rm.offset; s.dr = p.drom + rm.doff; 
-  s.rom_mask = (rm.size == 2048 && !ROMS) ? 0x7FFu : 0xFFFu;
+  s.rom_mask = (rm.size == 2048 && ROMS != 1) ? 0x7FFu : 0xFFFu;
   // ---- a2 action latch (C.11)
   if (live0) {
     uint32_t act = p.actions[ei]; if (act >= 18u) act = 0;
@@ -1327,7 +1342,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   }
   s.wsync = (fl & TF_WSYNC) != 0;
   s.relim(); s.rekey();
-  if constexpr (ROMS) mbar_wait(smem_u32(&s_bar), 0);
+  if constexpr (ROMS == 1) mbar_wait(smem_u32(&s_bar), 0);
   s.w = live0 ? s.fetch() : make_uint2(HC_COLD + H_SLOW, 0);
   Hot h;
   if (filed) { if (!live0) T::S(sl, S_FDONE) = s.fskip; h = s.store(); }
@@ -1532,9 +1547,9 @@ size_t step_smem_bytes(int block, bool roms, uint32_t max_rom, bool soft) {
   return (size_t)(S_WORDS * block + C_WORDS) * 4 + (roms ? (max_rom < 4096 ? 4096 : max_rom) + 16 : 0) + (soft ? (size_t)8 * block * 4 : 0);
 }
 
-template <int BLOCK, bool ROMS, int THREADS, bool SOFT, bool COUNT = false>
+template <int BLOCK, int ROMS, int THREADS, bool SOFT, bool COUNT = false>
 static cudaError_t launch_one(const StepParams &p, cudaStream_t stream) {
-  const size_t smem_bytes = step_smem_bytes(BLOCK, ROMS, p.max_rom, SOFT);
+  const size_t smem_bytes = step_smem_bytes(BLOCK, ROMS == 1, p.max_rom, SOFT);
   static size_t configured[64] = {0};                   // per device: the attribute belongs to the (function, device) pair
   int dev = 0; cudaGetDevice(&dev);
   if (dev < 0 || dev >= 64 || configured[dev] < smem_bytes) {
@@ -1549,16 +1564,18 @@ static cudaError_t launch_one(const StepParams &p, cudaStream_t stream) {
 
 cudaError_t launch_step(const StepParams &p, cudaStream_t stream) {
   if (p.n_instr > 0)                                       // vcs_step_instructions: one variant (128 envs per block, ROM through the read-only path)
-    return launch_one<128, false, 128, false, true>(p, stream);
+    return launch_one<128, 0, 128, false, true>(p, stream);
   if (p.soft_out)                                          // SOFT-STE mode: one variant (ROM through the read-only path, no regroup)
-    return launch_one<128, false, 128, true>(p, stream);
-  if (p.rom_smem && p.regroup && p.max_rom == 8192) {      // F8 carts present: one spare warp per block for the regroup
-    switch (p.block) { case 64: return launch_one<64, true, 96, false>(p, stream); case 256: return launch_one<256, true, 288, false>(p, stream); default: return launch_one<128, true, 160, false>(p, stream); }
+    return launch_one<128, 0, 128, true>(p, stream);
+  if (p.rom_smem && !p.rom_staged)                         // one ROM per block, 16 / 32 KB images: read through the read-only path (ROMS = 2); they are
+    switch (p.block) { case 64: return launch_one<64, 2, 96, false>(p, stream); case 256: return launch_one<256, 2, 288, false>(p, stream); default: return launch_one<128, 2, 160, false>(p, stream); }   // banked: spare warp
+  if (p.rom_smem && p.regroup && p.banked) {               // F8 carts present: one spare warp per block for the regroup
+    switch (p.block) { case 64: return launch_one<64, 1, 96, false>(p, stream); case 256: return launch_one<256, 1, 288, false>(p, stream); default: return launch_one<128, 1, 160, false>(p, stream); }
   }
   if (p.rom_smem) {
-    switch (p.block) { case 64: return launch_one<64, true, 64, false>(p, stream); case 256: return launch_one<256, true, 256, false>(p, stream); default: return launch_one<128, true, 128, false>(p, stream); }
+    switch (p.block) { case 64: return launch_one<64, 1, 64, false>(p, stream); case 256: return launch_one<256, 1, 256, false>(p, stream); default: return launch_one<128, 1, 128, false>(p, stream); }
   }
-  switch (p.block) { case 64: return launch_one<64, false, 64, false>(p, stream); case 256: return launch_one<256, false, 256, false>(p, stream); default: return launch_one<128, false, 128, false>(p, stream); }
+  switch (p.block) { case 64: return launch_one<64, 0, 64, false>(p, stream); case 256: return launch_one<256, 0, 256, false>(p, stream); default: return launch_one<128, 0, 128, false>(p, stream); }
 }
 
 }  // namespace vcs

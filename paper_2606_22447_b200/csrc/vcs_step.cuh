@@ -15,7 +15,8 @@ struct StepParams {
   int32_t batch, frameskip, y0, max_lines;
   const float *soft_w; const float *soft_tab; float *soft_out; float soft_alpha; int32_t soft_K;   // soft_out != nullptr: SOFT-STE mode (vcs_step_soft)
   const float4 *soft_ent;                                 // ... per decode entry: the soft sums of the instruction's own bytes
-  int32_t block, rom_smem, regroup; uint32_t max_rom;     // launch shape: envs per block (64/128/256), ROM staged in smem, largest image
+  int32_t block, rom_smem, regroup; uint32_t max_rom;     // launch shape: envs per block (64/128/256), one ROM per block, regroups allowed, largest image
+  int32_t rom_staged, banked;                             // the block's ROM is staged in smem (images <= 8 KB); some cartridge is a plain F8 / F6 / F4
   int32_t n_instr;                                        // > 0: vcs_step_instructions — run this many instructions per env instead of `frameskip` frames
 };
 
