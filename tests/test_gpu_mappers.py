@@ -158,3 +158,31 @@ def test_format_errors(torch):
     g = VCS([e0_rom(1)], env_seeds(1, 4), mappers=["E0"])
     with pytest.raises(VcsError):
         g.step_soft(torch.zeros(4, dtype=torch.uint8, device="cuda"), 1, 1.0, 4.0)   # hard mode only
+
+
+# ---- blocks that hold ONE banked cartridge regroup their envs at bank switches: F6 / F4 with
+# four / eight banks (the image read from global memory, classes padded to warp boundaries while the spare warp's lanes
+# last) and the Superchip variants.  Which thread runs which env never shows in the results.
+@pytest.mark.parametrize("kind,nb", [("f6", 4), ("f4", 8)])
+@pytest.mark.parametrize("flags", ["VCS_F_BLOCK_64", "VCS_F_BLOCK_128", "VCS_F_BLOCK_256", "VCS_F_BLOCK_128|VCS_F_NO_REGROUP"])
+def test_one_banked_rom_per_block_regroups(torch, kind, nb, flags):
+    import paper_2606_22447_b200.binding as b
+    fl = 0
+    for f in flags.split("|"): fl |= getattr(b, f)
+    n = 300                                                               # full blocks and a ragged last one at every block size
+    g, o = pair([make_rom(940 + nb, FEATURES[kind])], env_seeds(41, n), flags=fl)
+    r = SplitMix64(77 + nb)
+    for t in range(8):
+        a = np.array([r.rnd(18) for _ in range(n)], np.uint8)
+        g.step(torch.from_numpy(a).cuda(), 3); o.step(a, 3, threads=NCPU)
+        compare(g, o, f"{kind} {flags} step {t}")
+    banks = g.regs_host()["bank"]
+    assert banks.max() < nb and len(set(banks.tolist())) > 2
+    g.close(); o.close()
+
+
+@pytest.mark.parametrize("kind", ["F8SC", "F6SC", "F4SC"])
+def test_one_superchip_rom_per_block_regroups(torch, kind):
+    import paper_2606_22447_b200.binding as b
+    regs = run_kinds(torch, [superchip_rom(kind, 23)], [kind], [0] * 300, 9, kind + " one rom", max_lines=200, flags=b.VCS_F_BLOCK_128)
+    assert len(set(regs["bank"].tolist())) > 1
