@@ -20,7 +20,10 @@
  * source other than the [R] readings exists in this container): per-register TIA write
  * latencies, mid-line HMOVE, RSYNC, double/quad-size player 1-clock shift, bus residue
  * in TIA reads, same-cycle INTIM/underflow, F8 start bank, power-on timer/RAM state, y0,
- * and decimal-mode results for invalid BCD operands (cited algorithm only).
+ * the Superchip / E0 / FE power-up states and the read of a Superchip write port (R16),
+ * and the format guess of ovcs_detect_mapper against the paper's (xitari's) signatures (R17).
+ * Decimal-mode results for invalid BCD operands are pinned against the digit-wise
+ * definition since round 2 (tests/test_oracle_pins_cpu.py).
  */
 #ifndef OVCS_H
 #define OVCS_H
