@@ -321,8 +321,11 @@ def main():
     work = None
     if not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
-        s = oracle_sample(make_workload(args.workload), 32 * cores, 24, cores)       # ~10-20 s of wall clock on the box's cores
-        s1 = oracle_sample(make_workload(args.workload), 64, 16, 1)                  # the same oracle on ONE core (~4 s)
+        wo = make_workload(args.workload)                # the config at its stated batch (a sample of it is timed)
+        if args.cart is not None:
+            wo.roms = w.roms; wo.mappers = mappers
+        s = oracle_sample(wo, 32 * cores, 96, cores)     # ~10 s of wall clock on the box's 16 cores (~170 core-seconds)
+        s1 = oracle_sample(wo, 64, 48, 1)                # the same oracle on ONE core (~9 s)
         work = s["work"]
         cpu = {"value": s["value"], "unit": "env-steps/s", "cores": cores, "kind": "oracle", "sample": s["sample"],
                "emulated_cycles_per_s": s["cycles_per_s"], "seconds": s["seconds"],
