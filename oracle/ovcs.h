@@ -104,6 +104,10 @@ int  ovcs_destroy(ovcs_t *h);
  * always 0) and the largest |soft - hard|. */
 int  ovcs_step_soft_range(ovcs_t *h, const uint8_t *actions, int32_t frameskip, double T, double alpha,
                           double *out, int32_t lo, int32_t hi);
+/* n single-instruction steps per env in SOFT-STE (full = 0) or FULL mode (full = 1: PAPER.md appendix D, the fully
+ * relaxed forward whose casts act on the executed values; ovcs_soft.inc); out as above. */
+int  ovcs_step_instructions_soft_range(ovcs_t *h, const uint8_t *actions, int32_t n_instr, double T, double alpha, int full,
+                                       double *out, int32_t lo, int32_t hi);
 /* the soft primitives themselves, for the pins: eq. (6), eq. (10) with window K, eq. (8), eq. (9) in float32 */
 double ovcs_soft_peek(const double *r, int M, int a);
 double ovcs_soft_peek_relaxed(const double *r, int M, int a, double T, int K);

@@ -68,6 +68,7 @@ def lib():
         L.ovcs_boot.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, C.c_int32]
         L.ovcs_step_range.argtypes = [P, P, C.c_int32, C.c_int32, C.c_int32]
         L.ovcs_step_instructions_range.argtypes = [P, P, C.c_int32, C.c_int32, C.c_int32]
+        L.ovcs_step_instructions_soft_range.argtypes = [P, P, C.c_int32, C.c_double, C.c_double, C.c_int32, P, C.c_int32, C.c_int32]
         L.ovcs_detect_mapper.argtypes = [P, C.c_uint32]
         for f in ("ovcs_get_ram", "ovcs_get_regs", "ovcs_get_screen", "ovcs_get_cart_ram"):
             getattr(L, f).argtypes = [P, P]
@@ -149,6 +150,20 @@ class OracleVCS:
         with ThreadPoolExecutor(n) as ex:
             rcs = list(ex.map(lambda i: lib().ovcs_step_instructions_range(self.h, a.ctypes.data, int(n_instr), cuts[i], cuts[i + 1]), range(n)))
         assert all(rc == 0 for rc in rcs)
+
+    def step_instructions_soft(self, actions, n_instr, T, alpha, full, threads=1):
+        """n_instr single-instruction steps per env in SOFT-STE (full False) or FULL mode (full True: the fully relaxed
+        forward of PAPER.md appendix D).  Returns [batch][8] float64 as step_soft."""
+        a = np.ascontiguousarray(actions, dtype=np.uint8)
+        assert a.shape == (self.batch,)
+        out = np.zeros((self.batch, 8), dtype=np.float64)
+        n = max(1, min(threads, self.batch))
+        cuts = [self.batch * i // n for i in range(n + 1)]
+        with ThreadPoolExecutor(n) as ex:
+            rcs = list(ex.map(lambda i: lib().ovcs_step_instructions_soft_range(self.h, a.ctypes.data, int(n_instr), float(T), float(alpha),
+                                                                                 1 if full else 0, out.ctypes.data, cuts[i], cuts[i + 1]), range(n)))
+        assert all(rc == 0 for rc in rcs)
+        return out
 
     @staticmethod
     def _u8(x):
