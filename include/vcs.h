@@ -178,6 +178,22 @@ int vcs_get_booting(vcs_t h, uint8_t *out_dev, void *cuda_stream);
 int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float T, float alpha,
                   float *soft_out_dev, void *cuda_stream);
 
+/* The soft modes in the paper's own step unit (forward part): latch the actions, then
+ * exactly n_instr instructions per env as vcs_step_instructions, with the soft primitives of vcs_step_soft.
+ *   full = 0  SOFT-STE: the state equals vcs_step_instructions' bit for bit (Theorem 1/3).
+ *   full = 1  FULL, the fully relaxed forward of PAPER.md appendix D (L425-459; Table 2; reading R18 in
+ *             DESIGN.md §2): no straight-through correction — a value read returns round(soft), a conditional branch
+ *             sets PC = round(pc_nb + sigma(alpha z) delta), both cast in float32; dispatch stays the hard switch on the
+ *             (cast) opcode byte; an instruction's cycles and discarded reads follow its hard branch decision.  The
+ *             state equals hard mode's exactly while every cast rounds to the hard value (for every program when
+ *             alpha >= 6 and T <= 0.14, L459) and leaves it at the first cast that does not (Table 3's N_div).  The soft
+ *             values are evaluated tap by tap in double with the host's e^{-k/T} and gates, so that the casts are the
+ *             oracle's casts: this mode is exact, not fast.
+ * soft_out_dev as for vcs_step_soft; entry 6 counts the casts of this call that did not round to the hard value.
+ * 1 <= n_instr <= 1,000,000; 0 < T <= 60, alpha finite; Superchip / E0 / FE cartridges: VCS_EINVAL. */
+int vcs_step_instructions_soft(vcs_t h, const uint8_t *actions_dev, int32_t n_instr, float T, float alpha, int32_t full,
+                               float *soft_out_dev, void *cuda_stream);
+
 /* Copies into caller-owned DEVICE buffers. */
 int vcs_get_ram(vcs_t h, uint8_t *out_dev /* [batch][128] */, void *cuda_stream);
 int vcs_get_regs(vcs_t h, vcs_regs *out_dev /* [batch] */, void *cuda_stream);

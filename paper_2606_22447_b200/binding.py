@@ -20,7 +20,7 @@ VCS_F_NO_SPIN, VCS_F_NO_FUSE, VCS_F_NO_REGROUP, VCS_F_ROM_GLOBAL, VCS_F_NO_BALAN
 VCS_F_BLOCK_64, VCS_F_BLOCK_128, VCS_F_BLOCK_256 = 1 << 8, 2 << 8, 3 << 8
 _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
 
-EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_instructions", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_cart_ram", "vcs_get_screen", "vcs_detect_mapper", "vcs_step_host",
+EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_instructions", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_step_instructions_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_cart_ram", "vcs_get_screen", "vcs_detect_mapper", "vcs_step_host",
            "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_block_times", "vcs_launch_count",
            "vcs_optable", "vcs_issue_peak", "vcs_destroy", "vcs_last_error"]
 
@@ -63,6 +63,7 @@ def load_library() -> C.CDLL:
     L.vcs_step.argtypes = [P, P, C.c_int32, P]
     L.vcs_step_host.argtypes = [P, P, C.c_int32, P]
     L.vcs_step_instructions.argtypes = [P, P, C.c_int32, P]
+    L.vcs_step_instructions_soft.argtypes = [P, P, C.c_int32, C.c_float, C.c_float, C.c_int32, P, P]
     L.vcs_step_masked.argtypes = [P, P, C.c_int32, P, P]
     L.vcs_set_switches.argtypes = [P, P, P]
     L.vcs_boot.argtypes = [P, P, C.c_int32, C.c_int32, P, C.c_int32, C.c_int32, P]
@@ -170,6 +171,16 @@ class VCS:
         """vcs_step_instructions: exactly n_instr CPU instructions per env (the paper's step unit); the screen is not updated."""
         assert actions.is_cuda and actions.dtype == self.torch.uint8 and actions.numel() == self.batch and actions.is_contiguous()
         self._chk(self.L.vcs_step_instructions(self.h, actions.data_ptr(), int(n_instr), _stream_ptr(stream)), "vcs_step_instructions")
+
+    def step_instructions_soft(self, actions, n_instr, T, alpha, full, out=None, stream=None):
+        """vcs_step_instructions_soft: n_instr instructions per env in SOFT-STE (full False) or FULL mode (full True, the
+        fully relaxed forward); returns the device float[batch][8] of per-env soft sums."""
+        t = self.torch
+        assert actions.is_cuda and actions.dtype == t.uint8 and actions.numel() == self.batch and actions.is_contiguous()
+        out = t.empty((self.batch, 8), dtype=t.float32, device=self.device) if out is None else out
+        self._chk(self.L.vcs_step_instructions_soft(self.h, actions.data_ptr(), int(n_instr), float(T), float(alpha), 1 if full else 0,
+                                                    out.data_ptr(), _stream_ptr(stream)), "vcs_step_instructions_soft")
+        return out
 
     def _u8(self, x, what):
         if x is None:

@@ -6,6 +6,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <string>
 #include <vector>
 
 #include "../../include/vcs.h"
@@ -156,7 +157,7 @@ StepParams params_of(Handle *h, const uint8_t *actions, int frameskip) {
   p.rom_blob = h->d_rom_blob; p.drom = h->d_drom; p.rom_meta = h->d_rom_meta; p.env_rom = h->d_env_rom;
   p.actions = actions; p.switches = h->d_switches; p.mask = nullptr; p.boot = h->d_boot_ctr; p.perm = h->d_perm; p.blk_time = nullptr; p.batch = h->batch; p.frameskip = frameskip; p.y0 = h->y0; p.max_lines = h->max_lines;
   p.block = h->block; p.rom_smem = h->rom_smem; p.regroup = h->regroup; p.max_rom = h->max_rom; p.rom_staged = h->rom_staged; p.banked = h->banked;
-  p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_ent = nullptr; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0; p.n_instr = 0;
+  p.soft_w = nullptr; p.soft_tab = nullptr; p.soft_ent = nullptr; p.soft_wd = nullptr; p.soft_full = 0; p.soft_out = nullptr; p.soft_alpha = 0.f; p.soft_K = 0; p.n_instr = 0;
   return p;
 }
 
@@ -425,16 +426,11 @@ int vcs_get_booting(vcs_t h, uint8_t *out_dev, void *cuda_stream) {
   return VCS_OK;
 }
 
-int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float T, float alpha, float *soft_out_dev, void *cuda_stream) {
-  DEV_OK(h);
-  if (!actions_dev || !soft_out_dev) return fail(h, VCS_EINVAL, "vcs_step_soft: NULL buffer");
-  if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31)) return fail(h, VCS_EINVAL, "vcs_step_soft: frameskip out of range");
-  if (!(T > 0.f) || T > 60.f || !(alpha == alpha) || alpha > 1e30f || alpha < -1e30f) return fail(h, VCS_EINVAL, "vcs_step_soft: T or alpha out of range");
-  if (h->special_carts) return fail(h, VCS_EINVAL, "vcs_step_soft: Superchip / E0 / FE cartridges run in hard mode only");
-  cudaStream_t s = (cudaStream_t)cuda_stream;
-  if (h->soft_tab_T != T) {                            // a new temperature: e^{-k/T} and W(T) x ROM, once
+// soft modes: e^{-k/T}, W(T) x ROM and the per-entry sums for this temperature (once per temperature)
+static int soft_prepare(vcs_t h, float T, cudaStream_t s) {
+  if (h->soft_tab_T != T) {
     int K = (int)ceil(17.0 * (double)T); if (K < 1) K = 1; if (K > 1023) K = 1023;
-    CU(h, cudaEventSynchronize(h->soft_w_done));       // (the previous upload from the handle's pinned buffer; long since done)
+    CU(h, cudaEventSynchronize(h->soft_w_done));       // (the previous upload from the handle's pinned buffers; long since done)
     for (int k = 0; k < SOFT_W_N; ++k) h->h_soft_w[k] = k <= K ? (float)exp(-(double)k / (double)T) : 0.f;
     double cw = 0.0;                                   // normaliser of a RAM-tape window reaching n cells to one side (soft_ram_read)
     for (int n = 0; n < 128; ++n) { if (n <= K) cw += exp(-(double)n / (double)T); h->h_soft_w[SOFT_CW + n] = (float)cw; }
@@ -442,12 +438,27 @@ int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float 
     CU(h, cudaEventRecord(h->soft_w_done, s));
     cudaError_t ce0 = launch_soft_table(h->d_rom_blob, h->d_rom_meta_soft, h->n_roms, h->d_soft_w, K, h->d_soft_tab, s);
     h->launches += 1;
-    if (ce0 != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_soft table launch", ce0);
+    if (ce0 != cudaSuccess) return fail(h, VCS_ECUDA, "soft mode: table launch", ce0);
     ce0 = launch_soft_entries(h->d_rom_blob, h->d_rom_meta_soft, h->n_roms, h->d_drom_soft, h->d_soft_tab, h->d_soft_ent, s);
     h->launches += 1;
-    if (ce0 != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_soft entry-table launch", ce0);
+    if (ce0 != cudaSuccess) return fail(h, VCS_ECUDA, "soft mode: entry-table launch", ce0);
     h->soft_tab_T = T; h->soft_K = K;
   }
+  return VCS_OK;
+}
+static int soft_args_ok(vcs_t h, const char *who, float T, float alpha) {
+  if (!(T > 0.f) || T > 60.f || !(alpha == alpha) || alpha > 1e30f || alpha < -1e30f) return fail(h, VCS_EINVAL, (std::string(who) + ": T or alpha out of range").c_str());
+  if (h->special_carts) return fail(h, VCS_EINVAL, (std::string(who) + ": Superchip / E0 / FE cartridges run in hard mode only").c_str());
+  return VCS_OK;
+}
+
+int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float T, float alpha, float *soft_out_dev, void *cuda_stream) {
+  DEV_OK(h);
+  if (!actions_dev || !soft_out_dev) return fail(h, VCS_EINVAL, "vcs_step_soft: NULL buffer");
+  if (frameskip < 1 || (long long)frameskip * h->max_lines * LINE_CYC >= (1ll << 31)) return fail(h, VCS_EINVAL, "vcs_step_soft: frameskip out of range");
+  if (int rc = soft_args_ok(h, "vcs_step_soft", T, alpha)) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (int rc = soft_prepare(h, T, s)) return rc;
   CU(h, cudaMemsetAsync(soft_out_dev, 0, sizeof(float) * 8 * (size_t)h->batch, s));
   StepParams p = params_of(h, actions_dev, frameskip);
   p.drom = h->d_drom_soft; p.rom_meta = h->d_rom_meta_soft;
@@ -456,6 +467,44 @@ int vcs_step_soft(vcs_t h, const uint8_t *actions_dev, int32_t frameskip, float 
   cudaError_t ce = launch_step(p, s);
   h->launches += 1;
   if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_soft launch", ce);
+  return VCS_OK;
+}
+
+int vcs_step_instructions_soft(vcs_t h, const uint8_t *actions_dev, int32_t n_instr, float T, float alpha, int32_t full,
+                               float *soft_out_dev, void *cuda_stream) {
+  DEV_OK(h);
+  if (!actions_dev || !soft_out_dev) return fail(h, VCS_EINVAL, "vcs_step_instructions_soft: NULL buffer");
+  if (n_instr < 1 || n_instr > 1000000) return fail(h, VCS_EINVAL, "vcs_step_instructions_soft: n_instr out of range (1 .. 1,000,000)");
+  if (int rc = soft_args_ok(h, "vcs_step_instructions_soft", T, alpha)) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (int rc = soft_prepare(h, T, s)) return rc;
+  if (full) {
+    if (!h->d_drom_slow) {                             // every entry: "decode at run time" (the cast bytes decide what runs)
+      std::vector<DWord> slow(h->soft_tab_n + 8, DWord{(uint32_t)(HC_COLD + H_SLOW) | DW_LEADER, 0});
+      CU(h, cudaMalloc((void **)&h->d_drom_slow, sizeof(DWord) * slow.size()));
+      CU(h, cudaMemcpy(h->d_drom_slow, slow.data(), sizeof(DWord) * slow.size(), cudaMemcpyHostToDevice));
+      CU(h, cudaMalloc((void **)&h->d_soft_wd, sizeof(double) * SOFT_WD_WORDS));
+      CU(h, cudaMallocHost((void **)&h->h_soft_wd, sizeof(double) * SOFT_WD_WORDS));
+      h->soft_wd_T = -1.f; h->soft_wd_alpha = 0.f;
+    }
+    if (h->soft_wd_T != T || h->soft_wd_alpha != alpha) {   // the weights and the two gates in double, by the host's exp
+      CU(h, cudaEventSynchronize(h->soft_w_done));
+      const double Td = (double)T, ad = (double)alpha;
+      for (int k = 0; k < SOFT_WD_GATE; ++k) h->h_soft_wd[k] = k <= h->soft_K ? exp(-(double)k / Td) : 0.0;
+      h->h_soft_wd[SOFT_WD_GATE] = 1.0 / (1.0 + exp(-ad * 1.0)); h->h_soft_wd[SOFT_WD_GATE + 1] = 1.0 / (1.0 + exp(-ad * -1.0));
+      CU(h, cudaMemcpyAsync(h->d_soft_wd, h->h_soft_wd, sizeof(double) * SOFT_WD_WORDS, cudaMemcpyHostToDevice, s));
+      CU(h, cudaEventRecord(h->soft_w_done, s));
+      h->soft_wd_T = T; h->soft_wd_alpha = alpha;
+    }
+  }
+  CU(h, cudaMemsetAsync(soft_out_dev, 0, sizeof(float) * 8 * (size_t)h->batch, s));
+  StepParams p = params_of(h, actions_dev, 0x7FFFFFF0);
+  p.n_instr = n_instr; p.drom = full ? h->d_drom_slow : h->d_drom_soft; p.rom_meta = h->d_rom_meta_soft; p.perm = nullptr; p.regroup = 0;
+  p.soft_w = h->d_soft_w; p.soft_tab = h->d_soft_tab; p.soft_ent = h->d_soft_ent; p.soft_out = soft_out_dev; p.soft_alpha = alpha; p.soft_K = h->soft_K;
+  p.soft_wd = h->d_soft_wd; p.soft_full = full ? 1 : 0;
+  cudaError_t ce = launch_step(p, s);
+  h->launches += 1;
+  if (ce != cudaSuccess) return fail(h, VCS_ECUDA, "vcs_step_instructions_soft launch", ce);
   return VCS_OK;
 }
 
@@ -583,7 +632,7 @@ int vcs_destroy(vcs_t h) {
   if (cur != h->device) cudaSetDevice(h->device);     // free on the handle's own device, then give the caller's back
   cudaDeviceSynchronize();
   cudaFree(h->d_st); cudaFree(h->d_ram); cudaFree(h->d_sc_ram); cudaFree(h->d_cyc); cudaFree(h->d_screen); cudaFree(h->d_rom_blob); cudaFree(h->d_drom); cudaFree(h->d_drom_plain);
-  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_soft_ent); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr); cudaFree(h->d_perm); cudaFree(h->d_blk_time); cudaFree(h->d_w_avg);
+  cudaFree(h->d_rom_meta); cudaFree(h->d_drom_soft); cudaFree(h->d_rom_meta_soft); cudaFree(h->d_soft_w); cudaFree(h->d_soft_tab); cudaFree(h->d_soft_ent); cudaFree(h->d_drom_slow); cudaFree(h->d_soft_wd); if (h->h_soft_wd) cudaFreeHost(h->h_soft_wd); cudaFree(h->d_env_rom); cudaFree(h->d_seeds); cudaFree(h->d_actions_stage); cudaFree(h->d_switches); cudaFree(h->d_boot); cudaFree(h->d_boot_ctr); cudaFree(h->d_perm); cudaFree(h->d_blk_time); cudaFree(h->d_w_avg);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   if (h->h_soft_w) cudaFreeHost(h->h_soft_w);
   if (h->soft_w_done) cudaEventDestroy(h->soft_w_done);

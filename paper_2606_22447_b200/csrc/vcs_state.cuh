@@ -85,7 +85,8 @@ static_assert(S_STATUS == 58 && S_CART == 60, "file layout");
 // per-block context, in words after the thread files (block-uniform values the out-of-line paths need)
 enum CtxWord { C_SCREEN_LO = 0, C_SCREEN_HI, C_Y0, C_FRAMESKIP, C_BATCH, C_ENV0, C_CAP, C_ROMOFF, C_REGROUP,
                C_META_LO, C_META_HI, C_BLOB_LO, C_BLOB_HI, C_DROM_LO, C_DROM_HI,
-               C_SOFT_OUT_LO, C_SOFT_OUT_HI, C_SOFT_W_LO, C_SOFT_W_HI, C_SOFT_K, C_SOFT_ALPHA, C_SOFT_TAB_LO, C_SOFT_TAB_HI,
+               C_SOFT_WD_LO, C_SOFT_WD_HI,     // FULL mode: e^{-k/T} (k <= K) and the two branch gates in double, as the host computed them
+               C_SOFT_W_LO, C_SOFT_W_HI, C_SOFT_K, C_SOFT_ALPHA, C_SOFT_TAB_LO, C_SOFT_TAB_HI,
                C_HS,           // bank hotspots of the block's ROM (ROM staged in smem: one ROM per block): first address | count << 16 | HS_SC
                C_SCRAM_LO, C_SCRAM_HI,     // Superchip RAM of all envs, [32][batch] words like `ram` (nullptr when no cart has it)
                C_ROMG_LO, C_ROMG_HI,       // the block's ROM image in global memory (one ROM per block; read there when it is not staged, C_ROMOFF then = offset mask)
@@ -104,6 +105,8 @@ struct Handle {                 // host-side bookkeeping behind vcs_t
   uint8_t *d_rom_blob; uint2 *d_drom; RomMeta *d_rom_meta; int32_t *d_env_rom; unsigned long long *d_seeds;
   int device;                   // the CUDA device every pointer below belongs to
   float *h_soft_w; cudaEvent_t soft_w_done; int soft_K;            // soft mode: pinned e^{-k/T} staging buffer, its upload, window of the cached temperature
+  double *d_soft_wd, *h_soft_wd; float soft_wd_T, soft_wd_alpha;   // FULL mode: weights and gates in double (SOFT_WD_WORDS), what they were built for
+  uint2 *d_drom_slow;           // FULL mode: a decode table whose every entry says "decode at run time" (allocated on first use)
   float4 *d_soft_ent;           // soft mode: per decode entry of d_drom_soft, the soft sums of the instruction's own bytes at the cached temperature
   float *d_soft_tab; float soft_tab_T; size_t soft_tab_n;          // W(T) x ROM: the relaxed read of every ROM cell at the cached temperature
   uint2 *d_drom_plain;          // vcs_step_instructions: a decode table for 128-env blocks without fused / closed-form entries (one entry = one instruction)

@@ -152,7 +152,7 @@ template <int BLOCK> DEV void soft_note(uint32_t sl, int k, float soft_v, float 
 template <int BLOCK>
 __device__ __noinline__ uint32_t soft_ram_read(uint32_t sl, uint32_t cell, uint32_t hard) {
   using T = Tia<BLOCK>;
-  const int K = (int)T::ctx(C_SOFT_K);
+  const int K = (int)(T::ctx(C_SOFT_K) & 0x7FFFFFFFu);
   const float *wt = reinterpret_cast<const float *>((unsigned long long)T::ctx(C_SOFT_W_LO) | ((unsigned long long)T::ctx(C_SOFT_W_HI) << 32));
   const uint32_t *ramw = smem + sl;                        // RAM word i of this env at ramw[i * BLOCK], cell 4 i + j in byte j
   const float q = __ldg(wt + 1), q4 = (q * q) * (q * q);
@@ -412,16 +412,69 @@ struct Cpu {
     if constexpr (TAG == 1) fe_snoop(a, v);
   }
   // ---------------------------------------------------------------- SOFT-STE mode (include/vcs.h vcs_step_soft; eq. 8-10)
+  // FULL mode (appendix D; include/vcs.h vcs_step_instructions_soft): the cast of the soft value itself decides
+  // what the machine reads, so it is taken exactly as the oracle takes it — eq. (10) tap by tap in double, k = -K .. K,
+  // with the host's e^{-k/T} (no fused multiply-adds), then (float) and round.  Not a fast path and not meant to be.
+  DEV bool soft_full() const { return (T::ctx(C_SOFT_K) >> 31) != 0; }
+  DEV const double *soft_wd() const { return reinterpret_cast<const double *>((unsigned long long)T::ctx(C_SOFT_WD_LO) | ((unsigned long long)T::ctx(C_SOFT_WD_HI) << 32)); }
+  DEV uint32_t full_rom(uint32_t o, uint32_t hard) {
+    const int K = (int)(T::ctx(C_SOFT_K) & 0x7FFFFFFFu);
+    const double *wd = soft_wd();
+    double plane[8] = {0, 0, 0, 0, 0, 0, 0, 0}, den = 0.0;
+#pragma unroll 1
+    for (int k = -K; k <= K; ++k) {
+      const int i = (int)o + k; if (i < 0 || i >= 4096) continue;
+      const double w = wd[k < 0 ? -k : k];
+      const uint32_t b = rom_byte((di & 0x7000u) + ((uint32_t)i & rom_mask));
+#pragma unroll
+      for (int j = 0; j < 8; ++j) plane[j] = __dadd_rn(plane[j], ((b >> j) & 1u) ? w : 0.0);
+      den = __dadd_rn(den, w);
+    }
+    double soft = 0.0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) soft = __dadd_rn(soft, __dmul_rn((double)(1 << j), __ddiv_rn(plane[j], den)));
+    const float sv = (float)soft;
+    soft_note<BLOCK>(sl, 0, sv, (float)hard, sv);
+    return (uint32_t)(int)rintf(sv) & 0xFFu;
+  }
+  DEV uint32_t full_ram(uint32_t cell, uint32_t hard) {
+    const int K = (int)(T::ctx(C_SOFT_K) & 0x7FFFFFFFu);
+    const double *wd = soft_wd();
+    double num = 0.0, den = 0.0;
+#pragma unroll 1
+    for (int k = -K; k <= K; ++k) {
+      const int i = (int)cell + k; if (i < 0 || i >= 128) continue;
+      const double w = wd[k < 0 ? -k : k];
+      num = __dadd_rn(num, __dmul_rn(w, (double)ram_rd_off((((uint32_t)i & 0x7Cu) * BLOCK) | ((uint32_t)i & 3u))));
+      den = __dadd_rn(den, w);
+    }
+    const float sv = (float)__ddiv_rn(num, den);
+    soft_note<BLOCK>(sl, 1, sv, (float)hard, sv);
+    return (uint32_t)(int)rintf(sv) & 0xFFu;
+  }
+  DEV uint32_t full_branch(uint32_t f, bool set_sense, int32_t delta, bool taken) {        // -> PC = round(pc_nb + g delta)
+    const double g = soft_wd()[SOFT_WD_GATE + ((f != 0) == set_sense ? 0 : 1)];            // z = s (2 f - 1) = +1 / -1
+    const uint32_t pc_nb = pc();
+    const float v = rintf((float)__dadd_rn((double)pc_nb, __dmul_rn(g, (double)delta)));
+    const float pc_hard = (float)pc_nb + (taken ? (float)delta : 0.f);
+    soft_note<BLOCK>(sl, 2, (float)g, pc_hard, v);
+    return (uint32_t)(int)v & 0xFFFFu;
+  }
   DEV uint32_t soft_rom(uint32_t o, uint32_t hard) {       // eq. (10) on the 4096 x 8 bit tensor of the visible bank, then STE + round
+    if (soft_full()) return full_rom(o, hard);
     // the ROM is constant, so W(T) x ROM is computed once per temperature (soft_table_kernel): a fetch is one lookup
     const float sv = __ldg(soft_tab + (di & 0x7000u) + o);
     const float h = (float)hard, ste = sv + (h - sv);      // eq. (9), forward
     soft_note<BLOCK>(sl, 0, sv, h, ste);
     return (uint32_t)(int)rintf(ste) & 0xFFu;
   }
-  DEV uint32_t soft_ram(uint32_t cell, uint32_t hard) { return soft_ram_read<BLOCK>(sl, cell, hard); }
-  DEV void soft_branch(uint32_t f, float sense, float delta, bool taken) {   // the PC itself is set by the hard path (R14)
+  DEV uint32_t soft_ram(uint32_t cell, uint32_t hard) { return soft_full() ? full_ram(cell, hard) : soft_ram_read<BLOCK>(sl, cell, hard); }
+  // SOFT-STE: the PC itself is set by the hard path (R14), returns NO_PC; FULL: returns the PC the cast gives (R18)
+  static constexpr uint32_t NO_PC = 0xFFFFFFFFu;
+  DEV uint32_t soft_branch(uint32_t f, float sense, float delta, bool taken) {
+    if (soft_full()) return full_branch(f, sense > 0.f, (int32_t)delta, taken);
     soft_branch_note<BLOCK>(sl, f, sense, delta, taken, (float)pc());
+    return NO_PC;
   }
   DEV uint32_t pack_p() const {
     return ((zn & 0x180u) ? 0x80u : 0u) | (fV << 6) | 0x20u | fDI | (((zn & 0xFFu) == 0) ? 2u : 0u) | fC;
@@ -622,7 +675,7 @@ struct Cpu {
   DEV bool exec_one(uint32_t cx, uint32_t pl) {
     {
       bool slow = false;                                   // run-time decoded
-      uint32_t ea = 0, v = 0, wv = 0, op2 = 0, hid;
+      uint32_t ea = 0, v = 0, wv = 0, op2 = 0, hid, cast_pc = 0xFFFFFFFFu;     // cast_pc: FULL mode, the PC a branch's cast gives
       int k = 0, i0 = 0, total = 0, kb = 0;
       if constexpr (!GEN) { if (kind >= MK_F8SC) return true; }          // Superchip / E0 / FE carts: the generic executor knows their ports
     dispatch:
@@ -718,8 +771,8 @@ struct Cpu {
           switch (kk >> 1) { case 0: f = (zn & 0x180u) ? 1u : 0u; break; case 1: f = fV; break; case 2: f = fC; break;
                              default: f = (zn & 0xFFu) ? 0u : 1u; break; }
           const bool taken = f == (kk & 1u);
-          if constexpr (SOFT) soft_branch(f, (kk & 1u) ? 1.f : -1.f, (float)(int32_t)pl, taken);
-          if (!taken) break;
+          if constexpr (SOFT) cast_pc = soft_branch(f, (kk & 1u) ? 1.f : -1.f, (float)(int32_t)pl, taken);
+          if (!taken) { if constexpr (SOFT) { if (cast_pc != 0xFFFFFFFFu) set_pc(cast_pc); } break; }
         } goto br_taken;
         // ---- control transfers and stack
         case H_JMP: set_pc(pl); goto ctl;
@@ -832,6 +885,7 @@ struct Cpu {
             if ((cx >> DW_OP2_SHIFT) == 2u) dummy_rd((next & 0xFF00u) | (target & 0xFFu), 1);
             set_pc(target);
           } else di += pl;
+          if constexpr (SOFT) { if (cast_pc != 0xFFFFFFFFu) set_pc(cast_pc); }     // (cycles and discarded reads are the hard decision's)
           cyc += (int32_t)(cx >> DW_OP2_SHIFT);
           goto ctl;
         tia_store: {
@@ -1271,7 +1325,7 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
     { const unsigned long long v = reinterpret_cast<unsigned long long>(p.sc_ram); s_ctx[C_SCRAM_LO] = (uint32_t)v; s_ctx[C_SCRAM_HI] = (uint32_t)(v >> 32); }
     auto put = [&](int lo, const void *q) { const unsigned long long v = reinterpret_cast<unsigned long long>(q); s_ctx[lo] = (uint32_t)v; s_ctx[lo + 1] = (uint32_t)(v >> 32); };
     put(C_META_LO, p.rom_meta); put(C_BLOB_LO, p.rom_blob); put(C_DROM_LO, p.drom); put(C_ROMG_LO, p.rom_blob + rm.offset);
-    put(C_SOFT_OUT_LO, p.soft_out); put(C_SOFT_W_LO, p.soft_w); put(C_SOFT_TAB_LO, p.soft_tab); s_ctx[C_SOFT_K] = (uint32_t)p.soft_K; s_ctx[C_SOFT_ALPHA] = __float_as_uint(p.soft_alpha);
+    put(C_SOFT_WD_LO, p.soft_wd); put(C_SOFT_W_LO, p.soft_w); put(C_SOFT_TAB_LO, p.soft_tab); s_ctx[C_SOFT_K] = (uint32_t)p.soft_K | (p.soft_full ? 0x80000000u : 0u); s_ctx[C_SOFT_ALPHA] = __float_as_uint(p.soft_alpha);
     if constexpr (ROMS == 1) { mbar_init(smem_u32(&s_bar), 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
   }
   __syncthreads();
@@ -1563,6 +1617,8 @@ static cudaError_t launch_one(const StepParams &p, cudaStream_t stream) {
 }
 
 cudaError_t launch_step(const StepParams &p, cudaStream_t stream) {
+  if (p.n_instr > 0 && p.soft_out)                         // vcs_step_instructions_soft (SOFT-STE or FULL, per instruction)
+    return launch_one<128, 0, 128, true, true>(p, stream);
   if (p.n_instr > 0)                                       // vcs_step_instructions: one variant (128 envs per block, ROM through the read-only path)
     return launch_one<128, 0, 128, false, true>(p, stream);
   if (p.soft_out)                                          // SOFT-STE mode: one variant (ROM through the read-only path, no regroup)
