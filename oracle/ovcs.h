@@ -22,6 +22,7 @@
  * in TIA reads, same-cycle INTIM/underflow, F8 start bank, power-on timer/RAM state, y0,
  * the Superchip / E0 / FE power-up states and the read of a Superchip write port (R16),
  * and the format guess of ovcs_detect_mapper against the paper's (xitari's) signatures (R17).
+ * FULL mode (R18) is pinned by the paper's closed forms; its Table 3 N_div values need a ROM that is not here.
  * Decimal-mode results for invalid BCD operands are pinned against the digit-wise
  * definition since round 2 (tests/test_oracle_pins_cpu.py).
  */

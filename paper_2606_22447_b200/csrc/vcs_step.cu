@@ -34,6 +34,9 @@
 #include "vcs_decode.cuh"
 #include "vcs_step.cuh"
 
+#ifndef VCS_PAD
+#define VCS_PAD 0
+#endif
 namespace vcs {
 
 __constant__ uint32_t c_gen[256];       // generic decode per opcode (vcs_decode.cuh generic_entry) for H_SLOW
@@ -1302,6 +1305,14 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
   uint32_t *s_ctx = smem + S_WORDS * BLOCK;
   constexpr uint32_t ROM_OFF = (S_WORDS * BLOCK + C_WORDS) * 4;          // byte offset of the ROM image in smem
   const int tid = threadIdx.x;
+  // Code placement.  The kernel is instruction-cache bound and its hot device functions follow the kernel body in the
+  // image, so where their 128-byte lines begin moves with the body's size (+-4 % from placement alone).
+  // VCS_PAD filler instructions (one clock read each, executed once per thread) in the headline variant's prologue
+  // put that offset where it measured best; 0..7 cover every placement modulo 128 bytes.
+  if constexpr (BLOCK == 256 && ROMS == 1 && THREADS == 288 && !SOFT && !COUNT) {
+#pragma unroll
+    for (int i = 0; i < VCS_PAD; ++i) { uint32_t t; asm volatile("mov.u32 %0, %%clock;" : "=r"(t)); }
+  }
   if (p.blk_time && tid == 0) {                            // placement bookkeeping: when and where this block ran
     unsigned long long t; uint32_t sm;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
