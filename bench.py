@@ -118,10 +118,14 @@ def run_paper_axis(args):
     from vcs_inputs import make_workload
     torch.cuda.set_device(0)
     rows = []
+    mode = args.axis_mode                                  # hard | ste | full (the soft modes at the paper's corner alpha = 6, T = 0.14)
     for n in (1, 16, 64, 256, 1024, 4096, 16384, 65536):
         w = make_workload(2, batch=n)
         env = VCS(w.roms, w.seeds, w.env_rom)
         acts = torch.from_numpy(w.actions(0, 16)).cuda()
+        if mode != "hard":
+            so = torch.empty((n, 8), dtype=torch.float32, device="cuda")
+            env.step_instructions = lambda a, k, _e=env, _so=so: _e.step_instructions_soft(a, k, 0.14, 6.0, mode == "full", out=_so)
         for t in range(3):
             env.step_instructions(acts[t], 3000)                   # warm-up rollouts
         torch.cuda.synchronize()
@@ -136,7 +140,9 @@ def run_paper_axis(args):
                      "instructions_per_s": n * 3000 / (float(ms.mean()) * 1e-3)})
         env.close()
     print(json.dumps({"metric": "emulated CPU instructions/s, 3,000-instruction rollouts (PAPER.md Table 7 axis)", "unit": "instructions/s",
-                      "mode": "hard (integer) mode, vcs_step_instructions; the paper's rows are float32 soft mode on a GTX 1080 Ti with the Pong ROM",
+                      "mode": {"hard": "hard (integer) mode, vcs_step_instructions", "ste": "SOFT-STE mode per instruction (alpha 6, T 0.14), vcs_step_instructions_soft",
+                               "full": "FULL mode, the fully relaxed forward (alpha 6, T 0.14: its exact corner), vcs_step_instructions_soft"}[mode]
+                              + "; the paper's rows are float32 soft mode on a GTX 1080 Ti with the Pong ROM",
                       "workload": "config 2: N envs sharing one seeded 4K ROM, per-env random actions", "rows": rows}), flush=True)
 
 
@@ -196,6 +202,7 @@ def main():
     ap.add_argument("--paper-axis", action="store_true",
                     help="the paper's own throughput axis (PAPER.md Table 7, L566-576; L582 one step = one CPU instruction): "
                          "3,000-instruction rollouts (vcs_step_instructions) of one shared 4K ROM at N in {1, 16, ..., 65536}; prints a table line")
+    ap.add_argument("--axis-mode", default="hard", choices=["hard", "ste", "full"], help="with --paper-axis: which forward the rollouts run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
