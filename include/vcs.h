@@ -207,6 +207,29 @@ int vcs_get_ram_host(vcs_t h, uint8_t *out_host, void *cuda_stream);
 int vcs_get_regs_host(vcs_t h, vcs_regs *out_host, void *cuda_stream);
 int vcs_get_screen_host(vcs_t h, uint8_t *out_host, void *cuda_stream);
 
+/* A host-buffer step that allocates NOTHING, for callers that may not call cudaMalloc while they run (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it).  The calls above allocate their pinned / device stage
+ * on first use (and when the batch grows); this one stages in a static device array that is part of the library:
+ * VCS_NOALLOC_MAX_BATCH envs x (1 + 128 + 32) bytes + 256 = 10,551,552 bytes, held by every GPU that loads the library
+ * until the process exits.  One call = vcs_step(actions, frameskip) followed by the read-back of RAM and registers:
+ *   actions_host    HOST uint8[batch]       (in)   as vcs_step_host
+ *   ram_out_host    HOST uint8[batch][128]  (out)  as vcs_get_ram_host
+ *   regs_out_host   HOST vcs_regs[batch]    (out)  as vcs_get_regs_host
+ *   n_flagged_host  HOST int32              (out)  number of envs whose vcs_regs.status is non-zero after the step
+ * Everything is ENQUEUED on `cuda_stream` and the call returns: the outputs are valid once the caller has synchronised
+ * that stream, and all four host buffers must stay valid until then (pinned host memory for copies that really are
+ * asynchronous; under stream capture it must be pinned).  No cudaMalloc, cudaFree or other allocating call is made;
+ * the first call on a device takes the array's address (cudaGetSymbolAddress), so make one call before capturing.
+ * Errors: VCS_EINVAL when batch > VCS_NOALLOC_MAX_BATCH (vcs_last_error says so), on a NULL buffer, a frameskip out of
+ * range or a device index above 63; VCS_ECUDA as vcs_step.
+ * SHARED SCRATCH: every call of the process on one GPU, whatever its handle, uses the same array, which keeps the last
+ * call's contents (the call clears the one word that must start at zero and overwrites the rest before reading it).
+ * Calls on ONE stream are ordered and safe; calls that can overlap on the GPU — two streams, two threads, two handles
+ * — race on the array and return garbage: serialise them. */
+#define VCS_NOALLOC_MAX_BATCH 65536
+int vcs_step_host_noalloc(vcs_t h, const uint8_t *actions_host, int32_t frameskip, uint8_t *ram_out_host,
+                          vcs_regs *regs_out_host, int32_t *n_flagged_host, void *cuda_stream);
+
 /* Device pointer to the library-owned front screen [batch][210][160] (valid until vcs_destroy; contents
  * change with every vcs_step).  Zero-copy alternative to vcs_get_screen. */
 int vcs_screen_ptr(vcs_t h, const uint8_t **out_dev_ptr);

@@ -20,9 +20,11 @@ VCS_F_NO_SPIN, VCS_F_NO_FUSE, VCS_F_NO_REGROUP, VCS_F_ROM_GLOBAL, VCS_F_NO_BALAN
 VCS_F_BLOCK_64, VCS_F_BLOCK_128, VCS_F_BLOCK_256 = 1 << 8, 2 << 8, 3 << 8
 _ERR = {VCS_EINVAL: "VCS_EINVAL", VCS_ECUDA: "VCS_ECUDA", VCS_ENOMEM: "VCS_ENOMEM", VCS_EROM: "VCS_EROM"}
 
-EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_instructions", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_step_instructions_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_cart_ram", "vcs_get_screen", "vcs_detect_mapper", "vcs_step_host",
+EXPORTS = ["vcs_create", "vcs_reset", "vcs_step", "vcs_step_instructions", "vcs_step_masked", "vcs_set_switches", "vcs_boot", "vcs_auto_reset", "vcs_get_booting", "vcs_step_soft", "vcs_step_instructions_soft", "vcs_get_ram", "vcs_get_regs", "vcs_get_cart_ram", "vcs_get_screen", "vcs_detect_mapper", "vcs_step_host", "vcs_step_host_noalloc",
            "vcs_get_ram_host", "vcs_get_regs_host", "vcs_get_screen_host", "vcs_screen_ptr", "vcs_block_times", "vcs_launch_count",
            "vcs_optable", "vcs_issue_peak", "vcs_destroy", "vcs_last_error"]
+
+NOALLOC_MAX_BATCH = 65536        # VCS_NOALLOC_MAX_BATCH (include/vcs.h)
 
 REGS_DTYPE = np.dtype([("cycles", "<u8"), ("frame", "<u4"), ("pc", "<u2"), ("a", "u1"), ("x", "u1"), ("y", "u1"),
                        ("sp", "u1"), ("p", "u1"), ("bank", "u1"), ("line", "<u2"), ("cyc_in_line", "u1"),
@@ -62,6 +64,7 @@ def load_library() -> C.CDLL:
     L.vcs_reset.argtypes = [P, P, P]
     L.vcs_step.argtypes = [P, P, C.c_int32, P]
     L.vcs_step_host.argtypes = [P, P, C.c_int32, P]
+    L.vcs_step_host_noalloc.argtypes = [P, P, C.c_int32, P, P, P, P]
     L.vcs_step_instructions.argtypes = [P, P, C.c_int32, P]
     L.vcs_step_instructions_soft.argtypes = [P, P, C.c_int32, C.c_float, C.c_float, C.c_int32, P, P]
     L.vcs_step_masked.argtypes = [P, P, C.c_int32, P, P]
@@ -247,6 +250,22 @@ class VCS:
     def step_host(self, actions: np.ndarray, frameskip=4, stream=None):
         a = np.ascontiguousarray(actions, dtype=np.uint8); assert a.shape == (self.batch,)
         self._chk(self.L.vcs_step_host(self.h, a.ctypes.data, int(frameskip), _stream_ptr(stream)), "vcs_step_host")
+
+    def step_host_noalloc(self, actions: np.ndarray, frameskip=4, ram_out=None, regs_out=None, flagged_out=None, stream=None, sync=True):
+        """vcs_step_host_noalloc: step + read-back of RAM / regs / number of envs with a status bit, staged in the library's
+        static device array (no allocation on the CUDA side; batch <= NOALLOC_MAX_BATCH).  The C call only enqueues: with
+        sync=True the stream is synchronised here and (ram, regs, n_flagged) are returned ready to read."""
+        a = np.ascontiguousarray(actions, dtype=np.uint8); assert a.shape == (self.batch,)
+        ram = np.empty((self.batch, 128), dtype=np.uint8) if ram_out is None else ram_out
+        regs = np.empty(self.batch, dtype=REGS_DTYPE) if regs_out is None else regs_out
+        flagged = np.full(1, -1, dtype=np.int32) if flagged_out is None else flagged_out
+        sp = _stream_ptr(stream)
+        self._keep = (a, ram, regs, flagged)                # the buffers must outlive the enqueued copies
+        self._chk(self.L.vcs_step_host_noalloc(self.h, a.ctypes.data, int(frameskip), ram.ctypes.data, regs.ctypes.data, flagged.ctypes.data, sp),
+                  "vcs_step_host_noalloc")
+        if sync:
+            (self.torch.cuda.current_stream() if stream is None else stream).synchronize()
+        return ram, regs, flagged
 
     def ram_host(self, stream=None) -> np.ndarray:
         out = np.empty((self.batch, 128), dtype=np.uint8)

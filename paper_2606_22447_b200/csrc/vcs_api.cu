@@ -593,6 +593,86 @@ int vcs_block_times(vcs_t h, uint64_t *times_host, int32_t *perm_host, int32_t c
 
 int64_t vcs_launch_count(vcs_t h) { return h ? h->launches : -1; }
 
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// vcs_step_host_noalloc (include/vcs.h): a host-buffer step for callers that cannot call cudaMalloc.  Its device-side
+// staging — the actions on their way in, the transposed RAM and the vcs_regs on their way out, a flag counter — lives
+// in ONE file-scope array instead of the handle's lazily allocated stage: VCS_NOALLOC_MAX_BATCH envs x (1 + 128 + 32)
+// bytes + 256 = 10,551,552 bytes, held by every GPU that loads the library until the process exits.  All calls of a
+// process share it, per device.
+//
+// The array's name below is a DEVICE symbol: in host code it is a host-side stand-in, not a device address, so the host
+// side takes the address with cudaGetSymbolAddress — once per device, with that device current (noalloc_base) — and
+// passes that pointer on; only device code (noalloc_count_flags_kernel) names the array itself.
+constexpr size_t NOALLOC_OFF_ACT = 0;                                                     // uint8 [MAX]       actions, staged for the step kernel
+constexpr size_t NOALLOC_OFF_RAM = NOALLOC_OFF_ACT + (size_t)VCS_NOALLOC_MAX_BATCH;       // uint8 [MAX][128]  get_ram_kernel's output
+constexpr size_t NOALLOC_OFF_REGS = NOALLOC_OFF_RAM + 128 * (size_t)VCS_NOALLOC_MAX_BATCH; // vcs_regs [MAX]    get_regs_kernel's output
+constexpr size_t NOALLOC_OFF_CTR = NOALLOC_OFF_REGS + 32 * (size_t)VCS_NOALLOC_MAX_BATCH; // uint32            envs with a status bit set: MUST start at zero
+constexpr size_t NOALLOC_BYTES = NOALLOC_OFF_CTR + 256;
+static_assert(NOALLOC_OFF_RAM % 256 == 0 && NOALLOC_OFF_REGS % 256 == 0 && NOALLOC_OFF_CTR % 256 == 0, "scratch regions keep the array's alignment");
+static __device__ __align__(256) unsigned char vcs_noalloc_scratch[NOALLOC_BYTES];
+
+namespace {
+
+// envs whose vcs_regs.status (byte 23) is non-zero, added up in the counter word of the scratch array
+__global__ void noalloc_count_flags_kernel(int B) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= B) return;
+  if (vcs_noalloc_scratch[NOALLOC_OFF_REGS + 32 * (size_t)e + 23] != 0)
+    atomicAdd(reinterpret_cast<unsigned int *>(vcs_noalloc_scratch + NOALLOC_OFF_CTR), 1u);
+}
+
+// the array's device address on the current device: resolved once per device (no allocation: the array came with the module)
+int noalloc_base(Handle *h, unsigned char **out) {
+  static unsigned char *base[64] = {nullptr};
+  if (h->device < 0 || h->device >= 64) return fail(h, VCS_EINVAL, "vcs_step_host_noalloc: device index above 63");
+  if (!base[h->device]) {                              // (DEV_OK has checked that h->device is the current device)
+    void *ptr = nullptr;
+    const cudaError_t ce = cudaGetSymbolAddress(&ptr, vcs_noalloc_scratch);
+    if (ce != cudaSuccess || !ptr) return fail(h, VCS_ECUDA, "vcs_step_host_noalloc: cudaGetSymbolAddress(vcs_noalloc_scratch)", ce);
+    base[h->device] = static_cast<unsigned char *>(ptr);
+  }
+  *out = base[h->device];
+  return VCS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int vcs_step_host_noalloc(vcs_t h, const uint8_t *actions_host, int32_t frameskip, uint8_t *ram_out_host, vcs_regs *regs_out_host,
+                          int32_t *n_flagged_host, void *cuda_stream) {
+  DEV_OK(h);
+  if (!actions_host || !ram_out_host || !regs_out_host || !n_flagged_host) return fail(h, VCS_EINVAL, "vcs_step_host_noalloc: NULL buffer");
+  if (h->batch > VCS_NOALLOC_MAX_BATCH) {
+    char msg[160];
+    snprintf(msg, sizeof msg, "vcs_step_host_noalloc: batch %d exceeds VCS_NOALLOC_MAX_BATCH = %d (the size of the library's static scratch array)",
+             h->batch, (int)VCS_NOALLOC_MAX_BATCH);
+    return fail(h, VCS_EINVAL, msg);
+  }
+  unsigned char *base = nullptr;
+  if (int rc = noalloc_base(h, &base)) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const size_t B = (size_t)h->batch;
+  uint8_t *d_act = base + NOALLOC_OFF_ACT, *d_ram = base + NOALLOC_OFF_RAM;
+  vcs_regs *d_regs = reinterpret_cast<vcs_regs *>(base + NOALLOC_OFF_REGS);
+  // the array keeps the previous call's contents: the counter must start at zero; every other byte this call reads
+  // (actions, RAM, regs of envs [0, batch)) is written by this call first
+  CU(h, cudaMemsetAsync(base + NOALLOC_OFF_CTR, 0, 256, s));
+  CU(h, cudaMemcpyAsync(d_act, actions_host, B, cudaMemcpyHostToDevice, s));
+  if (int rc = vcs_step(h, d_act, frameskip, cuda_stream)) return rc;
+  if (int rc = vcs_get_ram(h, d_ram, cuda_stream)) return rc;
+  if (int rc = vcs_get_regs(h, d_regs, cuda_stream)) return rc;
+  noalloc_count_flags_kernel<<<(h->batch + 255) / 256, 256, 0, s>>>(h->batch);
+  h->launches += 1;
+  CU(h, cudaGetLastError());
+  CU(h, cudaMemcpyAsync(ram_out_host, d_ram, 128 * B, cudaMemcpyDeviceToHost, s));
+  CU(h, cudaMemcpyAsync(regs_out_host, d_regs, 32 * B, cudaMemcpyDeviceToHost, s));
+  CU(h, cudaMemcpyAsync(n_flagged_host, base + NOALLOC_OFF_CTR, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+  return VCS_OK;                                        // enqueued: the outputs are valid once the caller has synchronised the stream
+}
+
 // Format guess from size and content (reading R17).  Host only.
 int vcs_detect_mapper(const uint8_t *data, uint32_t size) {
   if (!data) return VCS_EINVAL;
