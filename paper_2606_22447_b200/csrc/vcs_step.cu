@@ -1050,7 +1050,7 @@ DEV uint32_t rom_byte_hot(uint32_t off) {                  // byte `off` (bank <
 // SOFT: `se` = per decode entry {sum of the soft values of the instruction's own bytes, their count, their largest
 // |soft - hard|, STE mismatches among them} (soft_entry_kernel); data reads of RAM and branches are noted where they run.
 template <int BLOCK, int ROMS, int THREADS, bool SOFT, bool COUNT = false>
-DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl, const float4 *se = nullptr, const float *stab = nullptr) {
+DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl, const uint32_t live, const float4 *se = nullptr, const float *stab = nullptr) {
   using T = Tia<BLOCK>;
   uint8_t *const ramb = reinterpret_cast<uint8_t *>(smem) + 4u * sl;
   auto soft_cell = [&](uint32_t a, uint32_t hard) -> uint32_t {          // SOFT: a value read of RAM cell a & 0x7F (else the byte as it is)
@@ -1275,14 +1275,16 @@ DEV void run_block(Hot &h, const uint2 *dr, const uint32_t sl, const float4 *se 
     alu(h, aux, v);
   seq:                                                     // sequential successor
     h.wx = wn.x | late0; h.wy = wn.y | late0;
-    // a leader is where another lane of the warp may be waiting: re-form the group — unless all 32 lanes are in this
-    // group already (nobody can be waiting; which lanes run together never changes results, only the time they take)
-    if (!(h.wx & DW_LEADER) || __activemask() == 0xFFFFFFFFu) continue;
+    // a leader is where another lane of the warp may be waiting: re-form the group — unless every lane of the warp that
+    // can run at all (`live`: holds an env, not parked, not done — as of the last scheduling pass; a lane can only
+    // leave that set before the next pass) is in this group already: nobody can be waiting, and which lanes run
+    // together never changes results, only the time they take
+    if (!(h.wx & DW_LEADER) || __activemask() == live) continue;
     return;
   ctl:                                                     // taken branch / jump: fetch at the new PC, re-schedule
     if (!((h.pbase + h.di) & 0x1000u)) { h.wx = HC_COLD + H_SLOW; h.wy = 0; }
     else { const uint2 t = __ldg(dr + h.di); h.wx = t.x; h.wy = t.y; }
-    if (__activemask() == 0xFFFFFFFFu) continue;           // (the whole warp took it together)
+    if (__activemask() == live) continue;                  // (every runnable lane of the warp took it together)
     return;
   }
 }
@@ -1428,7 +1430,8 @@ __global__ void __launch_bounds__(THREADS, 512 / BLOCK) vcs_step_kernel(StepPara
       const uint32_t key = h.keyhi | ((h.pbase + h.di) & 0xFFFFu);
       const uint32_t mk = __reduce_min_sync(0xFFFFFFFFu, key);
       if (mk >= KEY_PARKED) break;                         // every lane is parked or has finished the step
-      if (key == mk) run_block<BLOCK, ROMS, THREADS, SOFT, COUNT>(h, dr, cur, se, stab);
+      const uint32_t live = __ballot_sync(0xFFFFFFFFu, key < KEY_PARKED);      // the lanes that can run
+      if (key == mk) run_block<BLOCK, ROMS, THREADS, SOFT, COUNT>(h, dr, cur, live, se, stab);
       if (h.aux == AUX_GENERIC) h = cold_exec_generic<BLOCK, ROMS, THREADS, SOFT>(h, cur, h.wx, h.wy);   // (a rare bus pattern: see cold_exec)
     }
     if (!regroups) break;
