@@ -12,7 +12,8 @@ SOURCES = ["vcs_api.cu", "vcs_step.cu", "vcs_peak.cu"]
 HEADERS = ["vcs_decode.cuh", "vcs_tia.cuh", "vcs_state.cuh", "vcs_step.cuh", "vcs_optable.cuh", os.path.join("..", "..", "include", "vcs.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--use_fast_math",
-              "-maxrregcount=48"]     # caps the out-of-line device functions (the kernels carry __launch_bounds__): measured 9.70 -> 9.51 ms on config 4, 4K carts 8.4 -> 7.9 ms
+              "-maxrregcount=56"]     # caps the out-of-line device functions (the kernels carry __launch_bounds__): round 1 measured 9.70 -> 9.51 ms
+                                      # on config 4 with 48; on the round-2 kernel 40 / 48 / 56 / 64 / 80 give 7.05 / 6.97 / 6.92 / 7.15 / 7.10 ms
 
 
 def needs_build() -> bool:
